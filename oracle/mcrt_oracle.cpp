@@ -1,0 +1,679 @@
+// oracle/mcrt_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, serial-in-spirit fp64 CPU implementation of the hot path of
+// Siebenmorgen, Heymann & Kruegel, "PAH in vectorized three dimensional Monte Carlo dust
+// radiative transfer models", following the paper's section 2 step by step:
+//
+//   PAPER.md L23  "The space is partitioned into cubes and, where a finer grid is needed,
+//                  the cubes are further divided into subcubes (cells). The star emits photon
+//                  packages of constant energy eps, but different frequencies. A package
+//                  entering on its flight path a cell may be absorbed there or scattered. The
+//                  probability for such an interaction is given by the extinction optical
+//                  depth along the path within the cell. When the package is scattered, it
+//                  only changes direction determined in a probabilistic manner by the phase
+//                  function. When it is absorbed, a new package of the same energy, but
+//                  usually different frequency nu_new is emitted from the spot of absorption.
+//                  The emission is isotropic. Each absorption event raises the energy of the
+//                  cell by eps, and accordingly its temperature."
+//   PAPER.md L25-27  nu_new is drawn "using the cell temperature before absorption", and the
+//                  Bjorkman & Wood correction is omitted (Eqn 11.67 instead of 11.65 of
+//                  Kruegel 2006): dP/dnu ~ kappa_nu B_nu(T_before).
+//
+// Where the paper is silent the readings R1..R33 of SURVEY.md 8(c) / DESIGN.md section 3 are
+// taken; each function below names the step (O0..O8) and reading it implements.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+// load this file.  It shares no code, header, table or constant generator with the CUDA
+// path under paper_1201_3588_b200/csrc/.
+//
+// Pins (tests/test_oracle_pins.py): Philox vs the cuRAND host library; isotropy and HG
+// moments; Planck sum vs sigma T^4/pi; Q(T) vs the Gamma*zeta closed form; CDF sampling vs
+// its definition; temperature-inversion identity; integer packet accounting; pure-scattering
+// bin-by-bin conservation; Beer-Lambert escape vs brute-force chords; optically thin
+// T ~ r^(-2/(4+beta)); per-flight agreement with an "intersect every box" walker (a second,
+// independent algorithm, also re-implemented in numpy in the tests); split invariance on a
+// two-level grid; external-field mean chord 2a/3.
+// PARITY UNPINNED: the full multi-scattering + re-emission SED and temperatures at
+// tau_V >= 1 have no closed form and the paper's benchmarks are not
+// available; they are held only by the component pins above.
+//
+// The per-packet loop may run under OpenMP (packets are independent within a batch: T is
+// frozen, every packet has its own Philox stream, tallies are integers), which changes no
+// result.
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+// ---- O0 constants (cgs, CODATA 2018) --------------------------------------------------
+const double H_PLANCK = 6.62607015e-27;
+const double C_LIGHT = 2.99792458e10;
+const double K_BOLTZ = 1.380649e-16;
+const double PI = 3.14159265358979323846;
+
+const uint32_t TAG_EMIT = 0, TAG_FLIGHT = 1, TAG_REEMIT = 2;
+const uint32_t K_MAX_FLIGHTS = 10000000u;   // R20
+const int COMP_DIRECT = 0, COMP_SCATTERED = 1, COMP_THERMAL = 2;
+
+// ---- O3 Philox4x32-10 (Salmon et al. 2011) -------------------------------------------
+void philox4x32_10(const uint32_t key_in[2], const uint32_t ctr_in[4], uint32_t out[4]) {
+  const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+  uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3];
+  uint32_t k0 = key_in[0], k1 = key_in[1];
+  for (int r = 0; r < 10; ++r) {
+    if (r > 0) { k0 += W0; k1 += W1; }
+    uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// R18/R19: block of four uniforms in (0,1) for (seed, packet id, k, tag).
+void draw4(uint64_t seed, uint64_t pid, uint32_t k, uint32_t tag, double u[4]) {
+  uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  uint32_t ctr[4] = {(uint32_t)pid, (uint32_t)(pid >> 32), k, tag};
+  uint32_t x[4];
+  philox4x32_10(key, ctr, x);
+  for (int i = 0; i < 4; ++i) u[i] = ((double)x[i] + 0.5) * (1.0 / 4294967296.0);
+}
+
+// ---- O2 Planck -------------------------------------------------------------------------
+double planck_nu(double nu, double T) {
+  double x = H_PLANCK * nu / (K_BOLTZ * T);
+  double e = std::expm1(x);
+  if (!(e < 1e300)) return 0.0;
+  return (2.0 * H_PLANCK * nu * nu * nu / (C_LIGHT * C_LIGHT)) / e;
+}
+
+// ---- O6 direction draws ----------------------------------------------------------------
+void isotropic_dir(double u2, double u3, double d[3]) {
+  double mu = 2.0 * u2 - 1.0, phi = 2.0 * PI * u3;
+  double s = std::sqrt(std::max(0.0, 1.0 - mu * mu));
+  d[0] = s * std::cos(phi); d[1] = s * std::sin(phi); d[2] = mu;
+}
+
+double hg_cos(double g, double u) {   // R15
+  if (std::fabs(g) < 1e-3) return 2.0 * u - 1.0;
+  double t = (1.0 - g * g) / (1.0 - g + 2.0 * g * u);
+  double c = (1.0 + g * g - t * t) / (2.0 * g);
+  return std::min(1.0, std::max(-1.0, c));
+}
+
+void rotate_dir(const double d[3], double ct, double phi, double out[3]) {
+  double st = std::sqrt(std::max(0.0, 1.0 - ct * ct));
+  double cp = std::cos(phi), sp = std::sin(phi);
+  if (std::fabs(d[2]) < 1.0 - 1e-10) {
+    double q = std::sqrt(1.0 - d[2] * d[2]);
+    out[0] = st * (d[0] * d[2] * cp - d[1] * sp) / q + d[0] * ct;
+    out[1] = st * (d[1] * d[2] * cp + d[0] * sp) / q + d[1] * ct;
+    out[2] = -st * cp * q + d[2] * ct;
+  } else {
+    out[0] = st * cp; out[1] = st * sp; out[2] = (d[2] >= 0 ? 1.0 : -1.0) * ct;
+  }
+  double n = std::sqrt(out[0] * out[0] + out[1] * out[1] + out[2] * out[2]);
+  out[0] /= n; out[1] /= n; out[2] /= n;
+}
+
+struct Source { int type; double pos[3]; double L; double Tbb; };
+
+struct Counters { uint64_t emitted, escaped, lost, absorptions, scatterings, flights, crossings; };
+
+struct Ctx {
+  // grid (O1 of the build: D1, D2; layout R22). Positions are in root-cube units.
+  int N = 0, S = 1;
+  double origin[3] = {0, 0, 0}, root_size = 1;
+  std::vector<int32_t> refidx;          // [N^3]: k-th refined cube, or -1
+  int64_t n_ref = 0, slots = 0;
+  std::vector<double> rho;              // [slots] g cm^-3
+  // opacity tables (O1, O2)
+  int nb = 0;
+  std::vector<double> nu, dnu, kabs, ksca, kext, alb, g;
+  int nT = 0; double Tmin = 1, Tmax = 1e4, dlnT = 0;
+  std::vector<double> Q, C;             // Q[nT], C[nT*nb]
+  // sources
+  std::vector<Source> src; std::vector<double> Lcdf, Csrc; double Ltot = 0;
+  // state
+  std::vector<uint64_t> cum; std::vector<double> T; uint64_t Ncum = 0;
+  std::vector<uint64_t> sed, emitted_per_bin; Counters cnt{};
+  int walker = 0;                       // 0 = cell walk (O5), 1 = brute force (tests)
+  bool have_opacity = false, have_source = false;
+};
+
+inline int64_t root_lin(const Ctx& c, const int i[3]) {
+  return (int64_t)i[0] + (int64_t)c.N * ((int64_t)i[1] + (int64_t)c.N * i[2]);
+}
+inline int64_t leaf_slot(const Ctx& c, const int ir[3], const int is[3], bool refined) {
+  int64_t r = root_lin(c, ir);
+  if (!refined) return r;
+  int64_t k = c.refidx[r];
+  return (int64_t)c.N * c.N * c.N + k * (int64_t)(c.S * c.S * c.S) +
+         (is[0] + c.S * (is[1] + c.S * is[2]));
+}
+
+struct Packet {
+  double x[3], d[3];
+  int bin, comp;
+  int ir[3], is[3];
+  bool refined;
+};
+
+// R7: direction-aware location of the start cell, per axis in finest-level units.
+bool locate(const Ctx& c, Packet& p) {
+  for (int a = 0; a < 3; ++a) {
+    double xf = p.x[a] * c.S;
+    long f = (p.d[a] >= 0) ? (long)std::floor(xf) : (long)std::ceil(xf) - 1;
+    if (f < 0 || f >= (long)c.N * c.S) return false;
+    p.ir[a] = (int)(f / c.S);
+    p.is[a] = (int)(f % c.S);
+  }
+  p.refined = c.refidx[root_lin(c, p.ir)] >= 0;
+  if (!p.refined) p.is[0] = p.is[1] = p.is[2] = 0;
+  return true;
+}
+
+// ---- O5: one flight by the cell walk.  Returns 1 = interaction in leaf *slot at p.x,
+//      0 = escaped.  crossings is incremented once per leaf left through a face (R27).
+int walk_cells(const Ctx& c, Packet& p, double tau_star, int64_t* slot, uint64_t* crossings) {
+  const double hs = 1.0 / c.S;
+  double tau_acc = 0.0;
+  const double kx = c.kext[p.bin] * c.root_size;   // optical depth per (g cm^-3) per root unit
+  for (;;) {
+    double lo[3], hi[3];
+    for (int a = 0; a < 3; ++a) {
+      if (p.refined) { lo[a] = p.ir[a] + p.is[a] * hs; hi[a] = lo[a] + hs; }
+      else { lo[a] = p.ir[a]; hi[a] = p.ir[a] + 1.0; }
+    }
+    double ell = 1e300; int ax = -1;
+    for (int a = 0; a < 3; ++a) {
+      if (std::fabs(p.d[a]) < 1e-30) continue;     // R21
+      double t = ((p.d[a] > 0 ? hi[a] : lo[a]) - p.x[a]) / p.d[a];
+      if (t < 0) t = 0;
+      if (t < ell) { ell = t; ax = a; }            // strict <: ties -> lowest axis
+    }
+    int64_t s = leaf_slot(c, p.ir, p.is, p.refined);
+    double alpha = c.rho[s] * kx;
+    if (alpha > 0 && tau_acc + alpha * ell >= tau_star) {
+      double dl = (tau_star - tau_acc) / alpha;
+      for (int a = 0; a < 3; ++a) p.x[a] += p.d[a] * dl;
+      *slot = s;
+      return 1;
+    }
+    tau_acc += alpha * ell;
+    for (int a = 0; a < 3; ++a) p.x[a] += p.d[a] * ell;
+    p.x[ax] = (p.d[ax] > 0) ? hi[ax] : lo[ax];
+    ++*crossings;
+    int step = p.d[ax] > 0 ? 1 : -1;
+    bool leave_root = true;
+    if (p.refined) {
+      int ns = p.is[ax] + step;
+      if (ns >= 0 && ns < c.S) { p.is[ax] = ns; leave_root = false; }
+    }
+    if (leave_root) {
+      p.ir[ax] += step;
+      if (p.ir[ax] < 0 || p.ir[ax] >= c.N) return 0;          // escape by integer index
+      p.refined = c.refidx[root_lin(c, p.ir)] >= 0;
+      if (p.refined) {
+        for (int b = 0; b < 3; ++b) {
+          if (b == ax) { p.is[b] = step > 0 ? 0 : c.S - 1; continue; }
+          int v = (int)std::floor((p.x[b] - p.ir[b]) / hs);
+          p.is[b] = std::min(c.S - 1, std::max(0, v));
+        }
+      } else { p.is[0] = p.is[1] = p.is[2] = 0; }
+    }
+  }
+}
+
+// ---- second, independent walker for the pins: intersect EVERY leaf box with the ray by the
+//      slab method, sort by entry distance, accumulate optical depth.  O(leaves) per flight.
+int walk_bruteforce(const Ctx& c, Packet& p, double tau_star, int64_t* slot,
+                    uint64_t* crossings) {
+  struct Seg { double t0, t1; int64_t slot; int ir[3], is[3]; bool refined; };
+  std::vector<Seg> segs;
+  const double hs = 1.0 / c.S;
+  const double kx = c.kext[p.bin] * c.root_size;
+  auto clip = [&](const double lo[3], const double hi[3], double& t0, double& t1) {
+    t0 = 0.0; t1 = 1e300;
+    for (int a = 0; a < 3; ++a) {
+      if (std::fabs(p.d[a]) < 1e-30) {
+        if (p.x[a] < lo[a] || p.x[a] > hi[a]) return false;
+        continue;
+      }
+      double ta = (lo[a] - p.x[a]) / p.d[a], tb = (hi[a] - p.x[a]) / p.d[a];
+      if (ta > tb) std::swap(ta, tb);
+      t0 = std::max(t0, ta); t1 = std::min(t1, tb);
+    }
+    return t1 > t0;
+  };
+  for (int z = 0; z < c.N; ++z) for (int y = 0; y < c.N; ++y) for (int x = 0; x < c.N; ++x) {
+    int ir[3] = {x, y, z};
+    bool ref = c.refidx[root_lin(c, ir)] >= 0;
+    int n = ref ? c.S : 1;
+    for (int sz = 0; sz < n; ++sz) for (int sy = 0; sy < n; ++sy) for (int sx = 0; sx < n; ++sx) {
+      int is[3] = {sx, sy, sz};
+      double lo[3], hi[3];
+      for (int a = 0; a < 3; ++a) {
+        lo[a] = ref ? ir[a] + is[a] * hs : ir[a];
+        hi[a] = lo[a] + (ref ? hs : 1.0);
+      }
+      double t0, t1;
+      if (!clip(lo, hi, t0, t1)) continue;
+      Seg s; s.t0 = t0; s.t1 = t1; s.slot = leaf_slot(c, ir, is, ref); s.refined = ref;
+      for (int a = 0; a < 3; ++a) { s.ir[a] = ir[a]; s.is[a] = is[a]; }
+      segs.push_back(s);
+    }
+  }
+  std::sort(segs.begin(), segs.end(), [](const Seg& a, const Seg& b) { return a.t0 < b.t0; });
+  double tau_acc = 0.0;
+  for (const Seg& s : segs) {
+    double alpha = c.rho[s.slot] * kx, ell = s.t1 - s.t0;
+    if (alpha > 0 && tau_acc + alpha * ell >= tau_star) {
+      double t = s.t0 + (tau_star - tau_acc) / alpha;
+      for (int a = 0; a < 3; ++a) { p.x[a] += p.d[a] * t; p.ir[a] = s.ir[a]; p.is[a] = s.is[a]; }
+      p.refined = s.refined;
+      *slot = s.slot;
+      return 1;
+    }
+    tau_acc += alpha * ell;
+    ++*crossings;
+  }
+  return 0;
+}
+
+// first j with cdf[j] >= u (R19: zero-probability bins are never selected)
+int search_cdf(const double* cdf, int n, double u) {
+  int lo = 0, hi = n - 1;
+  while (lo < hi) { int mid = (lo + hi) / 2; if (cdf[mid] >= u) hi = mid; else lo = mid + 1; }
+  return lo;
+}
+
+// O6 / R11: emission bin at temperature T from the table rows, stochastic row choice.
+int sample_emission_bin(const Ctx& c, double T, double u0, double u1) {
+  double t = (std::log(T) - std::log(c.Tmin)) / c.dlnT;
+  t = std::min((double)(c.nT - 1), std::max(0.0, t));
+  int k0 = (int)std::floor(t);
+  double w = t - k0;
+  int row = (u1 < w && k0 + 1 < c.nT) ? k0 + 1 : k0;
+  return search_cdf(&c.C[(size_t)row * c.nb], c.nb, u0);
+}
+
+// O7 / R12: invert Q(T) = q by bracketing + log-log interpolation; clamp.
+double temperature_from_q(const Ctx& c, double q) {
+  if (!(q > c.Q[0])) return c.Tmin;
+  if (q >= c.Q[c.nT - 1]) return c.Tmax;
+  int lo = 0, hi = c.nT - 1;                 // Q[lo] <= q < Q[hi]
+  while (hi - lo > 1) { int mid = (lo + hi) / 2; if (c.Q[mid] <= q) lo = mid; else hi = mid; }
+  double f = (std::log(q) - std::log(c.Q[lo])) / (std::log(c.Q[lo + 1]) - std::log(c.Q[lo]));
+  double lnT = std::log(c.Tmin) + c.dlnT * (lo + f);
+  return std::min(c.Tmax, std::max(c.Tmin, std::exp(lnT)));
+}
+
+// O4: emission of packet pid.  Returns false if the source lies outside the grid.
+bool emit(const Ctx& c, uint64_t seed, uint64_t pid, Packet& p) {
+  double u[4];
+  draw4(seed, pid, 0, TAG_EMIT, u);
+  int s = 0;
+  while (s < (int)c.src.size() - 1 && c.Lcdf[s] < u[0]) ++s;      // s = min{s: Lcdf_s >= u0}
+  p.bin = search_cdf(&c.Csrc[(size_t)s * c.nb], c.nb, u[1]);
+  p.comp = COMP_DIRECT;
+  if (c.src[s].type == 0) {
+    isotropic_dir(u[2], u[3], p.d);
+    for (int a = 0; a < 3; ++a) p.x[a] = c.src[s].pos[a];
+  } else {                                                         // R25 external field
+    double v[4];
+    draw4(seed, pid, 1, TAG_EMIT, v);
+    int f = std::min(5, (int)std::floor(6.0 * v[0]));
+    int ax = f / 2, side = f % 2, b1 = (ax + 1) % 3, b2 = (ax + 2) % 3;
+    double mu = std::sqrt(u[2]), phi = 2.0 * PI * u[3];
+    double st = std::sqrt(std::max(0.0, 1.0 - mu * mu));
+    p.d[ax] = side == 0 ? mu : -mu;
+    p.d[b1] = st * std::cos(phi);
+    p.d[b2] = st * std::sin(phi);
+    p.x[ax] = side == 0 ? 0.0 : (double)c.N;
+    p.x[b1] = v[1] * c.N;
+    p.x[b2] = v[2] * c.N;
+  }
+  return locate(c, p);
+}
+
+struct Event { int32_t type; int32_t bin; int64_t slot; double x[3]; };  // for traces
+
+// O4..O6: full life of one packet with temperatures frozen.  Tallies are integer atomics.
+void run_packet(Ctx& c, uint64_t seed, uint64_t pid, std::vector<uint64_t>& batch,
+                Event* trace, int trace_cap, int* trace_n) {
+  Packet p;
+  Counters loc{};
+  auto rec = [&](int type, int64_t slot) {
+    if (trace && *trace_n < trace_cap) {
+      Event& e = trace[(*trace_n)++];
+      e.type = type; e.bin = p.bin; e.slot = slot;
+      for (int a = 0; a < 3; ++a) e.x[a] = p.x[a];
+    }
+  };
+  bool ok = emit(c, seed, pid, p);
+  loc.emitted = 1;
+#pragma omp atomic
+  c.emitted_per_bin[p.bin] += 1;
+  rec(0, -1);
+  if (!ok) { loc.lost = 1; }
+  uint32_t k = 0;
+  while (ok) {
+    if (k >= K_MAX_FLIGHTS) { loc.lost = 1; break; }            // R20
+    double u[4];
+    draw4(seed, pid, k, TAG_FLIGHT, u);
+    double tau_star = -std::log(u[0]);                           // R17
+    loc.flights++;
+    int64_t slot = -1;
+    int hit = (c.walker == 0) ? walk_cells(c, p, tau_star, &slot, &loc.crossings)
+                              : walk_bruteforce(c, p, tau_star, &slot, &loc.crossings);
+    if (!hit) {                                                  // escape -> SED (R24)
+      loc.escaped = 1;
+#pragma omp atomic
+      c.sed[(size_t)p.comp * c.nb + p.bin] += 1;
+      rec(3, -1);
+      break;
+    }
+    if (u[1] < c.alb[p.bin]) {                                   // scatter (R16)
+      loc.scatterings++;
+      double ct = hg_cos(c.g[p.bin], u[2]);
+      double nd[3];
+      rotate_dir(p.d, ct, 2.0 * PI * u[3], nd);
+      p.d[0] = nd[0]; p.d[1] = nd[1]; p.d[2] = nd[2];
+      if (p.comp == COMP_DIRECT) p.comp = COMP_SCATTERED;
+      rec(1, slot);
+    } else {                                                     // absorb + re-emit
+      loc.absorptions++;
+#pragma omp atomic
+      batch[slot] += 1;
+      double r[4];
+      draw4(seed, pid, k, TAG_REEMIT, r);
+      p.bin = sample_emission_bin(c, c.T[slot], r[0], r[1]);     // T frozen = T before absorption
+      isotropic_dir(r[2], r[3], p.d);
+      p.comp = COMP_THERMAL;
+      rec(2, slot);
+    }
+    ++k;
+  }
+#pragma omp atomic
+  c.cnt.emitted += loc.emitted;
+#pragma omp atomic
+  c.cnt.escaped += loc.escaped;
+#pragma omp atomic
+  c.cnt.lost += loc.lost;
+#pragma omp atomic
+  c.cnt.absorptions += loc.absorptions;
+#pragma omp atomic
+  c.cnt.scatterings += loc.scatterings;
+#pragma omp atomic
+  c.cnt.flights += loc.flights;
+#pragma omp atomic
+  c.cnt.crossings += loc.crossings;
+}
+
+double leaf_mass(const Ctx& c, int64_t slot) {
+  double V = c.root_size * c.root_size * c.root_size;
+  if (slot >= (int64_t)c.N * c.N * c.N) V /= (double)(c.S * c.S * c.S);
+  return c.rho[slot] * V;
+}
+
+// O7: merge the batch tally and update every leaf temperature (R9 reading B, R10, R12).
+void batch_end(Ctx& c, const std::vector<uint64_t>& batch, uint64_t n_packets) {
+  for (int64_t i = 0; i < c.slots; ++i) c.cum[i] += batch[i];
+  c.Ncum += n_packets;
+  for (int64_t i = 0; i < c.slots; ++i) {
+    double m = leaf_mass(c, i);
+    if (m > 0 && c.cum[i] > 0) {
+      double q = (double)c.cum[i] * c.Ltot / ((double)c.Ncum * 4.0 * PI * m);
+      c.T[i] = temperature_from_q(c, q);
+    } else {
+      c.T[i] = c.Tmin;
+    }
+  }
+}
+
+}  // namespace
+
+// =======================================================================================
+// C interface for ctypes (tests, smoke, cpu_baseline only)
+// =======================================================================================
+extern "C" {
+
+void* orc_create(int n_root, int sub, const double* origin, double root_size,
+                 const uint8_t* refine, const float* rho_root, const float* rho_sub) {
+  if (n_root < 1 || root_size <= 0) return nullptr;
+  Ctx* c = new Ctx;
+  c->N = n_root; c->S = sub > 1 ? sub : 1; c->root_size = root_size;
+  for (int a = 0; a < 3; ++a) c->origin[a] = origin[a];
+  int64_t n3 = (int64_t)n_root * n_root * n_root;
+  c->refidx.assign(n3, -1);
+  int64_t k = 0;
+  if (refine && c->S > 1)
+    for (int64_t i = 0; i < n3; ++i) if (refine[i]) c->refidx[i] = (int32_t)k++;
+  c->n_ref = k;
+  if (k == 0) c->S = 1;
+  int64_t s3 = (int64_t)c->S * c->S * c->S;
+  c->slots = n3 + k * s3;
+  c->rho.assign(c->slots, 0.0);
+  for (int64_t i = 0; i < n3; ++i) c->rho[i] = c->refidx[i] >= 0 ? 0.0 : (double)rho_root[i];
+  for (int64_t i = 0; i < k * s3; ++i) c->rho[n3 + i] = (double)rho_sub[i];
+  c->cum.assign(c->slots, 0);
+  c->T.assign(c->slots, 1.0);
+  return c;
+}
+
+void orc_destroy(void* h) { delete (Ctx*)h; }
+int64_t orc_leaf_slots(void* h) { return ((Ctx*)h)->slots; }
+void orc_set_walker(void* h, int w) { ((Ctx*)h)->walker = w; }
+
+// O1 + O2 (R4, R5, R6, R11, R13, R33): tables in fp64 from the fp32 input opacities.
+int orc_set_opacity(void* h, int n_bins, const double* lambda_edges_um, int n_species,
+                    const double* weight, const float* kabs, const float* ksca, const float* g,
+                    double Tmin, double Tmax, int nT) {
+  Ctx& c = *(Ctx*)h;
+  if (n_bins < 1 || n_species < 1) return -1;
+  if (nT <= 0) { Tmin = 1.0; Tmax = 1.0e4; nT = 801; }
+  c.nb = n_bins; c.nT = nT; c.Tmin = Tmin; c.Tmax = Tmax;
+  c.dlnT = (std::log(Tmax) - std::log(Tmin)) / (nT - 1);
+  c.nu.resize(n_bins); c.dnu.resize(n_bins);
+  for (int j = 0; j < n_bins; ++j) {
+    double l0 = lambda_edges_um[j] * 1e-4, l1 = lambda_edges_um[j + 1] * 1e-4;   // cm
+    c.nu[j] = C_LIGHT / std::sqrt(l0 * l1);
+    c.dnu[j] = C_LIGHT / l0 - C_LIGHT / l1;
+  }
+  c.kabs.assign(n_bins, 0); c.ksca.assign(n_bins, 0); c.kext.assign(n_bins, 0);
+  c.alb.assign(n_bins, 0); c.g.assign(n_bins, 0);
+  for (int j = 0; j < n_bins; ++j) {
+    double gs = 0;
+    for (int s = 0; s < n_species; ++s) {
+      c.kabs[j] += weight[s] * (double)kabs[(size_t)s * n_bins + j];
+      c.ksca[j] += weight[s] * (double)ksca[(size_t)s * n_bins + j];
+      gs += weight[s] * (double)ksca[(size_t)s * n_bins + j] * (double)g[(size_t)s * n_bins + j];
+    }
+    c.kext[j] = c.kabs[j] + c.ksca[j];
+    c.alb[j] = c.kext[j] > 0 ? c.ksca[j] / c.kext[j] : 0.0;
+    c.g[j] = c.ksca[j] > 0 ? gs / c.ksca[j] : 0.0;
+  }
+  c.Q.assign(nT, 0); c.C.assign((size_t)nT * n_bins, 0);
+  for (int k = 0; k < nT; ++k) {
+    double T = Tmin * std::pow(Tmax / Tmin, (double)k / (nT - 1));
+    double acc = 0;
+    for (int j = 0; j < n_bins; ++j) {
+      acc += c.kabs[j] * planck_nu(c.nu[j], T) * c.dnu[j];
+      c.C[(size_t)k * n_bins + j] = acc;
+    }
+    c.Q[k] = acc;
+    for (int j = 0; j < n_bins; ++j)
+      c.C[(size_t)k * n_bins + j] = acc > 0 ? c.C[(size_t)k * n_bins + j] / acc : 1.0;
+    c.C[(size_t)k * n_bins + n_bins - 1] = 1.0;
+  }
+  c.sed.assign((size_t)3 * n_bins, 0);
+  c.emitted_per_bin.assign(n_bins, 0);
+  c.have_opacity = true;
+  return 0;
+}
+
+// O2 (sources): spectrum CDF by the same midpoint rule, luminosity CDF.  pos in cm.
+int orc_set_source(void* h, int n_src, const int* type, const double* pos, const double* L,
+                   const double* Tbb) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.have_opacity || n_src < 1) return -2;
+  c.src.resize(n_src); c.Lcdf.resize(n_src); c.Csrc.assign((size_t)n_src * c.nb, 0);
+  c.Ltot = 0;
+  for (int s = 0; s < n_src; ++s) c.Ltot += L[s];
+  double acc = 0;
+  for (int s = 0; s < n_src; ++s) {
+    c.src[s].type = type[s]; c.src[s].L = L[s]; c.src[s].Tbb = Tbb[s];
+    for (int a = 0; a < 3; ++a) c.src[s].pos[a] = (pos[3 * s + a] - c.origin[a]) / c.root_size;
+    acc += L[s]; c.Lcdf[s] = acc / c.Ltot;
+    double sum = 0;
+    for (int j = 0; j < c.nb; ++j) {
+      sum += planck_nu(c.nu[j], Tbb[s]) * c.dnu[j];
+      c.Csrc[(size_t)s * c.nb + j] = sum;
+    }
+    for (int j = 0; j < c.nb; ++j) c.Csrc[(size_t)s * c.nb + j] /= sum;
+    c.Csrc[(size_t)s * c.nb + c.nb - 1] = 1.0;
+  }
+  c.Lcdf[n_src - 1] = 1.0;
+  c.have_source = true;
+  return 0;
+}
+
+// O4..O7 for packets [first, first+n): transport with T frozen, then batch end.
+int orc_run_batch(void* h, uint64_t seed, uint64_t first, uint64_t n, int n_threads) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.have_source) return -2;
+  std::vector<uint64_t> batch(c.slots, 0);
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t i = 0; i < (int64_t)n; ++i)
+    run_packet(c, seed, first + (uint64_t)i, batch, nullptr, 0, nullptr);
+  batch_end(c, batch, n);
+  return 0;
+}
+
+int orc_max_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// Event trace of a single packet against the current (frozen) temperatures; tallies ARE
+// updated in a scratch copy only (the context is left untouched except counters/SED).
+int orc_trace_packet(void* h, uint64_t seed, uint64_t pid, int cap, int32_t* type,
+                     int32_t* bin, int64_t* slot, double* xyz) {
+  Ctx& c = *(Ctx*)h;
+  std::vector<uint64_t> batch(c.slots, 0);
+  std::vector<Event> ev(cap);
+  int n = 0;
+  Counters save = c.cnt;
+  std::vector<uint64_t> sed = c.sed, epb = c.emitted_per_bin;
+  run_packet(c, seed, pid, batch, ev.data(), cap, &n);
+  c.cnt = save; c.sed = sed; c.emitted_per_bin = epb;
+  for (int i = 0; i < n; ++i) {
+    type[i] = ev[i].type; bin[i] = ev[i].bin; slot[i] = ev[i].slot;
+    for (int a = 0; a < 3; ++a) xyz[3 * i + a] = ev[i].x[a];
+  }
+  return n;
+}
+
+// getters (O8)
+void orc_get_cell_energy(void* h, uint64_t* n_abs, double* eps) {
+  Ctx& c = *(Ctx*)h;
+  std::memcpy(n_abs, c.cum.data(), sizeof(uint64_t) * c.slots);
+  *eps = c.Ncum ? c.Ltot / (double)c.Ncum : 0.0;
+}
+void orc_get_cell_temperature(void* h, double* T) {
+  Ctx& c = *(Ctx*)h; std::memcpy(T, c.T.data(), sizeof(double) * c.slots);
+}
+void orc_set_cell_temperature(void* h, const double* T) {      // tests: fixed-T emission pins
+  Ctx& c = *(Ctx*)h; std::memcpy(c.T.data(), T, sizeof(double) * c.slots);
+}
+void orc_get_sed(void* h, uint64_t* out) {
+  Ctx& c = *(Ctx*)h; std::memcpy(out, c.sed.data(), sizeof(uint64_t) * 3 * c.nb);
+}
+void orc_get_counters(void* h, uint64_t* out7, uint64_t* emitted_per_bin) {
+  Ctx& c = *(Ctx*)h;
+  out7[0] = c.cnt.emitted; out7[1] = c.cnt.escaped; out7[2] = c.cnt.lost;
+  out7[3] = c.cnt.absorptions; out7[4] = c.cnt.scatterings; out7[5] = c.cnt.flights;
+  out7[6] = c.cnt.crossings;
+  if (emitted_per_bin) std::memcpy(emitted_per_bin, c.emitted_per_bin.data(), 8 * c.nb);
+}
+void orc_reset_tallies(void* h, int what) {
+  Ctx& c = *(Ctx*)h;
+  if (what & 1) { std::fill(c.sed.begin(), c.sed.end(), 0);
+                  std::fill(c.emitted_per_bin.begin(), c.emitted_per_bin.end(), 0); c.cnt = Counters{}; }
+  if (what & 2) { std::fill(c.cum.begin(), c.cum.end(), 0); std::fill(c.T.begin(), c.T.end(), c.Tmin);
+                  c.Ncum = 0; }
+}
+void orc_get_tables(void* h, double* nu, double* dnu, double* kabs, double* kext, double* alb,
+                    double* g, double* Q, double* C) {
+  Ctx& c = *(Ctx*)h;
+  auto cp = [](double* d, const std::vector<double>& v) { if (d) std::memcpy(d, v.data(), 8 * v.size()); };
+  cp(nu, c.nu); cp(dnu, c.dnu); cp(kabs, c.kabs); cp(kext, c.kext); cp(alb, c.alb); cp(g, c.g);
+  cp(Q, c.Q); cp(C, c.C);
+}
+void orc_get_source_cdf(void* h, double* Csrc, double* Lcdf) {
+  Ctx& c = *(Ctx*)h;
+  std::memcpy(Csrc, c.Csrc.data(), 8 * c.Csrc.size());
+  std::memcpy(Lcdf, c.Lcdf.data(), 8 * c.Lcdf.size());
+}
+
+// ---- component entry points for the pins ------------------------------------------------
+void orc_philox(const uint32_t* key2, const uint32_t* ctr4, uint32_t* out4) {
+  philox4x32_10(key2, ctr4, out4);
+}
+void orc_draw4(uint64_t seed, uint64_t pid, uint32_t k, uint32_t tag, double* u4) {
+  draw4(seed, pid, k, tag, u4);
+}
+void orc_isotropic(double u2, double u3, double* d) { isotropic_dir(u2, u3, d); }
+double orc_hg_cos(double g, double u) { return hg_cos(g, u); }
+void orc_rotate(const double* d, double ct, double phi, double* out) { rotate_dir(d, ct, phi, out); }
+double orc_planck(double nu, double T) { return planck_nu(nu, T); }
+int orc_sample_emission_bin(void* h, double T, double u0, double u1) {
+  return sample_emission_bin(*(Ctx*)h, T, u0, u1);
+}
+double orc_temperature_from_q(void* h, double q) { return temperature_from_q(*(Ctx*)h, q); }
+double orc_leaf_mass(void* h, int64_t slot) { return leaf_mass(*(Ctx*)h, slot); }
+
+// One emission (O4): position (root units), direction, bin, start leaf slot.
+int orc_emit(void* h, uint64_t seed, uint64_t pid, double* x, double* d, int* bin, int64_t* slot) {
+  Ctx& c = *(Ctx*)h;
+  Packet p;
+  bool ok = emit(c, seed, pid, p);
+  for (int a = 0; a < 3; ++a) { x[a] = p.x[a]; d[a] = p.d[a]; }
+  *bin = p.bin;
+  *slot = ok ? leaf_slot(c, p.ir, p.is, p.refined) : -1;
+  return ok ? 0 : -1;
+}
+
+// One flight (O5) from x (root units) along d in frequency bin `bin` with optical depth
+// tau_star, using walker w.  Returns 1 = interaction (slot, x_out), 0 = escaped, -1 = outside.
+int orc_walk(void* h, int w, const double* x, const double* d, int bin, double tau_star,
+             int64_t* slot, double* x_out, uint64_t* crossings) {
+  Ctx& c = *(Ctx*)h;
+  Packet p;
+  for (int a = 0; a < 3; ++a) { p.x[a] = x[a]; p.d[a] = d[a]; }
+  p.bin = bin; p.comp = 0;
+  if (!locate(c, p)) return -1;
+  *crossings = 0; *slot = -1;
+  int r = w == 0 ? walk_cells(c, p, tau_star, slot, crossings)
+                 : walk_bruteforce(c, p, tau_star, slot, crossings);
+  for (int a = 0; a < 3; ++a) x_out[a] = p.x[a];
+  return r;
+}
+
+}  // extern "C"
