@@ -1,0 +1,173 @@
+/* mcrt.h -- C ABI of the B200-native Monte Carlo dust radiative-transfer hot path.
+ *
+ * Method: Siebenmorgen, Heymann & Kruegel, "PAH in vectorized three dimensional Monte Carlo
+ * dust radiative transfer models", section 2:
+ *   PAPER.md L23   space partitioned into cubes, some divided into subcubes (cells); the star
+ *                  emits photon packages of constant energy eps at different frequencies; in
+ *                  each cell on its flight path a package may be absorbed or scattered with a
+ *                  probability given by the extinction optical depth along the path in the cell;
+ *                  scattering changes the direction by the phase function; absorption raises the
+ *                  cell energy by eps (and so its temperature) and a new package of the same
+ *                  energy is emitted isotropically from the spot at a new frequency.
+ *   PAPER.md L25-27  many packages are followed simultaneously; the new frequency is drawn at
+ *                  the cell temperature BEFORE absorption without the Bjorkman-Wood correction
+ *                  (Eqn 11.67 instead of 11.65 of Kruegel 2006): dP/dnu ~ kappa_nu B_nu(T).
+ * The call names are the ones BASELINE.json north_star fixes; everything below the names is this
+ * build's reading (readings R1..R33).
+ *
+ * General rules
+ *  - cgs units.  Wavelengths in micron.  Plain pointers and sizes only; no C++ types.
+ *  - Every call returns mcrt_status (0 = ok, < 0 = error) and never aborts or throws.  The text of
+ *    the last error of a context is available from mcrt_last_error().
+ *  - The caller owns every pointer it passes.  The library copies during the call and never keeps
+ *    a caller pointer.  Outputs are written into caller-allocated buffers.  A buffer tagged
+ *    MCRT_DEVICE is device memory on the current CUDA device (e.g. torch.Tensor.data_ptr()).
+ *  - The context owns the device memory it allocates; mcrt_destroy releases it.
+ *  - Call order: mcrt_grid_create -> mcrt_set_opacity -> mcrt_set_source -> mcrt_run_batch (any
+ *    number) -> getters.  A call out of order returns MCRT_ESTATE.
+ *  - All arithmetic of the method runs in CUDA kernels on an sm_100a device.  There is no CPU
+ *    fallback: without a usable device every call that needs one returns MCRT_ECUDA.
+ *  - Determinism: results depend only on (grid, opacity, sources, seed, the sequence of
+ *    (first_packet_id, n_packets) batches), never on thread scheduling: temperatures are frozen
+ *    within a batch, every packet owns the Philox4x32-10 stream keyed by (seed, packet id), and
+ *    all tallies are integers.
+ */
+#ifndef MCRT_H_
+#define MCRT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mcrt_ctx mcrt_ctx; /* opaque */
+
+typedef enum {
+  MCRT_OK = 0,
+  MCRT_EINVAL = -1, /* NULL pointer, bad size, source outside the grid, ... */
+  MCRT_ESTATE = -2, /* call out of order */
+  MCRT_ENOMEM = -3, /* host or device allocation failed */
+  MCRT_ECUDA = -4   /* CUDA runtime error or no usable device; see mcrt_last_error */
+} mcrt_status;
+
+typedef enum { MCRT_HOST = 0, MCRT_DEVICE = 1 } mcrt_mem;
+
+/* ---- grid ("cubes ... further divided into subcubes (cells)") ------------------
+ * Root grid of n_root^3 cubes, x fastest.  A cube flagged in `refine` is divided into sub^3
+ * subcubes.  Leaf slots (layout R22), used by every per-cell getter:
+ *   slot = ix + n_root*(iy + n_root*iz)                      for an unrefined cube,
+ *   slot = n_root^3 + sub^3*k + (sx + sub*(sy + sub*sz))     for a subcube of the k-th refined
+ *                                                            cube (k counts flagged cubes in
+ *                                                            x-fastest order);
+ * the slot of a refined root cube itself is unused (density 0, tally 0, T = T_min).
+ * Densities that are negative or NaN are taken as 0. */
+typedef struct {
+  int32_t n_root;        /* N >= 1; N^3 + n_ref*sub^3 must be < 2^31                          */
+  int32_t sub;           /* S: 0 or 1 = no refinement, else 2..8 subcubes per edge            */
+  double origin[3];      /* cm, low corner of the box                                         */
+  double root_size;      /* cm, edge of a root cube, > 0                                      */
+  const uint8_t* refine; /* [N^3] 1 = cube is subdivided; NULL = none                         */
+  const float* rho_root; /* [N^3] g cm^-3 of dust; ignored where refine = 1                   */
+  const float* rho_sub;  /* [n_ref*S^3]; NULL iff no cube is refined                          */
+  mcrt_mem mem;          /* where refine / rho_root / rho_sub live                            */
+} mcrt_grid_desc;
+
+/* Creates a context on the current CUDA device and uploads the grid. */
+mcrt_status mcrt_grid_create(const mcrt_grid_desc* desc, mcrt_ctx** out);
+mcrt_status mcrt_destroy(mcrt_ctx* ctx);
+/* Number of leaf slots = length of every per-cell array.  < 0 on a NULL context. */
+int64_t mcrt_leaf_slots(const mcrt_ctx* ctx);
+
+/* ---- opacity (cross-sections per dust component and abundances) -------------
+ * n_bins frequency bins given by n_bins+1 ascending wavelength edges (R4); bin centre = geometric
+ * mean of its edges; a packet's frequency is a bin index.  The species are mixed by mass weight
+ * into one grain with one temperature per cell (R13).  The library builds, in fp64 kernels and
+ * stored as fp32: mixed kappa_ext, albedo, g; Q(T_k) = sum_j kappa_abs,j B_j(T_k) dnu_j on
+ * T_k = T_min (T_max/T_min)^(k/(n_T-1)); and the emission inverse-CDF rows C_k[j] (midpoint rule,
+ * R5; PAPER.md L27 Eqn 11.67).  All pointers are HOST pointers (the tables are small). */
+typedef struct {
+  int32_t n_bins;                /* 1..4096                                                   */
+  const double* lambda_edges_um; /* [n_bins+1] ascending, > 0                                 */
+  int32_t n_species;             /* >= 1                                                      */
+  const double* weight;          /* [n_species] mass fractions                                */
+  const float* kabs;             /* [n_species][n_bins] cm^2 g^-1                             */
+  const float* ksca;             /* [n_species][n_bins] cm^2 g^-1                             */
+  const float* g;                /* [n_species][n_bins] <cos theta> of Henyey-Greenstein      */
+  double T_min, T_max;           /* K; temperature table range                                */
+  int32_t n_T;                   /* rows; 0 = defaults T_min 1 K, T_max 1e4 K, n_T 801 (R11)  */
+} mcrt_opacity_desc;
+mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* desc);
+
+/* ---- sources ("The star emits photon packages of constant energy") -------------
+ * type 0: isotropic point source at pos (must lie inside the box, else MCRT_EINVAL);
+ * type 1: external isotropic field entering through the six box faces (R25), pos ignored.
+ * Each source radiates a blackbody spectrum of temperature T_bb truncated to the band (R6) with
+ * in-band luminosity L.  A packet picks its source with probability L_s / sum L (R26).
+ * Replaces all sources.  Host pointer. */
+typedef struct {
+  int32_t type;
+  double pos[3]; /* cm */
+  double L;      /* erg s^-1, > 0 */
+  double T_bb;   /* K, > 0 */
+} mcrt_source;
+mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src);
+
+/* ---- the hot path -----------------------------------------------------------
+ * Transports packets first_packet_id .. first_packet_id + n_packets - 1 with the cell
+ * temperatures frozen (emission, free-flight optical depth tau* = -ln xi, cell walk through
+ * cubes/subcubes, scatter or absorb + re-emit at nu ~ kappa_nu B_nu(T_cell), escape into the SED),
+ * then adds the batch to the cumulative tallies and updates every cell temperature from
+ * radiative equilibrium: 4 pi rho_i V_i Q(T_i) = cum_i * L_tot / N_cum (R9).
+ * Asynchronous on `cuda_stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream;
+ * NULL = the legacy default stream); getters synchronise with it.  n_packets = 0 is allowed
+ * (only the temperature update runs). */
+mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first_packet_id,
+                           uint64_t n_packets, void* cuda_stream);
+
+/* ---- results ---------------------------------------------------------------------------------
+ * n_abs_out[leaf slots]: cumulative number of packages absorbed per leaf (exact integers; "cell
+ * energy" in units of eps, R23).  *eps_out (host pointer, may be NULL) = L_tot / N_cum in erg s^-1
+ * per package, so that the absorbed power of a cell is n_abs * eps. */
+mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps_out, mcrt_mem mem);
+/* T_out[leaf slots] in K; T_min for cells that absorbed nothing or hold no dust. */
+mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem);
+/* counts_out[3][n_bins]: escaped packages per bin; component 0 = direct (never interacted),
+ * 1 = scattered only, 2 = thermal (re-emitted at least once) (R24). */
+mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
+
+typedef struct {
+  uint64_t emitted, escaped, lost, absorptions, scatterings, flights, crossings;
+} mcrt_counters;
+/* Cumulative event counters (host struct) and, if not NULL, emitted packages per bin
+ * (host, [n_bins]).  `crossings` counts every exit of a packet from a leaf through a face,
+ * including the final exit from the box (R27).  `lost` counts packets dropped at the flight cap
+ * of 10^7 (R20) and must be 0. */
+mcrt_status mcrt_get_counters(mcrt_ctx* ctx, mcrt_counters* out, uint64_t* emitted_per_bin);
+/* what: bit 0 = SED + counters, bit 1 = cell energy + temperatures + N_cum. */
+mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what);
+
+/* ---- tuning and introspection (do not change results) ---------------------------------------
+ * Launch shape of the transport kernel: threads per block (multiple of 32, <= 1024) and resident
+ * blocks per SM; 0 keeps the default. */
+mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t blocks_per_sm);
+/* Device times in ms of the mcrt_run_batch calls made since the previous call of this function
+ * (oldest first, at most `cap`), split into the two kernels of a batch (transport, temperature
+ * update), from CUDA events recorded on each batch's stream.  Synchronises with those streams.
+ * *n_out (host) receives the number written.  Either array may be NULL. */
+mcrt_status mcrt_get_batch_times(mcrt_ctx* ctx, float* transport_ms, float* update_ms, int32_t cap,
+                                 int32_t* n_out);
+/* Copies the built tables (fp32, device -> host) for inspection: opac[n_bins][4] = (kappa_ext *
+ * root_size, albedo, g, kappa_abs), lnQ[n_T], cdf[n_T][n_bins].  Any pointer may be NULL. */
+mcrt_status mcrt_get_tables(mcrt_ctx* ctx, float* opac, float* lnQ, float* cdf);
+/* Number of kernels launched by this library since the context was created. */
+int64_t mcrt_kernel_launches(const mcrt_ctx* ctx);
+/* Raw Philox4x32-10 blocks computed on the device (test hook for the generator pin):
+ * out[4*i..4*i+3] = Philox(key = (key2[0], key2[1]), counter = ctr[4*i..4*i+3]).  Host pointers. */
+mcrt_status mcrt_philox_blocks(const uint32_t* key2, const uint32_t* ctr, uint32_t* out, int64_t n);
+const char* mcrt_last_error(const mcrt_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MCRT_H_ */

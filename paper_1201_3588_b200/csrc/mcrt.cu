@@ -1,0 +1,480 @@
+// mcrt.cu -- C-ABI boundary (include/mcrt.h) of the sm_100a Monte Carlo radiative-transfer path.
+// Host code here only validates arguments, owns device memory and launches kernels; every step
+// of the method (table build, emission, walk, interactions, tallies, temperature update) runs in
+// the kernels of transport.cuh / tables.cuh.  There is no CPU fallback.
+#include "mcrt.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "tables.cuh"
+#include "transport.cuh"
+
+using namespace mcrt;
+
+struct BatchEvents { cudaEvent_t e0, e1, e2; };
+
+struct mcrt_ctx {
+  int device = 0, sm_count = 0;
+  int N = 0, S = 1;
+  long long n3 = 0, n_ref = 0, slots = 0;
+  double origin[3] = {0, 0, 0}, root_size = 1;
+  float* d_rho = nullptr;
+  unsigned long long* d_tally = nullptr;
+  float* d_trow = nullptr;
+  // opacity
+  int nb = 0, nT = 0;
+  double Tmin = 1, Tmax = 1e4, dlnT = 0;
+  double *d_nu = nullptr, *d_dnu = nullptr, *d_kabs = nullptr;
+  float4* d_opac = nullptr;
+  float *d_lnQ = nullptr, *d_cdf = nullptr;
+  // sources
+  int nsrc = 0;
+  SrcDev* d_src = nullptr;
+  float* d_csrc = nullptr;
+  double Ltot = 0;
+  // tallies: [0] work-queue head, [1..CNT_N] counters, then sed[3*nb], emit_bin[nb]
+  unsigned long long* d_small = nullptr;
+  unsigned long long Ncum = 0;
+  cudaStream_t last_stream = nullptr;
+  std::vector<BatchEvents> pending, spare;
+  int threads = 256, blocks_per_sm = 4;
+  long long launches = 0;
+  bool have_opacity = false, have_source = false;
+  std::string err;
+};
+
+static std::string g_err;   // errors raised without a context
+
+static mcrt_status fail(mcrt_ctx* c, mcrt_status st, const std::string& msg) {
+  if (c) c->err = msg; else g_err = msg;
+  return st;
+}
+#define CU(call)                                                                          \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess)                                                                \
+      return fail(ctx, e_ == cudaErrorMemoryAllocation ? MCRT_ENOMEM : MCRT_ECUDA,        \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                    \
+  } while (0)
+
+static void free_opacity(mcrt_ctx* c) {
+  cudaFree(c->d_nu); cudaFree(c->d_dnu); cudaFree(c->d_kabs); cudaFree(c->d_opac);
+  cudaFree(c->d_lnQ); cudaFree(c->d_cdf); cudaFree(c->d_small);
+  c->d_nu = c->d_dnu = c->d_kabs = nullptr; c->d_opac = nullptr; c->d_lnQ = c->d_cdf = nullptr;
+  c->d_small = nullptr;
+}
+static void free_sources(mcrt_ctx* c) {
+  cudaFree(c->d_src); cudaFree(c->d_csrc);
+  c->d_src = nullptr; c->d_csrc = nullptr;
+}
+
+extern "C" {
+
+mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
+  mcrt_ctx* ctx = nullptr;
+  if (!d || !out) return fail(nullptr, MCRT_EINVAL, "mcrt_grid_create: NULL argument");
+  *out = nullptr;
+  if (d->n_root < 1 || d->n_root > 1290 || !(d->root_size > 0) || !d->rho_root)
+    return fail(nullptr, MCRT_EINVAL, "mcrt_grid_create: bad n_root / root_size / rho_root");
+  if (d->sub < 0 || d->sub > 8) return fail(nullptr, MCRT_EINVAL, "mcrt_grid_create: sub must be 0..8");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(nullptr, MCRT_ECUDA, "mcrt_grid_create: no CUDA device (there is no CPU fallback)");
+  ctx = new (std::nothrow) mcrt_ctx;
+  if (!ctx) return fail(nullptr, MCRT_ENOMEM, "mcrt_grid_create: host allocation failed");
+  struct Guard { mcrt_ctx* c; ~Guard() { if (c) mcrt_destroy(c); } } guard{ctx};
+  auto bail = [&](mcrt_status st) { g_err = ctx->err; return st; };
+#define CUG(call)                                                                         \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess)                                                                \
+      return bail(fail(ctx, e_ == cudaErrorMemoryAllocation ? MCRT_ENOMEM : MCRT_ECUDA,   \
+                       std::string(#call) + ": " + cudaGetErrorString(e_)));              \
+  } while (0)
+  CUG(cudaGetDevice(&ctx->device));
+  cudaDeviceProp prop;
+  CUG(cudaGetDeviceProperties(&prop, ctx->device));
+  if (prop.major < 10)
+    return bail(fail(ctx, MCRT_ECUDA, "mcrt_grid_create: device is not sm_100 class (built for sm_100a only)"));
+  ctx->sm_count = prop.multiProcessorCount;
+  ctx->N = d->n_root;
+  ctx->S = d->sub > 1 ? d->sub : 1;
+  ctx->root_size = d->root_size;
+  for (int a = 0; a < 3; ++a) ctx->origin[a] = d->origin[a];
+  const long long n3 = (long long)d->n_root * d->n_root * d->n_root;
+  ctx->n3 = n3;
+  // refined-cube numbering (k counts flagged cubes in x-fastest order)
+  std::vector<int> refidx;
+  long long k = 0;
+  if (d->refine && ctx->S > 1) {
+    std::vector<uint8_t> ref(n3);
+    if (d->mem == MCRT_DEVICE) CUG(cudaMemcpy(ref.data(), d->refine, n3, cudaMemcpyDeviceToHost));
+    else std::memcpy(ref.data(), d->refine, n3);
+    refidx.assign(n3, -1);
+    for (long long i = 0; i < n3; ++i) if (ref[i]) refidx[i] = (int)k++;
+  }
+  ctx->n_ref = k;
+  if (k == 0) ctx->S = 1;
+  const long long s3 = (long long)ctx->S * ctx->S * ctx->S;
+  ctx->slots = n3 + k * s3;
+  if (ctx->slots >= (1ll << 31)) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: more than 2^31-1 leaf slots"));
+  if (k > 0 && !d->rho_sub) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: rho_sub is NULL but cubes are refined"));
+  CUG(cudaMalloc(&ctx->d_rho, sizeof(float) * ctx->slots));
+  CUG(cudaMalloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->slots));
+  CUG(cudaMalloc(&ctx->d_trow, sizeof(float) * ctx->slots));
+  CUG(cudaMemset(ctx->d_tally, 0, sizeof(unsigned long long) * ctx->slots));
+  CUG(cudaMemset(ctx->d_trow, 0, sizeof(float) * ctx->slots));
+  // staging copies of caller data (freed before returning)
+  float *st_root = nullptr, *st_sub = nullptr;
+  int* d_refidx = nullptr;
+  const float *src_root = d->rho_root, *src_sub = d->rho_sub;
+  struct Tmp { float*& a; float*& b; int*& c; ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); } } tmp{st_root, st_sub, d_refidx};
+  if (d->mem == MCRT_HOST) {
+    CUG(cudaMalloc(&st_root, sizeof(float) * n3));
+    CUG(cudaMemcpy(st_root, d->rho_root, sizeof(float) * n3, cudaMemcpyHostToDevice));
+    src_root = st_root;
+    if (k > 0) {
+      CUG(cudaMalloc(&st_sub, sizeof(float) * k * s3));
+      CUG(cudaMemcpy(st_sub, d->rho_sub, sizeof(float) * k * s3, cudaMemcpyHostToDevice));
+      src_sub = st_sub;
+    }
+  }
+  if (k > 0) {
+    CUG(cudaMalloc(&d_refidx, sizeof(int) * n3));
+    CUG(cudaMemcpy(d_refidx, refidx.data(), sizeof(int) * n3, cudaMemcpyHostToDevice));
+  }
+  k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, (int)n3);
+  ctx->launches++;
+  if (k > 0) {
+    k_sanitize<<<(unsigned)((k * s3 + 255) / 256), 256>>>(src_sub, ctx->d_rho + n3, k * s3);
+    ctx->launches++;
+  }
+  CUG(cudaGetLastError());
+  CUG(cudaDeviceSynchronize());
+  guard.c = nullptr;
+  *out = ctx;
+  return MCRT_OK;
+#undef CUG
+}
+
+mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
+  if (!ctx) return MCRT_EINVAL;
+  if (ctx->last_stream || true) cudaDeviceSynchronize();
+  for (auto& b : ctx->pending) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
+  for (auto& b : ctx->spare) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
+  free_opacity(ctx);
+  free_sources(ctx);
+  cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
+  delete ctx;
+  return MCRT_OK;
+}
+
+int64_t mcrt_leaf_slots(const mcrt_ctx* ctx) { return ctx ? ctx->slots : -1; }
+
+mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!d || !d->lambda_edges_um || !d->weight || !d->kabs || !d->ksca || !d->g)
+    return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: NULL argument");
+  if (d->n_bins < 1 || d->n_bins > 4096 || d->n_species < 1)
+    return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: n_bins must be 1..4096, n_species >= 1");
+  for (int j = 0; j < d->n_bins; ++j)
+    if (!(d->lambda_edges_um[j] > 0) || !(d->lambda_edges_um[j + 1] > d->lambda_edges_um[j]))
+      return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: wavelength edges must be positive and ascending");
+  int nT = d->n_T;
+  double Tmin = d->T_min, Tmax = d->T_max;
+  if (nT == 0) { nT = 801; Tmin = 1.0; Tmax = 1.0e4; }
+  if (nT < 2 || nT > 8192 || !(Tmin > 0) || !(Tmax > Tmin))
+    return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: bad temperature table");
+  CU(cudaDeviceSynchronize());
+  free_opacity(ctx);
+  free_sources(ctx);
+  ctx->have_opacity = ctx->have_source = false;
+  const int nb = d->n_bins, ns = d->n_species;
+  ctx->nb = nb; ctx->nT = nT; ctx->Tmin = Tmin; ctx->Tmax = Tmax;
+  ctx->dlnT = (std::log(Tmax) - std::log(Tmin)) / (nT - 1);
+  double *d_edges = nullptr, *d_w = nullptr;
+  float *d_ka = nullptr, *d_ks = nullptr, *d_g = nullptr;
+  struct Tmp { double*& a; double*& b; float*& c; float*& d; float*& e;
+               ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); cudaFree(d); cudaFree(e); } } tmp{d_edges, d_w, d_ka, d_ks, d_g};
+  CU(cudaMalloc(&d_edges, 8 * (nb + 1))); CU(cudaMalloc(&d_w, 8 * ns));
+  CU(cudaMalloc(&d_ka, 4 * (size_t)ns * nb)); CU(cudaMalloc(&d_ks, 4 * (size_t)ns * nb));
+  CU(cudaMalloc(&d_g, 4 * (size_t)ns * nb));
+  CU(cudaMemcpy(d_edges, d->lambda_edges_um, 8 * (nb + 1), cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(d_w, d->weight, 8 * ns, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(d_ka, d->kabs, 4 * (size_t)ns * nb, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(d_ks, d->ksca, 4 * (size_t)ns * nb, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(d_g, d->g, 4 * (size_t)ns * nb, cudaMemcpyHostToDevice));
+  CU(cudaMalloc(&ctx->d_nu, 8 * nb)); CU(cudaMalloc(&ctx->d_dnu, 8 * nb)); CU(cudaMalloc(&ctx->d_kabs, 8 * nb));
+  CU(cudaMalloc(&ctx->d_opac, sizeof(float4) * nb));
+  CU(cudaMalloc(&ctx->d_lnQ, 4 * nT));
+  CU(cudaMalloc(&ctx->d_cdf, 4 * (size_t)nT * nb));
+  const size_t n_small = 1 + CNT_N + 4 * (size_t)nb;
+  CU(cudaMalloc(&ctx->d_small, 8 * n_small));
+  CU(cudaMemset(ctx->d_small, 0, 8 * n_small));
+  k_mix_opacity<<<(nb + 127) / 128, 128>>>(nb, ns, d_edges, d_w, d_ka, d_ks, d_g, ctx->root_size,
+                                           ctx->d_nu, ctx->d_dnu, ctx->d_kabs, ctx->d_opac);
+  k_build_emission_rows<<<nT, 128, 8 * (nb + 1)>>>(nb, nT, Tmin, Tmax, ctx->d_nu, ctx->d_dnu,
+                                                   ctx->d_kabs, ctx->d_lnQ, ctx->d_cdf);
+  ctx->launches += 2;
+  CU(cudaGetLastError());
+  CU(cudaDeviceSynchronize());
+  ctx->have_opacity = true;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_set_source: call mcrt_set_opacity first");
+  if (n_src < 1 || n_src > 65536 || !src) return fail(ctx, MCRT_EINVAL, "mcrt_set_source: bad n_src / NULL");
+  std::vector<SrcDev> h(n_src);
+  std::vector<double> Tbb(n_src);
+  double Ltot = 0;
+  for (int s = 0; s < n_src; ++s) {
+    if (!(src[s].L > 0) || !(src[s].T_bb > 0) || (src[s].type != 0 && src[s].type != 1))
+      return fail(ctx, MCRT_EINVAL, "mcrt_set_source: L and T_bb must be > 0, type 0 or 1");
+    Ltot += src[s].L;
+  }
+  double acc = 0;
+  const int Sf = ctx->S;
+  for (int s = 0; s < n_src; ++s) {
+    h[s].type = src[s].type;
+    Tbb[s] = src[s].T_bb;
+    acc += src[s].L;
+    h[s].lcdf = s == n_src - 1 ? 1.f : (float)(acc / Ltot);
+    for (int a = 0; a < 3; ++a) { h[s].fine[a] = 0; h[s].frac[a] = 0.f; }
+    if (src[s].type == 0) {
+      for (int a = 0; a < 3; ++a) {
+        double xf = (src[s].pos[a] - ctx->origin[a]) / ctx->root_size * Sf;   // finest-level units
+        if (!(xf > 0.0) || !(xf < (double)ctx->N * Sf))
+          return fail(ctx, MCRT_EINVAL, "mcrt_set_source: point source outside the grid");
+        double fl = std::floor(xf);
+        float fr = (float)(xf - fl);
+        if (fr >= 1.f) { fl += 1.0; fr = 0.f; }
+        h[s].fine[a] = (int)fl;
+        h[s].frac[a] = fr;
+      }
+    }
+  }
+  CU(cudaDeviceSynchronize());
+  free_sources(ctx);
+  ctx->have_source = false;
+  double* d_T = nullptr;
+  struct Tmp { double*& a; ~Tmp() { cudaFree(a); } } tmp{d_T};
+  CU(cudaMalloc(&d_T, 8 * n_src));
+  CU(cudaMemcpy(d_T, Tbb.data(), 8 * n_src, cudaMemcpyHostToDevice));
+  CU(cudaMalloc(&ctx->d_src, sizeof(SrcDev) * n_src));
+  CU(cudaMemcpy(ctx->d_src, h.data(), sizeof(SrcDev) * n_src, cudaMemcpyHostToDevice));
+  CU(cudaMalloc(&ctx->d_csrc, 4 * (size_t)n_src * ctx->nb));
+  k_build_source_cdf<<<n_src, 128, 8 * (ctx->nb + 1)>>>(ctx->nb, d_T, ctx->d_nu, ctx->d_dnu, ctx->d_csrc);
+  ctx->launches++;
+  CU(cudaGetLastError());
+  CU(cudaDeviceSynchronize());
+  ctx->nsrc = n_src;
+  ctx->Ltot = Ltot;
+  ctx->have_source = true;
+  return MCRT_OK;
+}
+
+static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
+  if (!ctx->spare.empty()) { *b = ctx->spare.back(); ctx->spare.pop_back(); return MCRT_OK; }
+  CU(cudaEventCreate(&b->e0)); CU(cudaEventCreate(&b->e1)); CU(cudaEventCreate(&b->e2));
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, void* stream_) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_run_batch: grid, opacity and sources must be set first");
+  cudaStream_t st = (cudaStream_t)stream_;
+  if (ctx->pending.size() >= 4096) {                         // nobody is reading the timings: recycle
+    CU(cudaEventSynchronize(ctx->pending.back().e2));
+    for (auto& b : ctx->pending) ctx->spare.push_back(b);
+    ctx->pending.clear();
+  }
+  BatchEvents ev;
+  mcrt_status rc = take_events(ctx, &ev);
+  if (rc != MCRT_OK) return rc;
+  const int nb = ctx->nb;
+  TransportParams P;
+  P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.trow = ctx->d_trow;
+  P.opac = ctx->d_opac; P.cdf = ctx->d_cdf; P.csrc = ctx->d_csrc; P.src = ctx->d_src;
+  P.next = ctx->d_small; P.counters = ctx->d_small + 1;
+  P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
+  P.seed = seed; P.first = first; P.count = n;
+  P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->n3;
+  CU(cudaEventRecord(ev.e0, st));
+  if (n > 0) {
+    CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
+    const int threads = ctx->threads;
+    long long want = ((long long)n + threads - 1) / threads;
+    long long grid = (long long)ctx->sm_count * ctx->blocks_per_sm;
+    if (want < grid) grid = want;
+    size_t smem = sizeof(float4) * nb + 4 * (size_t)nb * 4;
+    if (ctx->S > 1) k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
+    else k_transport<false><<<(unsigned)grid, threads, smem, st>>>(P);
+    ctx->launches++;
+    CU(cudaGetLastError());
+  }
+  CU(cudaEventRecord(ev.e1, st));
+  ctx->Ncum += n;
+  if (ctx->Ncum > 0) {
+    const double PI = 3.14159265358979323846;
+    double V = ctx->root_size * ctx->root_size * ctx->root_size;
+    float ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)ctx->Ncum) - std::log(4.0 * PI) - std::log(V));
+    float ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
+    long long blocks = (ctx->slots + 255) / 256;
+    long long cap = (long long)ctx->sm_count * 8;
+    if (blocks > cap) blocks = cap;
+    k_update_temperature<<<(unsigned)blocks, 256, 4 * ctx->nT, st>>>(ctx->d_rho, ctx->d_tally, ctx->d_trow, ctx->d_lnQ,
+                                                                    ctx->nT, ctx->slots, ctx->n3, ln_coef, ln_sub3);
+    ctx->launches++;
+    CU(cudaGetLastError());
+  }
+  CU(cudaEventRecord(ev.e2, st));
+  ctx->pending.push_back(ev);
+  ctx->last_stream = st;
+  return MCRT_OK;
+}
+
+static mcrt_status sync_last(mcrt_ctx* ctx) {
+  CU(cudaStreamSynchronize(ctx->last_stream));
+  return MCRT_OK;
+}
+
+static mcrt_status copy_out(mcrt_ctx* ctx, void* dst, const void* src, size_t bytes, mcrt_mem mem) {
+  CU(cudaMemcpyAsync(dst, src, bytes, mem == MCRT_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                     ctx->last_stream));
+  CU(cudaStreamSynchronize(ctx->last_stream));
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps_out, mcrt_mem mem) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!n_abs_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_energy: NULL output");
+  if (eps_out) *eps_out = ctx->Ncum ? ctx->Ltot / (double)ctx->Ncum : 0.0;
+  return copy_out(ctx, n_abs_out, ctx->d_tally, 8 * (size_t)ctx->slots, mem);
+}
+
+mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!T_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_temperature: NULL output");
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_cell_temperature: opacity not set");
+  float* d_T = T_out;
+  float* tmp = nullptr;
+  struct Tmp { float*& a; ~Tmp() { cudaFree(a); } } guard{tmp};
+  if (mem == MCRT_HOST) { CU(cudaMalloc(&tmp, 4 * (size_t)ctx->slots)); d_T = tmp; }
+  k_trow_to_T<<<(unsigned)((ctx->slots + 255) / 256), 256, 0, ctx->last_stream>>>(
+      ctx->d_trow, d_T, ctx->slots, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
+  ctx->launches++;
+  CU(cudaGetLastError());
+  if (mem == MCRT_HOST) return copy_out(ctx, T_out, tmp, 4 * (size_t)ctx->slots, MCRT_HOST);
+  return sync_last(ctx);
+}
+
+mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!counts_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_sed: NULL output");
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_sed: opacity not set");
+  return copy_out(ctx, counts_out, ctx->d_small + 1 + CNT_N, 8 * 3 * (size_t)ctx->nb, mem);
+}
+
+mcrt_status mcrt_get_counters(mcrt_ctx* ctx, mcrt_counters* out, uint64_t* emitted_per_bin) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!out) return fail(ctx, MCRT_EINVAL, "mcrt_get_counters: NULL output");
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_counters: opacity not set");
+  unsigned long long h[CNT_N];
+  mcrt_status rc = copy_out(ctx, h, ctx->d_small + 1, 8 * CNT_N, MCRT_HOST);
+  if (rc != MCRT_OK) return rc;
+  out->emitted = h[CNT_EMITTED]; out->escaped = h[CNT_ESCAPED]; out->lost = h[CNT_LOST];
+  out->absorptions = h[CNT_ABS]; out->scatterings = h[CNT_SCA]; out->flights = h[CNT_FLIGHTS];
+  out->crossings = h[CNT_CROSS];
+  if (emitted_per_bin)
+    return copy_out(ctx, emitted_per_bin, ctx->d_small + 1 + CNT_N + 3 * (size_t)ctx->nb, 8 * (size_t)ctx->nb, MCRT_HOST);
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what) {
+  if (!ctx) return MCRT_EINVAL;
+  CU(cudaStreamSynchronize(ctx->last_stream));
+  if ((what & 1) && ctx->d_small) CU(cudaMemset(ctx->d_small, 0, 8 * (1 + CNT_N + 4 * (size_t)ctx->nb)));
+  if (what & 2) {
+    CU(cudaMemset(ctx->d_tally, 0, 8 * (size_t)ctx->slots));
+    CU(cudaMemset(ctx->d_trow, 0, 4 * (size_t)ctx->slots));
+    ctx->Ncum = 0;
+  }
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads, int32_t blocks_per_sm) {
+  if (!ctx) return MCRT_EINVAL;
+  if (threads < 0 || threads > 256 || (threads % 32) != 0 || blocks_per_sm < 0 || blocks_per_sm > 32)
+    return fail(ctx, MCRT_EINVAL, "mcrt_set_launch: threads must be a multiple of 32 up to 256, blocks_per_sm <= 32");
+  if (threads) ctx->threads = threads;
+  if (blocks_per_sm) ctx->blocks_per_sm = blocks_per_sm;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_get_batch_times(mcrt_ctx* ctx, float* transport_ms, float* update_ms, int32_t cap, int32_t* n_out) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!n_out || cap < 0) return fail(ctx, MCRT_EINVAL, "mcrt_get_batch_times: bad arguments");
+  int n = 0;
+  for (auto& b : ctx->pending) {
+    CU(cudaEventSynchronize(b.e2));
+    if (n < cap) {
+      float a = 0, c = 0;
+      CU(cudaEventElapsedTime(&a, b.e0, b.e1));
+      CU(cudaEventElapsedTime(&c, b.e1, b.e2));
+      if (transport_ms) transport_ms[n] = a;
+      if (update_ms) update_ms[n] = c;
+      ++n;
+    }
+    ctx->spare.push_back(b);
+  }
+  ctx->pending.clear();
+  *n_out = n;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_get_tables(mcrt_ctx* ctx, float* opac, float* lnQ, float* cdf) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_tables: opacity not set");
+  if (opac) CU(cudaMemcpy(opac, ctx->d_opac, 16 * (size_t)ctx->nb, cudaMemcpyDeviceToHost));
+  if (lnQ) CU(cudaMemcpy(lnQ, ctx->d_lnQ, 4 * (size_t)ctx->nT, cudaMemcpyDeviceToHost));
+  if (cdf) CU(cudaMemcpy(cdf, ctx->d_cdf, 4 * (size_t)ctx->nT * ctx->nb, cudaMemcpyDeviceToHost));
+  return MCRT_OK;
+}
+
+int64_t mcrt_kernel_launches(const mcrt_ctx* ctx) { return ctx ? ctx->launches : -1; }
+
+__global__ void k_philox_blocks(uint32_t k0, uint32_t k1, const uint32_t* __restrict__ ctr,
+                                uint32_t* __restrict__ out, long long n) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint32_t x[4];
+  philox4x32_10(k0, k1, ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], x);
+  out[4 * i] = x[0]; out[4 * i + 1] = x[1]; out[4 * i + 2] = x[2]; out[4 * i + 3] = x[3];
+}
+
+mcrt_status mcrt_philox_blocks(const uint32_t* key2, const uint32_t* ctr, uint32_t* out, int64_t n) {
+  mcrt_ctx* ctx = nullptr;
+  if (!key2 || !ctr || !out || n < 0) return fail(nullptr, MCRT_EINVAL, "mcrt_philox_blocks: bad arguments");
+  if (n == 0) return MCRT_OK;
+  uint32_t *d_c = nullptr, *d_o = nullptr;
+  struct Tmp { uint32_t*& a; uint32_t*& b; ~Tmp() { cudaFree(a); cudaFree(b); } } tmp{d_c, d_o};
+  CU(cudaMalloc(&d_c, 16 * (size_t)n)); CU(cudaMalloc(&d_o, 16 * (size_t)n));
+  CU(cudaMemcpy(d_c, ctr, 16 * (size_t)n, cudaMemcpyHostToDevice));
+  k_philox_blocks<<<(unsigned)((n + 255) / 256), 256>>>(key2[0], key2[1], d_c, d_o, n);
+  CU(cudaGetLastError());
+  CU(cudaMemcpy(out, d_o, 16 * (size_t)n, cudaMemcpyDeviceToHost));
+  return MCRT_OK;
+}
+
+const char* mcrt_last_error(const mcrt_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
+
+}  // extern "C"
