@@ -1,0 +1,409 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the Monte Carlo transport hot path (BASELINE.json metric:
+photon packets/s and cell-crossings/s on B200; fraction of the gather-bandwidth roofline).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c1_tau1] [--impl reference]
+
+A step = one mcrt_run_batch (transport of one batch with frozen temperatures + tally merge +
+temperature update) of the workload's batch size.  Prints ONE JSON line (rank 0).
+DESIGN.md section 8 states every figure's definition.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1201_3588_b200 import workloads as W  # noqa: E402
+
+METRIC = "photon packets/sec"
+UNIT = "packets/s"
+
+
+def make_workload(name: str):
+    """Bench workloads.  c1_tau1 = BASELINE.json configs[1] at tau_V = 1 (the configuration the
+    10^8 packets/s target is quoted on)."""
+    if name.startswith("c1_tau"):
+        return W.c1(tau_v=float(name[6:]))
+    if name == "c0":
+        return W.c0()
+    if name == "c2":
+        return W.c2()
+    if name == "c3":
+        return W.c3()
+    if name == "c4":
+        return W.c4()
+    if name == "c4_256":
+        return W.c4(n_root=256, batch=1 << 22)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def describe(wl, name):
+    return {"workload": name, "grid": f"{wl.n_root}^3" + (f"+{wl.n_ref}x{wl.sub}^3" if wl.n_ref else ""),
+            "leaf_slots": wl.leaf_slots, "n_bins": wl.n_bins, "batch_packets": wl.batch,
+            "n_sources": len(wl.sources), "seed": wl.seed}
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks (profiling recipe: sample nvidia-smi DURING the timed region)
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            if len(r) < 6:
+                continue
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for name, v in zip(self.NAMES, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ---------------------------------------------------------------------------------------------
+def oracle_rate(wl, target_seconds=15.0, n_batches=4):
+    """Time the oracle, as it stands, on a bounded sample of the workload: packets
+    0..n-1 in n_batches equal batches (temperatures update in between, as in the method)."""
+    from oracle import oracle as O
+    O.build()
+    cores = O.max_threads()
+    orc = O.Oracle(wl)
+    probe = 4096
+    t0 = time.perf_counter()
+    orc.run_batch(wl.seed, 0, probe)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    n = int(min(max(probe * target_seconds / dt, 4 * probe), wl.n_packets))
+    per = max(n // n_batches, 1)
+    orc = O.Oracle(wl)
+    t0 = time.perf_counter()
+    done = 0
+    for b in range(n_batches):
+        orc.run_batch(wl.seed, done, per)
+        done += per
+    dt = time.perf_counter() - t0
+    c = orc.counters()
+    return {"value": done / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"packets 0..{done - 1} in {n_batches} batches of {per} "
+                      f"({dt:.1f} s wall, OpenMP over packets)",
+            "crossings_per_s": c["crossings"] / dt}
+
+
+def run_reference(args, wl, name):
+    """--impl reference: the fp64 oracle on the host cores; a step = a bounded sample batch."""
+    from oracle import oracle as O
+    O.build()
+    cores = O.max_threads()
+    orc = O.Oracle(wl)
+    t0 = time.perf_counter()
+    orc.run_batch(wl.seed, 0, 2048)
+    rate = 2048 / max(time.perf_counter() - t0, 1e-4)
+    budget = 120.0 / max(args.steps + args.warmup, 1)
+    per = int(min(max(rate * min(budget, 10.0), 1024), wl.batch))
+    orc = O.Oracle(wl)
+    first = 0
+    for _ in range(args.warmup):
+        orc.run_batch(wl.seed, first, per)
+        first += per
+    c0 = orc.counters()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.run_batch(wl.seed, first, per)
+        first += per
+    dt = time.perf_counter() - t0
+    c1 = orc.counters()
+    value = args.steps * per / dt
+    sample = f"{args.steps} steps of {per} packets (bounded sample of the {wl.batch}-packet batch)"
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+           "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": describe(wl, name),
+           "crossings_per_s": (c1["crossings"] - c0["crossings"]) / dt,
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                            "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0,
+                   "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+# ---------------------------------------------------------------------------------------------
+# GPU arm
+# ---------------------------------------------------------------------------------------------
+def algorithmic_bytes(wl, d_cross, d_abs):
+    """SURVEY.md 8(d) / DESIGN.md section 7: 4 B per crossing (density gather; the refined-cube
+    marker shares that array, the descent into a refined cube costs a second 4-B gather which
+    is counted as a crossing of 8 B only on two-level grids), per absorption 4 B temperature
+    gather + 8 B tally read-modify-write + ceil(log2 n_bins) * 4 B of CDF probes."""
+    per_cross = 8 if wl.n_ref else 4
+    per_abs = 4 + 8 + 4 * int(np.ceil(np.log2(wl.n_bins)))
+    return d_cross * per_cross + d_abs * per_abs, per_cross, per_abs
+
+
+def run_gpu(args, wl, name):
+    import torch
+    import torch.distributed as dist
+    from paper_1201_3588_b200 import build as B, mcrt
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; "
+                         "use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        B.build_library()
+    if world > 1:
+        dist.barrier()
+    mcrt.lib()
+
+    batch = wl.batch
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx = mcrt.from_workload(wl)
+    if args.threads or args.blocks_per_sm:
+        ctx.set_launch(args.threads, args.blocks_per_sm)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    step_no = [0]
+
+    def one_step():
+        """One batch of `batch` packets per rank: global packet ids are dealt to the ranks in
+        contiguous ranges; N > 1 sums the integer tallies over ranks before the T update."""
+        first = (step_no[0] * world + rank) * batch
+        step_no[0] += 1
+        if world == 1:
+            ctx.run_batch(wl.seed, first, batch, stream)
+        else:
+            ctx.transport_batch(wl.seed, first, batch, stream)
+            tally, _ = ctx.get_cell_energy(device=True)
+            dist.all_reduce(tally, op=dist.ReduceOp.SUM)
+            ctx.update_temperature(tally, step_no[0] * world * batch, stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        one_step()
+    barrier()
+    ctx.get_batch_times()
+    c_before = ctx.get_counters()
+    launches_before = ctx.kernel_launches()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    barrier()
+    t_wall = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)                      # L2 flush between timed iterations (not timed)
+        a.record()
+        one_step()
+        b.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop() if rank == 0 else None
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    t_tr, t_up = ctx.get_batch_times()
+    c_after = ctx.get_counters()
+    launches = ctx.kernel_launches() - launches_before
+    d = {k: c_after[k] - c_before[k] for k in ("emitted", "escaped", "absorptions",
+                                                "scatterings", "flights", "crossings", "lost")}
+    stats = torch.tensor([total_ms, float(t_tr.sum()), float(t_up.sum())], dtype=torch.float64,
+                         device="cuda")
+    sums = torch.tensor([d["emitted"], d["crossings"], d["absorptions"], d["scatterings"],
+                         d["lost"], launches], dtype=torch.int64, device="cuda")
+    if world > 1:
+        dist.all_reduce(stats, op=dist.ReduceOp.MAX)
+        dist.all_reduce(sums, op=dist.ReduceOp.SUM)
+    total_ms, tr_ms, up_ms = [float(v) for v in stats.cpu()]
+    n_emit, n_cross, n_abs, n_sca, n_lost, launches = [int(v) for v in sums.cpu()]
+
+    # ---- e2e: a whole user job from HOST buffers to HOST results -------
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(args, wl, mcrt, torch, dist, rank, world, stream)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    secs = total_ms * 1e-3
+    peak, peak_src = measured_peaks()
+    # dominant kernel = k_transport; per-launch figures from this rank's batches
+    bytes_alg, per_cross, per_abs = algorithmic_bytes(wl, d["crossings"], d["absorptions"])
+    tr_s = float(t_tr.sum()) * 1e-3
+    achieved = bytes_alg / tr_s / 1e9 if tr_s > 0 else 0.0
+    out = {"metric": METRIC, "value": n_emit / secs, "unit": UNIT, "n_gpus": world,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+           "data": "synthetic",
+           "config": dict(describe(wl, name), l2="flushed between timed steps (256 MiB write)",
+                          parallelism=f"packet-sharded x{world}",
+                          launch=f"{ctx_launch_desc(args)}"),
+           "crossings_per_s": n_cross / secs,
+           "per_packet": {"crossings": n_cross / max(n_emit, 1), "absorptions": n_abs / max(n_emit, 1),
+                          "scatterings": n_sca / max(n_emit, 1)},
+           "lost": n_lost,
+           "kernel_ms_per_step": {"transport": tr_ms / args.steps, "temperature_update": up_ms / args.steps},
+           "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
+           "roofline": {"bound": "hbm", "kernel": "k_transport", "achieved": achieved, "peak": peak,
+                        "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                        "peak_source": peak_src,
+                        "algorithmic_bytes": {"per_crossing": per_cross, "per_absorption": per_abs,
+                                              "per_launch": bytes_alg / args.steps},
+                        "kernel_ms": 1e3 * tr_s / args.steps,
+                        "kernel_share_of_step": tr_s / (float(sum(step_ms)) * 1e-3)},
+           "gpu_launches": launches, "clocks": clocks}
+    if e2e is not None:
+        out["e2e"] = e2e
+    if not args.no_cpu and world >= 1:
+        cb = oracle_rate(wl, target_seconds=args.cpu_seconds)
+        out["cpu_baseline"] = cb
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def ctx_launch_desc(args):
+    return f"threads={args.threads or 'default'} blocks_per_sm={args.blocks_per_sm or 'default'}"
+
+
+def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
+    """End to end through the public API with HOST buffers: every step re-creates nothing, but
+    the job starts from host arrays (grid_create/set_opacity/set_source copy them H2D inside the
+    timed region) and every step ends with a device->host read of that step's results (SED,
+    counters, cell energies, cell temperatures).  Value = packets of all steps / wall time,
+    device-synchronised, max over ranks."""
+    batch = wl.batch
+    rho = torch.from_numpy(np.ascontiguousarray(wl.rho_root)).pin_memory().numpy()
+    steps = args.warmup + args.steps
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    ctx = mcrt.Context()
+    ctx.grid_create(wl.n_root, wl.sub, wl.origin, wl.root_size, wl.refine, rho, wl.rho_sub)
+    ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g)
+    ctx.set_source(wl.sources)
+    d2h = 0
+    for s in range(steps):
+        first = (s * world + rank) * batch
+        if world == 1:
+            ctx.run_batch(wl.seed, first, batch, stream)
+        else:
+            ctx.transport_batch(wl.seed, first, batch, stream)
+            tally, _ = ctx.get_cell_energy(device=True)
+            dist.all_reduce(tally, op=dist.ReduceOp.SUM)
+            ctx.update_temperature(tally, (s + 1) * world * batch, stream)
+        sed = ctx.get_sed()
+        n_abs, _ = ctx.get_cell_energy()
+        T = ctx.get_cell_temperature()
+        c = ctx.get_counters()
+        d2h = sed.nbytes + n_abs.nbytes + T.nbytes + 7 * 8 + c["emitted_per_bin"].nbytes
+    torch.cuda.synchronize()
+    dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+    dt = float(dt.cpu())
+    h2d_job = wl.rho_root.nbytes + (0 if wl.rho_sub is None else wl.rho_sub.nbytes) \
+        + (0 if wl.refine is None else wl.refine.nbytes + 4 * wl.refine.size) \
+        + wl.kabs.nbytes * 3 + wl.lambda_edges_um.nbytes
+    ctx.destroy()
+    return {"value": steps * batch * world / dt, "unit": UNIT,
+            "h2d_bytes_per_step": h2d_job / steps, "d2h_bytes_per_step": d2h,
+            "what": f"one job of {steps} batches from host arrays: grid/opacity/source set-up "
+                    "(H2D) + run_batch + host read-back of SED, counters, cell energy and "
+                    "temperature after every batch; wall clock, device-synchronised"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--workload", default="c1_tau1")
+    ap.add_argument("--threads", type=int, default=0)
+    ap.add_argument("--blocks-per-sm", type=int, default=0)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "native" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        run_reference(args, make_workload(args.workload), args.workload)
+        return
+    run_gpu(args, make_workload(args.workload), args.workload)
+
+
+if __name__ == "__main__":
+    main()

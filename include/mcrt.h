@@ -125,6 +125,21 @@ mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src
 mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first_packet_id,
                            uint64_t n_packets, void* cuda_stream);
 
+/* ---- the same batch in two halves, for packet-sharded multi-GPU runs ("scales
+ * almost linearly with the number of graphical processing units") -----------------------------
+ * Within a batch packages are independent (frozen temperatures, per-packet Philox streams), so
+ * rank r of G transports its own range of packet ids with mcrt_transport_batch (rows a1..a8: no
+ * temperature update), the ranks sum their cumulative integer tallies (one all-reduce of
+ * mcrt_get_cell_energy(MCRT_DEVICE) arrays, done by the caller, e.g. NCCL through
+ * torch.distributed), and every rank calls mcrt_update_temperature with the summed tally
+ * (DEVICE pointer, [leaf slots]) and the number of packages emitted so far by ALL ranks (row a9).
+ * tally_sum = NULL uses the context's own tally and count, which makes
+ * transport_batch + update_temperature(NULL) identical to mcrt_run_batch. */
+mcrt_status mcrt_transport_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first_packet_id,
+                                 uint64_t n_packets, void* cuda_stream);
+mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, uint64_t n_cum,
+                                    void* cuda_stream);
+
 /* ---- results ---------------------------------------------------------------------------------
  * n_abs_out[leaf slots]: cumulative number of packages absorbed per leaf (exact integers; "cell
  * energy" in units of eps, R23).  *eps_out (host pointer, may be NULL) = L_tot / N_cum in erg s^-1

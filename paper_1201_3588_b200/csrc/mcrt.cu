@@ -288,18 +288,8 @@ static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
   return MCRT_OK;
 }
 
-mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, void* stream_) {
-  if (!ctx) return MCRT_EINVAL;
-  if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_run_batch: grid, opacity and sources must be set first");
-  cudaStream_t st = (cudaStream_t)stream_;
-  if (ctx->pending.size() >= 4096) {                         // nobody is reading the timings: recycle
-    CU(cudaEventSynchronize(ctx->pending.back().e2));
-    for (auto& b : ctx->pending) ctx->spare.push_back(b);
-    ctx->pending.clear();
-  }
-  BatchEvents ev;
-  mcrt_status rc = take_events(ctx, &ev);
-  if (rc != MCRT_OK) return rc;
+static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st) {
+  if (n == 0) return MCRT_OK;
   const int nb = ctx->nb;
   TransportParams P;
   P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.trow = ctx->d_trow;
@@ -308,38 +298,92 @@ mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_
   P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
   P.seed = seed; P.first = first; P.count = n;
   P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->n3;
-  CU(cudaEventRecord(ev.e0, st));
-  if (n > 0) {
-    CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
-    const int threads = ctx->threads;
-    long long want = ((long long)n + threads - 1) / threads;
-    long long grid = (long long)ctx->sm_count * ctx->blocks_per_sm;
-    if (want < grid) grid = want;
-    size_t smem = sizeof(float4) * nb + 4 * (size_t)nb * 4;
-    if (ctx->S > 1) k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
-    else k_transport<false><<<(unsigned)grid, threads, smem, st>>>(P);
-    ctx->launches++;
-    CU(cudaGetLastError());
+  CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
+  const int threads = ctx->threads;
+  long long want = ((long long)n + threads - 1) / threads;
+  long long grid = (long long)ctx->sm_count * ctx->blocks_per_sm;
+  if (want < grid) grid = want;
+  size_t smem = sizeof(float4) * nb + 4 * (size_t)nb * 4;
+  if (ctx->S > 1) k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
+  else k_transport<false><<<(unsigned)grid, threads, smem, st>>>(P);
+  ctx->launches++;
+  CU(cudaGetLastError());
+  return MCRT_OK;
+}
+
+// a9: T from `tally` (the context's own cumulative tally, or a caller's device array that
+// holds the sum over ranks) and n_cum packages emitted so far in the whole job.
+static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally, uint64_t n_cum, cudaStream_t st) {
+  if (n_cum == 0) return MCRT_OK;
+  const double PI = 3.14159265358979323846;
+  double V = ctx->root_size * ctx->root_size * ctx->root_size;
+  float ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)n_cum) - std::log(4.0 * PI) - std::log(V));
+  float ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
+  long long blocks = (ctx->slots + 255) / 256;
+  long long cap = (long long)ctx->sm_count * 8;
+  if (blocks > cap) blocks = cap;
+  k_update_temperature<<<(unsigned)blocks, 256, 4 * ctx->nT, st>>>(ctx->d_rho, tally, ctx->d_trow, ctx->d_lnQ,
+                                                                  ctx->nT, ctx->slots, ctx->n3, ln_coef, ln_sub3);
+  ctx->launches++;
+  CU(cudaGetLastError());
+  return MCRT_OK;
+}
+
+static mcrt_status begin_batch(mcrt_ctx* ctx, BatchEvents* ev) {
+  if (ctx->pending.size() >= 4096) {                         // nobody is reading the timings: recycle
+    CU(cudaEventSynchronize(ctx->pending.back().e2));
+    for (auto& b : ctx->pending) ctx->spare.push_back(b);
+    ctx->pending.clear();
   }
+  return take_events(ctx, ev);
+}
+
+mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, void* stream_) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_run_batch: grid, opacity and sources must be set first");
+  cudaStream_t st = (cudaStream_t)stream_;
+  BatchEvents ev;
+  mcrt_status rc = begin_batch(ctx, &ev);
+  if (rc != MCRT_OK) return rc;
+  CU(cudaEventRecord(ev.e0, st));
+  rc = launch_transport(ctx, seed, first, n, st);
+  if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
   CU(cudaEventRecord(ev.e1, st));
   ctx->Ncum += n;
-  if (ctx->Ncum > 0) {
-    const double PI = 3.14159265358979323846;
-    double V = ctx->root_size * ctx->root_size * ctx->root_size;
-    float ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)ctx->Ncum) - std::log(4.0 * PI) - std::log(V));
-    float ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
-    long long blocks = (ctx->slots + 255) / 256;
-    long long cap = (long long)ctx->sm_count * 8;
-    if (blocks > cap) blocks = cap;
-    k_update_temperature<<<(unsigned)blocks, 256, 4 * ctx->nT, st>>>(ctx->d_rho, ctx->d_tally, ctx->d_trow, ctx->d_lnQ,
-                                                                    ctx->nT, ctx->slots, ctx->n3, ln_coef, ln_sub3);
-    ctx->launches++;
-    CU(cudaGetLastError());
-  }
+  rc = launch_update(ctx, ctx->d_tally, ctx->Ncum, st);
+  if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
   CU(cudaEventRecord(ev.e2, st));
   ctx->pending.push_back(ev);
   ctx->last_stream = st;
   return MCRT_OK;
+}
+
+mcrt_status mcrt_transport_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, void* stream_) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_transport_batch: grid, opacity and sources must be set first");
+  cudaStream_t st = (cudaStream_t)stream_;
+  BatchEvents ev;
+  mcrt_status rc = begin_batch(ctx, &ev);
+  if (rc != MCRT_OK) return rc;
+  CU(cudaEventRecord(ev.e0, st));
+  rc = launch_transport(ctx, seed, first, n, st);
+  if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
+  CU(cudaEventRecord(ev.e1, st));
+  CU(cudaEventRecord(ev.e2, st));
+  ctx->pending.push_back(ev);
+  ctx->Ncum += n;
+  ctx->last_stream = st;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, uint64_t n_cum, void* stream_) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_update_temperature: grid, opacity and sources must be set first");
+  cudaStream_t st = (cudaStream_t)stream_;
+  mcrt_status rc = launch_update(ctx, tally_sum ? (const unsigned long long*)tally_sum : ctx->d_tally,
+                                 tally_sum ? n_cum : ctx->Ncum, st);
+  ctx->last_stream = st;
+  return rc;
 }
 
 static mcrt_status sync_last(mcrt_ctx* ctx) {

@@ -1,0 +1,314 @@
+"""Thin ctypes binding of the C-ABI library (include/mcrt.h).  Argument marshalling only:
+every step of the method runs in the CUDA kernels behind the `mcrt_*` calls.  PyTorch is used
+for device buffers and streams.  There is no CPU fallback: a missing library or device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MCRT_HOST, MCRT_DEVICE = 0, 1
+_lib = None
+
+
+class McrtError(RuntimeError):
+    pass
+
+
+class _GridDesc(C.Structure):
+    _fields_ = [("n_root", C.c_int32), ("sub", C.c_int32), ("origin", C.c_double * 3),
+                ("root_size", C.c_double), ("refine", C.c_void_p), ("rho_root", C.c_void_p),
+                ("rho_sub", C.c_void_p), ("mem", C.c_int)]
+
+
+class _OpacityDesc(C.Structure):
+    _fields_ = [("n_bins", C.c_int32), ("lambda_edges_um", C.c_void_p),
+                ("n_species", C.c_int32), ("weight", C.c_void_p), ("kabs", C.c_void_p),
+                ("ksca", C.c_void_p), ("g", C.c_void_p), ("T_min", C.c_double),
+                ("T_max", C.c_double), ("n_T", C.c_int32)]
+
+
+class _Source(C.Structure):
+    _fields_ = [("type", C.c_int32), ("pos", C.c_double * 3), ("L", C.c_double),
+                ("T_bb", C.c_double)]
+
+
+class _Counters(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("emitted", "escaped", "lost", "absorptions",
+                                          "scatterings", "flights", "crossings")]
+
+
+# every symbol include/mcrt.h declares
+SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opacity",
+           "mcrt_set_source", "mcrt_run_batch", "mcrt_transport_batch",
+           "mcrt_update_temperature", "mcrt_get_cell_energy",
+           "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_get_counters",
+           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_get_batch_times", "mcrt_get_tables",
+           "mcrt_kernel_launches", "mcrt_philox_blocks", "mcrt_last_error")
+
+
+def lib():
+    """Load libmcrt.so (built in-tree by build.py).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB_PATH
+        if not os.path.exists(path):
+            raise McrtError(f"{path} is missing: run `python -m paper_1201_3588_b200.build` "
+                            "(there is no CPU fallback)")
+        L = C.CDLL(path)
+        vp, i32, i64, u64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64
+        L.mcrt_grid_create.argtypes = [C.POINTER(_GridDesc), C.POINTER(vp)]
+        L.mcrt_destroy.argtypes = [vp]
+        L.mcrt_leaf_slots.restype = i64
+        L.mcrt_leaf_slots.argtypes = [vp]
+        L.mcrt_set_opacity.argtypes = [vp, C.POINTER(_OpacityDesc)]
+        L.mcrt_set_source.argtypes = [vp, i32, C.POINTER(_Source)]
+        L.mcrt_run_batch.argtypes = [vp, u64, u64, u64, vp]
+        L.mcrt_transport_batch.argtypes = [vp, u64, u64, u64, vp]
+        L.mcrt_update_temperature.argtypes = [vp, vp, u64, vp]
+        L.mcrt_get_cell_energy.argtypes = [vp, vp, C.POINTER(C.c_double), C.c_int]
+        L.mcrt_get_cell_temperature.argtypes = [vp, vp, C.c_int]
+        L.mcrt_get_sed.argtypes = [vp, vp, C.c_int]
+        L.mcrt_get_counters.argtypes = [vp, C.POINTER(_Counters), vp]
+        L.mcrt_reset_tallies.argtypes = [vp, i32]
+        L.mcrt_set_launch.argtypes = [vp, i32, i32]
+        L.mcrt_get_batch_times.argtypes = [vp, vp, vp, i32, C.POINTER(i32)]
+        L.mcrt_get_tables.argtypes = [vp, vp, vp, vp]
+        L.mcrt_kernel_launches.restype = i64
+        L.mcrt_kernel_launches.argtypes = [vp]
+        L.mcrt_philox_blocks.argtypes = [vp, vp, vp, i64]
+        L.mcrt_last_error.restype = C.c_char_p
+        L.mcrt_last_error.argtypes = [vp]
+        for name in ("mcrt_grid_create", "mcrt_destroy", "mcrt_set_opacity", "mcrt_set_source",
+                     "mcrt_run_batch", "mcrt_transport_batch", "mcrt_update_temperature",
+                     "mcrt_get_cell_energy", "mcrt_get_cell_temperature",
+                     "mcrt_get_sed", "mcrt_get_counters", "mcrt_reset_tallies",
+                     "mcrt_set_launch", "mcrt_get_batch_times", "mcrt_get_tables",
+                     "mcrt_philox_blocks"):
+            getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _np_ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _is_tensor(x):
+    return hasattr(x, "data_ptr")
+
+
+class Context:
+    """mcrt_ctx with the call names of include/mcrt.h.  Inputs may be numpy arrays (host) or
+    torch CUDA tensors (device); outputs are numpy arrays, or torch CUDA tensors with
+    device=True."""
+
+    def __init__(self):
+        self.h = None
+        self.n_bins = 0
+        self.n_T = 0
+        self._keep = None
+
+    # -- errors ---------------------------------------------------------------------------
+    def _check(self, rc, what):
+        if rc != 0:
+            msg = lib().mcrt_last_error(self.h)
+            raise McrtError(f"{what}: status {rc}: {msg.decode() if msg else ''}")
+
+    # -- set-up ---------------------------------------------------------------------------
+    def grid_create(self, n_root, sub, origin, root_size, refine, rho_root, rho_sub):
+        L = lib()
+        d = _GridDesc()
+        d.n_root, d.sub = int(n_root), int(sub)
+        d.origin = (C.c_double * 3)(*[float(v) for v in origin])
+        d.root_size = float(root_size)
+        if _is_tensor(rho_root):
+            import torch
+            keep = [rho_root.contiguous().to(torch.float32)]
+            d.rho_root = keep[0].data_ptr()
+            if refine is not None:
+                keep.append(refine.contiguous().to(torch.uint8))
+                d.refine = keep[-1].data_ptr()
+            if rho_sub is not None:
+                keep.append(rho_sub.contiguous().to(torch.float32))
+                d.rho_sub = keep[-1].data_ptr()
+            d.mem = MCRT_DEVICE
+        else:
+            keep = [np.ascontiguousarray(rho_root, dtype=np.float32)]
+            d.rho_root = _np_ptr(keep[0])
+            if refine is not None:
+                keep.append(np.ascontiguousarray(refine, dtype=np.uint8))
+                d.refine = _np_ptr(keep[-1])
+            if rho_sub is not None:
+                keep.append(np.ascontiguousarray(rho_sub, dtype=np.float32))
+                d.rho_sub = _np_ptr(keep[-1])
+            d.mem = MCRT_HOST
+        out = C.c_void_p()
+        rc = L.mcrt_grid_create(C.byref(d), C.byref(out))
+        if rc != 0:
+            msg = L.mcrt_last_error(None)
+            raise McrtError(f"mcrt_grid_create: status {rc}: {msg.decode() if msg else ''}")
+        self.h = out
+        self.slots = int(L.mcrt_leaf_slots(self.h))
+        return self
+
+    def set_opacity(self, lambda_edges_um, weight, kabs, ksca, g, T_min=0.0, T_max=0.0, n_T=0):
+        e = np.ascontiguousarray(lambda_edges_um, dtype=np.float64)
+        w = np.ascontiguousarray(weight, dtype=np.float64)
+        ka = np.ascontiguousarray(kabs, dtype=np.float32).reshape(len(w), -1)
+        ks = np.ascontiguousarray(ksca, dtype=np.float32).reshape(len(w), -1)
+        gg = np.ascontiguousarray(g, dtype=np.float32).reshape(len(w), -1)
+        d = _OpacityDesc()
+        d.n_bins, d.n_species = len(e) - 1, len(w)
+        d.lambda_edges_um, d.weight = _np_ptr(e), _np_ptr(w)
+        d.kabs, d.ksca, d.g = _np_ptr(ka), _np_ptr(ks), _np_ptr(gg)
+        d.T_min, d.T_max, d.n_T = float(T_min), float(T_max), int(n_T)
+        self._check(lib().mcrt_set_opacity(self.h, C.byref(d)), "mcrt_set_opacity")
+        self.n_bins = d.n_bins
+        self.n_T = n_T if n_T > 0 else 801
+        return self
+
+    def set_source(self, sources):
+        arr = (_Source * len(sources))()
+        for i, s in enumerate(sources):
+            arr[i].type = int(s.type)
+            arr[i].pos = (C.c_double * 3)(*[float(v) for v in s.pos])
+            arr[i].L, arr[i].T_bb = float(s.L), float(s.T_bb)
+        self._check(lib().mcrt_set_source(self.h, len(sources), arr), "mcrt_set_source")
+        return self
+
+    # -- hot path -------------------------------------------------------------------------
+    def run_batch(self, seed, first_packet_id, n_packets, stream=None):
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(lib().mcrt_run_batch(self.h, int(seed), int(first_packet_id),
+                                         int(n_packets), C.c_void_p(stream)), "mcrt_run_batch")
+
+    def transport_batch(self, seed, first_packet_id, n_packets, stream=None):
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(lib().mcrt_transport_batch(self.h, int(seed), int(first_packet_id),
+                                               int(n_packets), C.c_void_p(stream)),
+                    "mcrt_transport_batch")
+
+    def update_temperature(self, tally_sum=None, n_cum=0, stream=None):
+        """tally_sum: torch int64 CUDA tensor [leaf slots] (sum over ranks) or None."""
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        p = None if tally_sum is None else C.c_void_p(tally_sum.data_ptr())
+        self._check(lib().mcrt_update_temperature(self.h, p, int(n_cum), C.c_void_p(stream)),
+                    "mcrt_update_temperature")
+
+    # -- results --------------------------------------------------------------------------
+    def _out(self, shape, np_dtype, device):
+        if device:
+            import torch
+            t = torch.empty(shape, dtype=getattr(torch, np.dtype(np_dtype).name
+                                                 .replace("uint64", "int64")), device="cuda")
+            return t, C.c_void_p(t.data_ptr()), MCRT_DEVICE
+        a = np.zeros(shape, dtype=np_dtype)
+        return a, _np_ptr(a), MCRT_HOST
+
+    def get_cell_energy(self, device=False):
+        out, p, mem = self._out((self.slots,), np.uint64, device)
+        eps = C.c_double(0)
+        self._check(lib().mcrt_get_cell_energy(self.h, p, C.byref(eps), mem),
+                    "mcrt_get_cell_energy")
+        return out, eps.value
+
+    def get_cell_temperature(self, device=False):
+        out, p, mem = self._out((self.slots,), np.float32, device)
+        self._check(lib().mcrt_get_cell_temperature(self.h, p, mem),
+                    "mcrt_get_cell_temperature")
+        return out
+
+    def get_sed(self, device=False):
+        out, p, mem = self._out((3, self.n_bins), np.uint64, device)
+        self._check(lib().mcrt_get_sed(self.h, p, mem), "mcrt_get_sed")
+        return out
+
+    def get_counters(self):
+        c = _Counters()
+        e = np.zeros(self.n_bins, dtype=np.uint64)
+        self._check(lib().mcrt_get_counters(self.h, C.byref(c), _np_ptr(e)),
+                    "mcrt_get_counters")
+        d = {n: int(getattr(c, n)) for n, _ in _Counters._fields_}
+        d["emitted_per_bin"] = e
+        return d
+
+    def reset_tallies(self, what=3):
+        self._check(lib().mcrt_reset_tallies(self.h, int(what)), "mcrt_reset_tallies")
+
+    # -- tuning / introspection ---------------------------------------------------------
+    def set_launch(self, threads_per_block=0, blocks_per_sm=0):
+        self._check(lib().mcrt_set_launch(self.h, threads_per_block, blocks_per_sm),
+                    "mcrt_set_launch")
+
+    def get_batch_times(self, cap=4096):
+        t = np.zeros(cap, dtype=np.float32)
+        u = np.zeros(cap, dtype=np.float32)
+        n = C.c_int32(0)
+        self._check(lib().mcrt_get_batch_times(self.h, _np_ptr(t), _np_ptr(u), cap,
+                                               C.byref(n)), "mcrt_get_batch_times")
+        return t[:n.value].copy(), u[:n.value].copy()
+
+    def get_tables(self):
+        opac = np.zeros((self.n_bins, 4), dtype=np.float32)
+        lnQ = np.zeros(self.n_T, dtype=np.float32)
+        cdf = np.zeros((self.n_T, self.n_bins), dtype=np.float32)
+        self._check(lib().mcrt_get_tables(self.h, _np_ptr(opac), _np_ptr(lnQ), _np_ptr(cdf)),
+                    "mcrt_get_tables")
+        return opac, lnQ, cdf
+
+    def kernel_launches(self):
+        return int(lib().mcrt_kernel_launches(self.h))
+
+    def destroy(self):
+        if self.h is not None and _lib is not None:
+            _lib.mcrt_destroy(self.h)
+        self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def from_workload(wl, device_inputs=False, n_T=0, T_min=0.0, T_max=0.0) -> Context:
+    """grid_create -> set_opacity -> set_source for a workloads.Workload."""
+    ctx = Context()
+    refine, rho_root, rho_sub = wl.refine, wl.rho_root, wl.rho_sub
+    if device_inputs:
+        import torch
+        rho_root = torch.from_numpy(np.ascontiguousarray(rho_root)).cuda()
+        refine = None if refine is None else torch.from_numpy(np.ascontiguousarray(refine)).cuda()
+        rho_sub = None if rho_sub is None else torch.from_numpy(np.ascontiguousarray(rho_sub)).cuda()
+    ctx.grid_create(wl.n_root, wl.sub, wl.origin, wl.root_size, refine, rho_root, rho_sub)
+    ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g, T_min, T_max, n_T)
+    ctx.set_source(wl.sources)
+    return ctx
+
+
+def run_workload(wl, n_packets=None, batch=None, **kw) -> Context:
+    ctx = from_workload(wl, **kw)
+    for first, cnt in wl.batches(n_packets, batch):
+        ctx.run_batch(wl.seed, first, cnt)
+    return ctx
+
+
+def philox_blocks(key2, ctr):
+    k = np.ascontiguousarray(key2, dtype=np.uint32)
+    c = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    o = np.zeros_like(c)
+    rc = lib().mcrt_philox_blocks(_np_ptr(k), _np_ptr(c), _np_ptr(o), len(c))
+    if rc != 0:
+        raise McrtError(f"mcrt_philox_blocks: status {rc}: {lib().mcrt_last_error(None).decode()}")
+    return o

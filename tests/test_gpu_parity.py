@@ -1,0 +1,258 @@
+"""-m gpu: the CUDA path (through the C-ABI, include/mcrt.h) against the fp64 oracle on the same
+seeded inputs.  Tolerances: BASELINE.json north_star (tests/parity.py)."""
+import numpy as np
+import pytest
+
+import parity as PR
+from paper_1201_3588_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def M():
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    from paper_1201_3588_b200 import build, mcrt
+    build.build_library()
+    mcrt.lib()
+    return mcrt
+
+
+def _run_both(M, O, wl, n_packets=None, batch=None, threads=0):
+    ctx = M.run_workload(wl, n_packets, batch)
+    orc = O.Oracle(wl).run(n_packets, batch, threads=threads)
+    return ctx, orc
+
+
+def _compare(ctx, orc, groups=None, min_count=1000, expect_cells=True):
+    cg, co = ctx.get_counters(), orc.counters()
+    PR.check_accounting(cg, co)
+    ng, eps_g = ctx.get_cell_energy()
+    no, eps_o = orc.cell_energy()
+    sg, so = ctx.get_sed(), orc.sed()
+    PR.check_self_consistency(cg, ng, sg)
+    assert eps_g == pytest.approx(eps_o, rel=1e-12)
+    n_cells, n_groups = PR.check_cell_energy(ng, no, min_count=min_count, groups=groups)
+    if expect_cells:
+        assert n_cells + n_groups > 0
+    PR.check_temperature(ctx.get_cell_temperature(), orc.cell_temperature(), ng, no,
+                         min_count=min_count)
+    PR.check_sed(sg, so)
+    # event totals are sums of ~1e5+ events: 3 sigma + 0.5 %
+    for k in ("absorptions", "scatterings", "crossings"):
+        assert PR.counts_close(cg[k], co[k], 0.005), (k, cg[k], co[k])
+    return cg, co
+
+
+# ---- generator ------------------------------------------------------------------------------
+def test_philox_device_matches_oracle(M, oracle_mod):
+    rng = np.random.default_rng(7)
+    key = rng.integers(0, 2 ** 32, size=2, dtype=np.uint64).astype(np.uint32)
+    ctr = rng.integers(0, 2 ** 32, size=(20000, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    ctr[1] = 0xFFFFFFFF
+    out = M.philox_blocks(key, ctr)
+    for i in list(range(64)) + list(range(0, 20000, 97)):
+        assert np.array_equal(out[i], oracle_mod.philox(key, ctr[i])), i
+
+
+# ---- tables (row a0) ------------------------------------------------------------------------
+@pytest.mark.parametrize("maker", [W.c0, lambda: W.c2(n_root=8, n_packets=10, batch=10)])
+def test_tables_match_oracle(M, oracle_mod, maker):
+    wl = maker()
+    ctx = M.from_workload(wl)
+    orc = oracle_mod.Oracle(wl)
+    opac, lnQ, cdf = ctx.get_tables()
+    t = orc.tables()
+    np.testing.assert_allclose(opac[:, 0], t["kext"] * wl.root_size, rtol=2e-7)
+    np.testing.assert_allclose(opac[:, 1], t["alb"], rtol=2e-7, atol=1e-30)
+    np.testing.assert_allclose(opac[:, 2], t["g"], rtol=2e-7, atol=1e-30)
+    ok = t["Q"] > 1e-280
+    np.testing.assert_allclose(lnQ[ok], np.log(t["Q"][ok]), rtol=2e-7, atol=2e-6)
+    np.testing.assert_allclose(cdf, t["C"], rtol=0, atol=1.2e-7)
+
+
+# ---- C0 at full size ------------------------------------------------------------------------
+def test_c0_full(M, oracle_mod):
+    wl = W.c0()
+    ctx, orc = _run_both(M, oracle_mod, wl)
+    cg, co = _compare(ctx, orc, groups=PR.radial_shells(16, 8))
+    assert cg["emitted"] == 100_000
+
+
+def test_c0_bit_reproducible_and_launch_shape_invariant(M):
+    wl = W.c0()
+    a = M.run_workload(wl)
+    b = M.from_workload(wl)
+    b.set_launch(64, 2)
+    for first, cnt in wl.batches():
+        b.run_batch(wl.seed, first, cnt)
+    assert np.array_equal(a.get_cell_energy()[0], b.get_cell_energy()[0])
+    assert np.array_equal(a.get_sed(), b.get_sed())
+    assert np.array_equal(a.get_cell_temperature(), b.get_cell_temperature())
+    ca, cb = a.get_counters(), b.get_counters()
+    for k in ca:
+        assert np.array_equal(ca[k], cb[k]), k
+
+
+def test_pure_scattering_exact(M, oracle_mod):
+    """albedo 1: no tally, frequency never changes -> SED total per bin == emitted per bin
+    exactly, and batch-partition independent bit-exactly (R29)."""
+    wl = W.sphere(n_root=16, albedo=1.0, gval=0.4, n_packets=200_000, batch=50_000)
+    ctx = M.run_workload(wl)
+    c = ctx.get_counters()
+    sed = ctx.get_sed()
+    assert np.array_equal(sed.sum(0), c["emitted_per_bin"])
+    assert int(ctx.get_cell_energy()[0].sum()) == 0 and c["absorptions"] == 0
+    assert c["escaped"] == 200_000 and c["lost"] == 0
+    other = M.run_workload(wl, batch=200_000)
+    assert np.array_equal(other.get_sed(), sed)
+    co = other.get_counters()
+    assert co["crossings"] == c["crossings"] and co["scatterings"] == c["scatterings"]
+    orc = oracle_mod.Oracle(wl).run()
+    PR.check_accounting(c, orc.counters())
+    PR.check_sed(sed, orc.sed())
+
+
+def test_beer_lambert_direct_fraction(M):
+    """Pure absorber, central source: direct/emitted per bin = exp(-tau_j) within the voxel
+    staircase (closed form, BASELINE.json check 2) -- pins the GPU walk without the oracle."""
+    wl = W.sphere(n_root=32, albedo=0.0, tau_v=1.0, n_packets=2_000_000, batch=2_000_000)
+    ctx = M.run_workload(wl)
+    c = ctx.get_counters()
+    sed = ctx.get_sed()
+    kext = (wl.kabs[0] + wl.ksca[0]).astype(np.float64)
+    tau = kext * wl.meta["rho0"] * wl.meta["R_cm"]
+    em = c["emitted_per_bin"].astype(np.float64)
+    sel = em > 20000
+    frac = sed[0][sel] / em[sel]
+    # staircase: chord through filled voxels differs from R by O(1 cell) = 1/16 of R
+    lo, hi = np.exp(-tau[sel] * (1 + 1.5 / 16)), np.exp(-tau[sel] * (1 - 1.5 / 16))
+    sig = 3 * np.sqrt(frac * (1 - frac) / em[sel])
+    assert np.all(frac <= hi + sig) and np.all(frac >= lo - sig)
+
+
+# ---- C1 twins: 64^3, HG g = 0.6, several tiles of batches and a ragged tail ------------------
+@pytest.mark.parametrize("tau_v,n_packets", [(0.1, 1_000_000), (1.0, 1_000_000),
+                                             (10.0, 400_000), (100.0, 30_000)])
+def test_c1_twin(M, oracle_mod, tau_v, n_packets):
+    wl = W.c1(tau_v=tau_v, n_packets=n_packets, batch=n_packets // 10 + 7)
+    ctx, orc = _run_both(M, oracle_mod, wl)
+    _compare(ctx, orc, groups=PR.radial_shells(64, 16))
+
+
+# ---- two-level grids ------------------------------------------------------------------------
+@pytest.mark.parametrize("n_root,sub,n_ref,ext", [(2, 4, 1, False), (2, 4, 8, True),
+                                                  (3, 4, 5, False), (4, 2, 9, True),
+                                                  (3, 0, 0, True)])
+def test_tiny_grids(M, oracle_mod, n_root, sub, n_ref, ext):
+    wl = W.tiny_random(n_root=n_root, sub=sub, n_refined=n_ref, seed=11 + n_ref,
+                       external=ext, n_packets=400_000, batch=100_000)
+    ctx, orc = _run_both(M, oracle_mod, wl)
+    _compare(ctx, orc)
+
+
+def test_c2_twin_small_disk(M, oracle_mod):
+    """Disk twin: 32^3 root grid of the C2 recipe (refined inside r < 5 r0), tau_V = 100."""
+    wl = W.c2(n_root=32, n_packets=200_000, batch=20_000)
+    assert wl.n_ref > 0
+    ctx, orc = _run_both(M, oracle_mod, wl)
+    _compare(ctx, orc, min_count=1000)
+
+
+def test_c3_twin_small_disk(M, oracle_mod):
+    wl = W.c3(n_root=32, n_packets=200_000, batch=20_000)
+    assert wl.n_ref > 0
+    ctx, orc = _run_both(M, oracle_mod, wl)
+    _compare(ctx, orc, min_count=1000)
+
+
+def test_c4_twin_small_cube(M, oracle_mod):
+    """Clumpy cube twin: 64^3 of the C4 recipe, 10 point sources + external field."""
+    wl = W.c4(n_root=64, n_packets=300_000, batch=30_000, corr_cells=4.0)
+    ctx, orc = _run_both(M, oracle_mod, wl)
+    _compare(ctx, orc, groups=PR.super_blocks(64, 8))
+
+
+# ---- edge cases -----------------------------------------------------------------------------
+def test_empty_batch_and_single_packet(M, oracle_mod):
+    wl = W.c0()
+    ctx = M.from_workload(wl)
+    ctx.run_batch(1, 0, 0)
+    assert ctx.get_counters()["emitted"] == 0
+    assert np.all(ctx.get_cell_temperature() == np.float32(1.0))
+    ctx.run_batch(1, 5, 1)
+    c = ctx.get_counters()
+    assert c["emitted"] == 1 and c["escaped"] == 1
+    orc = oracle_mod.Oracle(wl)
+    orc.run_batch(1, 5, 1)
+    assert np.array_equal(ctx.get_sed(), orc.sed())
+
+
+def test_empty_grid_all_escape_direct(M):
+    wl = W.c0()
+    wl.rho_root = np.zeros_like(wl.rho_root)
+    ctx = M.run_workload(wl, 50_000, 50_000)
+    c = ctx.get_counters()
+    sed = ctx.get_sed()
+    assert c["escaped"] == 50_000 and c["flights"] == 50_000
+    assert sed[1:].sum() == 0 and np.array_equal(sed[0], c["emitted_per_bin"])
+    # centre vertex of a 16^3 grid: every packet leaves 8 cells per axis-ish; at least 8 crossings
+    assert c["crossings"] >= 8 * 50_000
+
+
+def test_packet_ids_beyond_32_bits(M, oracle_mod):
+    wl = W.c0()
+    first = (1 << 40) + 12345
+    ctx = M.from_workload(wl)
+    ctx.run_batch(3, first, 20_000)
+    orc = oracle_mod.Oracle(wl)
+    orc.run_batch(3, first, 20_000)
+    PR.check_accounting(ctx.get_counters(), orc.counters())
+    PR.check_sed(ctx.get_sed(), orc.sed())
+
+
+def test_device_inputs_and_outputs(M):
+    import torch
+    wl = W.c0()
+    a = M.run_workload(wl, 20_000, 10_000)
+    b = M.run_workload(wl, 20_000, 10_000, device_inputs=True)
+    n_dev, eps = b.get_cell_energy(device=True)
+    assert n_dev.is_cuda and np.array_equal(n_dev.cpu().numpy().astype(np.uint64),
+                                            a.get_cell_energy()[0])
+    assert np.array_equal(b.get_cell_temperature(device=True).cpu().numpy(),
+                          a.get_cell_temperature())
+    assert np.array_equal(b.get_sed(device=True).cpu().numpy().astype(np.uint64), a.get_sed())
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        c = M.run_workload(wl, 20_000, 10_000)
+    assert np.array_equal(c.get_sed(), a.get_sed())
+
+
+def test_error_paths(M):
+    ctx = M.Context()
+    wl = W.c0()
+    with pytest.raises(M.McrtError):
+        ctx.grid_create(0, 0, wl.origin, wl.root_size, None, wl.rho_root, None)
+    ctx.grid_create(wl.n_root, 0, wl.origin, wl.root_size, None, wl.rho_root, None)
+    with pytest.raises(M.McrtError):          # ESTATE: opacity not set
+        ctx.set_source(wl.sources)
+    with pytest.raises(M.McrtError):          # ESTATE
+        ctx.run_batch(1, 0, 10)
+    ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g)
+    with pytest.raises(M.McrtError):          # source outside the box
+        ctx.set_source([W.Source(W.SRC_POINT, (-1.0, 0.0, 0.0), W.LSUN, 5800.0)])
+    with pytest.raises(M.McrtError):
+        ctx.set_opacity(wl.lambda_edges_um[::-1], wl.weight, wl.kabs, wl.ksca, wl.g)
+
+
+def test_reset_tallies(M):
+    wl = W.c0()
+    ctx = M.run_workload(wl, 20_000, 10_000)
+    first = ctx.get_sed().copy()
+    ctx.reset_tallies(3)
+    assert ctx.get_sed().sum() == 0 and ctx.get_cell_energy()[0].sum() == 0
+    for f, c in wl.batches(20_000, 10_000):
+        ctx.run_batch(wl.seed, f, c)
+    assert np.array_equal(ctx.get_sed(), first)
