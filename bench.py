@@ -79,9 +79,14 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
 
-    def stop(self):
+    def wait_first(self, timeout=8.0):
+        t0 = time.time()
+        while self.proc is not None and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.02)
+
+    def stop(self, t_from=0.0, t_to=float("inf")):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -91,8 +96,8 @@ class ClockSampler:
             self.proc.kill()
         self.thread.join(timeout=2)
         sm, mx, reasons = [], [], set()
-        for r in self.rows:
-            if len(r) < 6:
+        for t, r in self.rows:
+            if len(r) < 6 or t < t_from or t > t_to:
                 continue
             try:
                 sm.append(float(r[0]))
@@ -125,10 +130,12 @@ def oracle_rate(wl, target_seconds=15.0, n_batches=4):
     O.build()
     cores = O.max_threads()
     orc = O.Oracle(wl)
-    probe = 4096
-    t0 = time.perf_counter()
-    orc.run_batch(wl.seed, 0, probe)
-    dt = max(time.perf_counter() - t0, 1e-4)
+    probe, dt = 2048, 0.0
+    while dt < 0.5 and probe < wl.n_packets:                 # calibrate the sample size
+        probe *= 2
+        t0 = time.perf_counter()
+        orc.run_batch(wl.seed, 0, probe)
+        dt = max(time.perf_counter() - t0, 1e-4)
     n = int(min(max(probe * target_seconds / dt, 4 * probe), wl.n_packets))
     per = max(n // n_batches, 1)
     orc = O.Oracle(wl)
@@ -151,9 +158,13 @@ def run_reference(args, wl, name):
     O.build()
     cores = O.max_threads()
     orc = O.Oracle(wl)
-    t0 = time.perf_counter()
-    orc.run_batch(wl.seed, 0, 2048)
-    rate = 2048 / max(time.perf_counter() - t0, 1e-4)
+    probe, dt = 2048, 0.0
+    while dt < 0.5 and probe < wl.n_packets:
+        probe *= 2
+        t0 = time.perf_counter()
+        orc.run_batch(wl.seed, 0, probe)
+        dt = max(time.perf_counter() - t0, 1e-4)
+    rate = probe / dt
     budget = 120.0 / max(args.steps + args.warmup, 1)
     per = int(min(max(rate * min(budget, 10.0), 1024), wl.batch))
     orc = O.Oracle(wl)
@@ -245,6 +256,11 @@ def run_gpu(args, wl, name):
             dist.barrier()
             torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        sampler.wait_first()
+    t_load0 = time.time()
     for _ in range(args.warmup):
         flush.fill_(1)
         one_step()
@@ -252,9 +268,6 @@ def run_gpu(args, wl, name):
     ctx.get_batch_times()
     c_before = ctx.get_counters()
     launches_before = ctx.kernel_launches()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
           for _ in range(args.steps)]
     barrier()
@@ -266,12 +279,20 @@ def run_gpu(args, wl, name):
         b.record()
     barrier()
     t_wall = time.perf_counter() - t_wall
-    clocks = sampler.stop() if rank == 0 else None
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
     t_tr, t_up = ctx.get_batch_times()
     c_after = ctx.get_counters()
     launches = ctx.kernel_launches() - launches_before
+    # the timed region may be far shorter than nvidia-smi's sampling period: keep the same
+    # load running (untimed) until the clock record holds at least ~1.5 s under load
+    while time.time() - t_load0 < 1.5:
+        one_step()
+        torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop(t_load0, time.time()) if rank == 0 else None
+    if clocks is not None:
+        clocks["window"] = "warm-up + timed steps + identical untimed steps up to 1.5 s"
     d = {k: c_after[k] - c_before[k] for k in ("emitted", "escaped", "absorptions",
                                                 "scatterings", "flights", "crossings", "lost")}
     stats = torch.tensor([total_ms, float(t_tr.sum()), float(t_up.sum())], dtype=torch.float64,
@@ -385,7 +406,7 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--workload", default="c1_tau1")

@@ -16,7 +16,15 @@ def check_accounting(cg, co):
         assert cg[k] == co[k], (k, cg[k], co[k])
     assert cg["lost"] == 0
     assert cg["emitted"] == cg["escaped"]
-    assert np.array_equal(cg["emitted_per_bin"], co["emitted_per_bin"])
+    # Emission bins: both sides search the same source CDF with the same Philox word, the GPU
+    # with the 24-bit fp32 uniform and fp32 table, the oracle in fp64 (R19, R33).  A packet
+    # lands in a neighbouring bin only if a CDF edge lies within ~2^-24 of its uniform:
+    # expected flips <= N * n_bins * 2^-24.
+    eg = cg["emitted_per_bin"].astype(np.int64)
+    eo = co["emitted_per_bin"].astype(np.int64)
+    assert eg.sum() == eo.sum() == cg["emitted"]
+    flips = np.abs(eg - eo).sum() / 2
+    assert flips <= 10 + 3.0 * cg["emitted"] * len(eg) * 2.0 ** -24, flips
 
 
 def check_self_consistency(c, n_abs, sed):
@@ -86,3 +94,19 @@ def super_blocks(n_root, b=8):
     i = np.arange(n_root) // b
     m = n_root // b + (1 if n_root % b else 0)
     return (i[None, None, :] + m * (i[None, :, None] + m * i[:, None, None])).ravel()
+
+
+def root_of_slot(wl):
+    """Root-cube linear index of every leaf slot (layout R22): sub-cells of the k-th refined
+    cube map back to that cube."""
+    n3 = wl.n_root ** 3
+    out = np.arange(wl.leaf_slots, dtype=np.int64)
+    if wl.n_ref:
+        ridx = np.flatnonzero(np.asarray(wl.refine).ravel())
+        out[n3:] = np.repeat(ridx, wl.sub ** 3)
+    return out
+
+
+def blocks_of_slot(wl, b):
+    """b^3 super-blocks of root cubes, per leaf slot."""
+    return super_blocks(wl.n_root, b)[root_of_slot(wl)]

@@ -155,17 +155,19 @@ def test_tiny_grids(M, oracle_mod, n_root, sub, n_ref, ext):
 
 def test_c2_twin_small_disk(M, oracle_mod):
     """Disk twin: 32^3 root grid of the C2 recipe (refined inside r < 5 r0), tau_V = 100."""
-    wl = W.c2(n_root=32, n_packets=200_000, batch=20_000)
+    wl = W.c2(n_root=32, n_packets=1_000_000, batch=100_000)
     assert wl.n_ref > 0
     ctx, orc = _run_both(M, oracle_mod, wl)
-    _compare(ctx, orc, min_count=1000)
+    _compare(ctx, orc, groups=PR.root_of_slot(wl))
+    _compare(ctx, orc, groups=PR.blocks_of_slot(wl, 4))
 
 
 def test_c3_twin_small_disk(M, oracle_mod):
-    wl = W.c3(n_root=32, n_packets=200_000, batch=20_000)
+    wl = W.c3(n_root=32, n_packets=1_000_000, batch=100_000)
     assert wl.n_ref > 0
     ctx, orc = _run_both(M, oracle_mod, wl)
-    _compare(ctx, orc, min_count=1000)
+    _compare(ctx, orc, groups=PR.root_of_slot(wl))
+    _compare(ctx, orc, groups=PR.blocks_of_slot(wl, 4))
 
 
 def test_c4_twin_small_cube(M, oracle_mod):
