@@ -112,6 +112,17 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
+def ncu_traffic(name):
+    """DRAM bytes per k_transport launch from the committed ncu capture of this workload."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            t = json.load(f).get(name)
+        if t:
+            return float(t["bytes_per_launch"])
+    return None
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -334,7 +345,7 @@ def run_gpu(args, wl, name):
            "kernel_ms_per_step": {"transport": tr_ms / args.steps, "temperature_update": up_ms / args.steps},
            "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
            "roofline": {"bound": "hbm", "kernel": "k_transport", "achieved": achieved, "peak": peak,
-                        "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                        "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(name),
                         "peak_source": peak_src,
                         "algorithmic_bytes": {"per_crossing": per_cross, "per_absorption": per_abs,
                                               "per_launch": bytes_alg / args.steps},
