@@ -246,20 +246,16 @@ def run_gpu(args, wl, name):
         ctx.set_launch(args.threads, args.blocks_per_sm)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
+    from paper_1201_3588_b200.sharding import ShardedRunner
+    runner = ShardedRunner(ctx, dist if world > 1 else None)
     step_no = [0]
 
     def one_step():
-        """One batch of `batch` packets per rank: global packet ids are dealt to the ranks in
-        contiguous ranges; N > 1 sums the integer tallies over ranks before the T update."""
-        first = (step_no[0] * world + rank) * batch
+        """One batch of `batch` packets per rank (weak scaling): the global batch of
+        world*batch packet ids is dealt to the ranks in contiguous ranges; N > 1 sums the
+        integer tallies over ranks before the T update (sharding.ShardedRunner)."""
+        runner.run_batch(wl.seed, step_no[0] * world * batch, world * batch, stream)
         step_no[0] += 1
-        if world == 1:
-            ctx.run_batch(wl.seed, first, batch, stream)
-        else:
-            ctx.transport_batch(wl.seed, first, batch, stream)
-            tally, _ = ctx.get_cell_energy(device=True)
-            dist.all_reduce(tally, op=dist.ReduceOp.SUM)
-            ctx.update_temperature(tally, step_no[0] * world * batch, stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -384,15 +380,10 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
     ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g)
     ctx.set_source(wl.sources)
     d2h = 0
+    from paper_1201_3588_b200.sharding import ShardedRunner
+    runner = ShardedRunner(ctx, dist if world > 1 else None)
     for s in range(steps):
-        first = (s * world + rank) * batch
-        if world == 1:
-            ctx.run_batch(wl.seed, first, batch, stream)
-        else:
-            ctx.transport_batch(wl.seed, first, batch, stream)
-            tally, _ = ctx.get_cell_energy(device=True)
-            dist.all_reduce(tally, op=dist.ReduceOp.SUM)
-            ctx.update_temperature(tally, (s + 1) * world * batch, stream)
+        runner.run_batch(wl.seed, s * world * batch, world * batch, stream)
         sed = ctx.get_sed()
         n_abs, _ = ctx.get_cell_energy()
         T = ctx.get_cell_temperature()

@@ -427,18 +427,25 @@ double leaf_mass(const Ctx& c, int64_t slot) {
 }
 
 // O7: merge the batch tally and update every leaf temperature (R9 reading B, R10, R12).
-void batch_end(Ctx& c, const std::vector<uint64_t>& batch, uint64_t n_packets) {
+void merge_tally(Ctx& c, const std::vector<uint64_t>& batch, uint64_t n_packets) {
   for (int64_t i = 0; i < c.slots; ++i) c.cum[i] += batch[i];
   c.Ncum += n_packets;
+}
+// temperatures from absorbed-package counts `cum` after n_cum emitted packages
+void update_temperatures(Ctx& c, const uint64_t* cum, uint64_t n_cum) {
   for (int64_t i = 0; i < c.slots; ++i) {
     double m = leaf_mass(c, i);
-    if (m > 0 && c.cum[i] > 0) {
-      double q = (double)c.cum[i] * c.Ltot / ((double)c.Ncum * 4.0 * PI * m);
+    if (m > 0 && cum[i] > 0) {
+      double q = (double)cum[i] * c.Ltot / ((double)n_cum * 4.0 * PI * m);
       c.T[i] = temperature_from_q(c, q);
     } else {
       c.T[i] = c.Tmin;
     }
   }
+}
+void batch_end(Ctx& c, const std::vector<uint64_t>& batch, uint64_t n_packets) {
+  merge_tally(c, batch, n_packets);
+  update_temperatures(c, c.cum.data(), c.Ncum);
 }
 
 }  // namespace
@@ -560,6 +567,30 @@ int orc_run_batch(void* h, uint64_t seed, uint64_t first, uint64_t n, int n_thre
   for (int64_t i = 0; i < (int64_t)n; ++i)
     run_packet(c, seed, first + (uint64_t)i, batch, nullptr, 0, nullptr);
   batch_end(c, batch, n);
+  return 0;
+}
+
+// The two halves of a batch, for packet-sharded runs: transport of this
+// rank's packets with T frozen and NO temperature update ...
+int orc_transport_batch(void* h, uint64_t seed, uint64_t first, uint64_t n, int n_threads) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.have_source) return -2;
+  std::vector<uint64_t> batch(c.slots, 0);
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t i = 0; i < (int64_t)n; ++i)
+    run_packet(c, seed, first + (uint64_t)i, batch, nullptr, 0, nullptr);
+  merge_tally(c, batch, n);
+  return 0;
+}
+// ... and O7's temperature step on counts summed over all ranks (n_cum = packages emitted by
+// all ranks so far).  Same arithmetic as batch_end; this rank's own cum/Ncum are not touched.
+int orc_update_temperature(void* h, const uint64_t* tally_sum, uint64_t n_cum) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.have_source || !tally_sum || n_cum == 0) return -2;
+  update_temperatures(c, tally_sum, n_cum);
   return 0;
 }
 

@@ -47,6 +47,9 @@ def lib():
         L.orc_set_source.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p]
         L.orc_run_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_int]
+        L.orc_transport_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64,
+                                          C.c_int]
+        L.orc_update_temperature.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
         L.orc_trace_packet.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_int, C.c_void_p,
                                        C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_cell_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -128,6 +131,18 @@ class Oracle:
 
     def run_batch(self, seed: int, first: int, n: int, threads: int = 0):
         rc = lib().orc_run_batch(self.h, seed, first, n, threads)
+        assert rc == 0
+
+    def transport_batch(self, seed: int, first: int, n: int, threads: int = 0):
+        """Transport only (T frozen, no temperature update): one rank's share of a batch."""
+        rc = lib().orc_transport_batch(self.h, seed, first, n, threads)
+        assert rc == 0
+
+    def update_temperature(self, tally_sum, n_cum: int):
+        """O7 on counts summed over ranks."""
+        t = np.ascontiguousarray(tally_sum, dtype=np.uint64)
+        assert t.shape == (self.slots,)
+        rc = lib().orc_update_temperature(self.h, _p(t), int(n_cum))
         assert rc == 0
 
     def run(self, n_packets=None, batch=None, threads: int = 0):
