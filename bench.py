@@ -241,9 +241,11 @@ def run_gpu(args, wl, name):
 
     batch = wl.batch
     stream = torch.cuda.current_stream().cuda_stream
-    ctx = mcrt.from_workload(wl)
+    ctx = mcrt.from_workload(wl, layout=args.layout)
     if args.threads or args.blocks_per_sm:
         ctx.set_launch(args.threads, args.blocks_per_sm)
+    if args.quorum:
+        ctx.set_walk_quorum(args.quorum)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
     from paper_1201_3588_b200.sharding import ShardedRunner
@@ -359,7 +361,8 @@ def run_gpu(args, wl, name):
 
 
 def ctx_launch_desc(args):
-    return f"threads={args.threads or 'default'} blocks_per_sm={args.blocks_per_sm or 'default'}"
+    return (f"threads={args.threads or 'default'} blocks_per_sm={args.blocks_per_sm or 'default'} "
+            f"quorum={args.quorum or 'default'} layout={args.layout or 'auto'}")
 
 
 def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
@@ -414,6 +417,8 @@ def main():
     ap.add_argument("--workload", default="c1_tau1")
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
+    ap.add_argument("--quorum", type=int, default=0, help="walk-loop quorum (0 = library default)")
+    ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 x-fastest, 2 bricked")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

@@ -71,6 +71,11 @@ typedef struct {
   const float* rho_root; /* [N^3] g cm^-3 of dust; ignored where refine = 1                   */
   const float* rho_sub;  /* [n_ref*S^3]; NULL iff no cube is refined                          */
   mcrt_mem mem;          /* where refine / rho_root / rho_sub live                            */
+  int32_t layout;        /* device storage order of a single-level grid (never visible in the
+                            getters, which always use the slot order above): 0 = automatic
+                            (x-fastest while the density array fits the L2 comfortably, else
+                            bricked), 1 = x-fastest, 2 = 8^3 bricks in Morton order.  Ignored
+                            for two-level grids.                                               */
 } mcrt_grid_desc;
 
 /* Creates a context on the current CUDA device and uploads the grid. */
@@ -166,6 +171,10 @@ mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what);
  * Launch shape of the transport kernel: threads per block (multiple of 32, <= 1024) and resident
  * blocks per SM; 0 keeps the default. */
 mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t blocks_per_sm);
+/* Single-level grids: a warp leaves the cell-walk loop to process its stopped lanes (escape,
+ * refill, scattering, absorption) when fewer than `quorum` of its 32 lanes are still walking
+ * (1..32; 0 keeps the default 16).  A scheduling knob only: results do not depend on it. */
+mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum);
 /* Device times in ms of the mcrt_run_batch calls made since the previous call of this function
  * (oldest first, at most `cap`), split into the two kernels of a batch (transport, temperature
  * update), from CUDA events recorded on each batch's stream.  Synchronises with those streams.

@@ -15,6 +15,7 @@
 
 #include "tables.cuh"
 #include "transport.cuh"
+#include "transport_u.cuh"
 
 using namespace mcrt;
 
@@ -44,6 +45,13 @@ struct mcrt_ctx {
   unsigned long long Ncum = 0;
   cudaStream_t last_stream = nullptr;
   std::vector<BatchEvents> pending, spare;
+  // single-level grids: storage layout (transport_u.cuh); `slots` stays the caller-visible count
+  bool uni = false;
+  LayoutU lay = {0, 0, 0};
+  long long store_slots = 0;
+  int* d_lut = nullptr;
+  unsigned long long* d_tally_scratch = nullptr;
+  int quorum = 16;
   int threads = 256, blocks_per_sm = 4;
   long long launches = 0;
   bool have_opacity = false, have_source = false;
@@ -126,11 +134,24 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
   ctx->slots = n3 + k * s3;
   if (ctx->slots >= (1ll << 31)) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: more than 2^31-1 leaf slots"));
   if (k > 0 && !d->rho_sub) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: rho_sub is NULL but cubes are refined"));
-  CUG(cudaMalloc(&ctx->d_rho, sizeof(float) * ctx->slots));
-  CUG(cudaMalloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->slots));
-  CUG(cudaMalloc(&ctx->d_trow, sizeof(float) * ctx->slots));
-  CUG(cudaMemset(ctx->d_tally, 0, sizeof(unsigned long long) * ctx->slots));
-  CUG(cudaMemset(ctx->d_trow, 0, sizeof(float) * ctx->slots));
+  ctx->store_slots = ctx->slots;
+  if (k == 0) {                                             // single-level grid: pick the storage order
+    if (d->layout < 0 || d->layout > 2) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: layout must be 0, 1 or 2"));
+    ctx->uni = true;
+    ctx->lay.N = d->n_root;
+    ctx->lay.nbk = (d->n_root + 7) / 8;
+    ctx->lay.bricked = d->layout == 2 || (d->layout == 0 && n3 * 4 > (48ll << 20));
+    ctx->store_slots = slots_of(ctx->lay);
+    if (ctx->store_slots >= (1ll << 31)) {                   // padding pushed it over: fall back
+      ctx->lay.bricked = 0;
+      ctx->store_slots = n3;
+    }
+  }
+  CUG(cudaMalloc(&ctx->d_rho, sizeof(float) * ctx->store_slots));
+  CUG(cudaMalloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->store_slots));
+  CUG(cudaMalloc(&ctx->d_trow, sizeof(float) * ctx->store_slots));
+  CUG(cudaMemset(ctx->d_tally, 0, sizeof(unsigned long long) * ctx->store_slots));
+  CUG(cudaMemset(ctx->d_trow, 0, sizeof(float) * ctx->store_slots));
   // staging copies of caller data (freed before returning)
   float *st_root = nullptr, *st_sub = nullptr;
   int* d_refidx = nullptr;
@@ -150,7 +171,25 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     CUG(cudaMalloc(&d_refidx, sizeof(int) * n3));
     CUG(cudaMemcpy(d_refidx, refidx.data(), sizeof(int) * n3, cudaMemcpyHostToDevice));
   }
-  k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, (int)n3);
+  if (ctx->uni) {
+    // per-axis slot-delta tables: forward (i -> i+1) and reversed (entry j: i = N-1-j -> i-1)
+    const int N = ctx->N;
+    std::vector<int> lut(6 * (size_t)N);
+    for (int a = 0; a < 3; ++a)
+      for (int i = 0; i < N; ++i) {
+        lut[(size_t)(2 * a) * N + i] = i == N - 1 ? kLutEscape
+            : (int)(axis_term(ctx->lay, a, i + 1) - axis_term(ctx->lay, a, i));
+        int ir = N - 1 - i;
+        lut[(size_t)(2 * a + 1) * N + i] = ir == 0 ? kLutEscape
+            : (int)(axis_term(ctx->lay, a, ir - 1) - axis_term(ctx->lay, a, ir));
+      }
+    CUG(cudaMalloc(&ctx->d_lut, sizeof(int) * lut.size()));
+    CUG(cudaMemcpy(ctx->d_lut, lut.data(), sizeof(int) * lut.size(), cudaMemcpyHostToDevice));
+    CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
+    k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho, ctx->lay, n3);
+  } else {
+    k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, (int)n3);
+  }
   ctx->launches++;
   if (k > 0) {
     k_sanitize<<<(unsigned)((k * s3 + 255) / 256), 256>>>(src_sub, ctx->d_rho + n3, k * s3);
@@ -172,6 +211,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_opacity(ctx);
   free_sources(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
+  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -290,6 +330,12 @@ static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
 
 static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st) {
   if (n == 0) return MCRT_OK;
+  const uint64_t kMaxLaunch = 1ull << 31;                    // the kernels number packages within a launch in 32 bits
+  if (n > kMaxLaunch) {
+    mcrt_status rc = launch_transport(ctx, seed, first, kMaxLaunch, st);
+    if (rc != MCRT_OK) return rc;
+    return launch_transport(ctx, seed, first + kMaxLaunch, n - kMaxLaunch, st);
+  }
   const int nb = ctx->nb;
   TransportParams P;
   P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.trow = ctx->d_trow;
@@ -304,8 +350,14 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   long long grid = (long long)ctx->sm_count * ctx->blocks_per_sm;
   if (want < grid) grid = want;
   size_t smem = sizeof(float4) * nb + 4 * (size_t)nb * 4;
-  if (ctx->S > 1) k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
-  else k_transport<false><<<(unsigned)grid, threads, smem, st>>>(P);
+  if (ctx->uni) {
+    TransportParamsU PU;
+    PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
+    smem += sizeof(int) * 6 * (size_t)ctx->N;
+    k_transport_u<<<(unsigned)grid, threads, smem, st>>>(PU);
+  } else {
+    k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
+  }
   ctx->launches++;
   CU(cudaGetLastError());
   return MCRT_OK;
@@ -319,11 +371,22 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
   double V = ctx->root_size * ctx->root_size * ctx->root_size;
   float ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)n_cum) - std::log(4.0 * PI) - std::log(V));
   float ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
-  long long blocks = (ctx->slots + 255) / 256;
+  if (tally != ctx->d_tally && ctx->uni && ctx->lay.bricked) {     // caller's sum is in slot order (R22)
+    if (!ctx->d_tally_scratch) {
+      CU(cudaMalloc(&ctx->d_tally_scratch, 8 * (size_t)ctx->store_slots));
+      CU(cudaMemsetAsync(ctx->d_tally_scratch, 0, 8 * (size_t)ctx->store_slots, st));
+    }
+    k_ext_to_store_u64<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(tally, ctx->d_tally_scratch, ctx->lay, ctx->n3);
+    ctx->launches++;
+    tally = ctx->d_tally_scratch;
+  }
+  long long blocks = (ctx->store_slots + 255) / 256;
   long long cap = (long long)ctx->sm_count * 8;
   if (blocks > cap) blocks = cap;
   k_update_temperature<<<(unsigned)blocks, 256, 4 * ctx->nT, st>>>(ctx->d_rho, tally, ctx->d_trow, ctx->d_lnQ,
-                                                                  ctx->nT, ctx->slots, ctx->n3, ln_coef, ln_sub3);
+                                                                  ctx->nT, ctx->store_slots,
+                                                                  ctx->uni ? ctx->store_slots : ctx->n3,
+                                                                  ln_coef, ln_sub3);
   ctx->launches++;
   CU(cudaGetLastError());
   return MCRT_OK;
@@ -402,6 +465,18 @@ mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps
   if (!ctx) return MCRT_EINVAL;
   if (!n_abs_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_energy: NULL output");
   if (eps_out) *eps_out = ctx->Ncum ? ctx->Ltot / (double)ctx->Ncum : 0.0;
+  if (ctx->uni && ctx->lay.bricked) {                        // storage order -> slot order (R22)
+    unsigned long long* d_out = (unsigned long long*)n_abs_out;
+    unsigned long long* tmp = nullptr;
+    struct Tmp { unsigned long long*& a; ~Tmp() { cudaFree(a); } } guard{tmp};
+    if (mem == MCRT_HOST) { CU(cudaMalloc(&tmp, 8 * (size_t)ctx->slots)); d_out = tmp; }
+    k_store_to_ext<unsigned long long><<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
+        ctx->d_tally, d_out, ctx->lay, ctx->n3);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    if (mem == MCRT_HOST) return copy_out(ctx, n_abs_out, tmp, 8 * (size_t)ctx->slots, MCRT_HOST);
+    return sync_last(ctx);
+  }
   return copy_out(ctx, n_abs_out, ctx->d_tally, 8 * (size_t)ctx->slots, mem);
 }
 
@@ -413,8 +488,12 @@ mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem)
   float* tmp = nullptr;
   struct Tmp { float*& a; ~Tmp() { cudaFree(a); } } guard{tmp};
   if (mem == MCRT_HOST) { CU(cudaMalloc(&tmp, 4 * (size_t)ctx->slots)); d_T = tmp; }
-  k_trow_to_T<<<(unsigned)((ctx->slots + 255) / 256), 256, 0, ctx->last_stream>>>(
-      ctx->d_trow, d_T, ctx->slots, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
+  if (ctx->uni)
+    k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
+        ctx->d_trow, d_T, ctx->lay, ctx->n3, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
+  else
+    k_trow_to_T<<<(unsigned)((ctx->slots + 255) / 256), 256, 0, ctx->last_stream>>>(
+        ctx->d_trow, d_T, ctx->slots, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
   ctx->launches++;
   CU(cudaGetLastError());
   if (mem == MCRT_HOST) return copy_out(ctx, T_out, tmp, 4 * (size_t)ctx->slots, MCRT_HOST);
@@ -448,8 +527,8 @@ mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what) {
   CU(cudaStreamSynchronize(ctx->last_stream));
   if ((what & 1) && ctx->d_small) CU(cudaMemset(ctx->d_small, 0, 8 * (1 + CNT_N + 4 * (size_t)ctx->nb)));
   if (what & 2) {
-    CU(cudaMemset(ctx->d_tally, 0, 8 * (size_t)ctx->slots));
-    CU(cudaMemset(ctx->d_trow, 0, 4 * (size_t)ctx->slots));
+    CU(cudaMemset(ctx->d_tally, 0, 8 * (size_t)ctx->store_slots));
+    CU(cudaMemset(ctx->d_trow, 0, 4 * (size_t)ctx->store_slots));
     ctx->Ncum = 0;
   }
   return MCRT_OK;
@@ -461,6 +540,13 @@ mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads, int32_t blocks_per_s
     return fail(ctx, MCRT_EINVAL, "mcrt_set_launch: threads must be a multiple of 32 up to 256, blocks_per_sm <= 32");
   if (threads) ctx->threads = threads;
   if (blocks_per_sm) ctx->blocks_per_sm = blocks_per_sm;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
+  if (!ctx) return MCRT_EINVAL;
+  if (quorum < 0 || quorum > 32) return fail(ctx, MCRT_EINVAL, "mcrt_set_walk_quorum: quorum must be 0..32");
+  ctx->quorum = quorum ? quorum : 16;
   return MCRT_OK;
 }
 

@@ -1,0 +1,392 @@
+// transport_u.cuh -- sm_100a transport kernel for single-level (uniform) grids: rows a1..a8 of
+// SURVEY.md 8(a).  Same method and random-number slots as transport.cuh; what
+// differs is how a package is carried through the cells:
+//
+//  * The cell walk keeps ABSOLUTE path lengths along the current flight: t_a = path length at
+//    which the package meets its next face on axis a, tcur = path length so far.  One crossing
+//    is tnext = min(t_x,t_y,t_z); dtau = rho*kappa*(tnext - tcur); the axis whose t equals tnext
+//    (ties -> lowest axis, R21) advances by 1/|d_a|.  One FADD per crossing instead of three.
+//  * The cell's storage slot is advanced by a per-axis DELTA table held in shared memory
+//    (slot(ix,iy,iz) = A_x(ix) + A_y(iy) + A_z(iz) is separable, so the delta of a step depends
+//    on one coordinate only).  The tables make the memory layout a host decision -- x-fastest
+//    for L2-resident grids, 8^3 bricks in Morton order for grids larger than the L2 -- and mark
+//    the step that leaves the grid (INT_MIN), so the hot loop has no bounds check and no
+//    index arithmetic beyond one add.  Per axis there is a forward and a reversed table, so a
+//    table cursor always moves by +1 whatever the direction's sign.
+//  * The density of the NEXT cell is requested before the optical-depth test of the current
+//    cell (the geometric walk does not depend on rho), taking the gather latency off the
+//    dependent chain.
+//  * The walk loop runs until fewer than `quorum` lanes of the warp are still walking; then all
+//    stopped lanes go through ONE event pass (escape tally -> refill from the work queue ->
+//    emission / scattering / absorption+re-emission -> new flight).  Emission and re-emission
+//    share one instruction stream (Philox block -> CDF search -> isotropic direction).
+#pragma once
+#include <climits>
+#include "transport.cuh"
+
+namespace mcrt {
+
+// ---- storage layout of single-level grids (host and device) ----------------------------------
+struct LayoutU {
+  int N;          // root cells per axis
+  int bricked;    // 0: x-fastest;  1: 8^3 bricks (x-fastest over bricks), Morton order inside
+  int nbk;        // bricks per axis (bricked)
+};
+__host__ __device__ __forceinline__ unsigned dil3(unsigned v) {      // 3 bits -> every third bit
+  return (v & 1u) | ((v & 2u) << 2) | ((v & 4u) << 4);
+}
+__host__ __device__ __forceinline__ unsigned undil3(unsigned m) {
+  return (m & 1u) | ((m >> 2) & 2u) | ((m >> 4) & 4u);
+}
+// contribution of coordinate i on axis a to the storage slot
+__host__ __device__ __forceinline__ long long axis_term(const LayoutU& L, int a, int i) {
+  if (L.bricked) {
+    long long bs = a == 0 ? 1 : (a == 1 ? L.nbk : (long long)L.nbk * L.nbk);
+    return (long long)(dil3((unsigned)i & 7u) << a) + 512ll * (i >> 3) * bs;
+  }
+  long long s = a == 0 ? 1 : (a == 1 ? L.N : (long long)L.N * L.N);
+  return s * i;
+}
+__host__ __device__ __forceinline__ long long slot_of(const LayoutU& L, int ix, int iy, int iz) {
+  return axis_term(L, 0, ix) + axis_term(L, 1, iy) + axis_term(L, 2, iz);
+}
+__host__ __device__ __forceinline__ long long slots_of(const LayoutU& L) {
+  return L.bricked ? 512ll * L.nbk * L.nbk * L.nbk : (long long)L.N * L.N * L.N;
+}
+// storage slot -> x-fastest cell number (R22), or -1 for a padding slot
+__host__ __device__ __forceinline__ long long ext_of_slot(const LayoutU& L, long long s) {
+  if (!L.bricked) return s;
+  unsigned m = (unsigned)(s & 511);
+  long long b = s >> 9;
+  int bx = (int)(b % L.nbk), by = (int)((b / L.nbk) % L.nbk), bz = (int)(b / ((long long)L.nbk * L.nbk));
+  int ix = bx * 8 + (int)undil3(m), iy = by * 8 + (int)undil3(m >> 1), iz = bz * 8 + (int)undil3(m >> 2);
+  if (ix >= L.N || iy >= L.N || iz >= L.N) return -1;
+  return ix + (long long)L.N * (iy + (long long)L.N * iz);
+}
+
+struct TransportParamsU {
+  TransportParams base;          // rho / tally / trow are in STORAGE order here
+  const int* __restrict__ lut;   // [6][N] slot deltas: (axis, forward) at (2*axis)*N, reversed at (2*axis+1)*N
+  LayoutU lay;
+  int quorum;                    // leave the walk loop when fewer lanes than this are walking
+};
+
+constexpr int kLutEscape = INT_MIN;
+
+// SU_INTERACT_B: interaction found in the second step of a pair -> the cell's density is in the
+// alternate register (moved back in the event pass, never inside the walk loop where the move
+// would wait for the gather in flight).
+enum : int { SU_WALK = 0, SU_INTERACT = 1, SU_ESCAPE = 2, SU_FETCH = 3, SU_DONE = 4, SU_INTERACT_B = 5 };
+
+struct PacketU {
+  float d0, d1, d2;          // direction
+  float t0, t1, t2;          // path length (cell edges) at which the next face on each axis is met
+  float dt0, dt1, dt2;       // 1/|d_a|
+  float tcur, tau_rem, rho;  // path length so far in this flight; optical depth left; density here
+  uint32_t p0, p1, p2;       // cursors into the delta tables (shared-memory byte addresses)
+  int slot;                  // storage slot of the current cell
+  int cb;                    // bin | component << 16 (component: 0 direct, 1 scattered, 2 thermal)
+  uint32_t k;                // flight number
+  uint32_t off;              // package number within the batch: pid = first + off
+  float u1, u2, u3;          // uniforms of the current flight kept for the interaction
+};
+
+// Start a flight of a package sitting in cell (ix,iy,iz) at cell-local position (ux,uy,uz) with
+// direction (a,b,c): cursors, face path lengths, tcur = 0.
+__device__ __forceinline__ void begin_flight(PacketU& p, uint32_t lut, int N, int ix, int iy, int iz,
+                                             float ux, float uy, float uz, float a, float b, float c) {
+  if (fabsf(a) < 1e-12f) a = copysignf(1e-12f, a);          // G1: never the exit axis
+  if (fabsf(b) < 1e-12f) b = copysignf(1e-12f, b);
+  if (fabsf(c) < 1e-12f) c = copysignf(1e-12f, c);
+  p.d0 = a; p.d1 = b; p.d2 = c;
+  p.dt0 = __frcp_rn(fabsf(a)); p.dt1 = __frcp_rn(fabsf(b)); p.dt2 = __frcp_rn(fabsf(c));
+  p.t0 = (a > 0.f ? 1.f - ux : ux) * p.dt0;
+  p.t1 = (b > 0.f ? 1.f - uy : uy) * p.dt1;
+  p.t2 = (c > 0.f ? 1.f - uz : uz) * p.dt2;
+  p.p0 = lut + 4u * (uint32_t)(a > 0.f ? ix : 2 * N - 1 - ix);            // reversed table: entry N-1-i
+  p.p1 = lut + 4u * (uint32_t)(2 * N + (b > 0.f ? iy : 2 * N - 1 - iy));
+  p.p2 = lut + 4u * (uint32_t)(4 * N + (c > 0.f ? iz : 2 * N - 1 - iz));
+  p.tcur = 0.f;
+}
+// cell coordinates back from the cursors
+__device__ __forceinline__ void cell_of(const PacketU& p, uint32_t lut, int N, int& ix, int& iy, int& iz) {
+  int q0 = (int)((p.p0 - lut) >> 2), q1 = (int)((p.p1 - lut) >> 2) - 2 * N, q2 = (int)((p.p2 - lut) >> 2) - 4 * N;
+  ix = p.d0 > 0.f ? q0 : 2 * N - 1 - q0;
+  iy = p.d1 > 0.f ? q1 : 2 * N - 1 - q1;
+  iz = p.d2 > 0.f ? q2 : 2 * N - 1 - q2;
+}
+
+
+// O4 for a single-level grid: cell, cell-local position and (external field only) direction of
+// a new package.  r = Philox block (pid, 0, EMIT); iso = isotropic direction from (r2, r3).
+__device__ __forceinline__ int lds_s32(uint32_t addr) {
+  int v;
+  asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+
+// One crossing of the cell walk (O5).  `cur` holds the density of the current cell; the density
+// of the next cell is requested into `nxt` BEFORE the optical-depth test, so consecutive calls
+// alternate the two registers and no instruction waits on the gather except its real use.
+__device__ __forceinline__ void walk_step_u(const float* __restrict__ rho, PacketU& p, float& cur,
+                                            float& nxt, float kx, int& state, uint32_t& crossings) {
+  const float tnext = fminf(p.t0, fminf(p.t1, p.t2));
+  const bool a0 = p.t0 == tnext;                             // ties -> lowest axis (R21)
+  const bool a1 = !a0 && p.t1 == tnext;
+  const int dl = lds_s32(a0 ? p.p0 : (a1 ? p.p1 : p.p2));
+  const bool esc = dl == kLutEscape;
+  const int nslot = p.slot + dl;
+  if (!esc) nxt = __ldg(rho + nslot);
+  const float dtau = cur * kx * (tnext - p.tcur);
+  if (dtau >= p.tau_rem) {                                   // interaction inside this cell
+    state = SU_INTERACT;
+  } else {
+    p.tau_rem -= dtau;
+    p.tcur = tnext;
+    if (a0) { p.t0 += p.dt0; p.p0 += 4u; } else if (a1) { p.t1 += p.dt1; p.p1 += 4u; } else { p.t2 += p.dt2; p.p2 += 4u; }
+    ++crossings;
+    p.slot = nslot;
+    if (esc) state = SU_ESCAPE;
+  }
+}
+
+__device__ __forceinline__ void emit_position_u(const TransportParams& P, const SrcDev& sd,
+                                                unsigned long long pid, const float r[4], int& ix,
+                                                int& iy, int& iz, float& ux, float& uy, float& uz,
+                                                float& a, float& b, float& c) {
+  const int N = P.N;
+  if (sd.type == 0) {
+    ix = sd.fine[0]; iy = sd.fine[1]; iz = sd.fine[2];
+    ux = sd.frac[0]; uy = sd.frac[1]; uz = sd.frac[2];
+    if (a < 0.f && ux == 0.f) { --ix; ux = 1.f; }             // R7: ceil(x) - 1 for d < 0
+    if (b < 0.f && uy == 0.f) { --iy; uy = 1.f; }
+    if (c < 0.f && uz == 0.f) { --iz; uz = 1.f; }
+  } else {                                                    // R25 external isotropic field
+    float v[4];
+    draw4(P.seed, pid, 1, kTagEmit, v);
+    int f = min(5, (int)(6.f * v[0]));
+    int ax = f >> 1, side = f & 1;
+    float mu = sqrtf(r[2]);
+    float st = sqrtf(fmaxf(0.f, 1.f - mu * mu));
+    float sn, cs;
+    sincospif(2.f * r[3], &sn, &cs);
+    float dn = side == 0 ? mu : -mu, e1 = st * cs, e2 = st * sn;     // normal, axis+1, axis+2
+    float fN = (float)N;
+    float x1 = v[1] * fN, x2 = v[2] * fN;
+    int i1 = min(N - 1, (int)x1), i2 = min(N - 1, (int)x2);
+    float l1 = x1 - (float)i1, l2 = x2 - (float)i2;
+    if (e1 < 0.f && l1 == 0.f && i1 > 0) { --i1; l1 = 1.f; }
+    if (e2 < 0.f && l2 == 0.f && i2 > 0) { --i2; l2 = 1.f; }
+    int in = side == 0 ? 0 : N - 1;
+    float ln = side == 0 ? 0.f : 1.f;
+    if (ax == 0)      { a = dn; b = e1; c = e2; ix = in; iy = i1; iz = i2; ux = ln; uy = l1; uz = l2; }
+    else if (ax == 1) { a = e2; b = dn; c = e1; iy = in; iz = i1; ix = i2; uy = ln; uz = l1; ux = l2; }
+    else              { a = e1; b = e2; c = dn; iz = in; ix = i1; iy = i2; uz = ln; ux = l1; uy = l2; }
+  }
+}
+
+__global__ void __launch_bounds__(256, 4) k_transport_u(const TransportParamsU PU) {
+  const TransportParams& P = PU.base;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float4* s_opac = reinterpret_cast<float4*>(smem_raw);                    // [nb]
+  uint32_t* s_sed = reinterpret_cast<uint32_t*>(s_opac + P.nb);             // [3*nb]
+  uint32_t* s_emit = s_sed + 3 * P.nb;                                      // [nb]
+  int* s_lut = reinterpret_cast<int*>(s_emit + P.nb);                       // [6*N]
+  const uint32_t lut = (uint32_t)__cvta_generic_to_shared(s_lut);
+  const int N = P.N;
+  for (int i = threadIdx.x; i < P.nb; i += blockDim.x) { s_opac[i] = P.opac[i]; s_emit[i] = 0; }
+  for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x) s_sed[i] = 0;
+  for (int i = threadIdx.x; i < 6 * N; i += blockDim.x) s_lut[i] = PU.lut[i];
+  __syncthreads();
+
+  const unsigned lane = threadIdx.x & 31;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  // event counters kept per lane: crossings, absorptions, scatterings, flights.  Emitted and
+  // escaped packages are counted by the block's emission / SED histograms (summed at the end),
+  // lost packages (R20, must never happen) go straight to the global counter.
+  uint32_t n_cross = 0, n_abs = 0, n_sca = 0, n_flights = 0;
+
+  PacketU p;
+  p.d0 = p.d1 = p.d2 = 1.f; p.t0 = p.t1 = p.t2 = 0.f; p.dt0 = p.dt1 = p.dt2 = 1.f;
+  p.tcur = 0.f; p.tau_rem = 1.f; p.rho = 0.f; p.p0 = p.p1 = p.p2 = lut; p.slot = 0;
+  float rho_b = 0.f;                                         // the walk alternates p.rho / rho_b
+  p.cb = 0; p.k = 0; p.off = 0; p.u1 = p.u2 = p.u3 = 0.f;
+  float kx = 0.f;
+  int state = SU_FETCH;
+  int quorum = PU.quorum;
+
+  for (;;) {
+    // ---- a7: escaped packages -> SED; a8: refill from the work queue (one atomic per warp) ----
+    if (state == SU_ESCAPE) {
+      atomicAdd(&s_sed[(p.cb >> 16) * P.nb + (p.cb & 0xffff)], 1u);
+      state = SU_FETCH;
+    }
+    bool is_new = false;
+    const unsigned need = __ballot_sync(kFull, state == SU_FETCH);
+    if (need) {
+      unsigned long long base = 0;
+      if (lane == 0) base = atomicAdd(P.next, (unsigned long long)__popc(need));
+      base = __shfl_sync(kFull, base, 0);
+      if (base + 32ull > P.count) quorum = 1;                // queue (nearly) empty: no more refills
+      if (state == SU_FETCH) {
+        unsigned long long my = base + (unsigned long long)__popc(need & lt_mask);
+        if (my < P.count) { p.off = (uint32_t)my; is_new = true; }
+        else state = SU_DONE;
+      }
+    }
+    if (__all_sync(kFull, state == SU_DONE)) break;
+
+    // ---- one event pass for every lane that is not walking ----
+    if (is_new || state == SU_INTERACT || state == SU_INTERACT_B) {
+      if (state == SU_INTERACT_B) p.rho = rho_b;
+      const unsigned long long pid = P.first + p.off;
+      int bin = p.cb & 0xffff, comp = p.cb >> 16;
+      int ix = 0, iy = 0, iz = 0;
+      float ux = 0.f, uy = 0.f, uz = 0.f, a, b, c;
+      bool scatter = false;
+      if (!is_new) {                                         // where the interaction happened
+        cell_of(p, lut, N, ix, iy, iz);
+        // the interaction lies tau_rem / (rho kappa) further along this cell's segment
+        const float seg = fminf(p.t0, fminf(p.t1, p.t2)) - p.tcur;
+        const float ti = p.tcur + fminf(seg, p.tau_rem / (p.rho * kx));
+        float w0 = fminf(1.f, fmaxf(0.f, (p.t0 - ti) * fabsf(p.d0)));
+        float w1 = fminf(1.f, fmaxf(0.f, (p.t1 - ti) * fabsf(p.d1)));
+        float w2 = fminf(1.f, fmaxf(0.f, (p.t2 - ti) * fabsf(p.d2)));
+        ux = p.d0 > 0.f ? 1.f - w0 : w0;
+        uy = p.d1 > 0.f ? 1.f - w1 : w1;
+        uz = p.d2 > 0.f ? 1.f - w2 : w2;
+        scatter = p.u1 < s_opac[bin].y;                      // a4 (R16)
+      }
+      if (scatter) {                                         // a5
+        ++n_sca;
+        float ct = hg_cos(s_opac[bin].z, p.u2);
+        rotate_dir(p.d0, p.d1, p.d2, ct, p.u3, a, b, c);
+        if (comp == 0) comp = 1;
+        ++p.k;
+      } else {                                               // a1 emission / a6 absorption + re-emission
+        float r[4];
+        draw4(P.seed, pid, is_new ? 0u : p.k, is_new ? kTagEmit : kTagReemit, r);
+        const float* row;
+        float us;
+        int s = 0;
+        if (is_new) {
+          while (s < P.nsrc - 1 && P.src[s].lcdf < r[0]) ++s;
+          row = P.csrc + (size_t)s * P.nb;
+          us = r[1];
+        } else {
+          ++n_abs;
+          // warp-aggregated integer tally: one atomic per distinct cell per warp
+          unsigned peers = __match_any_sync(__activemask(), p.slot);
+          if ((int)lane == __ffs(peers) - 1)
+            atomicAdd(P.tally + p.slot, (unsigned long long)__popc(peers));
+          float tr = __ldg(P.trow + p.slot);                 // T frozen = T before absorption
+          int k0 = min(P.nT - 1, (int)tr);
+          float w = tr - (float)k0;
+          int rw = (r[1] < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
+          row = P.cdf + (size_t)rw * P.nb;
+          us = r[0];
+        }
+        bin = search_cdf(row, P.nb, us);
+        kx = s_opac[bin].x;
+        isotropic_dir(r[2], r[3], a, b, c);
+        if (is_new) {
+          emit_position_u(P, P.src[s], pid, r, ix, iy, iz, ux, uy, uz, a, b, c);
+          p.slot = (int)slot_of(PU.lay, ix, iy, iz);
+          p.rho = __ldg(P.rho + p.slot);
+          comp = 0; p.k = 0;
+          atomicAdd(&s_emit[bin], 1u);
+        } else {
+          comp = 2;
+          ++p.k;
+        }
+      }
+      // ---- a2: next flight ----
+      p.cb = bin | (comp << 16);
+      if (p.k >= kMaxFlights) {                              // R20
+        atomicAdd(P.counters + CNT_LOST, 1ull);
+        state = SU_FETCH;
+      } else {
+        begin_flight(p, lut, N, ix, iy, iz, ux, uy, uz, a, b, c);
+        float u[4];
+        draw4(P.seed, pid, p.k, kTagFlight, u);
+        p.tau_rem = -logf(u[0]);
+        p.u1 = u[1]; p.u2 = u[2]; p.u3 = u[3];
+        ++n_flights;
+        state = SU_WALK;
+      }
+    }
+
+    // ---- a3: cell walk until fewer than `quorum` lanes are walking ----
+#pragma unroll 1
+    for (;;) {
+      if (state == SU_WALK) walk_step_u(P.rho, p, p.rho, rho_b, kx, state, n_cross);
+      if (state == SU_WALK) {
+        walk_step_u(P.rho, p, rho_b, p.rho, kx, state, n_cross);
+        if (state == SU_INTERACT) state = SU_INTERACT_B;
+      }
+      if (__popc(__ballot_sync(kFull, state == SU_WALK)) < quorum) break;
+    }
+  }
+
+  // ---- flush block-private tallies ----
+  {
+    const int which[4] = {CNT_CROSS, CNT_ABS, CNT_SCA, CNT_FLIGHTS};
+    const uint32_t val[4] = {n_cross, n_abs, n_sca, n_flights};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      unsigned long long v = val[i];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+      if (lane == 0 && v) atomicAdd(P.counters + which[i], v);
+    }
+  }
+  __syncthreads();
+  unsigned long long esc = 0, emi = 0;
+  for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x)
+    if (s_sed[i]) { atomicAdd(P.sed + i, (unsigned long long)s_sed[i]); esc += s_sed[i]; }
+  for (int i = threadIdx.x; i < P.nb; i += blockDim.x)
+    if (s_emit[i]) { atomicAdd(P.emit_bin + i, (unsigned long long)s_emit[i]); emi += s_emit[i]; }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    esc += __shfl_xor_sync(kFull, esc, o);
+    emi += __shfl_xor_sync(kFull, emi, o);
+  }
+  if (lane == 0 && esc) atomicAdd(P.counters + CNT_ESCAPED, esc);
+  if (lane == 0 && emi) atomicAdd(P.counters + CNT_EMITTED, emi);
+}
+
+// ---- layout conversion (set-up and read-out; storage order never shows at the C ABI, R22) ----
+// x-fastest caller densities -> storage order (negative / NaN -> 0; padding slots stay 0)
+__global__ void k_encode_uniform(const float* __restrict__ rho_ext, float* __restrict__ rho_store,
+                                 LayoutU lay, long long n3) {
+  long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n3) return;
+  int ix = (int)(e % lay.N), iy = (int)((e / lay.N) % lay.N), iz = (int)(e / ((long long)lay.N * lay.N));
+  float v = rho_ext[e];
+  rho_store[slot_of(lay, ix, iy, iz)] = (v > 0.f) ? v : 0.f;
+}
+// storage order -> x-fastest output
+template <typename T>
+__global__ void k_store_to_ext(const T* __restrict__ store, T* __restrict__ ext, LayoutU lay, long long n3) {
+  long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n3) return;
+  int ix = (int)(e % lay.N), iy = (int)((e / lay.N) % lay.N), iz = (int)(e / ((long long)lay.N * lay.N));
+  ext[e] = store[slot_of(lay, ix, iy, iz)];
+}
+__global__ void k_trow_to_T_u(const float* __restrict__ trow_store, float* __restrict__ T_ext, LayoutU lay,
+                              long long n3, float lnTmin, float dlnT) {
+  long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n3) return;
+  int ix = (int)(e % lay.N), iy = (int)((e / lay.N) % lay.N), iz = (int)(e / ((long long)lay.N * lay.N));
+  T_ext[e] = expf(lnTmin + dlnT * trow_store[slot_of(lay, ix, iy, iz)]);
+}
+// x-fastest tally (sum over ranks, as read out by mcrt_get_cell_energy) -> storage order
+__global__ void k_ext_to_store_u64(const unsigned long long* __restrict__ ext, unsigned long long* __restrict__ store,
+                                   LayoutU lay, long long n3) {
+  long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n3) return;
+  int ix = (int)(e % lay.N), iy = (int)((e / lay.N) % lay.N), iz = (int)(e / ((long long)lay.N * lay.N));
+  store[slot_of(lay, ix, iy, iz)] = ext[e];
+}
+
+}  // namespace mcrt

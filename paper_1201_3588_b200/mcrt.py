@@ -22,7 +22,7 @@ class McrtError(RuntimeError):
 class _GridDesc(C.Structure):
     _fields_ = [("n_root", C.c_int32), ("sub", C.c_int32), ("origin", C.c_double * 3),
                 ("root_size", C.c_double), ("refine", C.c_void_p), ("rho_root", C.c_void_p),
-                ("rho_sub", C.c_void_p), ("mem", C.c_int)]
+                ("rho_sub", C.c_void_p), ("mem", C.c_int), ("layout", C.c_int32)]
 
 
 class _OpacityDesc(C.Structure):
@@ -47,7 +47,8 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_set_source", "mcrt_run_batch", "mcrt_transport_batch",
            "mcrt_update_temperature", "mcrt_get_cell_energy",
            "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_get_counters",
-           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_get_batch_times", "mcrt_get_tables",
+           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum",
+           "mcrt_get_batch_times", "mcrt_get_tables",
            "mcrt_kernel_launches", "mcrt_philox_blocks", "mcrt_last_error")
 
 
@@ -76,6 +77,7 @@ def lib():
         L.mcrt_get_counters.argtypes = [vp, C.POINTER(_Counters), vp]
         L.mcrt_reset_tallies.argtypes = [vp, i32]
         L.mcrt_set_launch.argtypes = [vp, i32, i32]
+        L.mcrt_set_walk_quorum.argtypes = [vp, i32]
         L.mcrt_get_batch_times.argtypes = [vp, vp, vp, i32, C.POINTER(i32)]
         L.mcrt_get_tables.argtypes = [vp, vp, vp, vp]
         L.mcrt_kernel_launches.restype = i64
@@ -87,7 +89,8 @@ def lib():
                      "mcrt_run_batch", "mcrt_transport_batch", "mcrt_update_temperature",
                      "mcrt_get_cell_energy", "mcrt_get_cell_temperature",
                      "mcrt_get_sed", "mcrt_get_counters", "mcrt_reset_tallies",
-                     "mcrt_set_launch", "mcrt_get_batch_times", "mcrt_get_tables",
+                     "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_get_batch_times",
+                     "mcrt_get_tables",
                      "mcrt_philox_blocks"):
             getattr(L, name).restype = C.c_int
         _lib = L
@@ -120,10 +123,11 @@ class Context:
             raise McrtError(f"{what}: status {rc}: {msg.decode() if msg else ''}")
 
     # -- set-up ---------------------------------------------------------------------------
-    def grid_create(self, n_root, sub, origin, root_size, refine, rho_root, rho_sub):
+    def grid_create(self, n_root, sub, origin, root_size, refine, rho_root, rho_sub, layout=0):
         L = lib()
         d = _GridDesc()
         d.n_root, d.sub = int(n_root), int(sub)
+        d.layout = int(layout)
         d.origin = (C.c_double * 3)(*[float(v) for v in origin])
         d.root_size = float(root_size)
         if _is_tensor(rho_root):
@@ -251,6 +255,9 @@ class Context:
         self._check(lib().mcrt_set_launch(self.h, threads_per_block, blocks_per_sm),
                     "mcrt_set_launch")
 
+    def set_walk_quorum(self, quorum):
+        self._check(lib().mcrt_set_walk_quorum(self.h, int(quorum)), "mcrt_set_walk_quorum")
+
     def get_batch_times(self, cap=4096):
         t = np.zeros(cap, dtype=np.float32)
         u = np.zeros(cap, dtype=np.float32)
@@ -282,7 +289,7 @@ class Context:
             pass
 
 
-def from_workload(wl, device_inputs=False, n_T=0, T_min=0.0, T_max=0.0) -> Context:
+def from_workload(wl, device_inputs=False, n_T=0, T_min=0.0, T_max=0.0, layout=0) -> Context:
     """grid_create -> set_opacity -> set_source for a workloads.Workload."""
     ctx = Context()
     refine, rho_root, rho_sub = wl.refine, wl.rho_root, wl.rho_sub
@@ -291,7 +298,8 @@ def from_workload(wl, device_inputs=False, n_T=0, T_min=0.0, T_max=0.0) -> Conte
         rho_root = torch.from_numpy(np.ascontiguousarray(rho_root)).cuda()
         refine = None if refine is None else torch.from_numpy(np.ascontiguousarray(refine)).cuda()
         rho_sub = None if rho_sub is None else torch.from_numpy(np.ascontiguousarray(rho_sub)).cuda()
-    ctx.grid_create(wl.n_root, wl.sub, wl.origin, wl.root_size, refine, rho_root, rho_sub)
+    ctx.grid_create(wl.n_root, wl.sub, wl.origin, wl.root_size, refine, rho_root, rho_sub,
+                    layout)
     ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g, T_min, T_max, n_T)
     ctx.set_source(wl.sources)
     return ctx

@@ -258,3 +258,63 @@ def test_reset_tallies(M):
     for f, c in wl.batches(20_000, 10_000):
         ctx.run_batch(wl.seed, f, c)
     assert np.array_equal(ctx.get_sed(), first)
+
+
+# ---- storage layouts of single-level grids (never visible in the getters, R22) ----------------
+def _run_layout(M, wl, layout, quorum=0, n_packets=None, batch=None):
+    ctx = M.from_workload(wl, layout=layout)
+    if quorum:
+        ctx.set_walk_quorum(quorum)
+    for first, cnt in wl.batches(n_packets, batch):
+        ctx.run_batch(wl.seed, first, cnt)
+    return ctx
+
+
+def _assert_identical(a, b):
+    assert np.array_equal(a.get_cell_energy()[0], b.get_cell_energy()[0])
+    assert np.array_equal(a.get_sed(), b.get_sed())
+    assert np.array_equal(a.get_cell_temperature(), b.get_cell_temperature())
+    ca, cb = a.get_counters(), b.get_counters()
+    for k in ca:
+        assert np.array_equal(ca[k], cb[k]), k
+
+
+@pytest.mark.parametrize("maker", [
+    lambda: W.c0(),
+    lambda: W.tiny_random(n_root=3, seed=4, external=True, n_packets=40_000, batch=10_000),
+    lambda: W.tiny_random(n_root=13, seed=5, external=True, tau_cell=0.2, n_packets=60_000,
+                          batch=20_000),
+    lambda: W.c4(n_root=24, n_packets=60_000, batch=20_000, corr_cells=3.0)])
+def test_bricked_layout_bit_identical_to_x_fastest(M, maker):
+    """Same walk, same Philox slots, integer tallies: the storage order (x-fastest vs 8^3 Morton
+    bricks, with padding when N is not a multiple of 8) must not change a single count."""
+    wl = maker()
+    a = _run_layout(M, wl, 1)
+    b = _run_layout(M, wl, 2)
+    _assert_identical(a, b)
+    assert a.get_counters()["emitted"] == wl.n_packets
+
+
+def test_walk_quorum_does_not_change_results(M):
+    wl = W.c4(n_root=24, n_packets=60_000, batch=20_000, corr_cells=3.0)
+    a = _run_layout(M, wl, 0, quorum=1)
+    b = _run_layout(M, wl, 0, quorum=32)
+    c = _run_layout(M, wl, 2, quorum=8)
+    _assert_identical(a, b)
+    _assert_identical(a, c)
+
+
+@pytest.mark.parametrize("layout", [1, 2])
+def test_split_batch_halves_equal_run_batch(M, layout):
+    """transport_batch + update_temperature(sum in slot order) == run_batch (multi-GPU path,
+    DESIGN.md section 12), for both storage layouts."""
+    wl = W.tiny_random(n_root=13, seed=6, tau_cell=0.3, n_packets=40_000, batch=10_000)
+    a = _run_layout(M, wl, layout)
+    b = M.from_workload(wl, layout=layout)
+    done = 0
+    for first, cnt in wl.batches():
+        b.transport_batch(wl.seed, first, cnt)
+        tally, _ = b.get_cell_energy(device=True)
+        done += cnt
+        b.update_temperature(tally, done)
+    _assert_identical(a, b)
