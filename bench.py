@@ -319,6 +319,14 @@ def run_gpu(args, wl, name):
     if not args.no_e2e:
         e2e = run_e2e(args, wl, mcrt, torch, dist, rank, world, stream)
 
+    # ---- gather roofline: independent 4-byte gathers over the density
+    # footprint of this workload, measured live by the library's calibration kernel ----------
+    gather = None
+    if rank == 0 and not args.no_gather:
+        foot = int(wl.leaf_slots) * 4
+        g_peak, g_sec = mcrt.gather_calibrate(foot, 1 << 31, stream)
+        gather = {"footprint_bytes": foot, "peak_gathers_per_s": g_peak, "calibration_s": g_sec}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -350,6 +358,14 @@ def run_gpu(args, wl, name):
                         "kernel_ms": 1e3 * tr_s / args.steps,
                         "kernel_share_of_step": tr_s / (float(sum(step_ms)) * 1e-3)},
            "gpu_launches": launches, "clocks": clocks}
+    if gather is not None:
+        # one density gather per crossing: crossings/s of the transport kernel alone vs the peak
+        gather["achieved_gathers_per_s"] = d["crossings"] / tr_s if tr_s > 0 else 0.0
+        gather["frac"] = gather["achieved_gathers_per_s"] / gather["peak_gathers_per_s"]
+        gather["what"] = ("peak = independent hash-indexed 4-byte gathers/s over an array of the "
+                          "density footprint at full occupancy (mcrt_gather_calibrate); achieved = "
+                          "cell crossings per second of k_transport on this rank")
+        out["gather_roofline"] = gather
     if e2e is not None:
         out["e2e"] = e2e
     if not args.no_cpu and world >= 1:
@@ -421,6 +437,7 @@ def main():
     ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 x-fastest, 2 bricked")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-gather", action="store_true", help="skip the gather-roofline calibration")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "native" else args.warmup

@@ -167,6 +167,16 @@ mcrt_status mcrt_get_counters(mcrt_ctx* ctx, mcrt_counters* out, uint64_t* emitt
 /* what: bit 0 = SED + counters, bit 1 = cell energy + temperatures + N_cum. */
 mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what);
 
+/* Gather-roofline calibration (BASELINE.json metric "% of gather-BW roofline"; SURVEY.md 8(d)
+ * item (iv)): times at least `n_gathers` independent, hash-indexed 4-byte gathers over a
+ * zero-filled device array of `footprint_bytes` (4 B .. 16 GiB; allocated and freed inside the
+ * call) at full occupancy on the current device and returns gathers per second (and the timed
+ * seconds if `seconds` is not NULL).  Host output pointers.  It is the ceiling for a cell walk
+ * in which every crossing costs one density gather and nothing else; the transport kernels'
+ * crossings per second are reported against it by bench.py. */
+mcrt_status mcrt_gather_calibrate(uint64_t footprint_bytes, uint64_t n_gathers, double* gathers_per_s,
+                                  double* seconds, void* cuda_stream);
+
 /* ---- tuning and introspection (do not change results) ---------------------------------------
  * Launch shape of the transport kernel: threads per block (multiple of 32, <= 1024) and resident
  * blocks per SM; 0 keeps the default. */

@@ -13,6 +13,7 @@
 
 #include <cuda_runtime.h>
 
+#include "calibrate.cuh"
 #include "tables.cuh"
 #include "transport.cuh"
 #include "transport_u.cuh"
@@ -602,6 +603,42 @@ mcrt_status mcrt_philox_blocks(const uint32_t* key2, const uint32_t* ctr, uint32
   k_philox_blocks<<<(unsigned)((n + 255) / 256), 256>>>(key2[0], key2[1], d_c, d_o, n);
   CU(cudaGetLastError());
   CU(cudaMemcpy(out, d_o, 16 * (size_t)n, cudaMemcpyDeviceToHost));
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_gather_calibrate(uint64_t footprint_bytes, uint64_t n_gathers, double* gathers_per_s,
+                                  double* seconds, void* stream_) {
+  mcrt_ctx* ctx = nullptr;
+  if (!gathers_per_s || footprint_bytes < 4 || footprint_bytes > (16ull << 30) || n_gathers == 0)
+    return fail(nullptr, MCRT_EINVAL, "mcrt_gather_calibrate: bad arguments (footprint 4 B .. 16 GiB, n_gathers > 0)");
+  int dev = 0, sms = 0;
+  CU(cudaGetDevice(&dev));
+  CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  cudaStream_t st = (cudaStream_t)stream_;
+  const uint32_t n_elems = (uint32_t)(footprint_bytes / 4);
+  float *d_a = nullptr, *d_sink = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  struct Tmp { float*& a; float*& b; cudaEvent_t& e0; cudaEvent_t& e1;
+               ~Tmp() { cudaFree(a); cudaFree(b); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); } } tmp{d_a, d_sink, e0, e1};
+  CU(cudaMalloc(&d_a, 4 * (size_t)n_elems));
+  CU(cudaMalloc(&d_sink, 4));
+  CU(cudaMemsetAsync(d_a, 0, 4 * (size_t)n_elems, st));
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  const unsigned blocks = (unsigned)sms * 8u, threads = 256u;
+  const uint64_t per_turn = 4ull * blocks * threads;
+  uint32_t turns = (uint32_t)((n_gathers + per_turn - 1) / per_turn);
+  if (turns < 1) turns = 1;
+  k_gather_calibrate<<<blocks, threads, 0, st>>>(d_a, n_elems, turns < 16 ? turns : 16, d_sink);   // warm-up
+  CU(cudaEventRecord(e0, st));
+  k_gather_calibrate<<<blocks, threads, 0, st>>>(d_a, n_elems, turns, d_sink);
+  CU(cudaEventRecord(e1, st));
+  CU(cudaGetLastError());
+  CU(cudaEventSynchronize(e1));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  const double sec = (double)ms * 1e-3;
+  *gathers_per_s = sec > 0 ? (double)turns * (double)per_turn / sec : 0.0;
+  if (seconds) *seconds = sec;
   return MCRT_OK;
 }
 

@@ -49,7 +49,7 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum",
            "mcrt_get_batch_times", "mcrt_get_tables",
-           "mcrt_kernel_launches", "mcrt_philox_blocks", "mcrt_last_error")
+           "mcrt_kernel_launches", "mcrt_philox_blocks", "mcrt_gather_calibrate", "mcrt_last_error")
 
 
 def lib():
@@ -83,6 +83,8 @@ def lib():
         L.mcrt_kernel_launches.restype = i64
         L.mcrt_kernel_launches.argtypes = [vp]
         L.mcrt_philox_blocks.argtypes = [vp, vp, vp, i64]
+        L.mcrt_gather_calibrate.argtypes = [u64, u64, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+        L.mcrt_gather_calibrate.restype = C.c_int
         L.mcrt_last_error.restype = C.c_char_p
         L.mcrt_last_error.argtypes = [vp]
         for name in ("mcrt_grid_create", "mcrt_destroy", "mcrt_set_opacity", "mcrt_set_source",
@@ -320,3 +322,16 @@ def philox_blocks(key2, ctr):
     if rc != 0:
         raise McrtError(f"mcrt_philox_blocks: status {rc}: {lib().mcrt_last_error(None).decode()}")
     return o
+
+
+def gather_calibrate(footprint_bytes, n_gathers=1 << 30, stream=None):
+    """Independent 4-byte gathers per second over an array of `footprint_bytes` (gather roofline)."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    g, sec = C.c_double(0), C.c_double(0)
+    rc = lib().mcrt_gather_calibrate(int(footprint_bytes), int(n_gathers), C.byref(g), C.byref(sec),
+                                     C.c_void_p(stream))
+    if rc != 0:
+        raise McrtError(f"mcrt_gather_calibrate: status {rc}: {lib().mcrt_last_error(None).decode()}")
+    return g.value, sec.value

@@ -318,3 +318,13 @@ def test_split_batch_halves_equal_run_batch(M, layout):
         done += cnt
         b.update_temperature(tally, done)
     _assert_identical(a, b)
+
+
+def test_gather_calibration_orders_by_footprint(M):
+    """The gather-roofline calibration returns a finite rate that falls as the footprint leaves
+    the caches (16 KB: L1; 64 MB: L2; 1 GB: HBM)."""
+    g = [M.gather_calibrate(fb, 1 << 28)[0] for fb in (16 << 10, 64 << 20, 1 << 30)]
+    assert all(np.isfinite(v) and v > 1e9 for v in g), g
+    assert g[0] > g[1] > g[2], g
+    with pytest.raises(M.McrtError):
+        M.gather_calibrate(0, 10)
