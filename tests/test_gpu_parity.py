@@ -328,3 +328,67 @@ def test_gather_calibration_orders_by_footprint(M):
     assert g[0] > g[1] > g[2], g
     with pytest.raises(M.McrtError):
         M.gather_calibrate(0, 10)
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times -------------------
+def _temperature_identity(M, ctx, wl, n_cum, sample=20000):
+    """4 pi m Q(T) N_cum / (cum L_tot) = 1 on sampled cells that are neither empty nor clamped
+    (O7; Q from the library's own ln Q table, interpolated as the update kernel does)."""
+    n_abs, eps = ctx.get_cell_energy()
+    T = ctx.get_cell_temperature().astype(np.float64)
+    _, lnQ, _ = ctx.get_tables()
+    lnQ = lnQ.astype(np.float64)
+    nT = len(lnQ)
+    rho = np.asarray(wl.rho_root, dtype=np.float64).ravel()
+    idx = np.flatnonzero((n_abs > 0) & (rho > 0))
+    rng = np.random.default_rng(3)
+    idx = rng.choice(idx, size=min(sample, len(idx)), replace=False)
+    t = np.log(T[idx]) / (np.log(1.0e4) / (nT - 1))          # row coordinate on the default T grid
+    ok = (t > 0.5) & (t < nT - 1.5)
+    idx, t = idx[ok], t[ok]
+    k = np.floor(t).astype(int)
+    lnq_T = lnQ[k] + (t - k) * (lnQ[k + 1] - lnQ[k])
+    Ltot = sum(s.L for s in wl.sources)
+    lnq = np.log(n_abs[idx].astype(np.float64)) + np.log(Ltot / (n_cum * 4 * np.pi * wl.root_size ** 3)) \
+        - np.log(rho[idx])
+    assert len(idx) > 100
+    assert np.abs(lnq_T - lnq).max() < 2e-3, np.abs(lnq_T - lnq).max()
+    assert eps == pytest.approx(Ltot / n_cum, rel=1e-12)
+
+
+def test_c1_full_batch_against_oracle(M, oracle_mod):
+    """One full 2^20-package batch of configs[1] (tau_V = 1) in bench.py's launch configuration:
+    the oracle runs the same batch; then a second batch for the temperature identity."""
+    wl = W.c1(tau_v=1.0)
+    n = wl.batch
+    assert n == 1 << 20
+    ctx = M.from_workload(wl)
+    ctx.run_batch(wl.seed, 0, n)
+    orc = oracle_mod.Oracle(wl)
+    orc.run_batch(wl.seed, 0, n)
+    cg, co = _compare(ctx, orc, groups=PR.radial_shells(64, 32))
+    assert cg["emitted"] == n
+    ctx.run_batch(wl.seed, n, n)
+    _temperature_identity(M, ctx, wl, 2 * n)
+
+
+def test_c4_full_grid_against_oracle(M, oracle_mod):
+    """configs[4]'s full 512^3 clumpy cube (bricked storage, 11 sources): 2^21 packages on both
+    sides compared by 8^3 super-blocks; then invariants on a second, 2^22-package batch."""
+    wl = W.c4()
+    assert wl.n_root == 512
+    n = 1 << 21
+    ctx = M.from_workload(wl)
+    ctx.run_batch(wl.seed, 0, n)
+    orc = oracle_mod.Oracle(wl)
+    orc.run_batch(wl.seed, 0, n)
+    _compare(ctx, orc, groups=PR.super_blocks(512, 8), expect_cells=True)
+    del orc
+    m = 1 << 22
+    ctx.run_batch(wl.seed, n, m)
+    c = ctx.get_counters()
+    n_abs, _ = ctx.get_cell_energy()
+    sed = ctx.get_sed()
+    assert c["emitted"] == c["escaped"] == n + m and c["lost"] == 0
+    PR.check_self_consistency(c, n_abs, sed)
+    _temperature_identity(M, ctx, wl, n + m)
