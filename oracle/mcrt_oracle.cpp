@@ -147,6 +147,11 @@ struct Ctx {
   std::vector<uint64_t> cum; std::vector<double> T; uint64_t Ncum = 0;
   std::vector<uint64_t> sed, emitted_per_bin; Counters cnt{};
   int walker = 0;                       // 0 = cell walk (O5), 1 = brute force (tests)
+  // O9 observer (reading R34): escape-direction binning
+  int n_mu = 0; std::vector<uint64_t> sed_mu;               // [n_mu][3][nb]
+  int n_pix = 0; double obs[3] = {0, 0, 1}, e1[3] = {1, 0, 0}, e2[3] = {0, 1, 0};
+  double cos_alpha = 1, half_width = 1; int img_lo = 0, img_hi = -1;
+  std::vector<uint64_t> image;                              // [n_pix][n_pix], row = e2, column = e1
   bool have_opacity = false, have_source = false;
 };
 
@@ -180,6 +185,36 @@ bool locate(const Ctx& c, Packet& p) {
   p.refined = c.refidx[root_lin(c, p.ir)] >= 0;
   if (!p.refined) p.is[0] = p.is[1] = p.is[2] = 0;
   return true;
+}
+
+// ---- O9 (R34): direction-resolved tallies of an escaping package.
+//  * inclination: mu = d_z, n_mu bins uniform in mu over [-1, 1]: SED_mu[m][comp][bin] += 1;
+//  * image: packages of bins img_lo..img_hi leaving within the cone d.obs >= cos(alpha) are
+//    binned by their impact vector b = r - (r.d) d (r = position relative to the box centre; b
+//    does not depend on where along the last flight it is taken) projected on the image axes
+//    e1, e2 (both normal to obs), n_pix x n_pix pixels over [-half_width, half_width]^2.
+void tally_observer(Ctx& c, const Packet& p) {
+  if (c.n_mu > 0) {
+    int m = (int)std::floor((p.d[2] + 1.0) * 0.5 * c.n_mu);
+    m = std::min(c.n_mu - 1, std::max(0, m));
+#pragma omp atomic
+    c.sed_mu[((size_t)m * 3 + p.comp) * c.nb + p.bin] += 1;
+  }
+  if (c.n_pix > 0 && p.bin >= c.img_lo && p.bin <= c.img_hi) {
+    double dot = p.d[0] * c.obs[0] + p.d[1] * c.obs[1] + p.d[2] * c.obs[2];
+    if (dot >= c.cos_alpha) {
+      double r[3], rd = 0;
+      for (int a = 0; a < 3; ++a) { r[a] = p.x[a] - 0.5 * c.N; rd += r[a] * p.d[a]; }
+      double X = 0, Y = 0;
+      for (int a = 0; a < 3; ++a) { double b = r[a] - rd * p.d[a]; X += b * c.e1[a]; Y += b * c.e2[a]; }
+      double fx = (X + c.half_width) / (2.0 * c.half_width) * c.n_pix;
+      double fy = (Y + c.half_width) / (2.0 * c.half_width) * c.n_pix;
+      if (fx >= 0 && fx < c.n_pix && fy >= 0 && fy < c.n_pix) {
+#pragma omp atomic
+        c.image[(size_t)std::floor(fy) * c.n_pix + (size_t)std::floor(fx)] += 1;
+      }
+    }
+  }
 }
 
 // ---- O5: one flight by the cell walk.  Returns 1 = interaction in leaf *slot at p.x,
@@ -380,6 +415,7 @@ void run_packet(Ctx& c, uint64_t seed, uint64_t pid, std::vector<uint64_t>& batc
       loc.escaped = 1;
 #pragma omp atomic
       c.sed[(size_t)p.comp * c.nb + p.bin] += 1;
+      tally_observer(c, p);
       rec(3, -1);
       break;
     }
@@ -594,6 +630,40 @@ int orc_update_temperature(void* h, const uint64_t* tally_sum, uint64_t n_cum) {
   return 0;
 }
 
+// O9: observer set-up.  dir need not be normalised; half_width in cm; n_mu = 0 / n_pix = 0 switch
+// the respective tally off.  Image axes: e1 = z x obs (or x if obs is along z), e2 = obs x e1.
+int orc_set_observer(void* h, int n_mu, int n_pix, const double* dir, double half_angle_deg,
+                     double half_width_cm, int bin_lo, int bin_hi) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.have_opacity || n_mu < 0 || n_pix < 0) return -2;
+  c.n_mu = n_mu; c.sed_mu.assign((size_t)n_mu * 3 * c.nb, 0);
+  c.n_pix = n_pix; c.image.assign((size_t)n_pix * n_pix, 0);
+  if (n_pix > 0) {
+    double n = std::sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
+    if (!(n > 0) || !(half_width_cm > 0)) return -1;
+    for (int a = 0; a < 3; ++a) c.obs[a] = dir[a] / n;
+    if (std::fabs(c.obs[2]) < 0.999) {
+      double q = std::sqrt(c.obs[0] * c.obs[0] + c.obs[1] * c.obs[1]);
+      c.e1[0] = -c.obs[1] / q; c.e1[1] = c.obs[0] / q; c.e1[2] = 0;          // z x obs
+    } else { c.e1[0] = 1; c.e1[1] = 0; c.e1[2] = 0; }
+    c.e2[0] = c.obs[1] * c.e1[2] - c.obs[2] * c.e1[1];
+    c.e2[1] = c.obs[2] * c.e1[0] - c.obs[0] * c.e1[2];
+    c.e2[2] = c.obs[0] * c.e1[1] - c.obs[1] * c.e1[0];
+    c.cos_alpha = std::cos(half_angle_deg * PI / 180.0);
+    c.half_width = half_width_cm / c.root_size;
+    c.img_lo = bin_lo; c.img_hi = bin_hi;
+  }
+  return 0;
+}
+void orc_get_sed_mu(void* h, uint64_t* out) {
+  Ctx& c = *(Ctx*)h;
+  for (size_t i = 0; i < c.sed_mu.size(); ++i) out[i] = c.sed_mu[i];
+}
+void orc_get_image(void* h, uint64_t* out) {
+  Ctx& c = *(Ctx*)h;
+  for (size_t i = 0; i < c.image.size(); ++i) out[i] = c.image[i];
+}
+
 int orc_max_threads() {
 #ifdef _OPENMP
   return omp_get_max_threads();
@@ -646,7 +716,8 @@ void orc_get_counters(void* h, uint64_t* out7, uint64_t* emitted_per_bin) {
 void orc_reset_tallies(void* h, int what) {
   Ctx& c = *(Ctx*)h;
   if (what & 1) { std::fill(c.sed.begin(), c.sed.end(), 0);
-                  std::fill(c.emitted_per_bin.begin(), c.emitted_per_bin.end(), 0); c.cnt = Counters{}; }
+                  std::fill(c.emitted_per_bin.begin(), c.emitted_per_bin.end(), 0); c.cnt = Counters{};
+                  std::fill(c.sed_mu.begin(), c.sed_mu.end(), 0); std::fill(c.image.begin(), c.image.end(), 0); }
   if (what & 2) { std::fill(c.cum.begin(), c.cum.end(), 0); std::fill(c.T.begin(), c.T.end(), c.Tmin);
                   c.Ncum = 0; }
 }

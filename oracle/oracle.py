@@ -50,6 +50,10 @@ def lib():
         L.orc_transport_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64,
                                           C.c_int]
         L.orc_update_temperature.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
+        L.orc_set_observer.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_double,
+                                       C.c_double, C.c_int, C.c_int]
+        L.orc_get_sed_mu.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_get_image.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_trace_packet.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_int, C.c_void_p,
                                        C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_cell_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -164,6 +168,27 @@ class Oracle:
     def set_cell_temperature(self, T):
         T = np.ascontiguousarray(np.broadcast_to(np.asarray(T, np.float64), (self.slots,)))
         lib().orc_set_cell_temperature(self.h, _p(T))
+
+    def set_observer(self, n_mu=0, n_pix=0, direction=(0.0, 0.0, 1.0), half_angle_deg=5.0,
+                     half_width_cm=1.0, bin_lo=0, bin_hi=-1):
+        """O9 (R34): inclination-binned SED and escape-direction image."""
+        d = np.ascontiguousarray(direction, dtype=np.float64)
+        if bin_hi < 0:
+            bin_hi = self.nb - 1
+        rc = lib().orc_set_observer(self.h, n_mu, n_pix, _p(d), float(half_angle_deg),
+                                    float(half_width_cm), int(bin_lo), int(bin_hi))
+        assert rc == 0
+        self.n_mu, self.n_pix = n_mu, n_pix
+
+    def sed_mu(self):
+        s = np.zeros((self.n_mu, 3, self.nb), dtype=np.uint64)
+        lib().orc_get_sed_mu(self.h, _p(s))
+        return s
+
+    def image(self):
+        s = np.zeros((self.n_pix, self.n_pix), dtype=np.uint64)
+        lib().orc_get_image(self.h, _p(s))
+        return s
 
     def sed(self):
         s = np.zeros((3, self.nb), dtype=np.uint64)
