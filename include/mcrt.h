@@ -177,6 +177,32 @@ mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what);
 mcrt_status mcrt_gather_calibrate(uint64_t footprint_bytes, uint64_t n_gathers, double* gathers_per_s,
                                   double* seconds, void* cuda_stream);
 
+/* ---- direction-resolved output (the paper's product is an 11.3 um image and
+ * flux profiles; reading R34) ---------------------------------
+ * Escaping packages are additionally binned by their direction:
+ *  - inclination: mu = d_z in n_mu bins uniform over [-1, 1]; counts [n_mu][3][n_bins] with
+ *    the components of mcrt_get_sed; summing over mu gives mcrt_get_sed exactly.
+ *  - image: packages of the bins bin_lo..bin_hi (bin_hi < 0 = last bin) that leave within
+ *    half_angle_deg of the direction `dir` (pointing from the grid TOWARDS the observer) are
+ *    binned by their impact vector b = r - (r.d) d (r = position relative to the box centre,
+ *    d = direction of flight) on the image axes e1 = z x dir (x if dir is along z) and
+ *    e2 = dir x e1: n_pix x n_pix pixels over [-half_width, half_width]^2 cm, row index along
+ *    e2, column index along e1; counts [n_pix][n_pix].
+ * n_mu = 0 / n_pix = 0 switch the respective tally off.  Needs the opacity (n_bins); calling
+ * mcrt_set_opacity again switches the observer off.  Setting an observer zeroes its tallies;
+ * mcrt_reset_tallies(bit 0) zeroes them too. */
+typedef struct {
+  int32_t n_mu;
+  int32_t n_pix;
+  double dir[3];
+  double half_angle_deg;   /* (0, 180]                                                       */
+  double half_width;       /* cm, > 0                                                        */
+  int32_t bin_lo, bin_hi;
+} mcrt_observer_desc;
+mcrt_status mcrt_set_observer(mcrt_ctx* ctx, const mcrt_observer_desc* desc);
+mcrt_status mcrt_get_sed_mu(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
+mcrt_status mcrt_get_image(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
+
 /* ---- tuning and introspection (do not change results) ---------------------------------------
  * Launch shape of the transport kernel: threads per block (multiple of 32, <= 1024) and resident
  * blocks per SM; 0 keeps the default. */

@@ -55,6 +55,8 @@ struct mcrt_ctx {
   int quorum = 16;
   int threads = 256, blocks_per_sm = 4;
   long long launches = 0;
+  // observer (O9 / R34): escape-direction tallies, off by default
+  ObserverDev obs = {0, 0, 0, -1, {0, 0, 1}, {1, 0, 0}, {0, 1, 0}, 1.f, 1.f, nullptr, nullptr};
   bool have_opacity = false, have_source = false;
   std::string err;
 };
@@ -78,6 +80,11 @@ static void free_opacity(mcrt_ctx* c) {
   cudaFree(c->d_lnQ); cudaFree(c->d_cdf); cudaFree(c->d_small);
   c->d_nu = c->d_dnu = c->d_kabs = nullptr; c->d_opac = nullptr; c->d_lnQ = c->d_cdf = nullptr;
   c->d_small = nullptr;
+}
+static void free_observer(mcrt_ctx* c) {
+  cudaFree(c->obs.sed_mu); cudaFree(c->obs.image);
+  c->obs.sed_mu = c->obs.image = nullptr;
+  c->obs.n_mu = c->obs.n_pix = 0;
 }
 static void free_sources(mcrt_ctx* c) {
   cudaFree(c->d_src); cudaFree(c->d_csrc);
@@ -211,6 +218,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   for (auto& b : ctx->spare) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   free_opacity(ctx);
   free_sources(ctx);
+  free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
   cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch);
   delete ctx;
@@ -236,6 +244,7 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
   CU(cudaDeviceSynchronize());
   free_opacity(ctx);
   free_sources(ctx);
+  free_observer(ctx);                                       // its tallies are sized by n_bins
   ctx->have_opacity = ctx->have_source = false;
   const int nb = d->n_bins, ns = d->n_species;
   ctx->nb = nb; ctx->nT = nT; ctx->Tmin = Tmin; ctx->Tmax = Tmax;
@@ -344,6 +353,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   P.next = ctx->d_small; P.counters = ctx->d_small + 1;
   P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
   P.seed = seed; P.first = first; P.count = n;
+  P.obs = ctx->obs;
   P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->n3;
   CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
   const int threads = ctx->threads;
@@ -508,6 +518,58 @@ mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem) {
   return copy_out(ctx, counts_out, ctx->d_small + 1 + CNT_N, 8 * 3 * (size_t)ctx->nb, mem);
 }
 
+mcrt_status mcrt_set_observer(mcrt_ctx* ctx, const mcrt_observer_desc* d) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!d) return fail(ctx, MCRT_EINVAL, "mcrt_set_observer: NULL argument");
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_set_observer: call mcrt_set_opacity first");
+  if (d->n_mu < 0 || d->n_mu > 4096 || d->n_pix < 0 || d->n_pix > 8192)
+    return fail(ctx, MCRT_EINVAL, "mcrt_set_observer: n_mu must be 0..4096, n_pix 0..8192");
+  double o[3] = {0, 0, 1}, e1[3] = {1, 0, 0}, e2[3] = {0, 1, 0};
+  if (d->n_pix > 0) {
+    const double n = std::sqrt(d->dir[0] * d->dir[0] + d->dir[1] * d->dir[1] + d->dir[2] * d->dir[2]);
+    if (!(n > 0) || !(d->half_width > 0) || !(d->half_angle_deg > 0) || d->half_angle_deg > 180)
+      return fail(ctx, MCRT_EINVAL, "mcrt_set_observer: dir must be non-zero, half_width > 0, 0 < half_angle_deg <= 180");
+    for (int a = 0; a < 3; ++a) o[a] = d->dir[a] / n;
+    if (std::fabs(o[2]) < 0.999) {                          // e1 = z x o
+      const double q = std::sqrt(o[0] * o[0] + o[1] * o[1]);
+      e1[0] = -o[1] / q; e1[1] = o[0] / q; e1[2] = 0;
+    }
+    e2[0] = o[1] * e1[2] - o[2] * e1[1];                    // e2 = o x e1
+    e2[1] = o[2] * e1[0] - o[0] * e1[2];
+    e2[2] = o[0] * e1[1] - o[1] * e1[0];
+  }
+  CU(cudaDeviceSynchronize());
+  free_observer(ctx);
+  if (d->n_mu > 0) {
+    CU(cudaMalloc(&ctx->obs.sed_mu, 8 * (size_t)d->n_mu * 3 * ctx->nb));
+    CU(cudaMemset(ctx->obs.sed_mu, 0, 8 * (size_t)d->n_mu * 3 * ctx->nb));
+  }
+  if (d->n_pix > 0) {
+    CU(cudaMalloc(&ctx->obs.image, 8 * (size_t)d->n_pix * d->n_pix));
+    CU(cudaMemset(ctx->obs.image, 0, 8 * (size_t)d->n_pix * d->n_pix));
+  }
+  ctx->obs.n_mu = d->n_mu; ctx->obs.n_pix = d->n_pix;
+  ctx->obs.bin_lo = d->bin_lo; ctx->obs.bin_hi = d->bin_hi < 0 ? ctx->nb - 1 : d->bin_hi;
+  for (int a = 0; a < 3; ++a) { ctx->obs.o[a] = (float)o[a]; ctx->obs.e1[a] = (float)e1[a]; ctx->obs.e2[a] = (float)e2[a]; }
+  ctx->obs.cos_alpha = d->n_pix > 0 ? (float)std::cos(d->half_angle_deg * 3.14159265358979323846 / 180.0) : 1.f;
+  ctx->obs.half_width = d->n_pix > 0 ? (float)(d->half_width / ctx->root_size) : 1.f;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_get_sed_mu(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!counts_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_sed_mu: NULL output");
+  if (!ctx->obs.sed_mu) return fail(ctx, MCRT_ESTATE, "mcrt_get_sed_mu: no inclination bins set (mcrt_set_observer)");
+  return copy_out(ctx, counts_out, ctx->obs.sed_mu, 8 * (size_t)ctx->obs.n_mu * 3 * ctx->nb, mem);
+}
+
+mcrt_status mcrt_get_image(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!counts_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_image: NULL output");
+  if (!ctx->obs.image) return fail(ctx, MCRT_ESTATE, "mcrt_get_image: no image set (mcrt_set_observer)");
+  return copy_out(ctx, counts_out, ctx->obs.image, 8 * (size_t)ctx->obs.n_pix * ctx->obs.n_pix, mem);
+}
+
 mcrt_status mcrt_get_counters(mcrt_ctx* ctx, mcrt_counters* out, uint64_t* emitted_per_bin) {
   if (!ctx) return MCRT_EINVAL;
   if (!out) return fail(ctx, MCRT_EINVAL, "mcrt_get_counters: NULL output");
@@ -527,6 +589,8 @@ mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what) {
   if (!ctx) return MCRT_EINVAL;
   CU(cudaStreamSynchronize(ctx->last_stream));
   if ((what & 1) && ctx->d_small) CU(cudaMemset(ctx->d_small, 0, 8 * (1 + CNT_N + 4 * (size_t)ctx->nb)));
+  if ((what & 1) && ctx->obs.sed_mu) CU(cudaMemset(ctx->obs.sed_mu, 0, 8 * (size_t)ctx->obs.n_mu * 3 * ctx->nb));
+  if ((what & 1) && ctx->obs.image) CU(cudaMemset(ctx->obs.image, 0, 8 * (size_t)ctx->obs.n_pix * ctx->obs.n_pix));
   if (what & 2) {
     CU(cudaMemset(ctx->d_tally, 0, 8 * (size_t)ctx->store_slots));
     CU(cudaMemset(ctx->d_trow, 0, 4 * (size_t)ctx->store_slots));

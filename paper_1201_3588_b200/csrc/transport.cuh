@@ -31,6 +31,16 @@ struct SrcDev {
   float lcdf;        // cumulative luminosity fraction
 };
 
+// Direction-resolved tallies of escaping packages (reading R34;
+// the paper's product is an image and flux profiles).  Off when n_mu = n_pix = 0.
+struct ObserverDev {
+  int n_mu, n_pix, bin_lo, bin_hi;
+  float o[3], e1[3], e2[3];                    // unit vector towards the observer; image axes
+  float cos_alpha, half_width;                 // acceptance cone; image half width in root-cube edges
+  unsigned long long* sed_mu;                  // [n_mu][3][nb]
+  unsigned long long* image;                   // [n_pix][n_pix], row = e2, column = e1
+};
+
 struct TransportParams {
   const float* __restrict__ rho;               // [slots] density / refined-cube marker
   unsigned long long* __restrict__ tally;      // [slots] cumulative absorbed-package counts
@@ -45,7 +55,35 @@ struct TransportParams {
   unsigned long long* counters;                // [CNT_N]
   unsigned long long seed, first, count;
   int N, S, nb, nT, nsrc, n3;
+  ObserverDev obs;
 };
+
+// O9 / R34: an escaping package at position (x,y,z) (root-cube edges from the box corner) with
+// direction d.  Inclination bin from mu = d_z; image pixel from the impact vector
+// b = r - (r.d) d, r relative to the box centre, projected on (e1, e2).
+__device__ __forceinline__ void tally_observer(const TransportParams& P, float x, float y, float z, float d0,
+                                               float d1, float d2, int bin, int comp) {
+  const ObserverDev& O = P.obs;
+  if (O.n_mu > 0) {
+    int m = (int)floorf((d2 + 1.f) * 0.5f * (float)O.n_mu);
+    m = min(O.n_mu - 1, max(0, m));
+    atomicAdd(O.sed_mu + ((size_t)m * 3 + comp) * P.nb + bin, 1ull);
+  }
+  if (O.n_pix > 0 && bin >= O.bin_lo && bin <= O.bin_hi) {
+    if (d0 * O.o[0] + d1 * O.o[1] + d2 * O.o[2] >= O.cos_alpha) {
+      const float h = 0.5f * (float)P.N;
+      const float r0 = x - h, r1 = y - h, r2 = z - h;
+      const float rd = r0 * d0 + r1 * d1 + r2 * d2;
+      const float b0 = r0 - rd * d0, b1 = r1 - rd * d1, b2 = r2 - rd * d2;
+      const float X = b0 * O.e1[0] + b1 * O.e1[1] + b2 * O.e1[2];
+      const float Y = b0 * O.e2[0] + b1 * O.e2[1] + b2 * O.e2[2];
+      const float fx = (X + O.half_width) / (2.f * O.half_width) * (float)O.n_pix;
+      const float fy = (Y + O.half_width) / (2.f * O.half_width) * (float)O.n_pix;
+      if (fx >= 0.f && fx < (float)O.n_pix && fy >= 0.f && fy < (float)O.n_pix)
+        atomicAdd(O.image + (size_t)floorf(fy) * O.n_pix + (size_t)floorf(fx), 1ull);
+    }
+  }
+}
 
 // ---- Philox4x32-10 (Salmon et al. 2011), counter = (pid_lo, pid_hi, k, tag), key = seed (R18) ----
 __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
@@ -445,6 +483,18 @@ __global__ void __launch_bounds__(256, 4) k_transport(const TransportParams P) {
 
     // ---- a7: escape -> SED ----
     if (state == ST_ESCAPE) {
+      if (P.obs.n_mu | P.obs.n_pix) {                        // exit point from the position-free state
+        const float h = (TL && p.lvl) ? 1.f / (float)P.S : 1.f;
+        float ux, uy, uz;
+        local_from_t(p, h, ux, uy, uz);
+        const int sx = (TL && p.lvl) ? (p.sub & 15) : 0, sy = (TL && p.lvl) ? ((p.sub >> 4) & 15) : 0,
+                  sz = (TL && p.lvl) ? ((p.sub >> 8) & 15) : 0;
+        const float fN = (float)P.N;
+        const float x = (unsigned)p.ix >= (unsigned)P.N ? (p.ix < 0 ? 0.f : fN) : (float)p.ix + ((float)sx + ux) * h;
+        const float y = (unsigned)p.iy >= (unsigned)P.N ? (p.iy < 0 ? 0.f : fN) : (float)p.iy + ((float)sy + uy) * h;
+        const float z = (unsigned)p.iz >= (unsigned)P.N ? (p.iz < 0 ? 0.f : fN) : (float)p.iz + ((float)sz + uz) * h;
+        tally_observer(P, x, y, z, p.d0, p.d1, p.d2, p.bin, p.comp);
+      }
       atomicAdd(&s_sed[p.comp * P.nb + p.bin], 1u);
       ++cnt[CNT_ESCAPED];
       state = ST_FETCH;

@@ -218,6 +218,15 @@ __global__ void __launch_bounds__(256, 4) k_transport_u(const TransportParamsU P
   for (;;) {
     // ---- a7: escaped packages -> SED; a8: refill from the work queue (one atomic per warp) ----
     if (state == SU_ESCAPE) {
+      if (P.obs.n_mu | P.obs.n_pix) {                        // exit point: cell from the cursors, offset from the t's
+        int ix, iy, iz;
+        cell_of(p, lut, N, ix, iy, iz);
+        const float w0 = fminf(1.f, fmaxf(0.f, (p.t0 - p.tcur) * fabsf(p.d0)));
+        const float w1 = fminf(1.f, fmaxf(0.f, (p.t1 - p.tcur) * fabsf(p.d1)));
+        const float w2 = fminf(1.f, fmaxf(0.f, (p.t2 - p.tcur) * fabsf(p.d2)));
+        tally_observer(P, (float)ix + (p.d0 > 0.f ? 1.f - w0 : w0), (float)iy + (p.d1 > 0.f ? 1.f - w1 : w1),
+                       (float)iz + (p.d2 > 0.f ? 1.f - w2 : w2), p.d0, p.d1, p.d2, p.cb & 0xffff, p.cb >> 16);
+      }
       atomicAdd(&s_sed[(p.cb >> 16) * P.nb + (p.cb & 0xffff)], 1u);
       state = SU_FETCH;
     }

@@ -37,6 +37,12 @@ class _Source(C.Structure):
                 ("T_bb", C.c_double)]
 
 
+class _ObserverDesc(C.Structure):
+    _fields_ = [("n_mu", C.c_int32), ("n_pix", C.c_int32), ("dir", C.c_double * 3),
+                ("half_angle_deg", C.c_double), ("half_width", C.c_double),
+                ("bin_lo", C.c_int32), ("bin_hi", C.c_int32)]
+
+
 class _Counters(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("emitted", "escaped", "lost", "absorptions",
                                           "scatterings", "flights", "crossings")]
@@ -46,7 +52,8 @@ class _Counters(C.Structure):
 SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opacity",
            "mcrt_set_source", "mcrt_run_batch", "mcrt_transport_batch",
            "mcrt_update_temperature", "mcrt_get_cell_energy",
-           "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_get_counters",
+           "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_observer",
+           "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum",
            "mcrt_get_batch_times", "mcrt_get_tables",
            "mcrt_kernel_launches", "mcrt_philox_blocks", "mcrt_gather_calibrate", "mcrt_last_error")
@@ -74,6 +81,9 @@ def lib():
         L.mcrt_get_cell_energy.argtypes = [vp, vp, C.POINTER(C.c_double), C.c_int]
         L.mcrt_get_cell_temperature.argtypes = [vp, vp, C.c_int]
         L.mcrt_get_sed.argtypes = [vp, vp, C.c_int]
+        L.mcrt_set_observer.argtypes = [vp, C.POINTER(_ObserverDesc)]
+        L.mcrt_get_sed_mu.argtypes = [vp, vp, C.c_int]
+        L.mcrt_get_image.argtypes = [vp, vp, C.c_int]
         L.mcrt_get_counters.argtypes = [vp, C.POINTER(_Counters), vp]
         L.mcrt_reset_tallies.argtypes = [vp, i32]
         L.mcrt_set_launch.argtypes = [vp, i32, i32]
@@ -90,7 +100,8 @@ def lib():
         for name in ("mcrt_grid_create", "mcrt_destroy", "mcrt_set_opacity", "mcrt_set_source",
                      "mcrt_run_batch", "mcrt_transport_batch", "mcrt_update_temperature",
                      "mcrt_get_cell_energy", "mcrt_get_cell_temperature",
-                     "mcrt_get_sed", "mcrt_get_counters", "mcrt_reset_tallies",
+                     "mcrt_get_sed", "mcrt_set_observer", "mcrt_get_sed_mu", "mcrt_get_image",
+                     "mcrt_get_counters", "mcrt_reset_tallies",
                      "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_get_batch_times",
                      "mcrt_get_tables",
                      "mcrt_philox_blocks"):
@@ -238,6 +249,26 @@ class Context:
     def get_sed(self, device=False):
         out, p, mem = self._out((3, self.n_bins), np.uint64, device)
         self._check(lib().mcrt_get_sed(self.h, p, mem), "mcrt_get_sed")
+        return out
+
+    def set_observer(self, n_mu=0, n_pix=0, direction=(0.0, 0.0, 1.0), half_angle_deg=5.0,
+                     half_width_cm=1.0, bin_lo=0, bin_hi=-1):
+        d = _ObserverDesc()
+        d.n_mu, d.n_pix = int(n_mu), int(n_pix)
+        d.dir = (C.c_double * 3)(*[float(v) for v in direction])
+        d.half_angle_deg, d.half_width = float(half_angle_deg), float(half_width_cm)
+        d.bin_lo, d.bin_hi = int(bin_lo), int(bin_hi)
+        self._check(lib().mcrt_set_observer(self.h, C.byref(d)), "mcrt_set_observer")
+        self.n_mu, self.n_pix = d.n_mu, d.n_pix
+
+    def get_sed_mu(self, device=False):
+        out, p, mem = self._out((self.n_mu, 3, self.n_bins), np.uint64, device)
+        self._check(lib().mcrt_get_sed_mu(self.h, p, mem), "mcrt_get_sed_mu")
+        return out
+
+    def get_image(self, device=False):
+        out, p, mem = self._out((self.n_pix, self.n_pix), np.uint64, device)
+        self._check(lib().mcrt_get_image(self.h, p, mem), "mcrt_get_image")
         return out
 
     def get_counters(self):
