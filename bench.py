@@ -142,12 +142,12 @@ def oracle_rate(wl, target_seconds=15.0, n_batches=4):
     cores = O.max_threads()
     orc = O.Oracle(wl)
     probe, dt = 2048, 0.0
-    while dt < 0.5 and probe < wl.n_packets:                 # calibrate the sample size
+    while dt < 0.5 and probe < (1 << 28):                    # calibrate the sample size
         probe *= 2
         t0 = time.perf_counter()
         orc.run_batch(wl.seed, 0, probe)
         dt = max(time.perf_counter() - t0, 1e-4)
-    n = int(min(max(probe * target_seconds / dt, 4 * probe), wl.n_packets))
+    n = int(min(max(probe * target_seconds / dt, 4 * probe), 1 << 31))       # ids may run past the config's count
     per = max(n // n_batches, 1)
     orc = O.Oracle(wl)
     t0 = time.perf_counter()
@@ -399,14 +399,21 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
     ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g)
     ctx.set_source(wl.sources)
     d2h = 0
+    # read-back buffers: pinned host memory, allocated once and reused every step
+    slots = wl.leaf_slots
+    pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory().numpy()
+    b_sed = pin((3, wl.n_bins), torch.int64).view(np.uint64)
+    b_abs = pin((slots,), torch.int64).view(np.uint64)
+    b_T = pin((slots,), torch.float32)
+    b_emit = pin((wl.n_bins,), torch.int64).view(np.uint64)
     from paper_1201_3588_b200.sharding import ShardedRunner
     runner = ShardedRunner(ctx, dist if world > 1 else None)
     for s in range(steps):
         runner.run_batch(wl.seed, s * world * batch, world * batch, stream)
-        sed = ctx.get_sed()
-        n_abs, _ = ctx.get_cell_energy()
-        T = ctx.get_cell_temperature()
-        c = ctx.get_counters()
+        sed = ctx.get_sed(out=b_sed)
+        n_abs, _ = ctx.get_cell_energy(out=b_abs)
+        T = ctx.get_cell_temperature(out=b_T)
+        c = ctx.get_counters(out=b_emit)
         d2h = sed.nbytes + n_abs.nbytes + T.nbytes + 7 * 8 + c["emitted_per_bin"].nbytes
     torch.cuda.synchronize()
     dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")

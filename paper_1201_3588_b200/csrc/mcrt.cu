@@ -52,6 +52,7 @@ struct mcrt_ctx {
   long long store_slots = 0;
   int* d_lut = nullptr;
   unsigned long long* d_tally_scratch = nullptr;
+  void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 16;
   int threads = 256, blocks_per_sm = 4;
   long long launches = 0;
@@ -220,7 +221,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_sources(ctx);
   free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
-  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch);
+  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -479,8 +480,10 @@ mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps
   if (ctx->uni && ctx->lay.bricked) {                        // storage order -> slot order (R22)
     unsigned long long* d_out = (unsigned long long*)n_abs_out;
     unsigned long long* tmp = nullptr;
-    struct Tmp { unsigned long long*& a; ~Tmp() { cudaFree(a); } } guard{tmp};
-    if (mem == MCRT_HOST) { CU(cudaMalloc(&tmp, 8 * (size_t)ctx->slots)); d_out = tmp; }
+    if (mem == MCRT_HOST) {
+      if (!ctx->d_out_scratch) CU(cudaMalloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
+      tmp = (unsigned long long*)ctx->d_out_scratch; d_out = tmp;
+    }
     k_store_to_ext<unsigned long long><<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
         ctx->d_tally, d_out, ctx->lay, ctx->n3);
     ctx->launches++;
@@ -497,8 +500,10 @@ mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem)
   if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_cell_temperature: opacity not set");
   float* d_T = T_out;
   float* tmp = nullptr;
-  struct Tmp { float*& a; ~Tmp() { cudaFree(a); } } guard{tmp};
-  if (mem == MCRT_HOST) { CU(cudaMalloc(&tmp, 4 * (size_t)ctx->slots)); d_T = tmp; }
+  if (mem == MCRT_HOST) {
+    if (!ctx->d_out_scratch) CU(cudaMalloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
+    tmp = (float*)ctx->d_out_scratch; d_T = tmp;
+  }
   if (ctx->uni)
     k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
         ctx->d_trow, d_T, ctx->lay, ctx->n3, (float)std::log(ctx->Tmin), (float)ctx->dlnT);

@@ -224,30 +224,37 @@ class Context:
                     "mcrt_update_temperature")
 
     # -- results --------------------------------------------------------------------------
-    def _out(self, shape, np_dtype, device):
+    def _out(self, shape, np_dtype, device, out=None):
+        """Output buffer: a torch CUDA tensor (device=True), the caller's `out` (a C-contiguous
+        numpy array of the right shape and dtype -- e.g. a view of pinned memory, reused from
+        call to call), or a fresh numpy array."""
         if device:
             import torch
             t = torch.empty(shape, dtype=getattr(torch, np.dtype(np_dtype).name
                                                  .replace("uint64", "int64")), device="cuda")
             return t, C.c_void_p(t.data_ptr()), MCRT_DEVICE
+        if out is not None:
+            if out.shape != tuple(shape) or out.dtype != np.dtype(np_dtype) or not out.flags.c_contiguous:
+                raise McrtError(f"out must be a C-contiguous {np.dtype(np_dtype)} array of shape {tuple(shape)}")
+            return out, _np_ptr(out), MCRT_HOST
         a = np.zeros(shape, dtype=np_dtype)
         return a, _np_ptr(a), MCRT_HOST
 
-    def get_cell_energy(self, device=False):
-        out, p, mem = self._out((self.slots,), np.uint64, device)
+    def get_cell_energy(self, device=False, out=None):
+        out, p, mem = self._out((self.slots,), np.uint64, device, out)
         eps = C.c_double(0)
         self._check(lib().mcrt_get_cell_energy(self.h, p, C.byref(eps), mem),
                     "mcrt_get_cell_energy")
         return out, eps.value
 
-    def get_cell_temperature(self, device=False):
-        out, p, mem = self._out((self.slots,), np.float32, device)
+    def get_cell_temperature(self, device=False, out=None):
+        out, p, mem = self._out((self.slots,), np.float32, device, out)
         self._check(lib().mcrt_get_cell_temperature(self.h, p, mem),
                     "mcrt_get_cell_temperature")
         return out
 
-    def get_sed(self, device=False):
-        out, p, mem = self._out((3, self.n_bins), np.uint64, device)
+    def get_sed(self, device=False, out=None):
+        out, p, mem = self._out((3, self.n_bins), np.uint64, device, out)
         self._check(lib().mcrt_get_sed(self.h, p, mem), "mcrt_get_sed")
         return out
 
@@ -271,9 +278,9 @@ class Context:
         self._check(lib().mcrt_get_image(self.h, p, mem), "mcrt_get_image")
         return out
 
-    def get_counters(self):
+    def get_counters(self, out=None):
         c = _Counters()
-        e = np.zeros(self.n_bins, dtype=np.uint64)
+        e = np.zeros(self.n_bins, dtype=np.uint64) if out is None else out
         self._check(lib().mcrt_get_counters(self.h, C.byref(c), _np_ptr(e)),
                     "mcrt_get_counters")
         d = {n: int(getattr(c, n)) for n, _ in _Counters._fields_}
