@@ -222,6 +222,11 @@ mcrt_status mcrt_get_batch_times(mcrt_ctx* ctx, float* transport_ms, float* upda
 mcrt_status mcrt_get_tables(mcrt_ctx* ctx, float* opac, float* lnQ, float* cdf);
 /* Number of kernels launched by this library since the context was created. */
 int64_t mcrt_kernel_launches(const mcrt_ctx* ctx);
+/* Library built with -DMCRT_CHECKS (paper_1201_3588_b200/build.py build_library(checks=True)):
+ * number of storage-slot indices the transport kernels found outside the grid's storage since
+ * the library was loaded (must stay 0); -1 if the library was built without the checks, -2 on
+ * a CUDA error.  Stands in for compute-sanitizer, which the GPU pool does not offer. */
+int64_t mcrt_debug_violations(void);
 /* Raw Philox4x32-10 blocks computed on the device (test hook for the generator pin):
  * out[4*i..4*i+3] = Philox(key = (key2[0], key2[1]), counter = ctr[4*i..4*i+3]).  Host pointers. */
 mcrt_status mcrt_philox_blocks(const uint32_t* key2, const uint32_t* ctr, uint32_t* out, int64_t n);

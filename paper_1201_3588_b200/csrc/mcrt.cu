@@ -356,6 +356,9 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   P.seed = seed; P.first = first; P.count = n;
   P.obs = ctx->obs;
   P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->n3;
+#ifdef MCRT_CHECKS
+  CU(cudaMemcpyToSymbolAsync(g_mcrt_nstore, &ctx->store_slots, sizeof(long long), 0, cudaMemcpyHostToDevice, st));
+#endif
   CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
   const int threads = ctx->threads;
   long long want = ((long long)n + threads - 1) / threads;
@@ -651,6 +654,17 @@ mcrt_status mcrt_get_tables(mcrt_ctx* ctx, float* opac, float* lnQ, float* cdf) 
 }
 
 int64_t mcrt_kernel_launches(const mcrt_ctx* ctx) { return ctx ? ctx->launches : -1; }
+
+int64_t mcrt_debug_violations(void) {
+#ifdef MCRT_CHECKS
+  unsigned long long v = 0;
+  if (cudaDeviceSynchronize() != cudaSuccess) return -2;
+  if (cudaMemcpyFromSymbol(&v, g_mcrt_violations, sizeof(v)) != cudaSuccess) return -2;
+  return (int64_t)v;
+#else
+  return -1;
+#endif
+}
 
 __global__ void k_philox_blocks(uint32_t k0, uint32_t k1, const uint32_t* __restrict__ ctr,
                                 uint32_t* __restrict__ out, long long n) {

@@ -16,6 +16,21 @@
 
 namespace mcrt {
 
+// Bounds checks of our own (compute-sanitizer is not available on the GPU pool): a library built
+// with -DMCRT_CHECKS counts every storage-slot index outside [0, store slots) before it is used;
+// tests/test_gpu_checks.py builds that variant and requires the count to stay 0.
+#ifdef MCRT_CHECKS
+__device__ unsigned long long g_mcrt_violations = 0ull;
+__device__ long long g_mcrt_nstore = 0;
+#define MCRT_CHECK_SLOT(s)                                                                     \
+  do {                                                                                         \
+    if ((unsigned long long)(long long)(s) >= (unsigned long long)g_mcrt_nstore)               \
+      atomicAdd(&g_mcrt_violations, 1ull);                                                     \
+  } while (0)
+#else
+#define MCRT_CHECK_SLOT(s) do { } while (0)
+#endif
+
 constexpr uint32_t kTagEmit = 0, kTagFlight = 1, kTagReemit = 2;
 constexpr uint32_t kMaxFlights = 10000000u;          // R20
 constexpr int kWalkChunk = 32;                       // crossings per outer iteration
@@ -206,6 +221,7 @@ __device__ __forceinline__ void place_in_root(const TransportParams& P, Packet& 
   int lin = p.ix + P.N * (p.iy + P.N * p.iz);
   p.lvl = 0; p.slot = lin;
   if (TL) {
+    MCRT_CHECK_SLOT(lin);
     int bits = __float_as_int(__ldg(P.rho + lin));
     if (bits < 0) {
       const int S = P.S;
@@ -251,7 +267,8 @@ __device__ __forceinline__ void emit_packet(const TransportParams& P, Packet& p,
     p.lvl = 0; p.slot = lin;
     bool refined = false;
     if (TL) {
-      int bits = __float_as_int(__ldg(P.rho + lin));
+      MCRT_CHECK_SLOT(lin);
+    int bits = __float_as_int(__ldg(P.rho + lin));
       if (bits < 0) {
         refined = true;
         p.lvl = 1; p.kref = bits & 0x7fffffff; p.sub = sx | (sy << 4) | (sz << 8);
@@ -294,6 +311,7 @@ __device__ __forceinline__ void emit_packet(const TransportParams& P, Packet& p,
 template <bool TL>
 __device__ __forceinline__ bool walk_step(const TransportParams& P, Packet& p, float kx, int& state,
                                           uint32_t& crossings) {
+  MCRT_CHECK_SLOT(p.slot);
   float rho = __ldg(P.rho + p.slot);
   float tmin = fminf(p.t0, fminf(p.t1, p.t2));
   float alpha = rho * kx;
@@ -328,6 +346,7 @@ __device__ __forceinline__ bool walk_step(const TransportParams& P, Packet& p, f
     int coord = a0 ? p.ix : (a1 ? p.iy : p.iz);
     if ((unsigned)coord >= (unsigned)P.N) { state = ST_ESCAPE; return false; }
     int lin = p.ix + P.N * (p.iy + P.N * p.iz);
+    MCRT_CHECK_SLOT(lin);
     int bits = __float_as_int(__ldg(P.rho + lin));
     if (bits < 0) {                                          // refined -> refined: sub faces line up
       int nf = step > 0 ? 0 : S - 1;
@@ -355,6 +374,7 @@ __device__ __forceinline__ bool walk_step(const TransportParams& P, Packet& p, f
   int lin = p.ix + P.N * (p.iy + P.N * p.iz);
   p.slot = lin;
   if (TL) {
+    MCRT_CHECK_SLOT(lin);
     int bits = __float_as_int(__ldg(P.rho + lin));
     if (bits < 0) {                                          // unrefined -> refined: descend
       const int S = P.S;
@@ -461,6 +481,7 @@ __global__ void __launch_bounds__(256, 4) k_transport(const TransportParams P) {
       } else {                                               // absorb + re-emit (Eqn 11.67)
         ++cnt[CNT_ABS];
         // a6: warp-aggregated integer tally: one atomic per distinct leaf per warp
+        MCRT_CHECK_SLOT(p.slot);
         unsigned peers = __match_any_sync(__activemask(), p.slot);
         if ((int)lane == __ffs(peers) - 1)
           atomicAdd(P.tally + p.slot, (unsigned long long)__popc(peers));

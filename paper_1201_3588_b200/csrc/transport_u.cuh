@@ -136,7 +136,7 @@ __device__ __forceinline__ void walk_step_u(const float* __restrict__ rho, Packe
   const int dl = lds_s32(a0 ? p.p0 : (a1 ? p.p1 : p.p2));
   const bool esc = dl == kLutEscape;
   const int nslot = p.slot + dl;
-  if (!esc) nxt = __ldg(rho + nslot);
+  if (!esc) { MCRT_CHECK_SLOT(nslot); nxt = __ldg(rho + nslot); }
   const float dtau = cur * kx * (tnext - p.tcur);
   if (dtau >= p.tau_rem) {                                   // interaction inside this cell
     state = SU_INTERACT;
@@ -285,6 +285,7 @@ __global__ void __launch_bounds__(256, 4) k_transport_u(const TransportParamsU P
         } else {
           ++n_abs;
           // warp-aggregated integer tally: one atomic per distinct cell per warp
+          MCRT_CHECK_SLOT(p.slot);
           unsigned peers = __match_any_sync(__activemask(), p.slot);
           if ((int)lane == __ffs(peers) - 1)
             atomicAdd(P.tally + p.slot, (unsigned long long)__popc(peers));
@@ -301,6 +302,7 @@ __global__ void __launch_bounds__(256, 4) k_transport_u(const TransportParamsU P
         if (is_new) {
           emit_position_u(P, P.src[s], pid, r, ix, iy, iz, ux, uy, uz, a, b, c);
           p.slot = (int)slot_of(PU.lay, ix, iy, iz);
+          MCRT_CHECK_SLOT(p.slot);
           p.rho = __ldg(P.rho + p.slot);
           comp = 0; p.k = 0;
           atomicAdd(&s_emit[bin], 1u);

@@ -56,14 +56,14 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum",
            "mcrt_get_batch_times", "mcrt_get_tables",
-           "mcrt_kernel_launches", "mcrt_philox_blocks", "mcrt_gather_calibrate", "mcrt_last_error")
+           "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_gather_calibrate", "mcrt_last_error")
 
 
 def lib():
     """Load libmcrt.so (built in-tree by build.py).  Fails loudly if it is missing."""
     global _lib
     if _lib is None:
-        path = _build.LIB_PATH
+        path = os.environ.get("MCRT_LIBRARY") or _build.LIB_PATH     # e.g. the -DMCRT_CHECKS variant
         if not os.path.exists(path):
             raise McrtError(f"{path} is missing: run `python -m paper_1201_3588_b200.build` "
                             "(there is no CPU fallback)")
@@ -92,6 +92,8 @@ def lib():
         L.mcrt_get_tables.argtypes = [vp, vp, vp, vp]
         L.mcrt_kernel_launches.restype = i64
         L.mcrt_kernel_launches.argtypes = [vp]
+        L.mcrt_debug_violations.restype = i64
+        L.mcrt_debug_violations.argtypes = []
         L.mcrt_philox_blocks.argtypes = [vp, vp, vp, i64]
         L.mcrt_gather_calibrate.argtypes = [u64, u64, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
         L.mcrt_gather_calibrate.restype = C.c_int
@@ -373,3 +375,8 @@ def gather_calibrate(footprint_bytes, n_gathers=1 << 30, stream=None):
     if rc != 0:
         raise McrtError(f"mcrt_gather_calibrate: status {rc}: {lib().mcrt_last_error(None).decode()}")
     return g.value, sec.value
+
+
+def debug_violations():
+    """Out-of-range storage indices seen by a -DMCRT_CHECKS library (-1: built without checks)."""
+    return int(lib().mcrt_debug_violations())
