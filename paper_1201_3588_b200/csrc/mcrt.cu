@@ -54,7 +54,7 @@ struct mcrt_ctx {
   unsigned long long* d_tally_scratch = nullptr;
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 16;
-  int threads = 256, blocks_per_sm = 4;
+  int threads = 256, blocks_per_sm = 0;   // 0 = automatic (4; 5 for the single-level kernel on L2-resident grids)
   long long launches = 0;
   // observer (O9 / R34): escape-direction tallies, off by default
   ObserverDev obs = {0, 0, 0, -1, {0, 0, 1}, {1, 0, 0}, {0, 1, 0}, 1.f, 1.f, nullptr, nullptr};
@@ -361,15 +361,19 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
 #endif
   CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
   const int threads = ctx->threads;
+  // resident blocks per SM: the caller's choice, else 5 for the single-level kernel on grids the
+  // L2 holds (x-fastest storage), 4 otherwise
+  const int bps = ctx->blocks_per_sm ? ctx->blocks_per_sm : (ctx->uni && !ctx->lay.bricked ? 5 : 4);
   long long want = ((long long)n + threads - 1) / threads;
-  long long grid = (long long)ctx->sm_count * ctx->blocks_per_sm;
+  long long grid = (long long)ctx->sm_count * bps;
   if (want < grid) grid = want;
   size_t smem = sizeof(float4) * nb + 4 * (size_t)nb * 4;
   if (ctx->uni) {
     TransportParamsU PU;
     PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
     smem += sizeof(int) * 6 * (size_t)ctx->N;
-    k_transport_u<<<(unsigned)grid, threads, smem, st>>>(PU);
+    if (bps * threads > 1024) k_transport_u<5><<<(unsigned)grid, threads, smem, st>>>(PU);   // 48 registers
+    else k_transport_u<4><<<(unsigned)grid, threads, smem, st>>>(PU);                        // 64 registers
   } else {
     k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
   }
@@ -612,7 +616,7 @@ mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads, int32_t blocks_per_s
   if (threads < 0 || threads > 256 || (threads % 32) != 0 || blocks_per_sm < 0 || blocks_per_sm > 32)
     return fail(ctx, MCRT_EINVAL, "mcrt_set_launch: threads must be a multiple of 32 up to 256, blocks_per_sm <= 32");
   if (threads) ctx->threads = threads;
-  if (blocks_per_sm) ctx->blocks_per_sm = blocks_per_sm;
+  ctx->blocks_per_sm = blocks_per_sm;                        // 0 = automatic
   return MCRT_OK;
 }
 

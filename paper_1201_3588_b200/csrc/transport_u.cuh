@@ -185,7 +185,12 @@ __device__ __forceinline__ void emit_position_u(const TransportParams& P, const 
   }
 }
 
-__global__ void __launch_bounds__(256, 4) k_transport_u(const TransportParamsU PU) {
+// MINBLOCKS = resident blocks per SM the kernel is compiled for: 4 (64 registers) or 5 (48
+// registers).  Five blocks hide more of the L2 latency on cache-resident grids (c1_tau1 0.371 ->
+// 0.338 ms per launch); on HBM-resident grids the extra threads thrash the L1 (c4 66 -> 74 ms),
+// so the host picks per grid (profiles/r01_summary.md).
+template <int MINBLOCKS>
+__global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportParamsU PU) {
   const TransportParams& P = PU.base;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* s_opac = reinterpret_cast<float4*>(smem_raw);                    // [nb]

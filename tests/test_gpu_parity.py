@@ -84,16 +84,17 @@ def test_c0_full(M, oracle_mod):
 def test_c0_bit_reproducible_and_launch_shape_invariant(M):
     wl = W.c0()
     a = M.run_workload(wl)
-    b = M.from_workload(wl)
-    b.set_launch(64, 2)
-    for first, cnt in wl.batches():
-        b.run_batch(wl.seed, first, cnt)
-    assert np.array_equal(a.get_cell_energy()[0], b.get_cell_energy()[0])
-    assert np.array_equal(a.get_sed(), b.get_sed())
-    assert np.array_equal(a.get_cell_temperature(), b.get_cell_temperature())
-    ca, cb = a.get_counters(), b.get_counters()
-    for k in ca:
-        assert np.array_equal(ca[k], cb[k]), k
+    for shape in ((64, 2), (256, 4), (256, 5), (128, 12)):    # 64- and 48-register builds of the kernel
+        b = M.from_workload(wl)
+        b.set_launch(*shape)
+        for first, cnt in wl.batches():
+            b.run_batch(wl.seed, first, cnt)
+        assert np.array_equal(a.get_cell_energy()[0], b.get_cell_energy()[0])
+        assert np.array_equal(a.get_sed(), b.get_sed())
+        assert np.array_equal(a.get_cell_temperature(), b.get_cell_temperature())
+        ca, cb = a.get_counters(), b.get_counters()
+        for k in ca:
+            assert np.array_equal(ca[k], cb[k]), k
 
 
 def test_pure_scattering_exact(M, oracle_mod):
