@@ -205,8 +205,8 @@ mcrt_status mcrt_get_image(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
 
 /* ---- tuning and introspection (do not change results) ---------------------------------------
  * Launch shape of the transport kernel: threads per block (multiple of 32, <= 256; 0 keeps the
- * current value) and resident blocks per SM (0 = automatic: 4, or 5 for a single-level grid the
- * L2 holds; more than 1024 resident threads per SM select the 48-register build of the kernel). */
+ * current value) and resident blocks per SM (0 = automatic: 5, or 4 for a single-level grid larger
+ * than the L2; more than 1024 resident threads per SM select the 48-register build of the kernel). */
 mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t blocks_per_sm);
 /* Single-level grids: a warp leaves the cell-walk loop to process its stopped lanes (escape,
  * refill, scattering, absorption) when fewer than `quorum` of its 32 lanes are still walking

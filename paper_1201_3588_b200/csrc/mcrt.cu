@@ -54,7 +54,7 @@ struct mcrt_ctx {
   unsigned long long* d_tally_scratch = nullptr;
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 16;
-  int threads = 256, blocks_per_sm = 0;   // 0 = automatic (4; 5 for the single-level kernel on L2-resident grids)
+  int threads = 256, blocks_per_sm = 0;   // 0 = automatic (5; 4 on HBM-resident single-level grids)
   long long launches = 0;
   // observer (O9 / R34): escape-direction tallies, off by default
   ObserverDev obs = {0, 0, 0, -1, {0, 0, 1}, {1, 0, 0}, {0, 1, 0}, 1.f, 1.f, nullptr, nullptr};
@@ -361,9 +361,9 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
 #endif
   CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
   const int threads = ctx->threads;
-  // resident blocks per SM: the caller's choice, else 5 for the single-level kernel on grids the
-  // L2 holds (x-fastest storage), 4 otherwise
-  const int bps = ctx->blocks_per_sm ? ctx->blocks_per_sm : (ctx->uni && !ctx->lay.bricked ? 5 : 4);
+  // resident blocks per SM: the caller's choice, else 5 (48-register kernels), except 4 for the
+  // single-level kernel on HBM-resident grids (bricked storage), where more threads thrash the L1
+  const int bps = ctx->blocks_per_sm ? ctx->blocks_per_sm : (ctx->uni && ctx->lay.bricked ? 4 : 5);
   long long want = ((long long)n + threads - 1) / threads;
   long long grid = (long long)ctx->sm_count * bps;
   if (want < grid) grid = want;

@@ -398,7 +398,9 @@ __device__ __forceinline__ bool walk_step(const TransportParams& P, Packet& p, f
 }
 
 template <bool TL>
-__global__ void __launch_bounds__(256, 4) k_transport(const TransportParams P) {
+// compiled for 5 resident blocks per SM (48 registers): c2 6.53 -> 6.41 ms, c3 15.9 -> 14.7 ms per
+// 2^22-package launch against the 64-register build (profiles/r01_summary.md)
+__global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* s_opac = reinterpret_cast<float4*>(smem_raw);                    // [nb]
   uint32_t* s_sed = reinterpret_cast<uint32_t*>(s_opac + P.nb);             // [3*nb]
