@@ -147,6 +147,9 @@ struct Ctx {
   std::vector<uint64_t> cum; std::vector<double> T; uint64_t Ncum = 0;
   std::vector<uint64_t> sed, emitted_per_bin; Counters cnt{};
   int walker = 0;                       // 0 = cell walk (O5), 1 = brute force (tests)
+  // O10: the ORIGINAL serial scheme the paper departs from:
+  // immediate temperature update at every absorption + Bjorkman & Wood (2001) corrected re-emission
+  bool bw_mode = false; uint64_t bw_ntotal = 0;
   // O9 observer (reading R34): escape-direction binning
   int n_mu = 0; std::vector<uint64_t> sed_mu;               // [n_mu][3][nb]
   int n_pix = 0; double obs[3] = {0, 0, 1}, e1[3] = {1, 0, 0}, e2[3] = {0, 1, 0};
@@ -342,6 +345,26 @@ int sample_emission_bin(const Ctx& c, double T, double u0, double u1) {
   return search_cdf(&c.C[(size_t)row * c.nb], c.nb, u0);
 }
 
+double leaf_mass(const Ctx& c, int64_t slot);
+
+// O10: Bjorkman & Wood (2001) temperature-corrected re-emission.  The cell went from T_old to
+// T_new by absorbing this package; the new package's frequency is drawn from
+// dP/dnu ~ kappa_nu [B_nu(T_new) - B_nu(T_old)], so that the sum of everything the cell has
+// emitted so far telescopes to kappa_nu B_nu(T_new).  CDF over the bins by the midpoint rule R5.
+int sample_bw_bin(const Ctx& c, double T_old, double T_new, double u) {
+  std::vector<double> cdf(c.nb);
+  double acc = 0;
+  for (int j = 0; j < c.nb; ++j) {
+    double w = c.kabs[j] * (planck_nu(c.nu[j], T_new) - planck_nu(c.nu[j], T_old)) * c.dnu[j];
+    acc += w > 0 ? w : 0.0;
+    cdf[j] = acc;
+  }
+  if (!(acc > 0)) return sample_emission_bin(c, T_new, u, 0.0);     // T did not move: Eqn 11.67 at T_new
+  for (int j = 0; j < c.nb; ++j) cdf[j] /= acc;
+  cdf[c.nb - 1] = 1.0;
+  return search_cdf(cdf.data(), c.nb, u);
+}
+
 // O7 / R12: invert Q(T) = q by bracketing + log-log interpolation; clamp.
 double temperature_from_q(const Ctx& c, double q) {
   if (!(q > c.Q[0])) return c.Tmin;
@@ -433,6 +456,14 @@ void run_packet(Ctx& c, uint64_t seed, uint64_t pid, std::vector<uint64_t>& batc
       batch[slot] += 1;
       double r[4];
       draw4(seed, pid, k, TAG_REEMIT, r);
+      if (c.bw_mode) {                                             // O10: serial only
+        double T_old = c.T[slot];
+        c.cum[slot] += 1;
+        double q = (double)c.cum[slot] * c.Ltot / ((double)c.bw_ntotal * 4.0 * PI * leaf_mass(c, slot));
+        double T_new = temperature_from_q(c, q);
+        c.T[slot] = T_new;
+        p.bin = sample_bw_bin(c, T_old, T_new, r[0]);
+      } else
       p.bin = sample_emission_bin(c, c.T[slot], r[0], r[1]);     // T frozen = T before absorption
       isotropic_dir(r[2], r[3], p.d);
       p.comp = COMP_THERMAL;
@@ -662,6 +693,21 @@ void orc_get_sed_mu(void* h, uint64_t* out) {
 void orc_get_image(void* h, uint64_t* out) {
   Ctx& c = *(Ctx*)h;
   for (size_t i = 0; i < c.image.size(); ++i) out[i] = c.image[i];
+}
+
+// O10: packages [first, first+n) of a job of n_total packages by the original serial scheme:
+// epsilon = L_tot / n_total fixed for the whole job (R9 reading A), every absorption raises the
+// cell's temperature at once, re-emission by sample_bw_bin.  Strictly serial (each absorption
+// changes T for the next package); cum[] holds the running counts, Ncum the packages run so far.
+int orc_run_bw(void* h, uint64_t seed, uint64_t first, uint64_t n, uint64_t n_total) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.have_source || n_total == 0) return -2;
+  c.bw_mode = true; c.bw_ntotal = n_total;
+  std::vector<uint64_t> unused(c.slots, 0);
+  for (uint64_t i = 0; i < n; ++i) run_packet(c, seed, first + i, unused, nullptr, 0, nullptr);
+  c.bw_mode = false;
+  c.Ncum += n;
+  return 0;
 }
 
 int orc_max_threads() {

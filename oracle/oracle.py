@@ -54,6 +54,7 @@ def lib():
                                        C.c_double, C.c_int, C.c_int]
         L.orc_get_sed_mu.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_get_image.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_run_bw.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64]
         L.orc_trace_packet.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_int, C.c_void_p,
                                        C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_cell_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -147,6 +148,11 @@ class Oracle:
         t = np.ascontiguousarray(tally_sum, dtype=np.uint64)
         assert t.shape == (self.slots,)
         rc = lib().orc_update_temperature(self.h, _p(t), int(n_cum))
+        assert rc == 0
+
+    def run_bw(self, seed: int, first: int, n: int, n_total: int):
+        """O10: the original serial scheme (immediate T update + Bjorkman-Wood correction)."""
+        rc = lib().orc_run_bw(self.h, seed, first, n, n_total)
         assert rc == 0
 
     def run(self, n_packets=None, batch=None, threads: int = 0):
