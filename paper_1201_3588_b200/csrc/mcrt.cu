@@ -52,6 +52,10 @@ struct mcrt_ctx {
   long long store_slots = 0;
   int* d_lut = nullptr;
   unsigned long long* d_tally_scratch = nullptr;
+  uint32_t* d_perm = nullptr;             // package numbers of a batch grouped by source
+  unsigned long long perm_cap = 0;
+  unsigned int* d_srccnt = nullptr;       // [2][nsrc] counts, cursors
+  int order_by_source = -1;               // -1 automatic (several sources and a grid larger than the L2), 0 off, 1 on
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 16;
   int threads = 256, blocks_per_sm = 0;   // 0 = automatic (5; 4 on HBM-resident single-level grids)
@@ -221,7 +225,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_sources(ctx);
   free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
-  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_out_scratch);
+  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -359,6 +363,25 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
 #ifdef MCRT_CHECKS
   CU(cudaMemcpyToSymbolAsync(g_mcrt_nstore, &ctx->store_slots, sizeof(long long), 0, cudaMemcpyHostToDevice, st));
 #endif
+  P.perm = nullptr;
+  const bool big = (size_t)ctx->store_slots * 4 > ((size_t)48 << 20);
+  const bool order = ctx->order_by_source < 0 ? (big && ctx->nsrc > 1) : (ctx->order_by_source != 0 && ctx->nsrc > 1);
+  if (order && ctx->nsrc <= kMaxOrderedSources && n >= 65536) {
+    if (ctx->perm_cap < n) {
+      cudaFree(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
+      CU(cudaMalloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
+      ctx->perm_cap = n;
+    }
+    if (!ctx->d_srccnt) CU(cudaMalloc(&ctx->d_srccnt, sizeof(unsigned int) * 2 * kMaxOrderedSources));
+    CU(cudaMemsetAsync(ctx->d_srccnt, 0, sizeof(unsigned int) * 2 * kMaxOrderedSources, st));
+    const unsigned gblocks = (unsigned)ctx->sm_count * 8u;
+    const size_t gsmem = sizeof(unsigned int) * 2 * (size_t)ctx->nsrc;
+    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, ctx->d_srccnt, nullptr, nullptr);
+    k_scan_sources<<<1, 32, 0, st>>>(ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->nsrc);
+    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->d_perm);
+    ctx->launches += 3;
+    P.perm = ctx->d_perm;
+  }
   CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
   const int threads = ctx->threads;
   // resident blocks per SM: the caller's choice, else 5 (48-register kernels), except 4 for the
@@ -624,6 +647,13 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
   if (!ctx) return MCRT_EINVAL;
   if (quorum < 0 || quorum > 32) return fail(ctx, MCRT_EINVAL, "mcrt_set_walk_quorum: quorum must be 0..32");
   ctx->quorum = quorum ? quorum : 16;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_set_source_order(mcrt_ctx* ctx, int32_t mode) {
+  if (!ctx) return MCRT_EINVAL;
+  if (mode < -1 || mode > 1) return fail(ctx, MCRT_EINVAL, "mcrt_set_source_order: mode must be -1, 0 or 1");
+  ctx->order_by_source = mode;
   return MCRT_OK;
 }
 

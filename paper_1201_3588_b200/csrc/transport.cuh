@@ -65,6 +65,7 @@ struct TransportParams {
   const float* __restrict__ csrc;              // [nsrc][nb] source spectrum CDFs
   const SrcDev* __restrict__ src;              // [nsrc]
   unsigned long long* next;                    // work-queue head (packet offset within the batch)
+  const uint32_t* __restrict__ perm;           // NULL, or the batch's package numbers grouped by source
   unsigned long long* sed;                     // [3][nb]
   unsigned long long* emit_bin;                // [nb]
   unsigned long long* counters;                // [CNT_N]
@@ -433,7 +434,7 @@ __global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
       if (state == ST_FETCH) {
         unsigned long long my = base + (unsigned long long)__popc(need & lt_mask);
         if (my < P.count) {
-          p.pid = P.first + my;
+          p.pid = P.first + (P.perm ? (unsigned long long)__ldg(P.perm + my) : my);
           emit_packet<TL>(P, p, s_opac);                    // a1
           kx = s_opac[p.bin].x;
           ++cnt[CNT_EMITTED];
@@ -537,6 +538,60 @@ __global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
     if (s_sed[i]) atomicAdd(P.sed + i, (unsigned long long)s_sed[i]);
   for (int i = threadIdx.x; i < P.nb; i += blockDim.x)
     if (s_emit[i]) atomicAdd(P.emit_bin + i, (unsigned long long)s_emit[i]);
+}
+
+
+// ---- a8, several sources: hand the packages out GROUPED BY SOURCE ----------------------------
+// Packages of one source cross the same neighbourhood, so when the packages in flight share a
+// source the L2 serves far more of their density gathers (profiles/r01_summary.md: 512^3 cube,
+// one source at a time 1.5-1.8e11 crossings/s against 1.17e11 with the eleven sources mixed).
+// The source of package i is the first decision of its emission (O4: u0 of its EMIT block), so a
+// pre-pass can group the batch's package numbers by source: count, exclusive scan, scatter.  The
+// order inside a group is arbitrary; integer tallies make the results independent of it.
+constexpr int kMaxOrderedSources = 2048;
+
+__device__ __forceinline__ int source_of(const TransportParams& P, unsigned long long pid) {
+  uint32_t x[4];
+  philox4x32_10((uint32_t)P.seed, (uint32_t)(P.seed >> 32), (uint32_t)pid, (uint32_t)(pid >> 32), 0u, kTagEmit, x);
+  const float u0 = u01(x[0]);
+  int s = 0;
+  while (s < P.nsrc - 1 && P.src[s].lcdf < u0) ++s;
+  return s;
+}
+
+// counts[s] += packages of source s (cursor == NULL), or perm[cursor[s]++] = package number
+__global__ void k_group_by_source(const TransportParams P, unsigned int* __restrict__ counts,
+                                  unsigned int* __restrict__ cursor, uint32_t* __restrict__ perm) {
+  extern __shared__ unsigned int s_cnt[];                    // [2 * nsrc]: block histogram, block bases
+  for (int i = threadIdx.x; i < 2 * P.nsrc; i += blockDim.x) s_cnt[i] = 0;
+  __syncthreads();
+  const unsigned long long per_block = (P.count + gridDim.x - 1) / gridDim.x;
+  const unsigned long long lo = per_block * blockIdx.x, hi = min(P.count, lo + per_block);
+  for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x)
+    atomicAdd(&s_cnt[source_of(P, P.first + i)], 1u);
+  __syncthreads();
+  if (!cursor) {
+    for (int i = threadIdx.x; i < P.nsrc; i += blockDim.x)
+      if (s_cnt[i]) atomicAdd(&counts[i], s_cnt[i]);
+    return;
+  }
+  for (int i = threadIdx.x; i < P.nsrc; i += blockDim.x) {   // reserve this block's range in every group
+    s_cnt[P.nsrc + i] = s_cnt[i] ? atomicAdd(&cursor[i], s_cnt[i]) : 0u;
+    s_cnt[i] = 0;
+  }
+  __syncthreads();
+  for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+    const int s = source_of(P, P.first + i);
+    perm[s_cnt[P.nsrc + s] + atomicAdd(&s_cnt[s], 1u)] = (uint32_t)i;
+  }
+}
+
+// cursor[s] = sum of counts[0..s) (one block; nsrc <= kMaxOrderedSources)
+__global__ void k_scan_sources(const unsigned int* __restrict__ counts, unsigned int* __restrict__ cursor, int nsrc) {
+  if (threadIdx.x == 0) {
+    unsigned int acc = 0;
+    for (int s = 0; s < nsrc; ++s) { cursor[s] = acc; acc += counts[s]; }
+  }
 }
 
 }  // namespace mcrt

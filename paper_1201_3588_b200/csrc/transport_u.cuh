@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       if (base + 32ull > P.count) quorum = 1;                // queue (nearly) empty: no more refills
       if (state == SU_FETCH) {
         unsigned long long my = base + (unsigned long long)__popc(need & lt_mask);
-        if (my < P.count) { p.off = (uint32_t)my; is_new = true; }
+        if (my < P.count) { p.off = P.perm ? __ldg(P.perm + my) : (uint32_t)my; is_new = true; }
         else state = SU_DONE;
       }
     }

@@ -54,7 +54,7 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_update_temperature", "mcrt_get_cell_energy",
            "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_observer",
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
-           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum",
+           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
            "mcrt_get_batch_times", "mcrt_get_tables",
            "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_gather_calibrate", "mcrt_last_error")
 
@@ -88,6 +88,7 @@ def lib():
         L.mcrt_reset_tallies.argtypes = [vp, i32]
         L.mcrt_set_launch.argtypes = [vp, i32, i32]
         L.mcrt_set_walk_quorum.argtypes = [vp, i32]
+        L.mcrt_set_source_order.argtypes = [vp, i32]
         L.mcrt_get_batch_times.argtypes = [vp, vp, vp, i32, C.POINTER(i32)]
         L.mcrt_get_tables.argtypes = [vp, vp, vp, vp]
         L.mcrt_kernel_launches.restype = i64
@@ -104,7 +105,8 @@ def lib():
                      "mcrt_get_cell_energy", "mcrt_get_cell_temperature",
                      "mcrt_get_sed", "mcrt_set_observer", "mcrt_get_sed_mu", "mcrt_get_image",
                      "mcrt_get_counters", "mcrt_reset_tallies",
-                     "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_get_batch_times",
+                     "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
+                     "mcrt_get_batch_times",
                      "mcrt_get_tables",
                      "mcrt_philox_blocks"):
             getattr(L, name).restype = C.c_int
@@ -299,6 +301,9 @@ class Context:
 
     def set_walk_quorum(self, quorum):
         self._check(lib().mcrt_set_walk_quorum(self.h, int(quorum)), "mcrt_set_walk_quorum")
+
+    def set_source_order(self, mode):
+        self._check(lib().mcrt_set_source_order(self.h, int(mode)), "mcrt_set_source_order")
 
     def get_batch_times(self, cap=4096):
         t = np.zeros(cap, dtype=np.float32)

@@ -393,3 +393,22 @@ def test_c4_full_grid_against_oracle(M, oracle_mod):
     assert c["emitted"] == c["escaped"] == n + m and c["lost"] == 0
     PR.check_self_consistency(c, n_abs, sed)
     _temperature_identity(M, ctx, wl, n + m)
+
+
+@pytest.mark.parametrize("layout", [1, 2])
+def test_source_grouped_handout_does_not_change_results(M, layout):
+    """Several sources: handing the packages of a batch out grouped by source (mcrt_set_source_order)
+    only changes which lane carries which package; every count must be identical.  Batches of
+    2^17 packages so that the pre-pass really runs (it skips batches below 65536)."""
+    wl = W.c4(n_root=24, n_packets=3 << 17, batch=1 << 17, corr_cells=3.0)
+    assert len(wl.sources) == 11
+    runs = []
+    for mode in (0, 1):
+        ctx = M.from_workload(wl, layout=layout)
+        ctx.set_source_order(mode)
+        for first, cnt in wl.batches():
+            ctx.run_batch(wl.seed, first, cnt)
+        runs.append(ctx)
+    _assert_identical(runs[0], runs[1])
+    assert runs[1].get_counters()["emitted"] == wl.n_packets
+    assert runs[1].kernel_launches() == runs[0].kernel_launches() + 3 * 3      # three pre-pass kernels per batch
