@@ -55,7 +55,7 @@ struct mcrt_ctx {
   uint32_t* d_perm = nullptr;             // package numbers of a batch grouped by source
   unsigned long long perm_cap = 0;
   unsigned int* d_srccnt = nullptr;       // [2][nsrc] counts, cursors
-  int order_by_source = -1;               // -1 automatic (several sources and a grid larger than the L2), 0 off, 1 on
+  int order_by_source = -1;               // -1 automatic, 0 off, 1 by source, 2 by source and start direction
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 16;
   int threads = 256, blocks_per_sm = 0;   // 0 = automatic (5; 4 on HBM-resident single-level grids)
@@ -365,8 +365,12 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
 #endif
   P.perm = nullptr;
   const bool big = (size_t)ctx->store_slots * 4 > ((size_t)48 << 20);
-  const bool order = ctx->order_by_source < 0 ? (big && ctx->nsrc > 1) : (ctx->order_by_source != 0 && ctx->nsrc > 1);
-  if (order && ctx->nsrc <= kMaxOrderedSources && n >= 65536) {
+  // 0 off, 1 grouped by source, 2 by source and start direction; automatic: 2 on grids larger than the L2
+  int gmode = ctx->order_by_source < 0 ? (big ? 2 : 0) : ctx->order_by_source;
+  if (gmode == 1 && ctx->nsrc < 2) gmode = 0;
+  int sub = gmode == 2 ? 32 : 1;
+  if (sub * ctx->nsrc > kMaxOrderedSources) sub = 1;
+  if (gmode && sub * ctx->nsrc <= kMaxOrderedSources && (sub > 1 || ctx->nsrc > 1) && n >= 65536) {
     if (ctx->perm_cap < n) {
       cudaFree(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
       CU(cudaMalloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
@@ -375,10 +379,10 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
     if (!ctx->d_srccnt) CU(cudaMalloc(&ctx->d_srccnt, sizeof(unsigned int) * 2 * kMaxOrderedSources));
     CU(cudaMemsetAsync(ctx->d_srccnt, 0, sizeof(unsigned int) * 2 * kMaxOrderedSources, st));
     const unsigned gblocks = (unsigned)ctx->sm_count * 8u;
-    const size_t gsmem = sizeof(unsigned int) * 2 * (size_t)ctx->nsrc;
-    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, ctx->d_srccnt, nullptr, nullptr);
-    k_scan_sources<<<1, 32, 0, st>>>(ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->nsrc);
-    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->d_perm);
+    const size_t gsmem = sizeof(unsigned int) * 2 * (size_t)ctx->nsrc * sub;
+    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, nullptr, nullptr);
+    k_scan_sources<<<1, 32, 0, st>>>(ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->nsrc * sub);
+    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->d_perm);
     ctx->launches += 3;
     P.perm = ctx->d_perm;
   }
@@ -652,7 +656,7 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
 
 mcrt_status mcrt_set_source_order(mcrt_ctx* ctx, int32_t mode) {
   if (!ctx) return MCRT_EINVAL;
-  if (mode < -1 || mode > 1) return fail(ctx, MCRT_EINVAL, "mcrt_set_source_order: mode must be -1, 0 or 1");
+  if (mode < -1 || mode > 2) return fail(ctx, MCRT_EINVAL, "mcrt_set_source_order: mode must be -1, 0, 1 or 2");
   ctx->order_by_source = mode;
   return MCRT_OK;
 }

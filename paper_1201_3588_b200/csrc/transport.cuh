@@ -544,45 +544,57 @@ __global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
 // ---- a8, several sources: hand the packages out GROUPED BY SOURCE ----------------------------
 // Packages of one source cross the same neighbourhood, so when the packages in flight share a
 // source the L2 serves far more of their density gathers (profiles/r01_summary.md: 512^3 cube,
-// one source at a time 1.5-1.8e11 crossings/s against 1.17e11 with the eleven sources mixed).
+// one source at a time 1.5-1.8e11 crossings/s against 1.17e11 with the eleven sources mixed);
+// packages that also start in the same direction share their whole first flight.
 // The source of package i is the first decision of its emission (O4: u0 of its EMIT block), so a
 // pre-pass can group the batch's package numbers by source: count, exclusive scan, scatter.  The
 // order inside a group is arbitrary; integer tallies make the results independent of it.
 constexpr int kMaxOrderedSources = 2048;
 
-__device__ __forceinline__ int source_of(const TransportParams& P, unsigned long long pid) {
+// group key of a package: its source, refined (sub = 32) by where it starts to fly: 4 x 8 bins in
+// (mu, phi) of the emission direction for a point source, face x 2 x 2 tiles for the external field
+__device__ __forceinline__ int group_of(const TransportParams& P, unsigned long long pid, int sub) {
   uint32_t x[4];
   philox4x32_10((uint32_t)P.seed, (uint32_t)(P.seed >> 32), (uint32_t)pid, (uint32_t)(pid >> 32), 0u, kTagEmit, x);
   const float u0 = u01(x[0]);
   int s = 0;
   while (s < P.nsrc - 1 && P.src[s].lcdf < u0) ++s;
-  return s;
+  if (sub == 1) return s;
+  int b;
+  if (P.src[s].type == 0) {
+    b = min(3, (int)(4.f * u01(x[2]))) * 8 + min(7, (int)(8.f * u01(x[3])));
+  } else {
+    philox4x32_10((uint32_t)P.seed, (uint32_t)(P.seed >> 32), (uint32_t)pid, (uint32_t)(pid >> 32), 1u, kTagEmit, x);
+    b = min(5, (int)(6.f * u01(x[0]))) * 4 + (u01(x[1]) >= 0.5f ? 1 : 0) + (u01(x[2]) >= 0.5f ? 2 : 0);
+  }
+  return s * sub + b;
 }
 
-// counts[s] += packages of source s (cursor == NULL), or perm[cursor[s]++] = package number
-__global__ void k_group_by_source(const TransportParams P, unsigned int* __restrict__ counts,
+// counts[g] += packages of group g (cursor == NULL), or perm[cursor[g]++] = package number
+__global__ void k_group_by_source(const TransportParams P, const int sub, unsigned int* __restrict__ counts,
                                   unsigned int* __restrict__ cursor, uint32_t* __restrict__ perm) {
-  extern __shared__ unsigned int s_cnt[];                    // [2 * nsrc]: block histogram, block bases
-  for (int i = threadIdx.x; i < 2 * P.nsrc; i += blockDim.x) s_cnt[i] = 0;
+  extern __shared__ unsigned int s_cnt[];                    // [2 * ngroups]: block histogram, block bases
+  const int ng = P.nsrc * sub;
+  for (int i = threadIdx.x; i < 2 * ng; i += blockDim.x) s_cnt[i] = 0;
   __syncthreads();
   const unsigned long long per_block = (P.count + gridDim.x - 1) / gridDim.x;
   const unsigned long long lo = per_block * blockIdx.x, hi = min(P.count, lo + per_block);
   for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x)
-    atomicAdd(&s_cnt[source_of(P, P.first + i)], 1u);
+    atomicAdd(&s_cnt[group_of(P, P.first + i, sub)], 1u);
   __syncthreads();
   if (!cursor) {
-    for (int i = threadIdx.x; i < P.nsrc; i += blockDim.x)
+    for (int i = threadIdx.x; i < ng; i += blockDim.x)
       if (s_cnt[i]) atomicAdd(&counts[i], s_cnt[i]);
     return;
   }
-  for (int i = threadIdx.x; i < P.nsrc; i += blockDim.x) {   // reserve this block's range in every group
-    s_cnt[P.nsrc + i] = s_cnt[i] ? atomicAdd(&cursor[i], s_cnt[i]) : 0u;
+  for (int i = threadIdx.x; i < ng; i += blockDim.x) {       // reserve this block's range in every group
+    s_cnt[ng + i] = s_cnt[i] ? atomicAdd(&cursor[i], s_cnt[i]) : 0u;
     s_cnt[i] = 0;
   }
   __syncthreads();
   for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
-    const int s = source_of(P, P.first + i);
-    perm[s_cnt[P.nsrc + s] + atomicAdd(&s_cnt[s], 1u)] = (uint32_t)i;
+    const int g = group_of(P, P.first + i, sub);
+    perm[s_cnt[ng + g] + atomicAdd(&s_cnt[g], 1u)] = (uint32_t)i;
   }
 }
 

@@ -402,13 +402,15 @@ def test_source_grouped_handout_does_not_change_results(M, layout):
     2^17 packages so that the pre-pass really runs (it skips batches below 65536)."""
     wl = W.c4(n_root=24, n_packets=3 << 17, batch=1 << 17, corr_cells=3.0)
     assert len(wl.sources) == 11
-    runs = []
-    for mode in (0, 1):
+    runs, launches = [], []
+    for mode in (0, 1, 2):                                      # off / by source / by source and direction
         ctx = M.from_workload(wl, layout=layout)
         ctx.set_source_order(mode)
         for first, cnt in wl.batches():
             ctx.run_batch(wl.seed, first, cnt)
         runs.append(ctx)
+        launches.append(ctx.kernel_launches())                  # before any getter launches a conversion
     _assert_identical(runs[0], runs[1])
+    _assert_identical(runs[0], runs[2])
     assert runs[1].get_counters()["emitted"] == wl.n_packets
-    assert runs[1].kernel_launches() == runs[0].kernel_launches() + 3 * 3      # three pre-pass kernels per batch
+    assert launches[1] == launches[2] == launches[0] + 3 * 3    # three pre-pass kernels per batch
