@@ -215,10 +215,11 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum);
 /* Hand the packages of a batch to the lanes grouped by where they start (a pre-pass evaluates the
  * first decisions of every package's emission and groups the package numbers), so that the
  * packages in flight share a neighbourhood and the L2 serves more of their gathers.  mode 1 =
- * grouped by source, 2 = by source and start direction (4 x 8 bins in (mu, phi) for a point
- * source, face x 2 x 2 tiles for the external field), 0 = off, -1 = automatic (2 when the density
- * array is larger than the L2).  Batches below 65536 packages are never reordered; more than 64
- * sources fall back to mode 1, more than 2048 to 0.  Integer tallies: results do not depend on it. */
+ * grouped by source, 2 = by source and start direction (8 x 16 bins in (mu, phi) for a point
+ * source -- 4 x 8 with more than 16 sources --, face x 2 x 2 tiles for the external field), 0 =
+ * off, -1 = automatic (2 when the density array is larger than the L2 or the batch has at least
+ * 2^21 packages).  Batches below 65536 packages are never reordered; more than 64 sources fall
+ * back to mode 1, more than 2048 to 0.  Integer tallies: results do not depend on it. */
 mcrt_status mcrt_set_source_order(mcrt_ctx* ctx, int32_t mode);
 /* Device times in ms of the mcrt_run_batch calls made since the previous call of this function
  * (oldest first, at most `cap`), split into the two kernels of a batch (transport, temperature

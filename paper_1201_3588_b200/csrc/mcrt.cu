@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -365,11 +366,12 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
 #endif
   P.perm = nullptr;
   const bool big = (size_t)ctx->store_slots * 4 > ((size_t)48 << 20);
-  // 0 off, 1 grouped by source, 2 by source and start direction; automatic: 2 on grids larger than the L2
-  int gmode = ctx->order_by_source < 0 ? (big ? 2 : 0) : ctx->order_by_source;
+  // 0 off, 1 grouped by source, 2 by source and start direction; automatic: 2 when the pre-pass is
+  // small against the batch (grid larger than the L2, or at least 2^21 packages)
+  int gmode = ctx->order_by_source < 0 ? ((big || n >= (1ull << 21)) ? 2 : 0) : ctx->order_by_source;
   if (gmode == 1 && ctx->nsrc < 2) gmode = 0;
-  int sub = gmode == 2 ? 32 : 1;
-  if (sub * ctx->nsrc > kMaxOrderedSources) sub = 1;
+  int sub = 1;                                               // start-direction sub-groups per source
+  if (gmode == 2) sub = ctx->nsrc * 128 <= kMaxOrderedSources ? 128 : (ctx->nsrc * 32 <= kMaxOrderedSources ? 32 : 1);
   if (gmode && sub * ctx->nsrc <= kMaxOrderedSources && (sub > 1 || ctx->nsrc > 1) && n >= 65536) {
     if (ctx->perm_cap < n) {
       cudaFree(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;

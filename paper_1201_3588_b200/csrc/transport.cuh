@@ -551,8 +551,9 @@ __global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
 // order inside a group is arbitrary; integer tallies make the results independent of it.
 constexpr int kMaxOrderedSources = 2048;
 
-// group key of a package: its source, refined (sub = 32) by where it starts to fly: 4 x 8 bins in
-// (mu, phi) of the emission direction for a point source, face x 2 x 2 tiles for the external field
+// group key of a package: its source, refined by where it starts to fly: sub = 128 (32) bins, 8 x 16
+// (4 x 8) in (mu, phi) of the emission direction for a point source, face x 2 x 2 tiles for the
+// external field
 __device__ __forceinline__ int group_of(const TransportParams& P, unsigned long long pid, int sub) {
   uint32_t x[4];
   philox4x32_10((uint32_t)P.seed, (uint32_t)(P.seed >> 32), (uint32_t)pid, (uint32_t)(pid >> 32), 0u, kTagEmit, x);
@@ -562,7 +563,8 @@ __device__ __forceinline__ int group_of(const TransportParams& P, unsigned long 
   if (sub == 1) return s;
   int b;
   if (P.src[s].type == 0) {
-    b = min(3, (int)(4.f * u01(x[2]))) * 8 + min(7, (int)(8.f * u01(x[3])));
+    b = sub == 32 ? min(3, (int)(4.f * u01(x[2]))) * 8 + min(7, (int)(8.f * u01(x[3])))
+                  : min(7, (int)(8.f * u01(x[2]))) * 16 + min(15, (int)(16.f * u01(x[3])));
   } else {
     philox4x32_10((uint32_t)P.seed, (uint32_t)(P.seed >> 32), (uint32_t)pid, (uint32_t)(pid >> 32), 1u, kTagEmit, x);
     b = min(5, (int)(6.f * u01(x[0]))) * 4 + (u01(x[1]) >= 0.5f ? 1 : 0) + (u01(x[2]) >= 0.5f ? 2 : 0);
