@@ -32,7 +32,10 @@
 // bin-by-bin conservation; Beer-Lambert escape vs brute-force chords; optically thin
 // T ~ r^(-2/(4+beta)); per-flight agreement with an "intersect every box" walker (a second,
 // independent algorithm, also re-implemented in numpy in the tests); split invariance on a
-// two-level grid; external-field mean chord 2a/3.
+// two-level grid; external-field mean chord 2a/3.  O9 (direction-resolved tallies,
+// tests/test_oracle_observer.py): sum identity, isotropy in mu, cone fraction, hand-computed
+// projection geometry, symmetry.  O10 (serial Bjorkman-Wood scheme, tests/test_oracle_bw.py):
+// telescoping of the corrected emission to the Planck spectrum at the final temperature.
 // PARITY UNPINNED: the full multi-scattering + re-emission SED and temperatures at
 // tau_V >= 1 have no closed form and the paper's benchmarks are not
 // available; they are held only by the component pins above.
