@@ -238,6 +238,10 @@ def test_error_paths(M):
     wl = W.c0()
     with pytest.raises(M.McrtError):
         ctx.grid_create(0, 0, wl.origin, wl.root_size, None, wl.rho_root, None)
+    with pytest.raises(M.McrtError):          # beyond the largest grid (N^3 must stay below 2^31 slots)
+        ctx.grid_create(1291, 0, wl.origin, wl.root_size, None, wl.rho_root, None)
+    with pytest.raises(M.McrtError):          # unknown storage layout
+        ctx.grid_create(wl.n_root, 0, wl.origin, wl.root_size, None, wl.rho_root, None, layout=7)
     ctx.grid_create(wl.n_root, 0, wl.origin, wl.root_size, None, wl.rho_root, None)
     with pytest.raises(M.McrtError):          # ESTATE: opacity not set
         ctx.set_source(wl.sources)
