@@ -418,3 +418,26 @@ def test_source_grouped_handout_does_not_change_results(M, layout):
     _assert_identical(runs[0], runs[2])
     assert runs[1].get_counters()["emitted"] == wl.n_packets
     assert launches[1] == launches[2] == launches[0] + 3 * 3    # three pre-pass kernels per batch
+
+
+@pytest.mark.parametrize("maker", [W.c2, W.c3])
+def test_disk_configs_full_size_invariants(M, maker):
+    """configs[2] / configs[3] at their full grids (128^3 + 17 256 x 4^3, 256^3 + 224 872 x 4^3), one
+    full 2^22-package batch in bench.py's launch configuration (grouped hand-out on): exact
+    integer accounting and consistency of every tally; refined root slots stay untouched."""
+    wl = maker()
+    n = wl.batch
+    assert n == 1 << 22 and wl.n_ref > 0
+    ctx = M.from_workload(wl)
+    ctx.run_batch(wl.seed, 0, n)
+    c = ctx.get_counters()
+    n_abs, eps = ctx.get_cell_energy()
+    sed = ctx.get_sed()
+    assert c["emitted"] == c["escaped"] == n and c["lost"] == 0
+    PR.check_self_consistency(c, n_abs, sed)
+    assert int(c["emitted_per_bin"].sum()) == n
+    refined = np.flatnonzero(np.asarray(wl.refine).ravel())
+    assert n_abs[refined].sum() == 0                            # the slot of a refined cube is unused (R22)
+    T = ctx.get_cell_temperature()
+    assert np.all(T[refined] == np.float32(1.0)) and np.isfinite(T).all() and T.min() >= 1.0
+    assert (T[n_abs > 0] > 1.0).all()
