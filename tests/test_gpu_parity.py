@@ -441,3 +441,17 @@ def test_disk_configs_full_size_invariants(M, maker):
     T = ctx.get_cell_temperature()
     assert np.all(T[refined] == np.float32(1.0)) and np.isfinite(T).all() and T.min() >= 1.0
     assert (T[n_abs > 0] > 1.0).all()
+
+
+def test_grouped_handout_two_level_grid(M):
+    """The grouped hand-out on the two-level kernel (one star, direction groups only)."""
+    wl = W.c2(n_root=32, n_packets=3 << 17, batch=1 << 17)
+    runs = []
+    for mode in (0, 2):
+        ctx = M.from_workload(wl)
+        ctx.set_source_order(mode)
+        for first, cnt in wl.batches():
+            ctx.run_batch(wl.seed, first, cnt)
+        runs.append(ctx)
+    _assert_identical(runs[0], runs[1])
+    assert runs[1].get_counters()["emitted"] == wl.n_packets
