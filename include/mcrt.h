@@ -71,11 +71,11 @@ typedef struct {
   const float* rho_root; /* [N^3] g cm^-3 of dust; ignored where refine = 1                   */
   const float* rho_sub;  /* [n_ref*S^3]; NULL iff no cube is refined                          */
   mcrt_mem mem;          /* where refine / rho_root / rho_sub live                            */
-  int32_t layout;        /* device storage order of a single-level grid (never visible in the
-                            getters, which always use the slot order above): 0 = automatic
-                            (x-fastest while the density array fits the L2 comfortably, else
-                            bricked), 1 = x-fastest, 2 = 8^3 bricks in Morton order.  Ignored
-                            for two-level grids.                                               */
+  int32_t layout;        /* device storage order of the root grid (never visible in the getters,
+                            which always use the slot order above): 0 = automatic (bricked for
+                            a single-level grid larger than the L2, else x-fastest), 1 =
+                            x-fastest, 2 = 8^3 bricks in Morton order.  Subcubes always follow
+                            the root grid as blocks of sub^3.                                  */
 } mcrt_grid_desc;
 
 /* Creates a context on the current CUDA device and uploads the grid. */

@@ -27,6 +27,8 @@ struct mcrt_ctx {
   int device = 0, sm_count = 0;
   int N = 0, S = 1;
   long long n3 = 0, n_ref = 0, slots = 0;
+  long long store_n3 = 0;                 // storage slots of the root grid (sub-cells follow it)
+  int* d_axtab = nullptr;                 // two-level grids with a bricked root: [3][N] axis terms of the root slot
   double origin[3] = {0, 0, 0}, root_size = 1;
   float* d_rho = nullptr;
   unsigned long long* d_tally = nullptr;
@@ -148,19 +150,20 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
   ctx->slots = n3 + k * s3;
   if (ctx->slots >= (1ll << 31)) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: more than 2^31-1 leaf slots"));
   if (k > 0 && !d->rho_sub) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: rho_sub is NULL but cubes are refined"));
-  ctx->store_slots = ctx->slots;
-  if (k == 0) {                                             // single-level grid: pick the storage order
-    if (d->layout < 0 || d->layout > 2) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: layout must be 0, 1 or 2"));
-    ctx->uni = true;
-    ctx->lay.N = d->n_root;
-    ctx->lay.nbk = (d->n_root + 7) / 8;
-    ctx->lay.bricked = d->layout == 2 || (d->layout == 0 && n3 * 4 > (48ll << 20));
-    ctx->store_slots = slots_of(ctx->lay);
-    if (ctx->store_slots >= (1ll << 31)) {                   // padding pushed it over: fall back
-      ctx->lay.bricked = 0;
-      ctx->store_slots = n3;
-    }
+  // storage order of the root grid (both kinds of grid; sub-cells always follow as blocks of S^3)
+  if (d->layout < 0 || d->layout > 2) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: layout must be 0, 1 or 2"));
+  ctx->uni = k == 0;
+  ctx->lay.N = d->n_root;
+  ctx->lay.nbk = (d->n_root + 7) / 8;
+  // automatic: bricks for single-level grids larger than the L2; on two-level grids most crossings are in
+  // subcubes (already blocks of S^3) and the bricked root measured slower (c3 13.3 vs 12.2 ms per batch)
+  ctx->lay.bricked = d->layout == 2 || (d->layout == 0 && k == 0 && n3 * 4 > (48ll << 20));
+  ctx->store_n3 = slots_of(ctx->lay);
+  if (ctx->store_n3 + k * s3 >= (1ll << 31)) {               // padding pushed it over: fall back
+    ctx->lay.bricked = 0;
+    ctx->store_n3 = n3;
   }
+  ctx->store_slots = ctx->store_n3 + k * s3;
   CUG(cudaMalloc(&ctx->d_rho, sizeof(float) * ctx->store_slots));
   CUG(cudaMalloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->store_slots));
   CUG(cudaMalloc(&ctx->d_trow, sizeof(float) * ctx->store_slots));
@@ -202,11 +205,20 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
     k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho, ctx->lay, n3);
   } else {
-    k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, (int)n3);
+    if (ctx->lay.bricked) {                                  // the kernel adds three axis terms from shared memory
+      const int N = ctx->N;
+      std::vector<int> tab(3 * (size_t)N);
+      for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < N; ++i) tab[(size_t)a * N + i] = (int)axis_term(ctx->lay, a, i);
+      CUG(cudaMalloc(&ctx->d_axtab, sizeof(int) * tab.size()));
+      CUG(cudaMemcpy(ctx->d_axtab, tab.data(), sizeof(int) * tab.size(), cudaMemcpyHostToDevice));
+    }
+    CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
+    k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, ctx->lay, n3);
   }
   ctx->launches++;
   if (k > 0) {
-    k_sanitize<<<(unsigned)((k * s3 + 255) / 256), 256>>>(src_sub, ctx->d_rho + n3, k * s3);
+    k_sanitize<<<(unsigned)((k * s3 + 255) / 256), 256>>>(src_sub, ctx->d_rho + ctx->store_n3, k * s3);
     ctx->launches++;
   }
   CUG(cudaGetLastError());
@@ -226,7 +238,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_sources(ctx);
   free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
-  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
+  cudaFree(ctx->d_lut); cudaFree(ctx->d_axtab); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -360,7 +372,8 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
   P.seed = seed; P.first = first; P.count = n;
   P.obs = ctx->obs;
-  P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->n3;
+  P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->store_n3;
+  P.axtab = ctx->uni ? nullptr : ctx->d_axtab;
 #ifdef MCRT_CHECKS
   CU(cudaMemcpyToSymbolAsync(g_mcrt_nstore, &ctx->store_slots, sizeof(long long), 0, cudaMemcpyHostToDevice, st));
 #endif
@@ -404,6 +417,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
     if (bps * threads > 1024) k_transport_u<5><<<(unsigned)grid, threads, smem, st>>>(PU);   // 48 registers
     else k_transport_u<4><<<(unsigned)grid, threads, smem, st>>>(PU);                        // 64 registers
   } else {
+    if (P.axtab) smem += sizeof(int) * 3 * (size_t)ctx->N;
     k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
   }
   ctx->launches++;
@@ -419,13 +433,16 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
   double V = ctx->root_size * ctx->root_size * ctx->root_size;
   float ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)n_cum) - std::log(4.0 * PI) - std::log(V));
   float ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
-  if (tally != ctx->d_tally && ctx->uni && ctx->lay.bricked) {     // caller's sum is in slot order (R22)
+  if (tally != ctx->d_tally && ctx->lay.bricked) {                 // caller's sum is in slot order (R22)
     if (!ctx->d_tally_scratch) {
       CU(cudaMalloc(&ctx->d_tally_scratch, 8 * (size_t)ctx->store_slots));
       CU(cudaMemsetAsync(ctx->d_tally_scratch, 0, 8 * (size_t)ctx->store_slots, st));
     }
     k_ext_to_store_u64<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(tally, ctx->d_tally_scratch, ctx->lay, ctx->n3);
     ctx->launches++;
+    if (ctx->slots > ctx->n3)                                // sub-cells keep their order behind the root grid
+      CU(cudaMemcpyAsync(ctx->d_tally_scratch + ctx->store_n3, tally + ctx->n3, 8 * (size_t)(ctx->slots - ctx->n3),
+                         cudaMemcpyDeviceToDevice, st));
     tally = ctx->d_tally_scratch;
   }
   long long blocks = (ctx->store_slots + 255) / 256;
@@ -433,7 +450,7 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
   if (blocks > cap) blocks = cap;
   k_update_temperature<<<(unsigned)blocks, 256, 4 * ctx->nT, st>>>(ctx->d_rho, tally, ctx->d_trow, ctx->d_lnQ,
                                                                   ctx->nT, ctx->store_slots,
-                                                                  ctx->uni ? ctx->store_slots : ctx->n3,
+                                                                  ctx->uni ? ctx->store_slots : ctx->store_n3,
                                                                   ln_coef, ln_sub3);
   ctx->launches++;
   CU(cudaGetLastError());
@@ -513,7 +530,7 @@ mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps
   if (!ctx) return MCRT_EINVAL;
   if (!n_abs_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_energy: NULL output");
   if (eps_out) *eps_out = ctx->Ncum ? ctx->Ltot / (double)ctx->Ncum : 0.0;
-  if (ctx->uni && ctx->lay.bricked) {                        // storage order -> slot order (R22)
+  if (ctx->lay.bricked) {                                    // storage order -> slot order (R22)
     unsigned long long* d_out = (unsigned long long*)n_abs_out;
     unsigned long long* tmp = nullptr;
     if (mem == MCRT_HOST) {
@@ -524,6 +541,9 @@ mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps
         ctx->d_tally, d_out, ctx->lay, ctx->n3);
     ctx->launches++;
     CU(cudaGetLastError());
+    if (ctx->slots > ctx->n3)
+      CU(cudaMemcpyAsync(d_out + ctx->n3, ctx->d_tally + ctx->store_n3, 8 * (size_t)(ctx->slots - ctx->n3),
+                         cudaMemcpyDeviceToDevice, ctx->last_stream));
     if (mem == MCRT_HOST) return copy_out(ctx, n_abs_out, tmp, 8 * (size_t)ctx->slots, MCRT_HOST);
     return sync_last(ctx);
   }
@@ -540,13 +560,15 @@ mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem)
     if (!ctx->d_out_scratch) CU(cudaMalloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
     tmp = (float*)ctx->d_out_scratch; d_T = tmp;
   }
-  if (ctx->uni)
-    k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
-        ctx->d_trow, d_T, ctx->lay, ctx->n3, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
-  else
-    k_trow_to_T<<<(unsigned)((ctx->slots + 255) / 256), 256, 0, ctx->last_stream>>>(
-        ctx->d_trow, d_T, ctx->slots, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
+  k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
+      ctx->d_trow, d_T, ctx->lay, ctx->n3, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
   ctx->launches++;
+  if (ctx->slots > ctx->n3) {                                // sub-cells: same order in storage and in the getter
+    const long long ns = ctx->slots - ctx->n3;
+    k_trow_to_T<<<(unsigned)((ns + 255) / 256), 256, 0, ctx->last_stream>>>(
+        ctx->d_trow + ctx->store_n3, d_T + ctx->n3, ns, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
+    ctx->launches++;
+  }
   CU(cudaGetLastError());
   if (mem == MCRT_HOST) return copy_out(ctx, T_out, tmp, 4 * (size_t)ctx->slots, MCRT_HOST);
   return sync_last(ctx);

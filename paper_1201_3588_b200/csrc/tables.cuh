@@ -17,17 +17,6 @@ __device__ __forceinline__ double planck_nu(double nu, double T) {
   return (2.0 * MCRT_H_PLANCK * nu * nu * nu / (MCRT_C_LIGHT * MCRT_C_LIGHT)) / expm1(x);
 }
 
-// Grid encoding: density >= 0, or (sign bit | k) for the k-th refined root cube.
-__global__ void k_encode_root(const float* __restrict__ rho_root, const int* __restrict__ refidx,
-                              float* __restrict__ out, int n3) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n3) return;
-  int k = refidx ? refidx[i] : -1;
-  float v = rho_root[i];
-  v = (v > 0.f) ? v : 0.f;                                    // negative / NaN -> 0
-  out[i] = k >= 0 ? __int_as_float((int)(0x80000000u | (unsigned)k)) : v;
-}
-
 __global__ void k_sanitize(const float* __restrict__ in, float* __restrict__ out, long long n) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) { float v = in[i]; out[i] = (v > 0.f) ? v : 0.f; }

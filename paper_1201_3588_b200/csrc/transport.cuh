@@ -66,6 +66,7 @@ struct TransportParams {
   const SrcDev* __restrict__ src;              // [nsrc]
   unsigned long long* next;                    // work-queue head (packet offset within the batch)
   const uint32_t* __restrict__ perm;           // NULL, or the batch's package numbers grouped by source
+  const int* __restrict__ axtab;               // NULL (x-fastest root), or [3][N] axis terms of the root slot (bricked)
   unsigned long long* sed;                     // [3][nb]
   unsigned long long* emit_bin;                // [nb]
   unsigned long long* counters;                // [CNT_N]
@@ -215,11 +216,18 @@ __device__ __forceinline__ int sub_lin(int sub, int S) {
   return (sub & 15) + S * (((sub >> 4) & 15) + S * ((sub >> 8) & 15));
 }
 
+// storage slot of root cube (ix,iy,iz): x-fastest, or the sum of three axis terms (bricked root,
+// tables in shared memory)
+__device__ __forceinline__ int root_lin(const TransportParams& P, const int* s_ax, int ix, int iy, int iz) {
+  if (s_ax) return s_ax[ix] + s_ax[P.N + iy] + s_ax[2 * P.N + iz];
+  return ix + P.N * (iy + P.N * iz);
+}
+
 // Put a packet whose root cube (ix,iy,iz) and root-local position are known into its leaf.
 template <bool TL>
-__device__ __forceinline__ void place_in_root(const TransportParams& P, Packet& p, float ux, float uy,
+__device__ __forceinline__ void place_in_root(const TransportParams& P, const int* s_ax, Packet& p, float ux, float uy,
                                               float uz) {
-  int lin = p.ix + P.N * (p.iy + P.N * p.iz);
+  int lin = root_lin(P, s_ax, p.ix, p.iy, p.iz);
   p.lvl = 0; p.slot = lin;
   if (TL) {
     MCRT_CHECK_SLOT(lin);
@@ -244,7 +252,7 @@ __device__ __forceinline__ void place_in_root(const TransportParams& P, Packet& 
 
 // O4: emission of packet pid.
 template <bool TL>
-__device__ __forceinline__ void emit_packet(const TransportParams& P, Packet& p, const float4* s_opac) {
+__device__ __forceinline__ void emit_packet(const TransportParams& P, const int* s_ax, Packet& p, const float4* s_opac) {
   float u[4];
   draw4(P.seed, p.pid, 0, kTagEmit, u);
   int s = 0;
@@ -264,7 +272,7 @@ __device__ __forceinline__ void emit_packet(const TransportParams& P, Packet& p,
     if (p.d2 < 0.f && r2 == 0.f) { --f2; r2 = 1.f; }
     p.ix = f0 / Sf; p.iy = f1 / Sf; p.iz = f2 / Sf;
     int sx = f0 - p.ix * Sf, sy = f1 - p.iy * Sf, sz = f2 - p.iz * Sf;
-    int lin = p.ix + P.N * (p.iy + P.N * p.iz);
+    int lin = root_lin(P, s_ax, p.ix, p.iy, p.iz);
     p.lvl = 0; p.slot = lin;
     bool refined = false;
     if (TL) {
@@ -303,14 +311,14 @@ __device__ __forceinline__ void emit_packet(const TransportParams& P, Packet& p,
     if (ax == 0)      { set_dir(p, dn, e1, e2); p.ix = in; p.iy = i1; p.iz = i2; ux = ln; uy = l1; uz = l2; }
     else if (ax == 1) { set_dir(p, e2, dn, e1); p.iy = in; p.iz = i1; p.ix = i2; uy = ln; uz = l1; ux = l2; }
     else              { set_dir(p, e1, e2, dn); p.iz = in; p.ix = i1; p.iy = i2; uz = ln; ux = l1; uy = l2; }
-    place_in_root<TL>(P, p, ux, uy, uz);
+    place_in_root<TL>(P, s_ax, p, ux, uy, uz);
   }
 }
 
 // One crossing of the cell walk (O5).  Returns false when the packet stops walking
 // (interaction or escape; state says which).
 template <bool TL>
-__device__ __forceinline__ bool walk_step(const TransportParams& P, Packet& p, float kx, int& state,
+__device__ __forceinline__ bool walk_step(const TransportParams& P, const int* s_ax, Packet& p, float kx, int& state,
                                           uint32_t& crossings) {
   MCRT_CHECK_SLOT(p.slot);
   float rho = __ldg(P.rho + p.slot);
@@ -346,7 +354,7 @@ __device__ __forceinline__ bool walk_step(const TransportParams& P, Packet& p, f
     if (a0) p.ix += step; else if (a1) p.iy += step; else p.iz += step;
     int coord = a0 ? p.ix : (a1 ? p.iy : p.iz);
     if ((unsigned)coord >= (unsigned)P.N) { state = ST_ESCAPE; return false; }
-    int lin = p.ix + P.N * (p.iy + P.N * p.iz);
+    int lin = root_lin(P, s_ax, p.ix, p.iy, p.iz);
     MCRT_CHECK_SLOT(lin);
     int bits = __float_as_int(__ldg(P.rho + lin));
     if (bits < 0) {                                          // refined -> refined: sub faces line up
@@ -372,7 +380,7 @@ __device__ __forceinline__ bool walk_step(const TransportParams& P, Packet& p, f
   p.t0 = a0 ? p.td0 : p.t0; p.t1 = a1 ? p.td1 : p.t1; p.t2 = a2 ? p.td2 : p.t2;
   int coord = a0 ? p.ix : (a1 ? p.iy : p.iz);
   if ((unsigned)coord >= (unsigned)P.N) { state = ST_ESCAPE; return false; }
-  int lin = p.ix + P.N * (p.iy + P.N * p.iz);
+  int lin = root_lin(P, s_ax, p.ix, p.iy, p.iz);
   p.slot = lin;
   if (TL) {
     MCRT_CHECK_SLOT(lin);
@@ -406,6 +414,8 @@ __global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
   float4* s_opac = reinterpret_cast<float4*>(smem_raw);                    // [nb]
   uint32_t* s_sed = reinterpret_cast<uint32_t*>(s_opac + P.nb);             // [3*nb]
   uint32_t* s_emit = s_sed + 3 * P.nb;                                      // [nb]
+  int* s_ax = P.axtab ? reinterpret_cast<int*>(s_emit + P.nb) : nullptr;    // [3*N] (bricked root only)
+  if (s_ax) for (int i = threadIdx.x; i < 3 * P.N; i += blockDim.x) s_ax[i] = P.axtab[i];
   for (int i = threadIdx.x; i < P.nb; i += blockDim.x) { s_opac[i] = P.opac[i]; s_emit[i] = 0; }
   for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x) s_sed[i] = 0;
   __syncthreads();
@@ -435,7 +445,7 @@ __global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
         unsigned long long my = base + (unsigned long long)__popc(need & lt_mask);
         if (my < P.count) {
           p.pid = P.first + (P.perm ? (unsigned long long)__ldg(P.perm + my) : my);
-          emit_packet<TL>(P, p, s_opac);                    // a1
+          emit_packet<TL>(P, s_ax, p, s_opac);              // a1
           kx = s_opac[p.bin].x;
           ++cnt[CNT_EMITTED];
           atomicAdd(&s_emit[p.bin], 1u);
@@ -466,7 +476,7 @@ __global__ void __launch_bounds__(256, 5) k_transport(const TransportParams P) {
     if (state == ST_WALK) {
 #pragma unroll 1
       for (int it = 0; it < kWalkChunk; ++it)
-        if (!walk_step<TL>(P, p, kx, state, cnt[CNT_CROSS])) break;
+        if (!walk_step<TL>(P, s_ax, p, kx, state, cnt[CNT_CROSS])) break;
     }
 
     // ---- a4..a6: interaction ----

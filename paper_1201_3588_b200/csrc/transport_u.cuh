@@ -381,6 +381,18 @@ __global__ void k_encode_uniform(const float* __restrict__ rho_ext, float* __res
   float v = rho_ext[e];
   rho_store[slot_of(lay, ix, iy, iz)] = (v > 0.f) ? v : 0.f;
 }
+// Two-level grids: root array in storage order; density >= 0, or (sign bit | k) for the k-th
+// refined root cube (negative / NaN densities -> 0; padding slots stay 0)
+__global__ void k_encode_root(const float* __restrict__ rho_root, const int* __restrict__ refidx,
+                              float* __restrict__ out, LayoutU lay, long long n3) {
+  long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n3) return;
+  int ix = (int)(e % lay.N), iy = (int)((e / lay.N) % lay.N), iz = (int)(e / ((long long)lay.N * lay.N));
+  int k = refidx ? refidx[e] : -1;
+  float v = rho_root[e];
+  v = (v > 0.f) ? v : 0.f;
+  out[slot_of(lay, ix, iy, iz)] = k >= 0 ? __int_as_float((int)(0x80000000u | (unsigned)k)) : v;
+}
 // storage order -> x-fastest output
 template <typename T>
 __global__ void k_store_to_ext(const T* __restrict__ store, T* __restrict__ ext, LayoutU lay, long long n3) {

@@ -455,3 +455,28 @@ def test_grouped_handout_two_level_grid(M):
         runs.append(ctx)
     _assert_identical(runs[0], runs[1])
     assert runs[1].get_counters()["emitted"] == wl.n_packets
+
+
+@pytest.mark.parametrize("maker", [
+    lambda: W.tiny_random(n_root=2, sub=4, n_refined=8, seed=2, external=True, n_packets=40_000, batch=10_000),
+    lambda: W.tiny_random(n_root=3, sub=2, n_refined=5, seed=9, external=True, n_packets=40_000, batch=10_000),
+    lambda: W.c2(n_root=20, n_packets=60_000, batch=20_000),
+    lambda: W.c3(n_root=32, n_packets=60_000, batch=20_000)])
+def test_two_level_bricked_root_bit_identical_to_x_fastest(M, maker):
+    """Two-level grids: the root array in bricks (padding when N is not a multiple of 8) must not
+    change a single count, in the getters' slot order (root cells AND sub-cells), nor through the
+    split batch halves with a tally handed back in slot order."""
+    wl = maker()
+    assert wl.n_ref > 0
+    a = _run_layout(M, wl, 1)
+    b = _run_layout(M, wl, 2)
+    _assert_identical(a, b)
+    assert a.get_counters()["emitted"] == wl.n_packets
+    c = M.from_workload(wl, layout=2)
+    done = 0
+    for first, cnt in wl.batches():
+        c.transport_batch(wl.seed, first, cnt)
+        tally, _ = c.get_cell_energy(device=True)
+        done += cnt
+        c.update_temperature(tally, done)
+    _assert_identical(a, c)
