@@ -92,7 +92,8 @@ int64_t mcrt_leaf_slots(const mcrt_ctx* ctx);
  * T_k = T_min (T_max/T_min)^(k/(n_T-1)); and the emission inverse-CDF rows C_k[j] (midpoint rule,
  * R5; PAPER.md L27 Eqn 11.67).  All pointers are HOST pointers (the tables are small). */
 typedef struct {
-  int32_t n_bins;                /* 1..4096                                                   */
+  int32_t n_bins;                /* 1..4096; 32*n_bins + 24*n_root bytes of shared memory per
+                                    block must stay below 227 KB (else MCRT_EINVAL)            */
   const double* lambda_edges_um; /* [n_bins+1] ascending, > 0                                 */
   int32_t n_species;             /* >= 1                                                      */
   const double* weight;          /* [n_species] mass fractions                                */
@@ -185,8 +186,8 @@ mcrt_status mcrt_gather_calibrate(uint64_t footprint_bytes, uint64_t n_gathers, 
  *  - image: packages of the bins bin_lo..bin_hi (bin_hi < 0 = last bin) that leave within
  *    half_angle_deg of the direction `dir` (pointing from the grid TOWARDS the observer) are
  *    binned by their impact vector b = r - (r.d) d (r = position relative to the box centre,
- *    d = direction of flight) on the image axes e1 = z x dir (x if dir is along z) and
- *    e2 = dir x e1: n_pix x n_pix pixels over [-half_width, half_width]^2 cm, row index along
+ *    d = direction of flight) on the orthonormal image axes e1 = z x dir normalised (within
+ *    2.6 degrees of the z axis: the component of x normal to dir, normalised) and e2 = dir x e1: n_pix x n_pix pixels over [-half_width, half_width]^2 cm, row index along
  *    e2, column index along e1; counts [n_pix][n_pix].
  * n_mu = 0 / n_pix = 0 switch the respective tally off.  Needs the opacity (n_bins); calling
  * mcrt_set_opacity again switches the observer off.  Setting an observer zeroes its tallies;
@@ -240,6 +241,11 @@ int64_t mcrt_debug_violations(void);
 /* Raw Philox4x32-10 blocks computed on the device (test hook for the generator pin):
  * out[4*i..4*i+3] = Philox(key = (key2[0], key2[1]), counter = ctr[4*i..4*i+3]).  Host pointers. */
 mcrt_status mcrt_philox_blocks(const uint32_t* key2, const uint32_t* ctr, uint32_t* out, int64_t n);
+/* The kernels' maps from a random word to a uniform (test hook for reading R19): u[i] = the fp32
+ * uniform ((w >> 9) + 0.5) 2^-23 used for every draw of a flight, ud[i] = the fp64 uniform
+ * (w + 0.5) 2^-32 used for the two emission decisions (source, frequency bin), tau[i] = -ln u[i]
+ * as the free-flight draw computes it.  Both uniforms lie strictly inside (0,1).  Host pointers. */
+mcrt_status mcrt_uniforms(const uint32_t* words, float* u, double* ud, float* tau, int64_t n);
 const char* mcrt_last_error(const mcrt_ctx* ctx);
 
 #ifdef __cplusplus

@@ -4,20 +4,14 @@
 // Siebenmorgen, Heymann & Kruegel, "PAH in vectorized three dimensional Monte Carlo dust
 // radiative transfer models", following the paper's section 2 step by step:
 //
-//   PAPER.md L23  "The space is partitioned into cubes and, where a finer grid is needed,
-//                  the cubes are further divided into subcubes (cells). The star emits photon
-//                  packages of constant energy eps, but different frequencies. A package
-//                  entering on its flight path a cell may be absorbed there or scattered. The
-//                  probability for such an interaction is given by the extinction optical
-//                  depth along the path within the cell. When the package is scattered, it
-//                  only changes direction determined in a probabilistic manner by the phase
-//                  function. When it is absorbed, a new package of the same energy, but
-//                  usually different frequency nu_new is emitted from the spot of absorption.
-//                  The emission is isotropic. Each absorption event raises the energy of the
-//                  cell by eps, and accordingly its temperature."
-//   PAPER.md L25-27  nu_new is drawn "using the cell temperature before absorption", and the
-//                  Bjorkman & Wood correction is omitted (Eqn 11.67 instead of 11.65 of
-//                  Kruegel 2006): dP/dnu ~ kappa_nu B_nu(T_before).
+//   PAPER.md L23     cubes / subcubes (cells); packages of constant energy eps and different
+//                    frequencies; per cell an interaction with the probability given by the
+//                    extinction optical depth along the path in the cell; scattering changes the
+//                    direction by the phase function; absorption raises the cell's energy by eps
+//                    and a package of the same energy is re-emitted isotropically from the spot
+//                    at a new frequency (see the paper for the wording);
+//   PAPER.md L25-27  nu_new from the cell temperature BEFORE the absorption, no Bjorkman & Wood
+//                    correction (Eqn 11.67 instead of 11.65 of Kruegel 2006): dP/dnu ~ kappa_nu B_nu(T).
 //
 // Where the paper is silent the readings R1..R33 of SURVEY.md 8(c) / DESIGN.md section 3 are
 // taken; each function below names the step (O0..O8) and reading it implements.
@@ -32,7 +26,9 @@
 // bin-by-bin conservation; Beer-Lambert escape vs brute-force chords; optically thin
 // T ~ r^(-2/(4+beta)); per-flight agreement with an "intersect every box" walker (a second,
 // independent algorithm, also re-implemented in numpy in the tests); split invariance on a
-// two-level grid; external-field mean chord 2a/3.  O9 (direction-resolved tallies,
+// two-level grid; external-field mean chord 2a/3; tests/test_oracle_pins2.py: source pick
+// proportional to L_s (and its boundary case), sub-cell mass through the temperature identity
+// of an all-refined grid over two batches, albedo and g indexed per bin.  O9 (direction-resolved tallies,
 // tests/test_oracle_observer.py): sum identity, isotropy in mu, cone fraction, hand-computed
 // projection geometry, symmetry.  O10 (serial Bjorkman-Wood scheme, tests/test_oracle_bw.py):
 // telescoping of the corrected emission to the Planck spectrum at the final temperature.
@@ -665,7 +661,8 @@ int orc_update_temperature(void* h, const uint64_t* tally_sum, uint64_t n_cum) {
 }
 
 // O9: observer set-up.  dir need not be normalised; half_width in cm; n_mu = 0 / n_pix = 0 switch
-// the respective tally off.  Image axes: e1 = z x obs (or x if obs is along z), e2 = obs x e1.
+// the respective tally off.  Image axes: e1 = z x obs normalised (within 2.6 degrees of the pole: the
+// part of x normal to obs), e2 = obs x e1.
 int orc_set_observer(void* h, int n_mu, int n_pix, const double* dir, double half_angle_deg,
                      double half_width_cm, int bin_lo, int bin_hi) {
   Ctx& c = *(Ctx*)h;
@@ -678,8 +675,14 @@ int orc_set_observer(void* h, int n_mu, int n_pix, const double* dir, double hal
     for (int a = 0; a < 3; ++a) c.obs[a] = dir[a] / n;
     if (std::fabs(c.obs[2]) < 0.999) {
       double q = std::sqrt(c.obs[0] * c.obs[0] + c.obs[1] * c.obs[1]);
-      c.e1[0] = -c.obs[1] / q; c.e1[1] = c.obs[0] / q; c.e1[2] = 0;          // z x obs
-    } else { c.e1[0] = 1; c.e1[1] = 0; c.e1[2] = 0; }
+      c.e1[0] = -c.obs[1] / q; c.e1[1] = c.obs[0] / q; c.e1[2] = 0;          // z x obs, normalised
+    } else {
+      // near the pole z x obs is ill-conditioned: e1 = the part of x normal to obs, normalised
+      // (x itself for obs exactly along z, as R34 says), so that (e1, e2, obs) stays orthonormal
+      double v[3] = {1.0 - c.obs[0] * c.obs[0], -c.obs[0] * c.obs[1], -c.obs[0] * c.obs[2]};
+      double q = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+      for (int a = 0; a < 3; ++a) c.e1[a] = v[a] / q;
+    }
     c.e2[0] = c.obs[1] * c.e1[2] - c.obs[2] * c.e1[1];
     c.e2[1] = c.obs[2] * c.e1[0] - c.obs[0] * c.e1[2];
     c.e2[2] = c.obs[0] * c.e1[1] - c.obs[1] * c.e1[0];
@@ -688,6 +691,10 @@ int orc_set_observer(void* h, int n_mu, int n_pix, const double* dir, double hal
     c.img_lo = bin_lo; c.img_hi = bin_hi;
   }
   return 0;
+}
+void orc_get_observer_axes(void* h, double* obs, double* e1, double* e2) {
+  Ctx& c = *(Ctx*)h;
+  for (int a = 0; a < 3; ++a) { obs[a] = c.obs[a]; e1[a] = c.e1[a]; e2[a] = c.e2[a]; }
 }
 void orc_get_sed_mu(void* h, uint64_t* out) {
   Ctx& c = *(Ctx*)h;

@@ -19,20 +19,29 @@ _LIB = os.path.join(_HERE, "libmcrt_oracle.so")
 _lib = None
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with g++ (-O2, OpenMP).  Building the checker is not using it."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-shared", "-fPIC",
+_LIB_SAN = os.path.join(_HERE, "libmcrt_oracle_san.so")
+
+
+def build(force: bool = False, sanitize: bool = False) -> str:
+    """Compile the oracle with g++ (-O2, OpenMP).  Building the checker is not using it.
+    sanitize=True builds a second library with -fsanitize=address,undefined (SURVEY.md
+    section 5); tests/test_oracle_sanitizers.py runs the pins' workloads on it in a
+    subprocess (LD_PRELOAD of libasan, MCRT_ORACLE_LIBRARY pointing at it)."""
+    out = _LIB_SAN if sanitize else _LIB
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+        tmp = out + ".tmp.%d" % os.getpid()
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                 "-fno-omit-frame-pointer"] if sanitize else ["-O2"]
+        subprocess.check_call(["g++"] + flags + ["-std=c++17", "-fopenmp", "-shared", "-fPIC",
                                "-o", tmp, _SRC])
-        os.replace(tmp, _LIB)
-    return _LIB
+        os.replace(tmp, out)
+    return out
 
 
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
+        _lib = C.CDLL(os.environ.get("MCRT_ORACLE_LIBRARY") or build())
         L = _lib
         L.orc_create.restype = C.c_void_p
         L.orc_create.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_double, C.c_void_p,
@@ -52,6 +61,7 @@ def lib():
         L.orc_update_temperature.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
         L.orc_set_observer.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_double,
                                        C.c_double, C.c_int, C.c_int]
+        L.orc_get_observer_axes.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_sed_mu.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_get_image.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_run_bw.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64]
@@ -185,6 +195,11 @@ class Oracle:
                                     float(half_width_cm), int(bin_lo), int(bin_hi))
         assert rc == 0
         self.n_mu, self.n_pix = n_mu, n_pix
+
+    def observer_axes(self):
+        o, e1, e2 = np.zeros(3), np.zeros(3), np.zeros(3)
+        lib().orc_get_observer_axes(self.h, _p(o), _p(e1), _p(e2))
+        return o, e1, e2
 
     def sed_mu(self):
         s = np.zeros((self.n_mu, 3, self.nb), dtype=np.uint64)

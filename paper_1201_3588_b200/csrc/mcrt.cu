@@ -28,7 +28,6 @@ struct mcrt_ctx {
   int N = 0, S = 1;
   long long n3 = 0, n_ref = 0, slots = 0;
   long long store_n3 = 0;                 // storage slots of the root grid (sub-cells follow it)
-  int* d_axtab = nullptr;                 // two-level grids with a bricked root: [3][N] axis terms of the root slot
   double origin[3] = {0, 0, 0}, root_size = 1;
   float* d_rho = nullptr;
   unsigned long long* d_tally = nullptr;
@@ -42,11 +41,12 @@ struct mcrt_ctx {
   // sources
   int nsrc = 0;
   SrcDev* d_src = nullptr;
-  float* d_csrc = nullptr;
+  double* d_csrc = nullptr;               // [nsrc][nb] fp64 source CDFs (emission decisions are exact)
   double Ltot = 0;
   // tallies: [0] work-queue head, [1..CNT_N] counters, then sed[3*nb], emit_bin[nb]
   unsigned long long* d_small = nullptr;
-  unsigned long long Ncum = 0;
+  unsigned long long Ncum = 0;            // packages this context has transported since the last reset
+  unsigned long long Nglobal = 0;         // packages of ALL ranks behind the temperatures (= Ncum on one GPU)
   cudaStream_t last_stream = nullptr;
   std::vector<BatchEvents> pending, spare;
   // single-level grids: storage layout (transport_u.cuh); `slots` stays the caller-visible count
@@ -98,6 +98,13 @@ static void free_sources(mcrt_ctx* c) {
   cudaFree(c->d_src); cudaFree(c->d_csrc);
   c->d_src = nullptr; c->d_csrc = nullptr;
 }
+
+// dynamic shared memory of the transport kernel: opacity float4[nb], SED u32[3 nb], emitted u32[nb],
+// root delta tables int[6 N] (+ subcube tables int[6 * 8] on two-level grids)
+static size_t transport_smem_bytes(const mcrt_ctx* ctx) {
+  return 32 * (size_t)ctx->nb + sizeof(int) * (6 * (size_t)ctx->N + (ctx->uni ? 0 : 6 * kSubStride));
+}
+constexpr size_t kMaxSmemPerBlock = 227u << 10;              // B200: opt-in limit of dynamic shared memory
 
 extern "C" {
 
@@ -188,10 +195,12 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     CUG(cudaMalloc(&d_refidx, sizeof(int) * n3));
     CUG(cudaMemcpy(d_refidx, refidx.data(), sizeof(int) * n3, cudaMemcpyHostToDevice));
   }
-  if (ctx->uni) {
-    // per-axis slot-delta tables: forward (i -> i+1) and reversed (entry j: i = N-1-j -> i-1)
-    const int N = ctx->N;
-    std::vector<int> lut(6 * (size_t)N);
+  {
+    // per-axis slot-delta tables of the root grid: forward (i -> i+1) and reversed (entry j: i = N-1-j -> i-1);
+    // two-level grids: followed by the tables of the S^3 subcubes of a refined cube (entry j = directional
+    // subcube index: +-S^a, the last one = "leaves the cube")
+    const int N = ctx->N, S = ctx->S;
+    std::vector<int> lut(6 * (size_t)N + (ctx->uni ? 0 : 6 * kSubStride), 0);
     for (int a = 0; a < 3; ++a)
       for (int i = 0; i < N; ++i) {
         lut[(size_t)(2 * a) * N + i] = i == N - 1 ? kLutEscape
@@ -200,21 +209,21 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
         lut[(size_t)(2 * a + 1) * N + i] = ir == 0 ? kLutEscape
             : (int)(axis_term(ctx->lay, a, ir - 1) - axis_term(ctx->lay, a, ir));
       }
+    if (!ctx->uni) {
+      int stride = 1;
+      for (int a = 0; a < 3; ++a) {
+        for (int j = 0; j < S; ++j) {
+          lut[6 * (size_t)N + (size_t)(2 * a) * kSubStride + j] = j == S - 1 ? kLutLeave : stride;
+          lut[6 * (size_t)N + (size_t)(2 * a + 1) * kSubStride + j] = j == S - 1 ? kLutLeave : -stride;
+        }
+        stride *= S;
+      }
+    }
     CUG(cudaMalloc(&ctx->d_lut, sizeof(int) * lut.size()));
     CUG(cudaMemcpy(ctx->d_lut, lut.data(), sizeof(int) * lut.size(), cudaMemcpyHostToDevice));
     CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
-    k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho, ctx->lay, n3);
-  } else {
-    if (ctx->lay.bricked) {                                  // the kernel adds three axis terms from shared memory
-      const int N = ctx->N;
-      std::vector<int> tab(3 * (size_t)N);
-      for (int a = 0; a < 3; ++a)
-        for (int i = 0; i < N; ++i) tab[(size_t)a * N + i] = (int)axis_term(ctx->lay, a, i);
-      CUG(cudaMalloc(&ctx->d_axtab, sizeof(int) * tab.size()));
-      CUG(cudaMemcpy(ctx->d_axtab, tab.data(), sizeof(int) * tab.size(), cudaMemcpyHostToDevice));
-    }
-    CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
-    k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, ctx->lay, n3);
+    if (ctx->uni) k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho, ctx->lay, n3);
+    else k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, ctx->lay, n3);
   }
   ctx->launches++;
   if (k > 0) {
@@ -238,7 +247,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_sources(ctx);
   free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
-  cudaFree(ctx->d_lut); cudaFree(ctx->d_axtab); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
+  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -254,6 +263,12 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
   for (int j = 0; j < d->n_bins; ++j)
     if (!(d->lambda_edges_um[j] > 0) || !(d->lambda_edges_um[j + 1] > d->lambda_edges_um[j]))
       return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: wavelength edges must be positive and ascending");
+  {
+    mcrt_ctx probe;                                          // same formula as the launch, with the new n_bins
+    probe.nb = d->n_bins; probe.N = ctx->N; probe.uni = ctx->uni;
+    if (transport_smem_bytes(&probe) > kMaxSmemPerBlock)
+      return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: 32*n_bins + 24*n_root bytes of shared memory per block exceed 227 KB");
+  }
   int nT = d->n_T;
   double Tmin = d->T_min, Tmax = d->T_max;
   if (nT == 0) { nT = 801; Tmin = 1.0; Tmax = 1.0e4; }
@@ -315,7 +330,7 @@ mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src
     h[s].type = src[s].type;
     Tbb[s] = src[s].T_bb;
     acc += src[s].L;
-    h[s].lcdf = s == n_src - 1 ? 1.f : (float)(acc / Ltot);
+    h[s].lcdf = s == n_src - 1 ? 1.0 : acc / Ltot;
     for (int a = 0; a < 3; ++a) { h[s].fine[a] = 0; h[s].frac[a] = 0.f; }
     if (src[s].type == 0) {
       for (int a = 0; a < 3; ++a) {
@@ -324,7 +339,9 @@ mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src
           return fail(ctx, MCRT_EINVAL, "mcrt_set_source: point source outside the grid");
         double fl = std::floor(xf);
         float fr = (float)(xf - fl);
-        if (fr >= 1.f) { fl += 1.0; fr = 0.f; }
+        if (fr >= 1.f) { fl += 1.0; fr = 0.f; }             // the fraction rounded up to the next cell
+        if (fl >= (double)ctx->N * Sf)                       // ... which must still lie inside the grid
+          return fail(ctx, MCRT_EINVAL, "mcrt_set_source: point source outside the grid");
         h[s].fine[a] = (int)fl;
         h[s].frac[a] = fr;
       }
@@ -339,7 +356,7 @@ mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src
   CU(cudaMemcpy(d_T, Tbb.data(), 8 * n_src, cudaMemcpyHostToDevice));
   CU(cudaMalloc(&ctx->d_src, sizeof(SrcDev) * n_src));
   CU(cudaMemcpy(ctx->d_src, h.data(), sizeof(SrcDev) * n_src, cudaMemcpyHostToDevice));
-  CU(cudaMalloc(&ctx->d_csrc, 4 * (size_t)n_src * ctx->nb));
+  CU(cudaMalloc(&ctx->d_csrc, 8 * (size_t)n_src * ctx->nb));
   k_build_source_cdf<<<n_src, 128, 8 * (ctx->nb + 1)>>>(ctx->nb, d_T, ctx->d_nu, ctx->d_dnu, ctx->d_csrc);
   ctx->launches++;
   CU(cudaGetLastError());
@@ -373,7 +390,6 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   P.seed = seed; P.first = first; P.count = n;
   P.obs = ctx->obs;
   P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->store_n3;
-  P.axtab = ctx->uni ? nullptr : ctx->d_axtab;
 #ifdef MCRT_CHECKS
   CU(cudaMemcpyToSymbolAsync(g_mcrt_nstore, &ctx->store_slots, sizeof(long long), 0, cudaMemcpyHostToDevice, st));
 #endif
@@ -409,17 +425,18 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   long long want = ((long long)n + threads - 1) / threads;
   long long grid = (long long)ctx->sm_count * bps;
   if (want < grid) grid = want;
-  size_t smem = sizeof(float4) * nb + 4 * (size_t)nb * 4;
-  if (ctx->uni) {
-    TransportParamsU PU;
-    PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
-    smem += sizeof(int) * 6 * (size_t)ctx->N;
-    if (bps * threads > 1024) k_transport_u<5><<<(unsigned)grid, threads, smem, st>>>(PU);   // 48 registers
-    else k_transport_u<4><<<(unsigned)grid, threads, smem, st>>>(PU);                        // 64 registers
-  } else {
-    if (P.axtab) smem += sizeof(int) * 3 * (size_t)ctx->N;
-    k_transport<true><<<(unsigned)grid, threads, smem, st>>>(P);
-  }
+  const size_t smem = transport_smem_bytes(ctx);
+  TransportParamsU PU;
+  PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
+  const bool five = bps * threads > 1024;                    // 48-register build (5 blocks of 256) or 64-register build
+  void (*kern)(TransportParamsU) = ctx->uni ? (five ? k_transport_u<5, false> : k_transport_u<4, false>)
+                                            : (five ? k_transport_u<5, true> : k_transport_u<4, true>);
+  if (smem > (48u << 10)) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int resident = 0;                                          // large tables (many bins) lower the residency:
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem));   // size the grid to what fits
+  if (resident < 1) return fail(ctx, MCRT_EINVAL, "mcrt_run_batch: the transport kernel does not fit on an SM with these tables");
+  if ((long long)ctx->sm_count * resident < grid) grid = (long long)ctx->sm_count * resident;
+  kern<<<(unsigned)grid, threads, smem, st>>>(PU);
   ctx->launches++;
   CU(cudaGetLastError());
   return MCRT_OK;
@@ -478,6 +495,7 @@ mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_
   if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
   CU(cudaEventRecord(ev.e1, st));
   ctx->Ncum += n;
+  ctx->Nglobal = ctx->Ncum;
   rc = launch_update(ctx, ctx->d_tally, ctx->Ncum, st);
   if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
   CU(cudaEventRecord(ev.e2, st));
@@ -508,6 +526,7 @@ mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, ui
   if (!ctx) return MCRT_EINVAL;
   if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_update_temperature: grid, opacity and sources must be set first");
   cudaStream_t st = (cudaStream_t)stream_;
+  ctx->Nglobal = tally_sum ? n_cum : ctx->Ncum;             // eps of mcrt_get_cell_energy = L_tot / packages of all ranks
   mcrt_status rc = launch_update(ctx, tally_sum ? (const unsigned long long*)tally_sum : ctx->d_tally,
                                  tally_sum ? n_cum : ctx->Ncum, st);
   ctx->last_stream = st;
@@ -529,7 +548,10 @@ static mcrt_status copy_out(mcrt_ctx* ctx, void* dst, const void* src, size_t by
 mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps_out, mcrt_mem mem) {
   if (!ctx) return MCRT_EINVAL;
   if (!n_abs_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_energy: NULL output");
-  if (eps_out) *eps_out = ctx->Ncum ? ctx->Ltot / (double)ctx->Ncum : 0.0;
+  {
+    const unsigned long long n_eps = ctx->Nglobal > ctx->Ncum ? ctx->Nglobal : ctx->Ncum;
+    if (eps_out) *eps_out = n_eps ? ctx->Ltot / (double)n_eps : 0.0;
+  }
   if (ctx->lay.bricked) {                                    // storage order -> slot order (R22)
     unsigned long long* d_out = (unsigned long long*)n_abs_out;
     unsigned long long* tmp = nullptr;
@@ -593,9 +615,15 @@ mcrt_status mcrt_set_observer(mcrt_ctx* ctx, const mcrt_observer_desc* d) {
     if (!(n > 0) || !(d->half_width > 0) || !(d->half_angle_deg > 0) || d->half_angle_deg > 180)
       return fail(ctx, MCRT_EINVAL, "mcrt_set_observer: dir must be non-zero, half_width > 0, 0 < half_angle_deg <= 180");
     for (int a = 0; a < 3; ++a) o[a] = d->dir[a] / n;
-    if (std::fabs(o[2]) < 0.999) {                          // e1 = z x o
+    // e1 = z x o normalised (R34); within 2.6 degrees of the pole, where that is ill-conditioned, e1 = the
+    // component of x normal to o, normalised (Gram-Schmidt; exactly x for o along z)
+    if (std::fabs(o[2]) < 0.999) {
       const double q = std::sqrt(o[0] * o[0] + o[1] * o[1]);
       e1[0] = -o[1] / q; e1[1] = o[0] / q; e1[2] = 0;
+    } else {
+      const double v[3] = {1.0 - o[0] * o[0], -o[0] * o[1], -o[0] * o[2]};
+      const double q = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+      for (int a = 0; a < 3; ++a) e1[a] = v[a] / q;
     }
     e2[0] = o[1] * e1[2] - o[2] * e1[1];                    // e2 = o x e1
     e2[1] = o[2] * e1[0] - o[0] * e1[2];
@@ -658,6 +686,7 @@ mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what) {
     CU(cudaMemset(ctx->d_tally, 0, 8 * (size_t)ctx->store_slots));
     CU(cudaMemset(ctx->d_trow, 0, 4 * (size_t)ctx->store_slots));
     ctx->Ncum = 0;
+    ctx->Nglobal = 0;
   }
   return MCRT_OK;
 }
@@ -748,6 +777,30 @@ mcrt_status mcrt_philox_blocks(const uint32_t* key2, const uint32_t* ctr, uint32
   k_philox_blocks<<<(unsigned)((n + 255) / 256), 256>>>(key2[0], key2[1], d_c, d_o, n);
   CU(cudaGetLastError());
   CU(cudaMemcpy(out, d_o, 16 * (size_t)n, cudaMemcpyDeviceToHost));
+  return MCRT_OK;
+}
+
+__global__ void k_uniforms(const uint32_t* __restrict__ w, float* __restrict__ u, double* __restrict__ ud,
+                           float* __restrict__ tau, long long n) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  u[i] = u01(w[i]); ud[i] = u01d(w[i]); tau[i] = -logf(u01(w[i]));
+}
+
+mcrt_status mcrt_uniforms(const uint32_t* words, float* u, double* ud, float* tau, int64_t n) {
+  mcrt_ctx* ctx = nullptr;
+  if (!words || !u || !ud || !tau || n < 0) return fail(nullptr, MCRT_EINVAL, "mcrt_uniforms: bad arguments");
+  if (n == 0) return MCRT_OK;
+  uint32_t* d_w = nullptr; float *d_u = nullptr, *d_t = nullptr; double* d_ud = nullptr;
+  struct Tmp { uint32_t*& a; float*& b; float*& c; double*& d; ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); cudaFree(d); } } tmp{d_w, d_u, d_t, d_ud};
+  CU(cudaMalloc(&d_w, 4 * (size_t)n)); CU(cudaMalloc(&d_u, 4 * (size_t)n)); CU(cudaMalloc(&d_t, 4 * (size_t)n));
+  CU(cudaMalloc(&d_ud, 8 * (size_t)n));
+  CU(cudaMemcpy(d_w, words, 4 * (size_t)n, cudaMemcpyHostToDevice));
+  k_uniforms<<<(unsigned)((n + 255) / 256), 256>>>(d_w, d_u, d_ud, d_t, n);
+  CU(cudaGetLastError());
+  CU(cudaMemcpy(u, d_u, 4 * (size_t)n, cudaMemcpyDeviceToHost));
+  CU(cudaMemcpy(ud, d_ud, 8 * (size_t)n, cudaMemcpyDeviceToHost));
+  CU(cudaMemcpy(tau, d_t, 4 * (size_t)n, cudaMemcpyDeviceToHost));
   return MCRT_OK;
 }
 

@@ -70,9 +70,10 @@ __global__ void k_build_emission_rows(int nb, int nT, double Tmin, double Tmax,
     cdf[(size_t)k * nb + j] = (j == nb - 1 || !(Q > 0)) ? 1.f : (float)(s_term[j] / Q);
 }
 
-// Source spectra: blackbody truncated to the band, same midpoint rule (R5, R6).
+// Source spectra: blackbody truncated to the band, same midpoint rule (R5, R6).  Kept in fp64: the
+// emission bin is searched once per package with the fp64 uniform, so emitted-per-bin is exact.
 __global__ void k_build_source_cdf(int nb, const double* __restrict__ Tbb, const double* __restrict__ nu,
-                                   const double* __restrict__ dnu, float* __restrict__ csrc) {
+                                   const double* __restrict__ dnu, double* __restrict__ csrc) {
   extern __shared__ double s_term[];
   int s = blockIdx.x;
   double T = Tbb[s];
@@ -86,7 +87,7 @@ __global__ void k_build_source_cdf(int nb, const double* __restrict__ Tbb, const
   __syncthreads();
   double tot = s_term[nb];
   for (int j = threadIdx.x; j < nb; j += blockDim.x)
-    csrc[(size_t)s * nb + j] = (j == nb - 1 || !(tot > 0)) ? 1.f : (float)(s_term[j] / tot);
+    csrc[(size_t)s * nb + j] = (j == nb - 1 || !(tot > 0)) ? 1.0 : s_term[j] / tot;
 }
 
 // a9 / O7 (R9 reading B, R10, R12): per-leaf radiative-equilibrium temperature from the cumulative

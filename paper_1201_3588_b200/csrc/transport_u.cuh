@@ -1,21 +1,30 @@
-// transport_u.cuh -- sm_100a transport kernel for single-level (uniform) grids: rows a1..a8 of
-// SURVEY.md 8(a).  Same method and random-number slots as transport.cuh; what
-// differs is how a package is carried through the cells:
+// transport_u.cuh -- the sm_100a transport kernel: rows a1..a8 of SURVEY.md 8(a).
+// One photon package per thread, persistent threads with lane refill, for single-level grids
+// (template TL = false) and for two-level grids of cubes and subcubes (TL = true, PAPER.md L23
+// "the cubes are further divided into subcubes (cells)").  DESIGN.md section 6.
 //
-//  * The cell walk keeps ABSOLUTE path lengths along the current flight: t_a = path length at
-//    which the package meets its next face on axis a, tcur = path length so far.  One crossing
+//  * A package lives in registers and is never located from a floating-point position.  The cell
+//    walk keeps ABSOLUTE path lengths along the current flight: t_a = path length at which the
+//    package meets the next face of its leaf on axis a, tcur = path length so far.  One crossing
 //    is tnext = min(t_x,t_y,t_z); dtau = rho*kappa*(tnext - tcur); the axis whose t equals tnext
-//    (ties -> lowest axis, R21) advances by 1/|d_a|.  One FADD per crossing instead of three.
-//  * The cell's storage slot is advanced by a per-axis DELTA table held in shared memory
+//    (ties -> lowest axis, R21) advances by its pitch 1/|d_a| (times 1/S inside a refined cube).
+//  * The leaf's storage slot is advanced by a per-axis DELTA table held in shared memory
 //    (slot(ix,iy,iz) = A_x(ix) + A_y(iy) + A_z(iz) is separable, so the delta of a step depends
-//    on one coordinate only).  The tables make the memory layout a host decision -- x-fastest
-//    for L2-resident grids, 8^3 bricks in Morton order for grids larger than the L2 -- and mark
-//    the step that leaves the grid (INT_MIN), so the hot loop has no bounds check and no
-//    index arithmetic beyond one add.  Per axis there is a forward and a reversed table, so a
-//    table cursor always moves by +1 whatever the direction's sign.
-//  * The density of the NEXT cell is requested before the optical-depth test of the current
-//    cell (the geometric walk does not depend on rho), taking the gather latency off the
-//    dependent chain.
+//    on one coordinate only).  The tables make the memory layout of the root grid a host decision
+//    -- x-fastest, or 8^3 bricks in Morton order -- and mark the step that leaves the grid
+//    (kLutEscape), so the hot loop has no bounds check and no index arithmetic beyond one add.
+//    Per axis there is a forward and a reversed table, so a table cursor always moves by +1
+//    whatever the direction's sign.
+//  * Two-level grids use the SAME step: inside a refined cube the three cursors point into a tiny
+//    second table (S entries per axis and direction: +-S^a, the last entry = kLutLeave) and the
+//    pitch is 1/(S|d_a|); the root cursors and the root slot wait in three + one more registers.
+//    A step that reads kLutLeave takes the root table's delta instead and returns to the root
+//    level; a gathered density with the sign bit set is the marker of a refined cube (the density
+//    array doubles as the two-level index): the package descends into the
+//    subcube its remaining distances to the root faces select.  Root-level and sub-level lanes of
+//    a warp therefore run one instruction stream; only the two transitions diverge.
+//  * The density of the NEXT leaf is requested before the optical-depth test of the current one
+//    (the geometric walk does not depend on rho), taking the gather latency off the dependent chain.
 //  * The walk loop runs until fewer than `quorum` lanes of the warp are still walking; then all
 //    stopped lanes go through ONE event pass (escape tally -> refill from the work queue ->
 //    emission / scattering / absorption+re-emission -> new flight).  Emission and re-emission
@@ -26,7 +35,7 @@
 
 namespace mcrt {
 
-// ---- storage layout of single-level grids (host and device) ----------------------------------
+// ---- storage layout of the root grid (host and device) ----------------------------------------
 struct LayoutU {
   int N;          // root cells per axis
   int bricked;    // 0: x-fastest;  1: 8^3 bricks (x-fastest over bricks), Morton order inside
@@ -64,14 +73,17 @@ __host__ __device__ __forceinline__ long long ext_of_slot(const LayoutU& L, long
   return ix + (long long)L.N * (iy + (long long)L.N * iz);
 }
 
+constexpr int kLutEscape = INT_MIN;       // root table: the step leaves the grid
+constexpr int kLutLeave = INT_MIN + 1;    // sub table: the step leaves the refined root cube
+constexpr int kSubStride = 8;             // entries per (axis, direction) of the sub table (S <= 8)
+
 struct TransportParamsU {
   TransportParams base;          // rho / tally / trow are in STORAGE order here
-  const int* __restrict__ lut;   // [6][N] slot deltas: (axis, forward) at (2*axis)*N, reversed at (2*axis+1)*N
+  const int* __restrict__ lut;   // [6][N] root slot deltas: (axis, forward) at (2*axis)*N, reversed at
+                                 // (2*axis+1)*N; two-level grids: followed by [6][kSubStride] sub-cell deltas
   LayoutU lay;
   int quorum;                    // leave the walk loop when fewer lanes than this are walking
 };
-
-constexpr int kLutEscape = INT_MIN;
 
 // SU_INTERACT_B: interaction found in the second step of a pair -> the cell's density is in the
 // alternate register (moved back in the event pass, never inside the walk loop where the move
@@ -80,76 +92,173 @@ enum : int { SU_WALK = 0, SU_INTERACT = 1, SU_ESCAPE = 2, SU_FETCH = 3, SU_DONE 
 
 struct PacketU {
   float d0, d1, d2;          // direction
-  float t0, t1, t2;          // path length (cell edges) at which the next face on each axis is met
+  float t0, t1, t2;          // path length (root-cube edges) at which the next leaf face on each axis is met
   float dt0, dt1, dt2;       // 1/|d_a|
   float tcur, tau_rem, rho;  // path length so far in this flight; optical depth left; density here
   uint32_t p0, p1, p2;       // cursors into the delta tables (shared-memory byte addresses)
-  int slot;                  // storage slot of the current cell
+  int slot;                  // storage slot of the current leaf
   int cb;                    // bin | component << 16 (component: 0 direct, 1 scattered, 2 thermal)
   uint32_t k;                // flight number
   uint32_t off;              // package number within the batch: pid = first + off
   float u1, u2, u3;          // uniforms of the current flight kept for the interaction
+  // two-level grids only (dead registers otherwise): state of a package inside a refined cube
+  uint32_t r0, r1, r2;       // the root-level cursors while p0..p2 walk the sub table
+  int rslot;                 // storage slot of the refined root cube
+  float hs;                  // leaf edge in root-cube edges: 1, or 1/S inside a refined cube
 };
 
-// Start a flight of a package sitting in cell (ix,iy,iz) at cell-local position (ux,uy,uz) with
-// direction (a,b,c): cursors, face path lengths, tcur = 0.
-__device__ __forceinline__ void begin_flight(PacketU& p, uint32_t lut, int N, int ix, int iy, int iz,
-                                             float ux, float uy, float uz, float a, float b, float c) {
-  if (fabsf(a) < 1e-12f) a = copysignf(1e-12f, a);          // G1: never the exit axis
-  if (fabsf(b) < 1e-12f) b = copysignf(1e-12f, b);
-  if (fabsf(c) < 1e-12f) c = copysignf(1e-12f, c);
-  p.d0 = a; p.d1 = b; p.d2 = c;
-  p.dt0 = __frcp_rn(fabsf(a)); p.dt1 = __frcp_rn(fabsf(b)); p.dt2 = __frcp_rn(fabsf(c));
-  p.t0 = (a > 0.f ? 1.f - ux : ux) * p.dt0;
-  p.t1 = (b > 0.f ? 1.f - uy : uy) * p.dt1;
-  p.t2 = (c > 0.f ? 1.f - uz : uz) * p.dt2;
-  p.p0 = lut + 4u * (uint32_t)(a > 0.f ? ix : 2 * N - 1 - ix);            // reversed table: entry N-1-i
-  p.p1 = lut + 4u * (uint32_t)(2 * N + (b > 0.f ? iy : 2 * N - 1 - iy));
-  p.p2 = lut + 4u * (uint32_t)(4 * N + (c > 0.f ? iz : 2 * N - 1 - iz));
-  p.tcur = 0.f;
-}
-// cell coordinates back from the cursors
-__device__ __forceinline__ void cell_of(const PacketU& p, uint32_t lut, int N, int& ix, int& iy, int& iz) {
-  int q0 = (int)((p.p0 - lut) >> 2), q1 = (int)((p.p1 - lut) >> 2) - 2 * N, q2 = (int)((p.p2 - lut) >> 2) - 4 * N;
-  ix = p.d0 > 0.f ? q0 : 2 * N - 1 - q0;
-  iy = p.d1 > 0.f ? q1 : 2 * N - 1 - q1;
-  iz = p.d2 > 0.f ? q2 : 2 * N - 1 - q2;
-}
-
-
-// O4 for a single-level grid: cell, cell-local position and (external field only) direction of
-// a new package.  r = Philox block (pid, 0, EMIT); iso = isotropic direction from (r2, r3).
 __device__ __forceinline__ int lds_s32(uint32_t addr) {
   int v;
   asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
 
-// One crossing of the cell walk (O5).  `cur` holds the density of the current cell; the density
-// of the next cell is requested into `nxt` BEFORE the optical-depth test, so consecutive calls
+// direction of a new flight: components too small to ever be the exit axis are nudged (G1)
+__device__ __forceinline__ void set_direction(PacketU& p, float a, float b, float c) {
+  if (fabsf(a) < 1e-12f) a = copysignf(1e-12f, a);
+  if (fabsf(b) < 1e-12f) b = copysignf(1e-12f, b);
+  if (fabsf(c) < 1e-12f) c = copysignf(1e-12f, c);
+  p.d0 = a; p.d1 = b; p.d2 = c;
+  p.dt0 = __frcp_rn(fabsf(a)); p.dt1 = __frcp_rn(fabsf(b)); p.dt2 = __frcp_rn(fabsf(c));
+  p.tcur = 0.f;
+}
+// root-table cursors of root cube (ix,iy,iz) for the current direction (reversed table: entry N-1-i)
+__device__ __forceinline__ void root_cursors(const PacketU& p, uint32_t lut, int N, int ix, int iy, int iz,
+                                             uint32_t& c0, uint32_t& c1, uint32_t& c2) {
+  c0 = lut + 4u * (uint32_t)(p.d0 > 0.f ? ix : 2 * N - 1 - ix);
+  c1 = lut + 4u * (uint32_t)(2 * N + (p.d1 > 0.f ? iy : 2 * N - 1 - iy));
+  c2 = lut + 4u * (uint32_t)(4 * N + (p.d2 > 0.f ? iz : 2 * N - 1 - iz));
+}
+// root cube back from root-table cursors
+__device__ __forceinline__ void cell_of(const PacketU& p, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t lut,
+                                        int N, int& ix, int& iy, int& iz) {
+  int q0 = (int)((c0 - lut) >> 2), q1 = (int)((c1 - lut) >> 2) - 2 * N, q2 = (int)((c2 - lut) >> 2) - 4 * N;
+  ix = p.d0 > 0.f ? q0 : 2 * N - 1 - q0;
+  iy = p.d1 > 0.f ? q1 : 2 * N - 1 - q1;
+  iz = p.d2 > 0.f ? q2 : 2 * N - 1 - q2;
+}
+// Start a flight at the root level: the package sits in root cube (ix,iy,iz) at cube-local
+// position (ux,uy,uz) in [0,1]^3; direction already set.
+__device__ __forceinline__ void begin_flight(PacketU& p, uint32_t lut, int N, int ix, int iy, int iz,
+                                             float ux, float uy, float uz) {
+  p.t0 = (p.d0 > 0.f ? 1.f - ux : ux) * p.dt0;
+  p.t1 = (p.d1 > 0.f ? 1.f - uy : uy) * p.dt1;
+  p.t2 = (p.d2 > 0.f ? 1.f - uz : uz) * p.dt2;
+  root_cursors(p, lut, N, ix, iy, iz, p.p0, p.p1, p.p2);
+  p.hs = 1.f;
+}
+// sub-table cursor of (axis, direction sign, directional index j = number of subcubes behind)
+__device__ __forceinline__ uint32_t sub_cursor(uint32_t sublut, int axis, float d, int j) {
+  return sublut + 4u * (uint32_t)((2 * axis + (d > 0.f ? 0 : 1)) * kSubStride + j);
+}
+// Start a flight inside subcube (sx,sy,sz) of the refined root cube (ix,iy,iz) at subcube-local
+// position (fx,fy,fz) in [0,1]^3; direction already set; p.slot / p.rslot are the caller's.
+__device__ __forceinline__ void begin_flight_sub(PacketU& p, uint32_t lut, uint32_t sublut, int N, int S,
+                                                 int ix, int iy, int iz, int sx, int sy, int sz,
+                                                 float fx, float fy, float fz) {
+  const float hs = 1.f / (float)S;
+  p.t0 = (p.d0 > 0.f ? 1.f - fx : fx) * hs * p.dt0;
+  p.t1 = (p.d1 > 0.f ? 1.f - fy : fy) * hs * p.dt1;
+  p.t2 = (p.d2 > 0.f ? 1.f - fz : fz) * hs * p.dt2;
+  root_cursors(p, lut, N, ix, iy, iz, p.r0, p.r1, p.r2);
+  p.p0 = sub_cursor(sublut, 0, p.d0, p.d0 > 0.f ? sx : S - 1 - sx);
+  p.p1 = sub_cursor(sublut, 1, p.d1, p.d1 > 0.f ? sy : S - 1 - sy);
+  p.p2 = sub_cursor(sublut, 2, p.d2, p.d2 > 0.f ? sz : S - 1 - sz);
+  p.hs = hs;
+}
+// directional subcube index on one axis from a sub-table cursor
+__device__ __forceinline__ int sub_j(uint32_t cursor, uint32_t sublut) {
+  return (int)(((cursor - sublut) >> 2) & (uint32_t)(kSubStride - 1));
+}
+
+// A package at the root level whose gathered "density" is the marker of a refined cube (sign bit
+// | refined-cube number k): descend into the subcube it is in.  Per axis the remaining distance to
+// the cube's exit face, in subcube edges, W = (t_a - tcur)|d_a| S, selects the subcube: m =
+// ceil(W) - 1 whole subcubes lie between the package's subcube and that face (a package exactly on
+// a subcube face belongs to the subcube it flies into: direction-aware as R7; the entry axis has
+// W = S).  Then t_a shrinks to the subcube's own exit face and the cursors move to the sub table.
+__device__ __forceinline__ void descend(const TransportParams& P, PacketU& p, uint32_t sublut, float& cur) {
+  const int S = P.S;
+  const float fS = (float)S, hs = 1.f / fS;
+  const int kref = __float_as_int(cur) & 0x7fffffff;
+  const int m0 = min(S - 1, max(0, (int)ceilf((p.t0 - p.tcur) * fabsf(p.d0) * fS) - 1));
+  const int m1 = min(S - 1, max(0, (int)ceilf((p.t1 - p.tcur) * fabsf(p.d1) * fS) - 1));
+  const int m2 = min(S - 1, max(0, (int)ceilf((p.t2 - p.tcur) * fabsf(p.d2) * fS) - 1));
+  p.t0 = fmaxf(p.tcur, p.t0 - (float)m0 * hs * p.dt0);
+  p.t1 = fmaxf(p.tcur, p.t1 - (float)m1 * hs * p.dt1);
+  p.t2 = fmaxf(p.tcur, p.t2 - (float)m2 * hs * p.dt2);
+  p.r0 = p.p0; p.r1 = p.p1; p.r2 = p.p2;
+  p.rslot = p.slot;
+  const int j0 = S - 1 - m0, j1 = S - 1 - m1, j2 = S - 1 - m2;
+  p.p0 = sub_cursor(sublut, 0, p.d0, j0);
+  p.p1 = sub_cursor(sublut, 1, p.d1, j1);
+  p.p2 = sub_cursor(sublut, 2, p.d2, j2);
+  const int sx = p.d0 > 0.f ? j0 : m0, sy = p.d1 > 0.f ? j1 : m1, sz = p.d2 > 0.f ? j2 : m2;
+  p.slot = P.n3 + kref * (S * S * S) + sx + S * (sy + S * sz);
+  p.hs = hs;
+  MCRT_CHECK_SLOT(p.slot);
+  cur = __ldg(P.rho + p.slot);
+}
+
+// One crossing of the cell walk (O5).  `cur` holds the density of the current leaf; the density
+// of the next leaf is requested into `nxt` BEFORE the optical-depth test, so consecutive calls
 // alternate the two registers and no instruction waits on the gather except its real use.
-__device__ __forceinline__ void walk_step_u(const float* __restrict__ rho, PacketU& p, float& cur,
-                                            float& nxt, float kx, int& state, uint32_t& crossings) {
+// tau_rem > 0 always (u01 < 1, and a - b > 0 for a > b in IEEE arithmetic), so dtau >= tau_rem
+// implies rho*kappa > 0: no interaction in an empty leaf (R14).
+template <bool TL>
+__device__ __forceinline__ void walk_step_u(const TransportParams& P, PacketU& p, float& cur, float& nxt,
+                                            float kx, uint32_t sublut, int& state, uint32_t& crossings) {
+  if (TL) {
+    if (__float_as_int(cur) < 0) descend(P, p, sublut, cur);
+  }
   const float tnext = fminf(p.t0, fminf(p.t1, p.t2));
   const bool a0 = p.t0 == tnext;                             // ties -> lowest axis (R21)
   const bool a1 = !a0 && p.t1 == tnext;
-  const int dl = lds_s32(a0 ? p.p0 : (a1 ? p.p1 : p.p2));
+  int dl = lds_s32(a0 ? p.p0 : (a1 ? p.p1 : p.p2));
+  int from = p.slot;
+  bool leave = false;
+  if (TL) {
+    leave = dl == kLutLeave;
+    if (leave) {                                             // the step leaves the refined cube: root table
+      dl = lds_s32(a0 ? p.r0 : (a1 ? p.r1 : p.r2));
+      from = p.rslot;
+    }
+  }
   const bool esc = dl == kLutEscape;
-  const int nslot = p.slot + dl;
-  if (!esc) { MCRT_CHECK_SLOT(nslot); nxt = __ldg(rho + nslot); }
+  const int nslot = from + dl;
+  if (!esc) { MCRT_CHECK_SLOT(nslot); nxt = __ldg(P.rho + nslot); }
   const float dtau = cur * kx * (tnext - p.tcur);
-  if (dtau >= p.tau_rem) {                                   // interaction inside this cell
+  if (dtau >= p.tau_rem) {                                   // interaction inside this leaf
     state = SU_INTERACT;
   } else {
     p.tau_rem -= dtau;
     p.tcur = tnext;
-    if (a0) { p.t0 += p.dt0; p.p0 += 4u; } else if (a1) { p.t1 += p.dt1; p.p1 += 4u; } else { p.t2 += p.dt2; p.p2 += 4u; }
+    if (TL) {
+      if (leave) {                                           // back to the root level: the other two axes'
+        const int S = P.S;                                   // exits move out to the faces of the root cube
+        const float h = p.hs;
+        if (!a0) p.t0 += (float)(S - 1 - sub_j(p.p0, sublut)) * h * p.dt0;
+        if (a0 || !a1) p.t1 += (float)(S - 1 - sub_j(p.p1, sublut)) * h * p.dt1;
+        if (a0 || a1) p.t2 += (float)(S - 1 - sub_j(p.p2, sublut)) * h * p.dt2;
+        p.p0 = p.r0; p.p1 = p.r1; p.p2 = p.r2;
+        p.hs = 1.f;
+      }
+      if (a0) { p.t0 = fmaf(p.dt0, p.hs, p.t0); p.p0 += 4u; }
+      else if (a1) { p.t1 = fmaf(p.dt1, p.hs, p.t1); p.p1 += 4u; }
+      else { p.t2 = fmaf(p.dt2, p.hs, p.t2); p.p2 += 4u; }
+    } else {
+      if (a0) { p.t0 += p.dt0; p.p0 += 4u; } else if (a1) { p.t1 += p.dt1; p.p1 += 4u; } else { p.t2 += p.dt2; p.p2 += 4u; }
+    }
     ++crossings;
     p.slot = nslot;
     if (esc) state = SU_ESCAPE;
   }
 }
 
+// O4: where a new package starts.  Point source: finest-level cell fx.. and fractional position
+// in it (direction-aware on a face, R7).  External field (R25): a point on one of the six box
+// faces and an inward cosine-law direction; returns the ROOT cube and cube-local position.
+// r = float uniforms of the Philox block (pid, 0, EMIT).
 __device__ __forceinline__ void emit_position_u(const TransportParams& P, const SrcDev& sd,
                                                 unsigned long long pid, const float r[4], int& ix,
                                                 int& iy, int& iz, float& ux, float& uy, float& uz,
@@ -186,22 +295,23 @@ __device__ __forceinline__ void emit_position_u(const TransportParams& P, const 
 }
 
 // MINBLOCKS = resident blocks per SM the kernel is compiled for: 4 (64 registers) or 5 (48
-// registers).  Five blocks hide more of the L2 latency on cache-resident grids (c1_tau1 0.371 ->
-// 0.338 ms per launch); on HBM-resident grids the extra threads thrash the L1 (c4 66 -> 74 ms),
-// so the host picks per grid (profiles/r01_summary.md).
-template <int MINBLOCKS>
+// registers).  Five blocks hide more of the L2 latency on cache-resident grids; on HBM-resident
+// grids the extra threads thrash the L1, so the host picks per grid (profiles/).
+template <int MINBLOCKS, bool TL>
 __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportParamsU PU) {
   const TransportParams& P = PU.base;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* s_opac = reinterpret_cast<float4*>(smem_raw);                    // [nb]
   uint32_t* s_sed = reinterpret_cast<uint32_t*>(s_opac + P.nb);             // [3*nb]
   uint32_t* s_emit = s_sed + 3 * P.nb;                                      // [nb]
-  int* s_lut = reinterpret_cast<int*>(s_emit + P.nb);                       // [6*N]
+  int* s_lut = reinterpret_cast<int*>(s_emit + P.nb);                       // [6*N] (+ [6*kSubStride])
   const uint32_t lut = (uint32_t)__cvta_generic_to_shared(s_lut);
   const int N = P.N;
+  const uint32_t sublut = lut + 4u * (uint32_t)(6 * N);
+  const int n_lut = 6 * N + (TL ? 6 * kSubStride : 0);
   for (int i = threadIdx.x; i < P.nb; i += blockDim.x) { s_opac[i] = P.opac[i]; s_emit[i] = 0; }
   for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x) s_sed[i] = 0;
-  for (int i = threadIdx.x; i < 6 * N; i += blockDim.x) s_lut[i] = PU.lut[i];
+  for (int i = threadIdx.x; i < n_lut; i += blockDim.x) s_lut[i] = PU.lut[i];
   __syncthreads();
 
   const unsigned lane = threadIdx.x & 31;
@@ -214,6 +324,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   PacketU p;
   p.d0 = p.d1 = p.d2 = 1.f; p.t0 = p.t1 = p.t2 = 0.f; p.dt0 = p.dt1 = p.dt2 = 1.f;
   p.tcur = 0.f; p.tau_rem = 1.f; p.rho = 0.f; p.p0 = p.p1 = p.p2 = lut; p.slot = 0;
+  p.r0 = p.r1 = p.r2 = lut; p.rslot = 0; p.hs = 1.f;
   float rho_b = 0.f;                                         // the walk alternates p.rho / rho_b
   p.cb = 0; p.k = 0; p.off = 0; p.u1 = p.u2 = p.u3 = 0.f;
   float kx = 0.f;
@@ -223,9 +334,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   for (;;) {
     // ---- a7: escaped packages -> SED; a8: refill from the work queue (one atomic per warp) ----
     if (state == SU_ESCAPE) {
-      if (P.obs.n_mu | P.obs.n_pix) {                        // exit point: cell from the cursors, offset from the t's
-        int ix, iy, iz;
-        cell_of(p, lut, N, ix, iy, iz);
+      if (P.obs.n_mu | P.obs.n_pix) {                        // exit point: cube from the cursors, offset from the t's
+        int ix, iy, iz;                                      // (a package always leaves the grid at the root level)
+        cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
         const float w0 = fminf(1.f, fmaxf(0.f, (p.t0 - p.tcur) * fabsf(p.d0)));
         const float w1 = fminf(1.f, fmaxf(0.f, (p.t1 - p.tcur) * fabsf(p.d1)));
         const float w2 = fminf(1.f, fmaxf(0.f, (p.t2 - p.tcur) * fabsf(p.d2)));
@@ -255,20 +366,32 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       if (state == SU_INTERACT_B) p.rho = rho_b;
       const unsigned long long pid = P.first + p.off;
       int bin = p.cb & 0xffff, comp = p.cb >> 16;
-      int ix = 0, iy = 0, iz = 0;
+      int ix = 0, iy = 0, iz = 0, sx = 0, sy = 0, sz = 0;
       float ux = 0.f, uy = 0.f, uz = 0.f, a, b, c;
       bool scatter = false;
+      bool in_sub = TL && !is_new && p.hs < 1.f;             // the package sits in a subcube
       if (!is_new) {                                         // where the interaction happened
-        cell_of(p, lut, N, ix, iy, iz);
-        // the interaction lies tau_rem / (rho kappa) further along this cell's segment
+        // it lies tau_rem / (rho kappa) further along this leaf's segment (rho kappa > 0 here)
         const float seg = fminf(p.t0, fminf(p.t1, p.t2)) - p.tcur;
-        const float ti = p.tcur + fminf(seg, p.tau_rem / (p.rho * kx));
-        float w0 = fminf(1.f, fmaxf(0.f, (p.t0 - ti) * fabsf(p.d0)));
-        float w1 = fminf(1.f, fmaxf(0.f, (p.t1 - ti) * fabsf(p.d1)));
-        float w2 = fminf(1.f, fmaxf(0.f, (p.t2 - ti) * fabsf(p.d2)));
+        const float ak = p.rho * kx;
+        const float ti = p.tcur + (ak > 0.f ? fminf(seg, p.tau_rem / ak) : 0.f);
+        // fraction of the leaf's edge left to its exit face, per axis
+        const float ih = in_sub ? (float)P.S : 1.f;
+        float w0 = fminf(1.f, fmaxf(0.f, (p.t0 - ti) * fabsf(p.d0) * ih));
+        float w1 = fminf(1.f, fmaxf(0.f, (p.t1 - ti) * fabsf(p.d1) * ih));
+        float w2 = fminf(1.f, fmaxf(0.f, (p.t2 - ti) * fabsf(p.d2) * ih));
         ux = p.d0 > 0.f ? 1.f - w0 : w0;
         uy = p.d1 > 0.f ? 1.f - w1 : w1;
         uz = p.d2 > 0.f ? 1.f - w2 : w2;
+        if (in_sub) {
+          cell_of(p, p.r0, p.r1, p.r2, lut, N, ix, iy, iz);
+          const int S = P.S, j0 = sub_j(p.p0, sublut), j1 = sub_j(p.p1, sublut), j2 = sub_j(p.p2, sublut);
+          sx = p.d0 > 0.f ? j0 : S - 1 - j0;
+          sy = p.d1 > 0.f ? j1 : S - 1 - j1;
+          sz = p.d2 > 0.f ? j2 : S - 1 - j2;
+        } else {
+          cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
+        }
         scatter = p.u1 < s_opac[bin].y;                      // a4 (R16)
       }
       if (scatter) {                                         // a5
@@ -278,15 +401,14 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         if (comp == 0) comp = 1;
         ++p.k;
       } else {                                               // a1 emission / a6 absorption + re-emission
-        float r[4];
-        draw4(P.seed, pid, is_new ? 0u : p.k, is_new ? kTagEmit : kTagReemit, r);
-        const float* row;
-        float us;
+        uint32_t xw[4];
+        draw4w(P.seed, pid, is_new ? 0u : p.k, is_new ? kTagEmit : kTagReemit, xw);
+        const float r2 = u01(xw[2]), r3 = u01(xw[3]);
         int s = 0;
-        if (is_new) {
-          while (s < P.nsrc - 1 && P.src[s].lcdf < r[0]) ++s;
-          row = P.csrc + (size_t)s * P.nb;
-          us = r[1];
+        if (is_new) {                                        // O4: source by luminosity, bin by its spectrum (fp64)
+          const double u0 = u01d(xw[0]);
+          while (s < P.nsrc - 1 && P.src[s].lcdf < u0) ++s;
+          bin = search_cdf<double>(P.csrc + (size_t)s * P.nb, P.nb, u01d(xw[1]));
         } else {
           ++n_abs;
           // warp-aggregated integer tally: one atomic per distinct cell per warp
@@ -297,18 +419,35 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
           float tr = __ldg(P.trow + p.slot);                 // T frozen = T before absorption
           int k0 = min(P.nT - 1, (int)tr);
           float w = tr - (float)k0;
-          int rw = (r[1] < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
-          row = P.cdf + (size_t)rw * P.nb;
-          us = r[0];
+          int rw = (u01(xw[1]) < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
+          bin = search_cdf<float>(P.cdf + (size_t)rw * P.nb, P.nb, u01(xw[0]));
         }
-        bin = search_cdf(row, P.nb, us);
         kx = s_opac[bin].x;
-        isotropic_dir(r[2], r[3], a, b, c);
+        isotropic_dir(r2, r3, a, b, c);
         if (is_new) {
+          const float r[4] = {0.f, 0.f, r2, r3};
           emit_position_u(P, P.src[s], pid, r, ix, iy, iz, ux, uy, uz, a, b, c);
+          if (TL && P.src[s].type == 0) {                    // finest-level cell -> root cube + subcube
+            const int S = P.S;
+            sx = ix % S; sy = iy % S; sz = iz % S;
+            ix /= S; iy /= S; iz /= S;
+          }
           p.slot = (int)slot_of(PU.lay, ix, iy, iz);
           MCRT_CHECK_SLOT(p.slot);
           p.rho = __ldg(P.rho + p.slot);
+          if (TL && P.src[s].type == 0) {
+            if (__float_as_int(p.rho) < 0) {                 // the source sits in a refined cube
+              const int S = P.S;
+              p.rslot = p.slot;
+              p.slot = P.n3 + (__float_as_int(p.rho) & 0x7fffffff) * (S * S * S) + sx + S * (sy + S * sz);
+              MCRT_CHECK_SLOT(p.slot);
+              p.rho = __ldg(P.rho + p.slot);
+              in_sub = true;
+            } else {                                         // cube-local position from the finest-level one
+              const float hs = 1.f / (float)P.S;
+              ux = ((float)sx + ux) * hs; uy = ((float)sy + uy) * hs; uz = ((float)sz + uz) * hs;
+            }
+          }
           comp = 0; p.k = 0;
           atomicAdd(&s_emit[bin], 1u);
         } else {
@@ -322,7 +461,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         atomicAdd(P.counters + CNT_LOST, 1ull);
         state = SU_FETCH;
       } else {
-        begin_flight(p, lut, N, ix, iy, iz, ux, uy, uz, a, b, c);
+        set_direction(p, a, b, c);
+        if (TL && in_sub) begin_flight_sub(p, lut, sublut, N, P.S, ix, iy, iz, sx, sy, sz, ux, uy, uz);
+        else begin_flight(p, lut, N, ix, iy, iz, ux, uy, uz);
         float u[4];
         draw4(P.seed, pid, p.k, kTagFlight, u);
         p.tau_rem = -logf(u[0]);
@@ -335,9 +476,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
     // ---- a3: cell walk until fewer than `quorum` lanes are walking ----
 #pragma unroll 1
     for (;;) {
-      if (state == SU_WALK) walk_step_u(P.rho, p, p.rho, rho_b, kx, state, n_cross);
+      if (state == SU_WALK) walk_step_u<TL>(P, p, p.rho, rho_b, kx, sublut, state, n_cross);
       if (state == SU_WALK) {
-        walk_step_u(P.rho, p, rho_b, p.rho, kx, state, n_cross);
+        walk_step_u<TL>(P, p, rho_b, p.rho, kx, sublut, state, n_cross);
         if (state == SU_INTERACT) state = SU_INTERACT_B;
       }
       if (__popc(__ballot_sync(kFull, state == SU_WALK)) < quorum) break;

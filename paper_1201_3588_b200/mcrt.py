@@ -56,7 +56,7 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
            "mcrt_get_batch_times", "mcrt_get_tables",
-           "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_gather_calibrate", "mcrt_last_error")
+           "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_uniforms", "mcrt_gather_calibrate", "mcrt_last_error")
 
 
 def lib():
@@ -96,6 +96,7 @@ def lib():
         L.mcrt_debug_violations.restype = i64
         L.mcrt_debug_violations.argtypes = []
         L.mcrt_philox_blocks.argtypes = [vp, vp, vp, i64]
+        L.mcrt_uniforms.argtypes = [vp, vp, vp, vp, i64]
         L.mcrt_gather_calibrate.argtypes = [u64, u64, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
         L.mcrt_gather_calibrate.restype = C.c_int
         L.mcrt_last_error.restype = C.c_char_p
@@ -108,7 +109,7 @@ def lib():
                      "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
                      "mcrt_get_batch_times",
                      "mcrt_get_tables",
-                     "mcrt_philox_blocks"):
+                     "mcrt_philox_blocks", "mcrt_uniforms"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -367,6 +368,18 @@ def philox_blocks(key2, ctr):
     if rc != 0:
         raise McrtError(f"mcrt_philox_blocks: status {rc}: {lib().mcrt_last_error(None).decode()}")
     return o
+
+
+def uniforms(words):
+    """(fp32 uniform, fp64 uniform, -ln of the fp32 uniform) the kernels derive from random words."""
+    w = np.ascontiguousarray(words, dtype=np.uint32).ravel()
+    u = np.zeros(len(w), dtype=np.float32)
+    ud = np.zeros(len(w), dtype=np.float64)
+    tau = np.zeros(len(w), dtype=np.float32)
+    rc = lib().mcrt_uniforms(_np_ptr(w), _np_ptr(u), _np_ptr(ud), _np_ptr(tau), len(w))
+    if rc != 0:
+        raise McrtError(f"mcrt_uniforms: status {rc}: {lib().mcrt_last_error(None).decode()}")
+    return u, ud, tau
 
 
 def gather_calibrate(footprint_bytes, n_gathers=1 << 30, stream=None):

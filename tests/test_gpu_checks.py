@@ -18,7 +18,10 @@ assert mcrt.debug_violations() == 0, "library was not built with -DMCRT_CHECKS"
 cases = [W.c0(n_packets=20000, batch=10000),
          W.tiny_random(n_root=3, seed=4, external=True, n_packets=20000, batch=5000),
          W.tiny_random(n_root=2, sub=4, n_refined=8, seed=2, external=True, n_packets=20000, batch=5000),
+         W.tiny_random(n_root=3, sub=3, n_refined=7, seed=8, external=True, n_packets=20000, batch=5000),
+         W.tiny_random(n_root=2, sub=8, n_refined=3, seed=9, external=True, n_packets=20000, batch=5000),
          W.c2(n_root=16, n_packets=20000, batch=10000),
+         W.c3(n_root=32, n_packets=20000, batch=10000),
          W.c4(n_root=24, n_packets=20000, batch=10000, corr_cells=3.0)]
 for wl in cases:
     for layout in (1, 2):

@@ -70,10 +70,20 @@ def test_observer_clumpy_cube_with_external_field(M, oracle_mod):
 
 @pytest.mark.parametrize("direction", [(0.0, 0.0, 1.0), (0.0, 1.0, 0.15)])
 def test_observer_two_level_disk(M, oracle_mod, direction):
-    """Flared disk on a two-level grid (k_transport<true>): face-on and nearly edge-on."""
+    """Flared disk on a two-level grid (k_transport_u<., true>): face-on and nearly edge-on."""
     wl = W.c2(n_root=32, n_packets=300_000, batch=100_000)
     obs = dict(n_mu=8, n_pix=15, direction=direction, half_angle_deg=20.0,   # odd: the star is mid-pixel
                half_width_cm=16 * wl.root_size)
+    ctx, orc = _both(M, oracle_mod, wl, obs)
+    _check(ctx, orc)
+
+
+def test_observer_near_the_pole(M, oracle_mod):
+    """An observer 2 degrees off the z axis: the image axes are the orthonormal pair of R34's
+    near-polar rule on both sides (e1 = x there was not normal to the line of sight)."""
+    wl = W.c0()
+    obs = dict(n_mu=4, n_pix=9, direction=(0.03, 0.02, 1.0), half_angle_deg=25.0,
+               half_width_cm=9 * wl.root_size)
     ctx, orc = _both(M, oracle_mod, wl, obs)
     _check(ctx, orc)
 

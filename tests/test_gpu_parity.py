@@ -25,7 +25,11 @@ def _run_both(M, O, wl, n_packets=None, batch=None, threads=0):
     return ctx, orc
 
 
-def _compare(ctx, orc, groups=None, min_count=1000, expect_cells=True):
+def _compare(ctx, orc, groups=None, min_count=1000, expect_cells=True, expect_T_cells=0):
+    """GPU run against the oracle's run of the same packages.  `groups`: one array or a list of
+    arrays of aggregation indices per leaf slot.  Last of all the GPU's temperatures are checked on
+    every leaf slot against the oracle's temperature step applied to the GPU's own tally (this
+    overwrites the oracle's temperatures: _compare is the last use of `orc`)."""
     cg, co = ctx.get_counters(), orc.counters()
     PR.check_accounting(cg, co)
     ng, eps_g = ctx.get_cell_energy()
@@ -33,12 +37,20 @@ def _compare(ctx, orc, groups=None, min_count=1000, expect_cells=True):
     sg, so = ctx.get_sed(), orc.sed()
     PR.check_self_consistency(cg, ng, sg)
     assert eps_g == pytest.approx(eps_o, rel=1e-12)
-    n_cells, n_groups = PR.check_cell_energy(ng, no, min_count=min_count, groups=groups)
+    if groups is None or isinstance(groups, np.ndarray):
+        groups = [groups]
+    n_cells = n_groups = 0
+    for g in groups:
+        n_cells, k = PR.check_cell_energy(ng, no, min_count=min_count, groups=g)
+        n_groups += k
     if expect_cells:
         assert n_cells + n_groups > 0
-    PR.check_temperature(ctx.get_cell_temperature(), orc.cell_temperature(), ng, no,
-                         min_count=min_count)
+    Tg = ctx.get_cell_temperature()
+    n_T = PR.check_temperature(Tg, orc.cell_temperature(), ng, no, min_count=min_count)
+    assert n_T >= expect_T_cells, (n_T, expect_T_cells)
     PR.check_sed(sg, so)
+    n_slots, n_hot = PR.check_temperature_of_tally(Tg, orc, ng, cg["emitted"])
+    assert n_slots == len(ng) and 0.99 * (ng > 0).sum() <= n_hot <= (ng > 0).sum()
     # event totals are sums of ~1e5+ events: 3 sigma + 0.5 %
     for k in ("absorptions", "scatterings", "crossings"):
         assert PR.counts_close(cg[k], co[k], 0.005), (k, cg[k], co[k])
@@ -55,6 +67,22 @@ def test_philox_device_matches_oracle(M, oracle_mod):
     out = M.philox_blocks(key, ctr)
     for i in list(range(64)) + list(range(0, 20000, 97)):
         assert np.array_equal(out[i], oracle_mod.philox(key, ctr[i])), i
+
+
+def test_device_uniforms_stay_inside_the_unit_interval(M):
+    """R19: the fp32 uniform of a flight is ((w >> 9) + 0.5) 2^-23, exact in fp32 and
+    strictly inside (0,1) for every word -- in particular 0xFFFFFFFF, which a 24-bit variant
+    rounds to 1.0 -- so tau* = -ln u > 0; the fp64 uniform of the emission decisions is the
+    oracle's (w + 0.5) 2^-32."""
+    rng = np.random.default_rng(3)
+    w = np.concatenate([np.array([0, 1, 511, 512, 0x7FFFFFFF, 0x80000000, 0xFFFFFE00, 0xFFFFFFFF],
+                                 dtype=np.uint64), rng.integers(0, 2 ** 32, size=5000, dtype=np.uint64)])
+    u, ud, tau = M.uniforms(w.astype(np.uint32))
+    assert u.dtype == np.float32 and 0.0 < u.min() and u.max() < 1.0
+    assert np.array_equal(u.astype(np.float64), ((w >> 9).astype(np.float64) + 0.5) * 2.0 ** -23)
+    assert np.array_equal(ud, (w.astype(np.float64) + 0.5) * 2.0 ** -32)
+    assert tau.min() > 0.0 and np.isfinite(tau).all() and tau.max() < 16.7
+    assert u[7] == np.float32(1.0) - np.float32(2.0 ** -24)
 
 
 # ---- tables (row a0) ------------------------------------------------------------------------
@@ -146,7 +174,8 @@ def test_c1_twin(M, oracle_mod, tau_v, n_packets):
 # ---- two-level grids ------------------------------------------------------------------------
 @pytest.mark.parametrize("n_root,sub,n_ref,ext", [(2, 4, 1, False), (2, 4, 8, True),
                                                   (3, 4, 5, False), (4, 2, 9, True),
-                                                  (3, 0, 0, True)])
+                                                  (3, 0, 0, True), (3, 3, 11, True),
+                                                  (2, 8, 3, False), (5, 5, 40, True)])
 def test_tiny_grids(M, oracle_mod, n_root, sub, n_ref, ext):
     wl = W.tiny_random(n_root=n_root, sub=sub, n_refined=n_ref, seed=11 + n_ref,
                        external=ext, n_packets=400_000, batch=100_000)
@@ -159,16 +188,34 @@ def test_c2_twin_small_disk(M, oracle_mod):
     wl = W.c2(n_root=32, n_packets=1_000_000, batch=100_000)
     assert wl.n_ref > 0
     ctx, orc = _run_both(M, oracle_mod, wl)
-    _compare(ctx, orc, groups=PR.root_of_slot(wl))
-    _compare(ctx, orc, groups=PR.blocks_of_slot(wl, 4))
+    _compare(ctx, orc, groups=[PR.root_of_slot(wl), PR.blocks_of_slot(wl, 4)])
 
 
 def test_c3_twin_small_disk(M, oracle_mod):
     wl = W.c3(n_root=32, n_packets=1_000_000, batch=100_000)
     assert wl.n_ref > 0
     ctx, orc = _run_both(M, oracle_mod, wl)
-    _compare(ctx, orc, groups=PR.root_of_slot(wl))
-    _compare(ctx, orc, groups=PR.blocks_of_slot(wl, 4))
+    _compare(ctx, orc, groups=[PR.root_of_slot(wl), PR.blocks_of_slot(wl, 4)])
+
+
+@pytest.mark.parametrize("maker,n_ref", [(W.c2, 17_256), (W.c3, 224_872)])
+def test_disk_configs_full_grid_against_oracle(M, oracle_mod, maker, n_ref):
+    """configs[2] / configs[3] on their OWN grids (128^3 + 17 256 x 4^3, 256^3 + 224 872 x 4^3 leaf
+    slots, the two-level walk at full size): 2^22 packages in four batches of 2^20 on both sides
+    (temperatures feed back three times), compared per leaf, per root cube (sub-cells folded
+    back into their cube), per 4^3 and 8^3 super-block of cubes, SED, counters, and the
+    temperature of every leaf slot."""
+    wl = maker()
+    assert wl.n_ref == n_ref and wl.sub == 4
+    n, batch = 1 << 22, 1 << 20
+    ctx, orc = _run_both(M, oracle_mod, wl, n, batch)
+    cg, co = _compare(ctx, orc, groups=[PR.root_of_slot(wl), PR.blocks_of_slot(wl, 4),
+                                        PR.blocks_of_slot(wl, 8)])
+    assert cg["emitted"] == n and cg["absorptions"] > 100_000
+    n_abs, _ = ctx.get_cell_energy()
+    n3 = wl.n_root ** 3
+    assert n_abs[n3:].sum() > 0.5 * n_abs.sum()               # most absorptions happen in subcubes
+    assert n_abs[:n3][np.asarray(wl.refine).ravel() > 0].sum() == 0
 
 
 def test_c4_twin_small_cube(M, oracle_mod):

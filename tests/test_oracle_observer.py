@@ -95,3 +95,22 @@ def test_symmetric_sphere_is_uniform_in_mu(oracle_mod):
     sel = (img + rot) > 200
     z = (img - rot)[sel] / np.sqrt((img + rot)[sel])
     assert np.abs(z).max() < 5.0 and sel.sum() >= 9
+
+
+@pytest.mark.parametrize("obs", [(0.0, 0.0, 1.0), (0.03, 0.02, 1.0), (-0.04, 0.01, -1.0),
+                                 (0.044, 0.0, 0.999), (0.3, -0.2, 0.9), (1.0, 0.0, 0.0)])
+def test_image_axes_are_orthonormal(oracle_mod, obs):
+    """(e1, e2, obs) is a right-handed orthonormal triad for every observer direction, also within
+    2.6 degrees of the pole where z x obs is ill-conditioned (R34; the old rule kept
+    e1 = x there, which is not normal to obs)."""
+    o = oracle_mod.Oracle(W.c0())
+    o.set_observer(n_pix=3, direction=obs, half_width_cm=1.0)
+    d, e1, e2 = o.observer_axes()
+    want = np.array(obs) / np.linalg.norm(obs)
+    assert np.allclose(d, want, atol=1e-15)
+    for v in (e1, e2):
+        assert abs(np.linalg.norm(v) - 1) < 1e-14
+    assert abs(e1 @ d) < 1e-14 and abs(e2 @ d) < 1e-14 and abs(e1 @ e2) < 1e-14
+    assert np.allclose(np.cross(d, e1), e2, atol=1e-14)
+    if obs == (0.0, 0.0, 1.0):
+        assert np.array_equal(e1, [1.0, 0.0, 0.0])
