@@ -134,33 +134,40 @@ def measured_peaks():
 # ---------------------------------------------------------------------------------------------
 # CPU oracle legs
 # ---------------------------------------------------------------------------------------------
-def oracle_rate(wl, target_seconds=15.0, n_batches=4):
-    """Time the oracle, as it stands, on a bounded sample of the workload: packets
-    0..n-1 in n_batches equal batches (temperatures update in between, as in the method)."""
-    from oracle import oracle as O
-    O.build()
-    cores = O.max_threads()
+def _oracle_sample(O, wl, threads, target_seconds, n_batches=4):
+    """Time the oracle, as it stands, on packets 0..n-1 of the workload in n_batches equal batches
+    (temperatures update in between, as in the method) with `threads` OpenMP threads."""
     orc = O.Oracle(wl)
-    probe, dt = 2048, 0.0
-    while dt < 0.5 and probe < (1 << 28):                    # calibrate the sample size
+    probe, dt = 1024, 0.0
+    while dt < 0.4 and probe < (1 << 28):                    # calibrate the sample size
         probe *= 2
         t0 = time.perf_counter()
-        orc.run_batch(wl.seed, 0, probe)
+        orc.run_batch(wl.seed, 0, probe, threads)
         dt = max(time.perf_counter() - t0, 1e-4)
     n = int(min(max(probe * target_seconds / dt, 4 * probe), 1 << 31))       # ids may run past the config's count
     per = max(n // n_batches, 1)
     orc = O.Oracle(wl)
     t0 = time.perf_counter()
     done = 0
-    for b in range(n_batches):
-        orc.run_batch(wl.seed, done, per)
+    for _ in range(n_batches):
+        orc.run_batch(wl.seed, done, per, threads)
         done += per
     dt = time.perf_counter() - t0
     c = orc.counters()
-    return {"value": done / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"packets 0..{done - 1} in {n_batches} batches of {per} "
-                      f"({dt:.1f} s wall, OpenMP over packets)",
-            "crossings_per_s": c["crossings"] / dt}
+    return done / dt, c["crossings"] / dt, f"packets 0..{done - 1} in {n_batches} batches of {per} ({dt:.1f} s wall)"
+
+
+def oracle_rate(wl, target_seconds=15.0):
+    """cpu_baseline: the fp64 oracle on ONE core (the headline CPU figure) and on
+    all host cores (OpenMP over packets), each on a bounded sample of the same workload."""
+    from oracle import oracle as O
+    O.build()
+    cores = O.max_threads()
+    v1, x1, s1 = _oracle_sample(O, wl, 1, 0.4 * target_seconds)
+    vn, xn, sn = _oracle_sample(O, wl, cores, 0.6 * target_seconds)
+    return {"value": vn, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": sn + ", OpenMP over packets", "crossings_per_s": xn,
+            "one_core": {"value": v1, "unit": UNIT, "cores": 1, "crossings_per_s": x1, "sample": s1}}
 
 
 def run_reference(args, wl, name):
@@ -209,6 +216,9 @@ def run_reference(args, wl, name):
 # ---------------------------------------------------------------------------------------------
 # GPU arm
 # ---------------------------------------------------------------------------------------------
+L2_BYTES = 126 << 20
+
+
 def algorithmic_bytes(wl, d_cross, d_abs):
     """SURVEY.md 8(d) / DESIGN.md section 7: 4 B per crossing (density gather; the refined-cube
     marker shares that array, the descent into a refined cube costs a second 4-B gather which
@@ -217,6 +227,109 @@ def algorithmic_bytes(wl, d_cross, d_abs):
     per_cross = 8 if wl.n_ref else 4
     per_abs = 4 + 8 + 4 * int(np.ceil(np.log2(wl.n_bins)))
     return d_cross * per_cross + d_abs * per_abs, per_cross, per_abs
+
+
+def time_steps(torch, ctx, wl, runner, stream, world, steps, warmup, flush, barrier):
+    """`warmup` untimed + `steps` timed batches of wl.batch packages per rank.  Returns per-step CUDA
+    event times (ms), the kernel times recorded inside the library, counter deltas, launches."""
+    batch = wl.batch
+    step_no = [0]
+
+    def one_step():
+        runner.run_batch(wl.seed, step_no[0] * world * batch, world * batch, stream)
+        step_no[0] += 1
+
+    for _ in range(warmup):
+        flush.fill_(1)
+        one_step()
+    barrier()
+    ctx.get_batch_times()
+    c_before = ctx.get_counters()
+    launches_before = ctx.kernel_launches()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    barrier()
+    t_wall = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)                      # L2 flush between timed iterations (not timed)
+        a.record()
+        one_step()
+        b.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    t_tr, t_up = ctx.get_batch_times()
+    c_after = ctx.get_counters()
+    d = {k: c_after[k] - c_before[k] for k in ("emitted", "escaped", "absorptions", "scatterings",
+                                                "flights", "crossings", "lost")}
+    return dict(step_ms=step_ms, t_tr=t_tr, t_up=t_up, d=d, t_wall=t_wall,
+                launches=ctx.kernel_launches() - launches_before, one_step=one_step)
+
+
+def rooflines(wl, name, d, tr_s, steps, gather_peak):
+    """The bound that holds for this workload and the secondary figures (DESIGN.md sections 7, 8).
+    L2-resident density array: the walk is bound by the rate at which the SMs' L1TEX units serve
+    scattered 4-byte gathers (calibrated live, mcrt_gather_calibrate, at this footprint); density
+    array at or above the L2 size: HBM, algorithmic bytes against the measured copy bandwidth."""
+    peak, peak_src = measured_peaks()
+    bytes_alg, per_cross, per_abs = algorithmic_bytes(wl, d["crossings"], d["absorptions"])
+    hbm_achieved = bytes_alg / tr_s / 1e9 if tr_s > 0 else 0.0
+    foot = int(wl.leaf_slots) * 4
+    hbm = {"bound": "hbm", "kernel": "k_transport_u", "achieved": hbm_achieved, "peak": peak, "unit": "GB/s",
+           "frac": hbm_achieved / peak, "traffic": ncu_traffic(name), "peak_source": peak_src,
+           "algorithmic_bytes": {"per_crossing": per_cross, "per_absorption": per_abs,
+                                 "per_launch": bytes_alg / steps},
+           "kernel_ms": 1e3 * tr_s / steps}
+    if hbm["traffic"]:
+        hbm["traffic_over_algorithmic"] = hbm["traffic"] / (bytes_alg / steps)
+        hbm["dram_rate_gbs_from_capture"] = hbm["traffic"] / (tr_s / steps) / 1e9
+    gather = None
+    if gather_peak:
+        g_ach = d["crossings"] / tr_s if tr_s > 0 else 0.0
+        gather = {"footprint_bytes": foot, "peak_gathers_per_s": gather_peak, "achieved_gathers_per_s": g_ach,
+                  "frac": g_ach / gather_peak,
+                  "what": "peak = independent hash-indexed 4-byte gathers/s over an array of the density "
+                          "footprint at full occupancy (mcrt_gather_calibrate); achieved = cell crossings/s "
+                          "of k_transport_u.  A fraction above 1 means the walk's locality (bricks, grouped "
+                          "hand-out) lets one sector serve several crossings: then it is no ceiling and the "
+                          "hbm figures are the ones that bound"}
+    resident = foot <= 0.75 * L2_BYTES
+    if resident and gather:
+        roof = {"bound": "l1tex-gather", "kernel": "k_transport_u", "achieved": 4e-9 * gather["achieved_gathers_per_s"],
+                "peak": 4e-9 * gather_peak, "unit": "GB/s", "frac": gather["frac"], "traffic": hbm["traffic"],
+                "peak_source": "calibrated live: scattered 4-byte gathers over the density footprint x 4 B "
+                               "(density array is L2-resident: DRAM moves ~1 % of the algorithmic bytes)",
+                "algorithmic_bytes": {"per_crossing": 4, "per_launch": 4.0 * d["crossings"] / steps},
+                "kernel_ms": 1e3 * tr_s / steps, "hbm": hbm}
+    else:
+        roof = hbm
+    return roof, gather
+
+
+def measure_workload(torch, mcrt, wl, name, steps, warmup, stream, flush, args, calibrate=True):
+    """One entry of per_config: a fresh context, `warmup` + `steps` batches on this GPU."""
+    from paper_1201_3588_b200.sharding import ShardedRunner
+    ctx = mcrt.from_workload(wl)
+    runner = ShardedRunner(ctx, None)
+    r = time_steps(torch, ctx, wl, runner, stream, 1, steps, warmup, flush, torch.cuda.synchronize)
+    secs = float(sum(r["step_ms"])) * 1e-3
+    tr_s = float(r["t_tr"].sum()) * 1e-3
+    gpeak = mcrt.gather_calibrate(int(wl.leaf_slots) * 4, 1 << 30, stream)[0] if calibrate else None
+    roof, gather = rooflines(wl, name, r["d"], tr_s, steps, gpeak)
+    d = r["d"]
+    out = {"config": describe(wl, name), "steps": steps, "warmup": warmup,
+           "packets_per_s": d["emitted"] / secs, "crossings_per_s": d["crossings"] / secs,
+           "ms_per_step": 1e3 * secs / steps, "kernel_ms": 1e3 * tr_s / steps,
+           "update_ms": float(r["t_up"].sum()) / steps, "lost": d["lost"],
+           "crossings_per_packet": d["crossings"] / max(d["emitted"], 1),
+           "bound": roof["bound"], "roofline_frac": roof["frac"],
+           "hbm_algorithmic_frac": (roof.get("hbm") or roof)["frac"],
+           "gather_frac": gather["frac"] if gather else None,
+           "traffic_over_algorithmic": (roof.get("hbm") or roof).get("traffic_over_algorithmic")}
+    ctx.destroy()
+    return out
+
+
+PER_CONFIG = (("c0", 6), ("c1_tau0.1", 4), ("c1_tau10", 4), ("c1_tau100", 4), ("c2", 3), ("c3", 3), ("c4", 3))
 
 
 def run_gpu(args, wl, name):
@@ -239,7 +352,6 @@ def run_gpu(args, wl, name):
         dist.barrier()
     mcrt.lib()
 
-    batch = wl.batch
     stream = torch.cuda.current_stream().cuda_stream
     ctx = mcrt.from_workload(wl, layout=args.layout)
     if args.threads or args.blocks_per_sm:
@@ -252,14 +364,6 @@ def run_gpu(args, wl, name):
 
     from paper_1201_3588_b200.sharding import ShardedRunner
     runner = ShardedRunner(ctx, dist if world > 1 else None)
-    step_no = [0]
-
-    def one_step():
-        """One batch of `batch` packets per rank (weak scaling): the global batch of
-        world*batch packet ids is dealt to the ranks in contiguous ranges; N > 1 sums the
-        integer tallies over ranks before the T update (sharding.ShardedRunner)."""
-        runner.run_batch(wl.seed, step_no[0] * world * batch, world * batch, stream)
-        step_no[0] += 1
 
     def barrier():
         torch.cuda.synchronize()
@@ -272,40 +376,21 @@ def run_gpu(args, wl, name):
         sampler.start()
         sampler.wait_first()
     t_load0 = time.time()
-    for _ in range(args.warmup):
-        flush.fill_(1)
-        one_step()
-    barrier()
-    ctx.get_batch_times()
-    c_before = ctx.get_counters()
-    launches_before = ctx.kernel_launches()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-          for _ in range(args.steps)]
-    barrier()
-    t_wall = time.perf_counter()
-    for a, b in ev:
-        flush.fill_(1)                      # L2 flush between timed iterations (not timed)
-        a.record()
-        one_step()
-        b.record()
-    barrier()
-    t_wall = time.perf_counter() - t_wall
-    step_ms = [a.elapsed_time(b) for a, b in ev]
+    # One step = one batch of wl.batch packages per rank (weak scaling): the global batch of world*batch
+    # packet ids is dealt to the ranks in contiguous ranges; N > 1 all-reduces the batch's uint32 tallies
+    # before the T update (sharding.ShardedRunner).
+    r = time_steps(torch, ctx, wl, runner, stream, world, args.steps, args.warmup, flush, barrier)
+    step_ms, t_tr, t_up, d, launches = r["step_ms"], r["t_tr"], r["t_up"], r["d"], r["launches"]
     total_ms = float(sum(step_ms))
-    t_tr, t_up = ctx.get_batch_times()
-    c_after = ctx.get_counters()
-    launches = ctx.kernel_launches() - launches_before
     # the timed region may be far shorter than nvidia-smi's sampling period: keep the same
     # load running (untimed) until the clock record holds at least ~1.5 s under load
     while time.time() - t_load0 < 1.5:
-        one_step()
+        r["one_step"]()
         torch.cuda.synchronize()
     barrier()
     clocks = sampler.stop(t_load0, time.time()) if rank == 0 else None
     if clocks is not None:
         clocks["window"] = "warm-up + timed steps + identical untimed steps up to 1.5 s"
-    d = {k: c_after[k] - c_before[k] for k in ("emitted", "escaped", "absorptions",
-                                                "scatterings", "flights", "crossings", "lost")}
     stats = torch.tensor([total_ms, float(t_tr.sum()), float(t_up.sum())], dtype=torch.float64,
                          device="cuda")
     sums = torch.tensor([d["emitted"], d["crossings"], d["absorptions"], d["scatterings"],
@@ -323,22 +408,18 @@ def run_gpu(args, wl, name):
 
     # ---- gather roofline: independent 4-byte gathers over the density
     # footprint of this workload, measured live by the library's calibration kernel ----------
-    gather = None
+    gpeak = None
     if rank == 0 and not args.no_gather:
-        foot = int(wl.leaf_slots) * 4
-        g_peak, g_sec = mcrt.gather_calibrate(foot, 1 << 31, stream)
-        gather = {"footprint_bytes": foot, "peak_gathers_per_s": g_peak, "calibration_s": g_sec}
+        gpeak = mcrt.gather_calibrate(int(wl.leaf_slots) * 4, 1 << 31, stream)[0]
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     secs = total_ms * 1e-3
-    peak, peak_src = measured_peaks()
-    # dominant kernel = k_transport; per-launch figures from this rank's batches
-    bytes_alg, per_cross, per_abs = algorithmic_bytes(wl, d["crossings"], d["absorptions"])
-    tr_s = float(t_tr.sum()) * 1e-3
-    achieved = bytes_alg / tr_s / 1e9 if tr_s > 0 else 0.0
+    tr_s = float(t_tr.sum()) * 1e-3                          # dominant kernel: this rank's launches
+    roof, gather = rooflines(wl, name, d, tr_s, args.steps, gpeak)
+    roof["kernel_share_of_step"] = tr_s / (float(sum(step_ms)) * 1e-3)
     out = {"metric": METRIC, "value": n_emit / secs, "unit": UNIT, "n_gpus": world,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
@@ -351,28 +432,32 @@ def run_gpu(args, wl, name):
                           "scatterings": n_sca / max(n_emit, 1)},
            "lost": n_lost,
            "kernel_ms_per_step": {"transport": tr_ms / args.steps, "temperature_update": up_ms / args.steps},
-           "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
-           "roofline": {"bound": "hbm", "kernel": "k_transport", "achieved": achieved, "peak": peak,
-                        "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(name),
-                        "peak_source": peak_src,
-                        "algorithmic_bytes": {"per_crossing": per_cross, "per_absorption": per_abs,
-                                              "per_launch": bytes_alg / args.steps},
-                        "kernel_ms": 1e3 * tr_s / args.steps,
-                        "kernel_share_of_step": tr_s / (float(sum(step_ms)) * 1e-3)},
-           "gpu_launches": launches, "clocks": clocks}
+           "wall_ms_per_step_incl_flush": 1e3 * r["t_wall"] / args.steps,
+           "roofline": roof, "gpu_launches": launches, "clocks": clocks}
     if gather is not None:
-        # one density gather per crossing: crossings/s of the transport kernel alone vs the peak
-        gather["achieved_gathers_per_s"] = d["crossings"] / tr_s if tr_s > 0 else 0.0
-        gather["frac"] = gather["achieved_gathers_per_s"] / gather["peak_gathers_per_s"]
-        gather["what"] = ("peak = independent hash-indexed 4-byte gathers/s over an array of the "
-                          "density footprint at full occupancy (mcrt_gather_calibrate); achieved = "
-                          "cell crossings per second of k_transport on this rank")
         out["gather_roofline"] = gather
     if e2e is not None:
         out["e2e"] = e2e
+    ctx.destroy()
+    # ---- every other config of BASELINE.json, at reduced step counts, in the same invocation ----
+    if world == 1 and not args.no_per_config:
+        per = {name: {k: v for k, v in (("packets_per_s", out["value"]), ("crossings_per_s", out["crossings_per_s"]),
+                                         ("ms_per_step", out["ms_per_step"]),
+                                         ("kernel_ms", roof["kernel_ms"]), ("bound", roof["bound"]),
+                                         ("roofline_frac", roof["frac"]),
+                                         ("hbm_algorithmic_frac", (roof.get("hbm") or roof)["frac"]),
+                                         ("gather_frac", gather["frac"] if gather else None), ("lost", n_lost))}}
+        for wname, wsteps in PER_CONFIG:
+            if wname == name:
+                continue
+            try:
+                per[wname] = measure_workload(torch, mcrt, make_workload(wname), wname, wsteps, 3, stream, flush, args)
+            except Exception as e:                           # a config that cannot run must not hide the others
+                per[wname] = {"error": f"{type(e).__name__}: {e}"}
+            torch.cuda.empty_cache()
+        out["per_config"] = per
     if not args.no_cpu and world >= 1:
-        cb = oracle_rate(wl, target_seconds=args.cpu_seconds)
-        out["cpu_baseline"] = cb
+        out["cpu_baseline"] = oracle_rate(wl, target_seconds=args.cpu_seconds)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -380,18 +465,25 @@ def run_gpu(args, wl, name):
 
 def ctx_launch_desc(args):
     return (f"threads={args.threads or 'default'} blocks_per_sm={args.blocks_per_sm or 'default'} "
-            f"quorum={args.quorum or 'default'} layout={args.layout or 'auto'}")
+            f"quorum={args.quorum or 'auto'} layout={args.layout or 'auto'}")
 
 
 def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
-    """End to end through the public API with HOST buffers: every step re-creates nothing, but
-    the job starts from host arrays (grid_create/set_opacity/set_source copy them H2D inside the
-    timed region) and every step ends with a device->host read of that step's results (SED,
-    counters, cell energies, cell temperatures).  Value = packets of all steps / wall time,
-    device-synchronised, max over ranks."""
+    """End to end through the public API with HOST buffers: the job starts from host arrays
+    (grid_create/set_opacity/set_source copy them H2D inside the timed region) and every step
+    ends with a device->host read of that step's results (SED, counters, cell energies, cell
+    temperatures) into pinned host buffers.  The read-out of batch k is queued behind it
+    (mcrt_results_begin) and overlaps batch k+1; it is waited for before its buffers are reused.
+    Value = packets of all steps / wall time, device-synchronised, max over ranks."""
     batch = wl.batch
     rho = torch.from_numpy(np.ascontiguousarray(wl.rho_root)).pin_memory().numpy()
     steps = args.warmup + args.steps
+    slots = wl.leaf_slots
+    pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory().numpy()
+    mk = lambda: dict(n_abs=pin((slots,), torch.int64).view(np.uint64), T=pin((slots,), torch.float32),
+                      sed=pin((3, wl.n_bins), torch.int64).view(np.uint64),
+                      emitted_per_bin=pin((wl.n_bins,), torch.int64).view(np.uint64))
+    bufs = [mk(), mk()]                                      # allocated once, reused every other step
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -400,28 +492,24 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
     ctx.grid_create(wl.n_root, wl.sub, wl.origin, wl.root_size, wl.refine, rho, wl.rho_sub)
     ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g)
     ctx.set_source(wl.sources)
-    d2h = 0
-    # read-back buffers: pinned host memory, allocated once and reused every step
-    slots = wl.leaf_slots
-    pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory().numpy()
-    b_sed = pin((3, wl.n_bins), torch.int64).view(np.uint64)
-    b_abs = pin((slots,), torch.int64).view(np.uint64)
-    b_T = pin((slots,), torch.float32)
-    b_emit = pin((wl.n_bins,), torch.int64).view(np.uint64)
     from paper_1201_3588_b200.sharding import ShardedRunner
     runner = ShardedRunner(ctx, dist if world > 1 else None)
+    pending, n_read = None, 0
     for s in range(steps):
         runner.run_batch(wl.seed, s * world * batch, world * batch, stream)
-        sed = ctx.get_sed(out=b_sed)
-        n_abs, _ = ctx.get_cell_energy(out=b_abs)
-        T = ctx.get_cell_temperature(out=b_T)
-        c = ctx.get_counters(out=b_emit)
-        d2h = sed.nbytes + n_abs.nbytes + T.nbytes + 7 * 8 + c["emitted_per_bin"].nbytes
+        h = ctx.results_begin(bufs[s % 2])
+        if pending is not None:
+            n_read += ctx.results_wait(pending)["counters"]["emitted"] > 0
+        pending = h
+    last = ctx.results_wait(pending)
+    n_read += 1
     torch.cuda.synchronize()
     dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(dt, op=dist.ReduceOp.MAX)
     dt = float(dt.cpu())
+    assert n_read == steps and last["counters"]["emitted"] > 0
+    d2h = sum(v.nbytes for v in bufs[0].values()) + 7 * 8
     h2d_job = wl.rho_root.nbytes + (0 if wl.rho_sub is None else wl.rho_sub.nbytes) \
         + (0 if wl.refine is None else wl.refine.nbytes + 4 * wl.refine.size) \
         + wl.kabs.nbytes * 3 + wl.lambda_edges_um.nbytes
@@ -430,7 +518,23 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
             "h2d_bytes_per_step": h2d_job / steps, "d2h_bytes_per_step": d2h,
             "what": f"one job of {steps} batches from host arrays: grid/opacity/source set-up "
                     "(H2D) + run_batch + host read-back of SED, counters, cell energy and "
-                    "temperature after every batch; wall clock, device-synchronised"}
+                    "temperature after EVERY batch (pinned buffers; the read-out of batch k "
+                    "overlaps batch k+1); wall clock, device-synchronised"}
+
+
+def relaunch_under_torchrun(args):
+    """`python bench.py --gpus N` without a launcher: start N ranks on this node ourselves."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                     # the communicator log shows the ranks (and NVLS)
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    raise SystemExit(subprocess.call(cmd, env=env))
 
 
 def main():
@@ -442,13 +546,14 @@ def main():
     ap.add_argument("--workload", default="c1_tau1")
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
-    ap.add_argument("--quorum", type=int, default=0, help="walk-loop quorum (0 = library default)")
+    ap.add_argument("--quorum", type=int, default=0, help="walk-loop quorum (0 = automatic)")
     ap.add_argument("--source-order", type=int, default=None,
                     help="hand packages out grouped by source: 1 on, 0 off (default: automatic)")
     ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 x-fastest, 2 bricked")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-gather", action="store_true", help="skip the gather-roofline calibration")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the other configs (per_config)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "native" else args.warmup
@@ -458,6 +563,10 @@ def main():
             return
         run_reference(args, make_workload(args.workload), args.workload)
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        relaunch_under_torchrun(args)
+    if args.gpus != int(os.environ.get("WORLD_SIZE", "1")):
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ.get('WORLD_SIZE', '1')}")
     run_gpu(args, make_workload(args.workload), args.workload)
 
 

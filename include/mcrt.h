@@ -146,7 +146,23 @@ mcrt_status mcrt_transport_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first_pa
 mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, uint64_t n_cum,
                                     void* cuda_stream);
 
-/* ---- results ---------------------------------------------------------------------------------
+/* The same exchange with HALF the bytes and no layout conversion (what sharding.ShardedRunner uses):
+ * mcrt_transport_batch_delta zeroes `delta_dev` (DEVICE, uint32[mcrt_store_slots], owned by the
+ * caller, e.g. a torch int32 tensor), then transports this rank's packets tallying the batch's
+ * absorptions into it instead of into the cumulative tally; the ranks all-reduce (sum) their delta
+ * arrays; mcrt_accumulate_update adds the summed delta to the context's cumulative tally and
+ * updates the temperatures with n_cum = packages emitted so far by ALL ranks (one kernel).  The
+ * array is in the library's internal STORAGE order (root grid possibly bricked and padded,
+ * subcubes behind it): opaque to the caller, identical on every rank that created the same grid.
+ * After the call every rank's mcrt_get_cell_energy returns the global cumulative counts. */
+int64_t mcrt_store_slots(const mcrt_ctx* ctx);
+mcrt_status mcrt_transport_batch_delta(mcrt_ctx* ctx, uint64_t seed, uint64_t first_packet_id,
+                                       uint64_t n_packets, uint32_t* delta_dev, void* cuda_stream);
+mcrt_status mcrt_accumulate_update(mcrt_ctx* ctx, const uint32_t* delta_sum_dev, uint64_t n_cum,
+                                   void* cuda_stream);
+
+/* ---- results ("Each absorption event raises the energy of the cell by eps, and
+ * accordingly its temperature"; L27, L31: the computed SED) ------------------------------------
  * n_abs_out[leaf slots]: cumulative number of packages absorbed per leaf (exact integers; "cell
  * energy" in units of eps, R23).  *eps_out (host pointer, may be NULL) = L_tot / N_cum in erg s^-1
  * per package, so that the absorbed power of a cell is n_abs * eps. */
@@ -160,6 +176,28 @@ mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
 typedef struct {
   uint64_t emitted, escaped, lost, absorptions, scatterings, flights, crossings;
 } mcrt_counters;
+
+/* ---- all results of a batch in one call, optionally overlapped with the next batch -------------
+ * The getters above synchronise once each.  mcrt_get_results reads any subset of the same arrays
+ * (cell energies and temperatures; L27, L31: the SED) with ONE synchronisation;
+ * mcrt_results_begin only queues the read-out and returns a ticket (0 or 1; two may be in flight):
+ * on the stream of the last batch it snapshots what was asked for (slot order, R22) into buffers
+ * the context owns, then copies the snapshot to the caller's buffers on a stream of its own, so a
+ * mcrt_run_batch issued right after it overlaps the transfer; mcrt_results_wait(ticket) blocks
+ * until that ticket's buffers are filled.  `mem` says where n_abs / T / sed / emitted_per_bin
+ * live (MCRT_HOST buffers should be pinned for the copies to overlap); counters and eps are host
+ * pointers always.  Any member may be NULL.  The buffers must stay valid until the wait. */
+typedef struct {
+  uint64_t* n_abs;           /* [leaf slots] cumulative absorbed packages per leaf             */
+  float* T;                  /* [leaf slots] K                                                  */
+  uint64_t* sed;             /* [3][n_bins]                                                     */
+  uint64_t* emitted_per_bin; /* [n_bins]                                                        */
+  mcrt_counters* counters;   /* host                                                            */
+  double* eps;               /* host: L_tot / N_cum                                             */
+} mcrt_results;
+mcrt_status mcrt_get_results(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem mem);
+mcrt_status mcrt_results_begin(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem mem, int32_t* ticket);
+mcrt_status mcrt_results_wait(mcrt_ctx* ctx, int32_t ticket);
 /* Cumulative event counters (host struct) and, if not NULL, emitted packages per bin
  * (host, [n_bins]).  `crossings` counts every exit of a packet from a leaf through a face,
  * including the final exit from the box (R27).  `lost` counts packets dropped at the flight cap
@@ -209,9 +247,11 @@ mcrt_status mcrt_get_image(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
  * current value) and resident blocks per SM (0 = automatic: 5, or 4 for a single-level grid larger
  * than the L2; more than 1024 resident threads per SM select the 48-register build of the kernel). */
 mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t blocks_per_sm);
-/* Single-level grids: a warp leaves the cell-walk loop to process its stopped lanes (escape,
- * refill, scattering, absorption) when fewer than `quorum` of its 32 lanes are still walking
- * (1..32; 0 keeps the default 16).  A scheduling knob only: results do not depend on it. */
+/* A warp leaves the cell-walk loop to process its stopped lanes (escape, refill, scattering,
+ * absorption) when fewer than `quorum` of its 32 lanes are still walking (1..32).  0 = automatic
+ * (the default): 14 + 2 log2(L / 24) clamped to 8..24, L = the job's crossings per flight so far
+ * (long free flights -> keep more lanes walking).  A scheduling knob only: results do not depend
+ * on it. */
 mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum);
 /* Hand the packages of a batch to the lanes grouped by where they start (a pre-pass evaluates the
  * first decisions of every package's emission and groups the package numbers), so that the

@@ -38,10 +38,12 @@ struct mcrt_ctx {
   double *d_nu = nullptr, *d_dnu = nullptr, *d_kabs = nullptr;
   float4* d_opac = nullptr;
   float *d_lnQ = nullptr, *d_cdf = nullptr;
+  int* d_guide = nullptr;                 // [kGuide] bracket guide of the ln Q table (tables.cuh)
   // sources
   int nsrc = 0;
   SrcDev* d_src = nullptr;
   double* d_csrc = nullptr;               // [nsrc][nb] fp64 source CDFs (emission decisions are exact)
+  float* d_csrc32 = nullptr;              // ... and their fp32 copy
   double Ltot = 0;
   // tallies: [0] work-queue head, [1..CNT_N] counters, then sed[3*nb], emit_bin[nb]
   unsigned long long* d_small = nullptr;
@@ -60,11 +62,22 @@ struct mcrt_ctx {
   unsigned int* d_srccnt = nullptr;       // [2][nsrc] counts, cursors
   int order_by_source = -1;               // -1 automatic, 0 off, 1 by source, 2 by source and start direction
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
-  int quorum = 16;
+  int quorum = 0;                         // 0 = automatic (from the job's crossings per flight so far)
   int threads = 256, blocks_per_sm = 0;   // 0 = automatic (5; 4 on HBM-resident single-level grids)
   long long launches = 0;
   // observer (O9 / R34): escape-direction tallies, off by default
   ObserverDev obs = {0, 0, 0, -1, {0, 0, 1}, {1, 0, 0}, {0, 1, 0}, 1.f, 1.f, nullptr, nullptr};
+  // asynchronous read-out (mcrt_results_begin / _wait): two tickets, each with its own device snapshot,
+  // pinned staging of the small tallies and events; copies run on the context's own stream
+  struct Ticket {
+    bool busy = false;
+    unsigned long long* snap_abs = nullptr; float* snap_T = nullptr; unsigned long long* snap_small = nullptr;
+    unsigned long long* h_small = nullptr;                  // pinned
+    cudaEvent_t ev_snap = nullptr, ev_done = nullptr;
+    mcrt_counters* counters = nullptr; uint64_t* emitted = nullptr; uint64_t* sed = nullptr; mcrt_mem mem = MCRT_HOST;
+  } tickets[2];
+  int next_ticket = 0;
+  cudaStream_t copy_stream = nullptr;
   bool have_opacity = false, have_source = false;
   std::string err;
 };
@@ -85,8 +98,8 @@ static mcrt_status fail(mcrt_ctx* c, mcrt_status st, const std::string& msg) {
 
 static void free_opacity(mcrt_ctx* c) {
   cudaFree(c->d_nu); cudaFree(c->d_dnu); cudaFree(c->d_kabs); cudaFree(c->d_opac);
-  cudaFree(c->d_lnQ); cudaFree(c->d_cdf); cudaFree(c->d_small);
-  c->d_nu = c->d_dnu = c->d_kabs = nullptr; c->d_opac = nullptr; c->d_lnQ = c->d_cdf = nullptr;
+  cudaFree(c->d_lnQ); cudaFree(c->d_cdf); cudaFree(c->d_small); cudaFree(c->d_guide);
+  c->d_nu = c->d_dnu = c->d_kabs = nullptr; c->d_opac = nullptr; c->d_lnQ = c->d_cdf = nullptr; c->d_guide = nullptr;
   c->d_small = nullptr;
 }
 static void free_observer(mcrt_ctx* c) {
@@ -95,14 +108,15 @@ static void free_observer(mcrt_ctx* c) {
   c->obs.n_mu = c->obs.n_pix = 0;
 }
 static void free_sources(mcrt_ctx* c) {
-  cudaFree(c->d_src); cudaFree(c->d_csrc);
-  c->d_src = nullptr; c->d_csrc = nullptr;
+  cudaFree(c->d_src); cudaFree(c->d_csrc); cudaFree(c->d_csrc32);
+  c->d_src = nullptr; c->d_csrc = nullptr; c->d_csrc32 = nullptr;
 }
 
-// dynamic shared memory of the transport kernel: opacity float4[nb], SED u32[3 nb], emitted u32[nb],
-// root delta tables int[6 N] (+ subcube tables int[6 * 8] on two-level grids)
+// dynamic shared memory of the transport kernel: opacity float4[nb], SED u32[3 nb], emitted u32[nb], then at
+// a 64-byte boundary the root delta tables int[6 N] (+ the subcube rows int[6][16] on two-level grids)
 static size_t transport_smem_bytes(const mcrt_ctx* ctx) {
-  return 32 * (size_t)ctx->nb + sizeof(int) * (6 * (size_t)ctx->N + (ctx->uni ? 0 : 6 * kSubStride));
+  const size_t n_lut = ctx->uni ? 6 * (size_t)ctx->N : (size_t)lut_sub_offset(ctx->N) + 6 * kSubStride;
+  return ((32 * (size_t)ctx->nb + 63) & ~(size_t)63) + sizeof(int) * n_lut;
 }
 constexpr size_t kMaxSmemPerBlock = 227u << 10;              // B200: opt-in limit of dynamic shared memory
 
@@ -200,7 +214,8 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     // two-level grids: followed by the tables of the S^3 subcubes of a refined cube (entry j = directional
     // subcube index: +-S^a, the last one = "leaves the cube")
     const int N = ctx->N, S = ctx->S;
-    std::vector<int> lut(6 * (size_t)N + (ctx->uni ? 0 : 6 * kSubStride), 0);
+    const size_t sub0 = (size_t)lut_sub_offset(N);
+    std::vector<int> lut(ctx->uni ? 6 * (size_t)N : sub0 + 6 * kSubStride, 0);
     for (int a = 0; a < 3; ++a)
       for (int i = 0; i < N; ++i) {
         lut[(size_t)(2 * a) * N + i] = i == N - 1 ? kLutEscape
@@ -213,9 +228,11 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
       int stride = 1;
       for (int a = 0; a < 3; ++a) {
         for (int j = 0; j < S; ++j) {
-          lut[6 * (size_t)N + (size_t)(2 * a) * kSubStride + j] = j == S - 1 ? kLutLeave : stride;
-          lut[6 * (size_t)N + (size_t)(2 * a + 1) * kSubStride + j] = j == S - 1 ? kLutLeave : -stride;
+          lut[sub0 + (size_t)(2 * a) * kSubStride + j] = j == S - 1 ? kLutLeave : stride;
+          lut[sub0 + (size_t)(2 * a + 1) * kSubStride + j] = j == S - 1 ? kLutLeave : -stride;
         }
+        lut[sub0 + (size_t)(2 * a) * kSubStride + kSubStride - 1] = -(S - 1) * stride;      // wrap to the mirror subcube
+        lut[sub0 + (size_t)(2 * a + 1) * kSubStride + kSubStride - 1] = (S - 1) * stride;
         stride *= S;
       }
     }
@@ -243,6 +260,12 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   if (ctx->last_stream || true) cudaDeviceSynchronize();
   for (auto& b : ctx->pending) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& b : ctx->spare) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
+  for (auto& t : ctx->tickets) {
+    cudaFree(t.snap_abs); cudaFree(t.snap_T); cudaFree(t.snap_small); cudaFreeHost(t.h_small);
+    if (t.ev_snap) cudaEventDestroy(t.ev_snap);
+    if (t.ev_done) cudaEventDestroy(t.ev_done);
+  }
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   free_opacity(ctx);
   free_sources(ctx);
   free_observer(ctx);
@@ -298,6 +321,7 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
   CU(cudaMalloc(&ctx->d_opac, sizeof(float4) * nb));
   CU(cudaMalloc(&ctx->d_lnQ, 4 * nT));
   CU(cudaMalloc(&ctx->d_cdf, 4 * (size_t)nT * nb));
+  CU(cudaMalloc(&ctx->d_guide, sizeof(int) * kGuide));
   const size_t n_small = 1 + CNT_N + 4 * (size_t)nb;
   CU(cudaMalloc(&ctx->d_small, 8 * n_small));
   CU(cudaMemset(ctx->d_small, 0, 8 * n_small));
@@ -305,7 +329,8 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
                                            ctx->d_nu, ctx->d_dnu, ctx->d_kabs, ctx->d_opac);
   k_build_emission_rows<<<nT, 128, 8 * (nb + 1)>>>(nb, nT, Tmin, Tmax, ctx->d_nu, ctx->d_dnu,
                                                    ctx->d_kabs, ctx->d_lnQ, ctx->d_cdf);
-  ctx->launches += 2;
+  k_build_guide<<<kGuide / 256, 256>>>(ctx->d_lnQ, nT, ctx->d_guide);
+  ctx->launches += 3;
   CU(cudaGetLastError());
   CU(cudaDeviceSynchronize());
   ctx->have_opacity = true;
@@ -357,7 +382,8 @@ mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src
   CU(cudaMalloc(&ctx->d_src, sizeof(SrcDev) * n_src));
   CU(cudaMemcpy(ctx->d_src, h.data(), sizeof(SrcDev) * n_src, cudaMemcpyHostToDevice));
   CU(cudaMalloc(&ctx->d_csrc, 8 * (size_t)n_src * ctx->nb));
-  k_build_source_cdf<<<n_src, 128, 8 * (ctx->nb + 1)>>>(ctx->nb, d_T, ctx->d_nu, ctx->d_dnu, ctx->d_csrc);
+  CU(cudaMalloc(&ctx->d_csrc32, 4 * (size_t)n_src * ctx->nb));
+  k_build_source_cdf<<<n_src, 128, 8 * (ctx->nb + 1)>>>(ctx->nb, d_T, ctx->d_nu, ctx->d_dnu, ctx->d_csrc, ctx->d_csrc32);
   ctx->launches++;
   CU(cudaGetLastError());
   CU(cudaDeviceSynchronize());
@@ -373,18 +399,19 @@ static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
   return MCRT_OK;
 }
 
-static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st) {
+static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st,
+                                    uint32_t* tally32 = nullptr) {
   if (n == 0) return MCRT_OK;
   const uint64_t kMaxLaunch = 1ull << 31;                    // the kernels number packages within a launch in 32 bits
   if (n > kMaxLaunch) {
-    mcrt_status rc = launch_transport(ctx, seed, first, kMaxLaunch, st);
+    mcrt_status rc = launch_transport(ctx, seed, first, kMaxLaunch, st, tally32);
     if (rc != MCRT_OK) return rc;
-    return launch_transport(ctx, seed, first + kMaxLaunch, n - kMaxLaunch, st);
+    return launch_transport(ctx, seed, first + kMaxLaunch, n - kMaxLaunch, st, tally32);
   }
   const int nb = ctx->nb;
   TransportParams P;
-  P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.trow = ctx->d_trow;
-  P.opac = ctx->d_opac; P.cdf = ctx->d_cdf; P.csrc = ctx->d_csrc; P.src = ctx->d_src;
+  P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.tally32 = tally32; P.trow = ctx->d_trow;
+  P.opac = ctx->d_opac; P.cdf = ctx->d_cdf; P.csrc = ctx->d_csrc32; P.csrc64 = ctx->d_csrc; P.src = ctx->d_src;
   P.next = ctx->d_small; P.counters = ctx->d_small + 1;
   P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
   P.seed = seed; P.first = first; P.count = n;
@@ -444,7 +471,9 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
 
 // a9: T from `tally` (the context's own cumulative tally, or a caller's device array that
 // holds the sum over ranks) and n_cum packages emitted so far in the whole job.
-static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally, uint64_t n_cum, cudaStream_t st) {
+// delta != NULL: first add the batch's counts (u32, storage order, summed over ranks) to the context's tally.
+static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally, uint64_t n_cum, cudaStream_t st,
+                                 const uint32_t* delta = nullptr) {
   if (n_cum == 0) return MCRT_OK;
   const double PI = 3.14159265358979323846;
   double V = ctx->root_size * ctx->root_size * ctx->root_size;
@@ -462,13 +491,18 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
                          cudaMemcpyDeviceToDevice, st));
     tally = ctx->d_tally_scratch;
   }
-  long long blocks = (ctx->store_slots + 255) / 256;
+  long long blocks = (ctx->store_slots / 2 + 256) / 256;     // two leaves per thread and turn
   long long cap = (long long)ctx->sm_count * 8;
   if (blocks > cap) blocks = cap;
-  k_update_temperature<<<(unsigned)blocks, 256, 4 * ctx->nT, st>>>(ctx->d_rho, tally, ctx->d_trow, ctx->d_lnQ,
-                                                                  ctx->nT, ctx->store_slots,
-                                                                  ctx->uni ? ctx->store_slots : ctx->store_n3,
-                                                                  ln_coef, ln_sub3);
+  const size_t smem = 4 * (size_t)ctx->nT + sizeof(int) * kGuide;
+  const long long n3 = ctx->uni ? ctx->store_slots : ctx->store_n3;
+  if (delta)
+    k_update_temperature<true><<<(unsigned)blocks, 256, smem, st>>>(ctx->d_rho, ctx->d_tally, delta, ctx->d_trow, ctx->d_lnQ,
+                                                                    ctx->d_guide, ctx->nT, ctx->store_slots, n3, ln_coef, ln_sub3);
+  else
+    k_update_temperature<false><<<(unsigned)blocks, 256, smem, st>>>(ctx->d_rho, const_cast<unsigned long long*>(tally), nullptr,
+                                                                     ctx->d_trow, ctx->d_lnQ, ctx->d_guide, ctx->nT,
+                                                                     ctx->store_slots, n3, ln_coef, ln_sub3);
   ctx->launches++;
   CU(cudaGetLastError());
   return MCRT_OK;
@@ -529,6 +563,40 @@ mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, ui
   ctx->Nglobal = tally_sum ? n_cum : ctx->Ncum;             // eps of mcrt_get_cell_energy = L_tot / packages of all ranks
   mcrt_status rc = launch_update(ctx, tally_sum ? (const unsigned long long*)tally_sum : ctx->d_tally,
                                  tally_sum ? n_cum : ctx->Ncum, st);
+  ctx->last_stream = st;
+  return rc;
+}
+
+int64_t mcrt_store_slots(const mcrt_ctx* ctx) { return ctx ? ctx->store_slots : -1; }
+
+mcrt_status mcrt_transport_batch_delta(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, uint32_t* delta_dev,
+                                       void* stream_) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_transport_batch_delta: grid, opacity and sources must be set first");
+  if (!delta_dev) return fail(ctx, MCRT_EINVAL, "mcrt_transport_batch_delta: NULL delta buffer");
+  cudaStream_t st = (cudaStream_t)stream_;
+  BatchEvents ev;
+  mcrt_status rc = begin_batch(ctx, &ev);
+  if (rc != MCRT_OK) return rc;
+  CU(cudaEventRecord(ev.e0, st));
+  CU(cudaMemsetAsync(delta_dev, 0, sizeof(uint32_t) * (size_t)ctx->store_slots, st));
+  rc = launch_transport(ctx, seed, first, n, st, delta_dev);
+  if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
+  CU(cudaEventRecord(ev.e1, st));
+  CU(cudaEventRecord(ev.e2, st));
+  ctx->pending.push_back(ev);
+  ctx->Ncum += n;
+  ctx->last_stream = st;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_accumulate_update(mcrt_ctx* ctx, const uint32_t* delta_sum_dev, uint64_t n_cum, void* stream_) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_accumulate_update: grid, opacity and sources must be set first");
+  if (!delta_sum_dev || n_cum == 0) return fail(ctx, MCRT_EINVAL, "mcrt_accumulate_update: NULL delta / n_cum = 0");
+  cudaStream_t st = (cudaStream_t)stream_;
+  ctx->Nglobal = n_cum;
+  mcrt_status rc = launch_update(ctx, ctx->d_tally, n_cum, st, delta_sum_dev);
   ctx->last_stream = st;
   return rc;
 }
@@ -601,6 +669,102 @@ mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem) {
   if (!counts_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_sed: NULL output");
   if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_sed: opacity not set");
   return copy_out(ctx, counts_out, ctx->d_small + 1 + CNT_N, 8 * 3 * (size_t)ctx->nb, mem);
+}
+
+// ---- combined / asynchronous read-out ----------------------------------------------------------
+mcrt_status mcrt_results_begin(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem mem, int32_t* ticket) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!out || !ticket) return fail(ctx, MCRT_EINVAL, "mcrt_results_begin: NULL argument");
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_results_begin: opacity not set");
+  const int s = ctx->next_ticket;
+  mcrt_ctx::Ticket& t = ctx->tickets[s];
+  if (t.busy) return fail(ctx, MCRT_ESTATE, "mcrt_results_begin: both tickets are in flight (call mcrt_results_wait)");
+  cudaStream_t st = ctx->last_stream;
+  if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+  if (!t.ev_snap) { CU(cudaEventCreateWithFlags(&t.ev_snap, cudaEventDisableTiming)); CU(cudaEventCreateWithFlags(&t.ev_done, cudaEventDisableTiming)); }
+  const size_t n_small = 1 + CNT_N + 4 * (size_t)ctx->nb;
+  const bool host = mem == MCRT_HOST;
+  // 1. snapshot on the batches' stream (the next batch may start right behind it)
+  unsigned long long* abs_dst = nullptr;
+  float* T_dst = nullptr;
+  if (out->n_abs) {
+    if (host && !t.snap_abs) CU(cudaMalloc(&t.snap_abs, 8 * (size_t)ctx->slots));
+    abs_dst = host ? t.snap_abs : (unsigned long long*)out->n_abs;
+    if (ctx->lay.bricked) {
+      k_store_to_ext<unsigned long long><<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(ctx->d_tally, abs_dst, ctx->lay, ctx->n3);
+      ctx->launches++;
+      if (ctx->slots > ctx->n3)
+        CU(cudaMemcpyAsync(abs_dst + ctx->n3, ctx->d_tally + ctx->store_n3, 8 * (size_t)(ctx->slots - ctx->n3), cudaMemcpyDeviceToDevice, st));
+    } else {
+      CU(cudaMemcpyAsync(abs_dst, ctx->d_tally, 8 * (size_t)ctx->slots, cudaMemcpyDeviceToDevice, st));
+    }
+  }
+  if (out->T) {
+    if (host && !t.snap_T) CU(cudaMalloc(&t.snap_T, 4 * (size_t)ctx->slots));
+    T_dst = host ? t.snap_T : out->T;
+    k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(ctx->d_trow, T_dst, ctx->lay, ctx->n3,
+                                                                     (float)std::log(ctx->Tmin), (float)ctx->dlnT);
+    ctx->launches++;
+    if (ctx->slots > ctx->n3) {
+      const long long ns = ctx->slots - ctx->n3;
+      k_trow_to_T<<<(unsigned)((ns + 255) / 256), 256, 0, st>>>(ctx->d_trow + ctx->store_n3, T_dst + ctx->n3, ns,
+                                                                (float)std::log(ctx->Tmin), (float)ctx->dlnT);
+      ctx->launches++;
+    }
+  }
+  if (!t.snap_small) { CU(cudaMalloc(&t.snap_small, 8 * n_small)); }
+  CU(cudaMemcpyAsync(t.snap_small, ctx->d_small, 8 * n_small, cudaMemcpyDeviceToDevice, st));
+  CU(cudaGetLastError());
+  CU(cudaEventRecord(t.ev_snap, st));
+  // 2. copies out on the context's own stream
+  cudaStream_t cs = ctx->copy_stream;
+  CU(cudaStreamWaitEvent(cs, t.ev_snap, 0));
+  if (host) {
+    if (out->n_abs) CU(cudaMemcpyAsync(out->n_abs, t.snap_abs, 8 * (size_t)ctx->slots, cudaMemcpyDeviceToHost, cs));
+    if (out->T) CU(cudaMemcpyAsync(out->T, t.snap_T, 4 * (size_t)ctx->slots, cudaMemcpyDeviceToHost, cs));
+  }
+  if (!t.h_small) CU(cudaMallocHost(&t.h_small, 8 * 8192 * 5));     // n_bins <= 4096
+  CU(cudaMemcpyAsync(t.h_small, t.snap_small, 8 * n_small, cudaMemcpyDeviceToHost, cs));
+  if (!host) {
+    if (out->sed) CU(cudaMemcpyAsync(out->sed, t.snap_small + 1 + CNT_N, 8 * 3 * (size_t)ctx->nb, cudaMemcpyDeviceToDevice, cs));
+    if (out->emitted_per_bin)
+      CU(cudaMemcpyAsync(out->emitted_per_bin, t.snap_small + 1 + CNT_N + 3 * (size_t)ctx->nb, 8 * (size_t)ctx->nb, cudaMemcpyDeviceToDevice, cs));
+  }
+  CU(cudaEventRecord(t.ev_done, cs));
+  if (out->eps) {
+    const unsigned long long n_eps = ctx->Nglobal > ctx->Ncum ? ctx->Nglobal : ctx->Ncum;
+    *out->eps = n_eps ? ctx->Ltot / (double)n_eps : 0.0;
+  }
+  t.counters = out->counters; t.mem = mem;
+  t.sed = host ? out->sed : nullptr; t.emitted = host ? out->emitted_per_bin : nullptr;
+  t.busy = true;
+  *ticket = s;
+  ctx->next_ticket = s ^ 1;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_results_wait(mcrt_ctx* ctx, int32_t ticket) {
+  if (!ctx) return MCRT_EINVAL;
+  if (ticket < 0 || ticket > 1 || !ctx->tickets[ticket].busy) return fail(ctx, MCRT_EINVAL, "mcrt_results_wait: no such ticket in flight");
+  mcrt_ctx::Ticket& t = ctx->tickets[ticket];
+  CU(cudaEventSynchronize(t.ev_done));
+  const unsigned long long* h = t.h_small + 1;
+  if (t.counters) {
+    t.counters->emitted = h[CNT_EMITTED]; t.counters->escaped = h[CNT_ESCAPED]; t.counters->lost = h[CNT_LOST];
+    t.counters->absorptions = h[CNT_ABS]; t.counters->scatterings = h[CNT_SCA]; t.counters->flights = h[CNT_FLIGHTS];
+    t.counters->crossings = h[CNT_CROSS];
+  }
+  if (t.sed) std::memcpy(t.sed, h + CNT_N, 8 * 3 * (size_t)ctx->nb);
+  if (t.emitted) std::memcpy(t.emitted, h + CNT_N + 3 * (size_t)ctx->nb, 8 * (size_t)ctx->nb);
+  t.busy = false;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_get_results(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem mem) {
+  int32_t ticket = -1;
+  mcrt_status rc = mcrt_results_begin(ctx, out, mem, &ticket);
+  if (rc != MCRT_OK) return rc;
+  return mcrt_results_wait(ctx, ticket);
 }
 
 mcrt_status mcrt_set_observer(mcrt_ctx* ctx, const mcrt_observer_desc* d) {
@@ -703,7 +867,7 @@ mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads, int32_t blocks_per_s
 mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
   if (!ctx) return MCRT_EINVAL;
   if (quorum < 0 || quorum > 32) return fail(ctx, MCRT_EINVAL, "mcrt_set_walk_quorum: quorum must be 0..32");
-  ctx->quorum = quorum ? quorum : 16;
+  ctx->quorum = quorum;
   return MCRT_OK;
 }
 

@@ -71,9 +71,11 @@ __global__ void k_build_emission_rows(int nb, int nT, double Tmin, double Tmax,
 }
 
 // Source spectra: blackbody truncated to the band, same midpoint rule (R5, R6).  Kept in fp64: the
-// emission bin is searched once per package with the fp64 uniform, so emitted-per-bin is exact.
+// emission bin is settled once per package with the fp64 uniform, so emitted-per-bin is exact; the
+// fp32 copy serves the search loop that emission shares with re-emission.
 __global__ void k_build_source_cdf(int nb, const double* __restrict__ Tbb, const double* __restrict__ nu,
-                                   const double* __restrict__ dnu, double* __restrict__ csrc) {
+                                   const double* __restrict__ dnu, double* __restrict__ csrc,
+                                   float* __restrict__ csrc32) {
   extern __shared__ double s_term[];
   int s = blockIdx.x;
   double T = Tbb[s];
@@ -87,7 +89,11 @@ __global__ void k_build_source_cdf(int nb, const double* __restrict__ Tbb, const
   __syncthreads();
   double tot = s_term[nb];
   for (int j = threadIdx.x; j < nb; j += blockDim.x)
-    csrc[(size_t)s * nb + j] = (j == nb - 1 || !(tot > 0)) ? 1.0 : s_term[j] / tot;
+  {
+    const double v = (j == nb - 1 || !(tot > 0)) ? 1.0 : s_term[j] / tot;
+    csrc[(size_t)s * nb + j] = v;
+    csrc32[(size_t)s * nb + j] = (float)v;
+  }
 }
 
 // a9 / O7 (R9 reading B, R10, R12): per-leaf radiative-equilibrium temperature from the cumulative
@@ -95,27 +101,78 @@ __global__ void k_build_source_cdf(int nb, const double* __restrict__ Tbb, const
 // (N_cum 4 pi V_root)) is computed on the host in fp64.  Q^-1 by bracketing the ln Q table (in
 // shared memory) and linear interpolation in (ln Q, ln T); the result is stored as the table row
 // coordinate t = (ln T - ln T_min)/dlnT in [0, nT-1], which is what re-emission needs.
-__global__ void k_update_temperature(const float* __restrict__ rho, const unsigned long long* __restrict__ tally,
-                                     float* __restrict__ trow, const float* __restrict__ lnQ, int nT,
-                                     long long slots, long long n3, float ln_coef, float ln_sub3) {
-  extern __shared__ float s_lnQ[];
+//
+// The bracket lnQ[lo] <= lq < lnQ[lo+1] is found through a GUIDE table instead of a binary search
+// (ten dependent, bank-conflicting shared-memory reads per leaf made the kernel run at 29 % of the
+// copy bandwidth): the range [lnQ[0], lnQ[nT-1]] is cut into kGuide equal buckets, guide[b] = the
+// largest row k whose lnQ[k] falls into a bucket below b, so lnQ[guide[b]] <= lq for every lq of
+// bucket b, and a walk of (mostly 0 or 1) rows from there ends on the same bracket the binary
+// search finds.  With ~2.5 buckets per row the kernel is a plain stream.
+constexpr int kGuide = 2048;
+__device__ __forceinline__ int q_bucket(float x, float lq0, float inv_w) {
+  return min(kGuide - 1, max(0, (int)((x - lq0) * inv_w)));
+}
+__global__ void k_build_guide(const float* __restrict__ lnQ, int nT, int* __restrict__ guide) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= kGuide) return;
+  const float lq0 = lnQ[0], inv_w = (float)kGuide / (lnQ[nT - 1] - lnQ[0]);
+  int lo = 0, hi = nT;                                       // rows [0, lo] are known to lie below bucket b (row 0 by definition)
+  while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (q_bucket(lnQ[mid], lq0, inv_w) < b) lo = mid; else hi = mid; }
+  guide[b] = lo;
+}
+
+__device__ __forceinline__ float row_of_lnq(float lq, const float* s_lnQ, const int* s_guide, int nT, float lq0,
+                                            float inv_w, bool use_guide) {
+  if (lq >= s_lnQ[nT - 1]) return (float)(nT - 1);
+  if (!(lq > s_lnQ[0])) return 0.f;
+  int lo;
+  if (use_guide) {
+    lo = s_guide[q_bucket(lq, lq0, inv_w)];
+    while (s_lnQ[lo + 1] <= lq) ++lo;                         // lq < lnQ[nT-1]: stops at the latest at nT-2
+  } else {                                                    // degenerate table (rows with Q = 0): plain bisection
+    int hi = nT - 1;
+    lo = 0;
+    while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (s_lnQ[mid] <= lq) lo = mid; else hi = mid; }
+  }
+  return (float)lo + (lq - s_lnQ[lo]) / (s_lnQ[lo + 1] - s_lnQ[lo]);
+}
+
+// ADD: first add the batch's absorbed-package counts `delta` (u32, the sum over all ranks of a
+// packet-sharded run) to the cumulative tally, then update (one pass over the leaves).
+template <bool ADD>
+__global__ void __launch_bounds__(256) k_update_temperature(const float* __restrict__ rho,
+                                     unsigned long long* __restrict__ tally, const uint32_t* __restrict__ delta,
+                                     float* __restrict__ trow, const float* __restrict__ lnQ,
+                                     const int* __restrict__ guide, int nT, long long slots, long long n3,
+                                     float ln_coef, float ln_sub3) {
+  extern __shared__ float s_lnQ[];                            // [nT] + int[kGuide]
+  int* s_guide = reinterpret_cast<int*>(s_lnQ + nT);
   for (int i = threadIdx.x; i < nT; i += blockDim.x) s_lnQ[i] = lnQ[i];
+  for (int i = threadIdx.x; i < kGuide; i += blockDim.x) s_guide[i] = guide[i];
   __syncthreads();
-  long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < slots; i += stride) {
-    unsigned long long c = tally[i];
-    float r = rho[i];
-    float t = 0.f;
-    if (c > 0 && r > 0.f) {                                   // refined-root markers have r < 0
-      float lq = logf((float)c) + ln_coef - logf(r) + (i >= n3 ? ln_sub3 : 0.f);
-      if (lq >= s_lnQ[nT - 1]) t = (float)(nT - 1);
-      else if (lq > s_lnQ[0]) {
-        int lo = 0, hi = nT - 1;                              // lnQ[lo] <= lq < lnQ[hi]
-        while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (s_lnQ[mid] <= lq) lo = mid; else hi = mid; }
-        t = (float)lo + (lq - s_lnQ[lo]) / (s_lnQ[lo + 1] - s_lnQ[lo]);
+  const float lq0 = s_lnQ[0], inv_w = (float)kGuide / (s_lnQ[nT - 1] - s_lnQ[0]);
+  const bool use_guide = lq0 > -1e29f && s_lnQ[nT - 1] > lq0;
+  auto one = [&](unsigned long long c, float r, long long i) -> float {
+    if (c == 0 || !(r > 0.f)) return 0.f;                     // refined-root markers have r < 0
+    const float lq = logf((float)c) + ln_coef - logf(r) + (i >= n3 ? ln_sub3 : 0.f);
+    return row_of_lnq(lq, s_lnQ, s_guide, nT, lq0, inv_w, use_guide);
+  };
+  const long long stride = 2ll * gridDim.x * blockDim.x;
+  for (long long i = 2ll * ((long long)blockIdx.x * blockDim.x + threadIdx.x); i < slots; i += stride) {
+    if (i + 1 < slots) {                                      // two leaves per turn: 16-byte tally, 8-byte rho / trow accesses
+      ulonglong2 c = *reinterpret_cast<const ulonglong2*>(tally + i);
+      const float2 r = *reinterpret_cast<const float2*>(rho + i);
+      if (ADD) {
+        const uint2 d = *reinterpret_cast<const uint2*>(delta + i);
+        c.x += d.x; c.y += d.y;
+        *reinterpret_cast<ulonglong2*>(tally + i) = c;
       }
+      *reinterpret_cast<float2*>(trow + i) = make_float2(one(c.x, r.x, i), one(c.y, r.y, i + 1));
+    } else {
+      unsigned long long c = tally[i];
+      if (ADD) { c += delta[i]; tally[i] = c; }
+      trow[i] = one(c, rho[i], i);
     }
-    trow[i] = t;
   }
 }
 

@@ -50,10 +50,14 @@ struct ObserverDev {
 struct TransportParams {
   const float* __restrict__ rho;               // [slots] density / refined-cube marker
   unsigned long long* __restrict__ tally;      // [slots] cumulative absorbed-package counts
+  uint32_t* __restrict__ tally32;              // NULL, or [slots] this batch's counts only (packet-sharded runs:
+                                               // the ranks all-reduce this array, not the cumulative one)
   const float* __restrict__ trow;              // [slots] temperature as table row coordinate
   const float4* __restrict__ opac;             // [nb] (kappa_ext*root_size, albedo, g, kappa_abs)
   const float* __restrict__ cdf;               // [nT][nb] emission inverse-CDF rows
-  const double* __restrict__ csrc;             // [nsrc][nb] source spectrum CDFs (fp64, searched once per package)
+  const float* __restrict__ csrc;              // [nsrc][nb] source spectrum CDFs, fp32 copy: searched in the same
+                                               // instruction stream as the re-emission rows ...
+  const double* __restrict__ csrc64;           // ... and the fp64 table that settles the bin exactly
   const SrcDev* __restrict__ src;              // [nsrc]
   unsigned long long* next;                    // work-queue head (packet offset within the batch)
   const uint32_t* __restrict__ perm;           // NULL, or the batch's package numbers grouped by source

@@ -16,13 +16,18 @@
 //    Per axis there is a forward and a reversed table, so a table cursor always moves by +1
 //    whatever the direction's sign.
 //  * Two-level grids use the SAME step: inside a refined cube the three cursors point into a tiny
-//    second table (S entries per axis and direction: +-S^a, the last entry = kLutLeave) and the
-//    pitch is 1/(S|d_a|); the root cursors and the root slot wait in three + one more registers.
-//    A step that reads kLutLeave takes the root table's delta instead and returns to the root
-//    level; a gathered density with the sign bit set is the marker of a refined cube (the density
-//    array doubles as the two-level index): the package descends into the
-//    subcube its remaining distances to the root faces select.  Root-level and sub-level lanes of
-//    a warp therefore run one instruction stream; only the two transitions diverge.
+//    second table (per axis and direction S entries +-S^a, the last one = kLutLeave) and the pitch
+//    is 1/(S|d_a|); the root cursors, the root slot and the refined-cube number wait in five more
+//    registers.  A step that reads kLutLeave takes the root table's delta, requests the new root
+//    cube's entry and keeps walking at the sub level (the subcube index on the exit axis wraps,
+//    the other two carry over: the faces of neighbouring refined cubes line up).  The density array
+//    doubles as the two-level index: if the entry that comes back has its
+//    sign bit set it is the number of a refined cube and the leaf slot just moves to that cube
+//    (integer arithmetic only); if not, the package has left the refined region and its exits move
+//    out to the faces of the root cube.  A package that meets a marker at the root level descends
+//    into the subcube its remaining distances to the root faces select.  Root-level and sub-level
+//    lanes of a warp therefore run one instruction stream; the transitions between refined cubes
+//    cost a handful of predicated instructions, only entering / leaving the refined REGION diverges.
 //  * The density of the NEXT leaf is requested before the optical-depth test of the current one
 //    (the geometric walk does not depend on rho), taking the gather latency off the dependent chain.
 //  * The walk loop runs until fewer than `quorum` lanes of the warp are still walking; then all
@@ -75,15 +80,35 @@ __host__ __device__ __forceinline__ long long ext_of_slot(const LayoutU& L, long
 
 constexpr int kLutEscape = INT_MIN;       // root table: the step leaves the grid
 constexpr int kLutLeave = INT_MIN + 1;    // sub table: the step leaves the refined root cube
-constexpr int kSubStride = 8;             // entries per (axis, direction) of the sub table (S <= 8)
+constexpr int kSubStride = 16;            // ints per (axis, direction) row of the sub table (64-byte rows, S <= 8):
+                                          // [0..S-1] slot deltas (+-S^a, the last one kLutLeave), [15] = -(S-1) * delta
+constexpr int kPending = (int)0x80000000u; // PacketU::cb: the package crossed into a new root cube at the sub level
+                                          // and the cube's entry (density or marker) is still on its way
+
+// offset (ints) of the sub table behind the root tables, such that its rows are 64-byte aligned when the
+// table block itself is (the kernel places it at a 64-byte aligned shared-memory address)
+__host__ __device__ __forceinline__ int lut_sub_offset(int N) { return (6 * N + 15) & ~15; }
 
 struct TransportParamsU {
   TransportParams base;          // rho / tally / trow are in STORAGE order here
   const int* __restrict__ lut;   // [6][N] root slot deltas: (axis, forward) at (2*axis)*N, reversed at
-                                 // (2*axis+1)*N; two-level grids: followed by [6][kSubStride] sub-cell deltas
+                                 // (2*axis+1)*N; two-level grids: [6][kSubStride] sub-cell rows from lut_sub_offset(N)
   LayoutU lay;
-  int quorum;                    // leave the walk loop when fewer lanes than this are walking
+  int quorum;                    // leave the walk loop when fewer lanes than this are walking; 0 = automatic
 };
+
+// Automatic walk quorum.  A warp that walks until w lanes are left and then spends E instructions on
+// one event pass does about L (32 - w) crossings in c L ln(32/w) + E instructions (L = mean crossings
+// per flight, c = instructions per step), so the best w grows with L.  Measured optima (profiles/):
+// 12-16 at L = 38 (c1), ~19 at L = 160 (c2), 20-24 at L = 320 (c3): w = 14 + 2 log2(L / 24), 8..24.
+// L is taken from the job's own cumulative counters (crossings / flights so far; the first batch
+// starts at 16).  A scheduling knob only: results do not depend on it.
+__device__ __forceinline__ int auto_quorum(const unsigned long long* __restrict__ counters) {
+  const float cr = (float)counters[CNT_CROSS], fl = (float)counters[CNT_FLIGHTS];
+  if (fl < 1024.f) return 16;
+  const int q = 14 + (int)rintf(2.f * log2f(fmaxf(cr / fl, 1.f) * (1.f / 24.f)));
+  return min(24, max(8, q));
+}
 
 // SU_INTERACT_B: interaction found in the second step of a pair -> the cell's density is in the
 // alternate register (moved back in the event pass, never inside the walk loop where the move
@@ -104,6 +129,7 @@ struct PacketU {
   // two-level grids only (dead registers otherwise): state of a package inside a refined cube
   uint32_t r0, r1, r2;       // the root-level cursors while p0..p2 walk the sub table
   int rslot;                 // storage slot of the refined root cube
+  int kref;                  // its refined-cube number
   float hs;                  // leaf edge in root-cube edges: 1, or 1/S inside a refined cube
 };
 
@@ -166,9 +192,9 @@ __device__ __forceinline__ void begin_flight_sub(PacketU& p, uint32_t lut, uint3
   p.p2 = sub_cursor(sublut, 2, p.d2, p.d2 > 0.f ? sz : S - 1 - sz);
   p.hs = hs;
 }
-// directional subcube index on one axis from a sub-table cursor
-__device__ __forceinline__ int sub_j(uint32_t cursor, uint32_t sublut) {
-  return (int)(((cursor - sublut) >> 2) & (uint32_t)(kSubStride - 1));
+// directional subcube index on one axis from a sub-table cursor (rows are 64-byte aligned)
+__device__ __forceinline__ int sub_j(uint32_t cursor) {
+  return (int)((cursor >> 2) & (uint32_t)(kSubStride - 1));
 }
 
 // A package at the root level whose gathered "density" is the marker of a refined cube (sign bit
@@ -195,9 +221,48 @@ __device__ __forceinline__ void descend(const TransportParams& P, PacketU& p, ui
   p.p2 = sub_cursor(sublut, 2, p.d2, j2);
   const int sx = p.d0 > 0.f ? j0 : m0, sy = p.d1 > 0.f ? j1 : m1, sz = p.d2 > 0.f ? j2 : m2;
   p.slot = P.n3 + kref * (S * S * S) + sx + S * (sy + S * sz);
+  p.kref = kref;
   p.hs = hs;
   MCRT_CHECK_SLOT(p.slot);
   cur = __ldg(P.rho + p.slot);
+}
+
+// A package at the sub level whose exits must move out to the faces of its root cube (it has left
+// the refined region, or the grid): per axis (S - 1 - j) more subcube edges; cursors back to the
+// root tables.  The exit axis of a kLutLeave step has j = 0 by then, so one rule serves all three.
+__device__ __forceinline__ void to_root_level(const TransportParams& P, PacketU& p) {
+  const int S = P.S;
+  const float h = p.hs;
+  p.t0 = fmaf((float)(S - 1 - sub_j(p.p0)) * h, p.dt0, p.t0);
+  p.t1 = fmaf((float)(S - 1 - sub_j(p.p1)) * h, p.dt1, p.t1);
+  p.t2 = fmaf((float)(S - 1 - sub_j(p.p2)) * h, p.dt2, p.t2);
+  p.p0 = p.r0; p.p1 = p.r1; p.p2 = p.r2;
+  p.slot = p.rslot;
+  p.hs = 1.f;
+}
+
+// Start of a step on a two-level grid when the gathered entry is a refined-cube marker or the
+// package is waiting for the entry of the root cube it crossed into (kPending):
+//  * pending + marker: refined -> refined, the leaf slot moves to the same subcube of the new cube
+//    (the wrap of the exit axis was applied when the step was taken), then its density is gathered;
+//  * pending, no marker: the package has left the refined region -> root level, `cur` is its density;
+//  * marker, not pending: a package at the root level meets a refined cube -> descend().
+__device__ __forceinline__ void root_entry(const TransportParams& P, PacketU& p, uint32_t sublut, float& cur) {
+  const int bits = __float_as_int(cur);
+  if (p.cb < 0) {
+    p.cb &= ~kPending;
+    if (bits < 0) {
+      const int kref = bits & 0x7fffffff;
+      p.slot += (kref - p.kref) * (P.S * P.S * P.S);
+      p.kref = kref;
+      MCRT_CHECK_SLOT(p.slot);
+      cur = __ldg(P.rho + p.slot);
+    } else {
+      to_root_level(P, p);
+    }
+  } else {
+    descend(P, p, sublut, cur);
+  }
 }
 
 // One crossing of the cell walk (O5).  `cur` holds the density of the current leaf; the density
@@ -209,12 +274,13 @@ template <bool TL>
 __device__ __forceinline__ void walk_step_u(const TransportParams& P, PacketU& p, float& cur, float& nxt,
                                             float kx, uint32_t sublut, int& state, uint32_t& crossings) {
   if (TL) {
-    if (__float_as_int(cur) < 0) descend(P, p, sublut, cur);
+    if ((p.cb | __float_as_int(cur)) < 0) root_entry(P, p, sublut, cur);
   }
   const float tnext = fminf(p.t0, fminf(p.t1, p.t2));
   const bool a0 = p.t0 == tnext;                             // ties -> lowest axis (R21)
   const bool a1 = !a0 && p.t1 == tnext;
-  int dl = lds_s32(a0 ? p.p0 : (a1 ? p.p1 : p.p2));
+  const uint32_t csel = a0 ? p.p0 : (a1 ? p.p1 : p.p2);
+  int dl = lds_s32(csel);
   int from = p.slot;
   bool leave = false;
   if (TL) {
@@ -233,25 +299,33 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, PacketU& p
   } else {
     p.tau_rem -= dtau;
     p.tcur = tnext;
+    ++crossings;
     if (TL) {
-      if (leave) {                                           // back to the root level: the other two axes'
-        const int S = P.S;                                   // exits move out to the faces of the root cube
-        const float h = p.hs;
-        if (!a0) p.t0 += (float)(S - 1 - sub_j(p.p0, sublut)) * h * p.dt0;
-        if (a0 || !a1) p.t1 += (float)(S - 1 - sub_j(p.p1, sublut)) * h * p.dt1;
-        if (a0 || a1) p.t2 += (float)(S - 1 - sub_j(p.p2, sublut)) * h * p.dt2;
-        p.p0 = p.r0; p.p1 = p.r1; p.p2 = p.r2;
-        p.hs = 1.f;
+      uint32_t cnew = csel + 4u;
+      if (leave) {
+        // Keep walking at the sub level: the subcube index of the exit axis wraps (cursor back to the
+        // row's start, leaf slot to the mirror subcube), the root cursor of that axis advances, and
+        // the entry of the new root cube (density or marker) arrives with the next step (kPending).
+        cnew = csel & ~63u;
+        p.slot += lds_s32(cnew + 4u * (uint32_t)(kSubStride - 1));
+        p.rslot = nslot;
+        if (a0) p.r0 += 4u; else if (a1) p.r1 += 4u; else p.r2 += 4u;
+        p.cb |= kPending;
+      } else {
+        p.slot = nslot;
       }
-      if (a0) { p.t0 = fmaf(p.dt0, p.hs, p.t0); p.p0 += 4u; }
-      else if (a1) { p.t1 = fmaf(p.dt1, p.hs, p.t1); p.p1 += 4u; }
-      else { p.t2 = fmaf(p.dt2, p.hs, p.t2); p.p2 += 4u; }
+      if (a0) { p.t0 = fmaf(p.dt0, p.hs, p.t0); p.p0 = cnew; }
+      else if (a1) { p.t1 = fmaf(p.dt1, p.hs, p.t1); p.p1 = cnew; }
+      else { p.t2 = fmaf(p.dt2, p.hs, p.t2); p.p2 = cnew; }
+      if (esc) {
+        if (leave) { p.cb &= ~kPending; to_root_level(P, p); }   // left the grid from a subcube (rare)
+        state = SU_ESCAPE;
+      }
     } else {
       if (a0) { p.t0 += p.dt0; p.p0 += 4u; } else if (a1) { p.t1 += p.dt1; p.p1 += 4u; } else { p.t2 += p.dt2; p.p2 += 4u; }
+      p.slot = nslot;
+      if (esc) state = SU_ESCAPE;
     }
-    ++crossings;
-    p.slot = nslot;
-    if (esc) state = SU_ESCAPE;
   }
 }
 
@@ -300,15 +374,16 @@ __device__ __forceinline__ void emit_position_u(const TransportParams& P, const 
 template <int MINBLOCKS, bool TL>
 __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportParamsU PU) {
   const TransportParams& P = PU.base;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   float4* s_opac = reinterpret_cast<float4*>(smem_raw);                    // [nb]
   uint32_t* s_sed = reinterpret_cast<uint32_t*>(s_opac + P.nb);             // [3*nb]
   uint32_t* s_emit = s_sed + 3 * P.nb;                                      // [nb]
-  int* s_lut = reinterpret_cast<int*>(s_emit + P.nb);                       // [6*N] (+ [6*kSubStride])
+  // root delta tables [6*N] (+ the 64-byte aligned sub-table rows), at a 64-byte aligned address
+  int* s_lut = reinterpret_cast<int*>(smem_raw + ((32u * (unsigned)P.nb + 63u) & ~63u));
   const uint32_t lut = (uint32_t)__cvta_generic_to_shared(s_lut);
   const int N = P.N;
-  const uint32_t sublut = lut + 4u * (uint32_t)(6 * N);
-  const int n_lut = 6 * N + (TL ? 6 * kSubStride : 0);
+  const uint32_t sublut = lut + 4u * (uint32_t)lut_sub_offset(N);
+  const int n_lut = TL ? lut_sub_offset(N) + 6 * kSubStride : 6 * N;
   for (int i = threadIdx.x; i < P.nb; i += blockDim.x) { s_opac[i] = P.opac[i]; s_emit[i] = 0; }
   for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x) s_sed[i] = 0;
   for (int i = threadIdx.x; i < n_lut; i += blockDim.x) s_lut[i] = PU.lut[i];
@@ -324,12 +399,12 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   PacketU p;
   p.d0 = p.d1 = p.d2 = 1.f; p.t0 = p.t1 = p.t2 = 0.f; p.dt0 = p.dt1 = p.dt2 = 1.f;
   p.tcur = 0.f; p.tau_rem = 1.f; p.rho = 0.f; p.p0 = p.p1 = p.p2 = lut; p.slot = 0;
-  p.r0 = p.r1 = p.r2 = lut; p.rslot = 0; p.hs = 1.f;
+  p.r0 = p.r1 = p.r2 = lut; p.rslot = 0; p.kref = 0; p.hs = 1.f;
   float rho_b = 0.f;                                         // the walk alternates p.rho / rho_b
   p.cb = 0; p.k = 0; p.off = 0; p.u1 = p.u2 = p.u3 = 0.f;
   float kx = 0.f;
   int state = SU_FETCH;
-  int quorum = PU.quorum;
+  int quorum = PU.quorum > 0 ? PU.quorum : auto_quorum(P.counters);
 
   for (;;) {
     // ---- a7: escaped packages -> SED; a8: refill from the work queue (one atomic per warp) ----
@@ -385,7 +460,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         uz = p.d2 > 0.f ? 1.f - w2 : w2;
         if (in_sub) {
           cell_of(p, p.r0, p.r1, p.r2, lut, N, ix, iy, iz);
-          const int S = P.S, j0 = sub_j(p.p0, sublut), j1 = sub_j(p.p1, sublut), j2 = sub_j(p.p2, sublut);
+          const int S = P.S, j0 = sub_j(p.p0), j1 = sub_j(p.p1), j2 = sub_j(p.p2);
           sx = p.d0 > 0.f ? j0 : S - 1 - j0;
           sy = p.d1 > 0.f ? j1 : S - 1 - j1;
           sz = p.d2 > 0.f ? j2 : S - 1 - j2;
@@ -404,23 +479,38 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         uint32_t xw[4];
         draw4w(P.seed, pid, is_new ? 0u : p.k, is_new ? kTagEmit : kTagReemit, xw);
         const float r2 = u01(xw[2]), r3 = u01(xw[3]);
+        const float* row;
+        float us;
         int s = 0;
-        if (is_new) {                                        // O4: source by luminosity, bin by its spectrum (fp64)
+        if (is_new) {                                        // O4: source by luminosity (fp64, exact)
           const double u0 = u01d(xw[0]);
           while (s < P.nsrc - 1 && P.src[s].lcdf < u0) ++s;
-          bin = search_cdf<double>(P.csrc + (size_t)s * P.nb, P.nb, u01d(xw[1]));
+          row = P.csrc + (size_t)s * P.nb;
+          us = (float)u01d(xw[1]);
         } else {
           ++n_abs;
           // warp-aggregated integer tally: one atomic per distinct cell per warp
           MCRT_CHECK_SLOT(p.slot);
           unsigned peers = __match_any_sync(__activemask(), p.slot);
-          if ((int)lane == __ffs(peers) - 1)
-            atomicAdd(P.tally + p.slot, (unsigned long long)__popc(peers));
+          if ((int)lane == __ffs(peers) - 1) {
+            if (P.tally32) atomicAdd(P.tally32 + p.slot, (uint32_t)__popc(peers));
+            else atomicAdd(P.tally + p.slot, (unsigned long long)__popc(peers));
+          }
           float tr = __ldg(P.trow + p.slot);                 // T frozen = T before absorption
           int k0 = min(P.nT - 1, (int)tr);
           float w = tr - (float)k0;
           int rw = (u01(xw[1]) < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
-          bin = search_cdf<float>(P.cdf + (size_t)rw * P.nb, P.nb, u01(xw[0]));
+          row = P.cdf + (size_t)rw * P.nb;
+          us = u01(xw[0]);
+        }
+        bin = search_cdf<float>(row, P.nb, us);              // one search loop for emission and re-emission
+        if (is_new) {
+          // the emission bin is settled in fp64 against the fp64 table with the oracle's uniform: the fp32
+          // search lands within a bin or two of "first j with C[j] >= u", a short walk ends exactly on it
+          const double* c64 = P.csrc64 + (size_t)s * P.nb;
+          const double ud = u01d(xw[1]);
+          while (bin > 0 && __ldg(c64 + bin - 1) >= ud) --bin;
+          while (bin < P.nb - 1 && __ldg(c64 + bin) < ud) ++bin;
         }
         kx = s_opac[bin].x;
         isotropic_dir(r2, r3, a, b, c);
@@ -439,7 +529,8 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
             if (__float_as_int(p.rho) < 0) {                 // the source sits in a refined cube
               const int S = P.S;
               p.rslot = p.slot;
-              p.slot = P.n3 + (__float_as_int(p.rho) & 0x7fffffff) * (S * S * S) + sx + S * (sy + S * sz);
+              p.kref = __float_as_int(p.rho) & 0x7fffffff;
+              p.slot = P.n3 + p.kref * (S * S * S) + sx + S * (sy + S * sz);
               MCRT_CHECK_SLOT(p.slot);
               p.rho = __ldg(P.rho + p.slot);
               in_sub = true;

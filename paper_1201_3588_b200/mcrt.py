@@ -48,10 +48,18 @@ class _Counters(C.Structure):
                                           "scatterings", "flights", "crossings")]
 
 
+class _Results(C.Structure):
+    _fields_ = [("n_abs", C.c_void_p), ("T", C.c_void_p), ("sed", C.c_void_p),
+                ("emitted_per_bin", C.c_void_p), ("counters", C.POINTER(_Counters)),
+                ("eps", C.POINTER(C.c_double))]
+
+
 # every symbol include/mcrt.h declares
 SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opacity",
            "mcrt_set_source", "mcrt_run_batch", "mcrt_transport_batch",
-           "mcrt_update_temperature", "mcrt_get_cell_energy",
+           "mcrt_update_temperature", "mcrt_store_slots", "mcrt_transport_batch_delta",
+           "mcrt_accumulate_update", "mcrt_get_results", "mcrt_results_begin", "mcrt_results_wait",
+           "mcrt_get_cell_energy",
            "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_observer",
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
@@ -78,6 +86,13 @@ def lib():
         L.mcrt_run_batch.argtypes = [vp, u64, u64, u64, vp]
         L.mcrt_transport_batch.argtypes = [vp, u64, u64, u64, vp]
         L.mcrt_update_temperature.argtypes = [vp, vp, u64, vp]
+        L.mcrt_store_slots.restype = i64
+        L.mcrt_store_slots.argtypes = [vp]
+        L.mcrt_transport_batch_delta.argtypes = [vp, u64, u64, u64, vp, vp]
+        L.mcrt_accumulate_update.argtypes = [vp, vp, u64, vp]
+        L.mcrt_get_results.argtypes = [vp, C.POINTER(_Results), C.c_int]
+        L.mcrt_results_begin.argtypes = [vp, C.POINTER(_Results), C.c_int, C.POINTER(i32)]
+        L.mcrt_results_wait.argtypes = [vp, i32]
         L.mcrt_get_cell_energy.argtypes = [vp, vp, C.POINTER(C.c_double), C.c_int]
         L.mcrt_get_cell_temperature.argtypes = [vp, vp, C.c_int]
         L.mcrt_get_sed.argtypes = [vp, vp, C.c_int]
@@ -103,7 +118,8 @@ def lib():
         L.mcrt_last_error.argtypes = [vp]
         for name in ("mcrt_grid_create", "mcrt_destroy", "mcrt_set_opacity", "mcrt_set_source",
                      "mcrt_run_batch", "mcrt_transport_batch", "mcrt_update_temperature",
-                     "mcrt_get_cell_energy", "mcrt_get_cell_temperature",
+                     "mcrt_transport_batch_delta", "mcrt_accumulate_update", "mcrt_get_results",
+                     "mcrt_results_begin", "mcrt_results_wait", "mcrt_get_cell_energy", "mcrt_get_cell_temperature",
                      "mcrt_get_sed", "mcrt_set_observer", "mcrt_get_sed_mu", "mcrt_get_image",
                      "mcrt_get_counters", "mcrt_reset_tallies",
                      "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
@@ -228,7 +244,62 @@ class Context:
         self._check(lib().mcrt_update_temperature(self.h, p, int(n_cum), C.c_void_p(stream)),
                     "mcrt_update_temperature")
 
+    def transport_batch_delta(self, seed, first_packet_id, n_packets, stream=None):
+        """This rank's share of a batch, tallied into a per-batch uint32 array in the library's
+        storage order (a torch int32 CUDA tensor owned by this object, reused every batch): the
+        array the ranks of a packet-sharded run all-reduce."""
+        import torch
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        if getattr(self, "_delta", None) is None:
+            self._delta = torch.empty(int(lib().mcrt_store_slots(self.h)), dtype=torch.int32, device="cuda")
+        self._check(lib().mcrt_transport_batch_delta(self.h, int(seed), int(first_packet_id), int(n_packets),
+                                                     C.c_void_p(self._delta.data_ptr()), C.c_void_p(stream)),
+                    "mcrt_transport_batch_delta")
+        return self._delta
+
+    def accumulate_update(self, delta_sum, n_cum, stream=None):
+        """Adds the batch's counts summed over ranks to the cumulative tally and updates T."""
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(lib().mcrt_accumulate_update(self.h, C.c_void_p(delta_sum.data_ptr()), int(n_cum),
+                                                 C.c_void_p(stream)), "mcrt_accumulate_update")
+
     # -- results --------------------------------------------------------------------------
+    def _results_struct(self, bufs):
+        """bufs: dict with any of n_abs / T / sed / emitted_per_bin -> numpy arrays (host, ideally
+        views of pinned memory) or torch CUDA tensors; returns (struct, keep-alive, mem)."""
+        r = _Results()
+        dev = any(_is_tensor(v) for v in bufs.values())
+        for k in ("n_abs", "T", "sed", "emitted_per_bin"):
+            v = bufs.get(k)
+            if v is not None:
+                setattr(r, k, v.data_ptr() if _is_tensor(v) else v.ctypes.data)
+        c, eps = _Counters(), C.c_double(0)
+        r.counters, r.eps = C.pointer(c), C.pointer(eps)
+        return r, (c, eps, bufs), MCRT_DEVICE if dev else MCRT_HOST
+
+    def results_begin(self, bufs):
+        """Queue the read-out of a finished batch into `bufs` (see _results_struct); the next
+        run_batch may be issued at once.  Returns a handle for results_wait."""
+        r, keep, mem = self._results_struct(bufs)
+        t = C.c_int32(-1)
+        self._check(lib().mcrt_results_begin(self.h, C.byref(r), mem, C.byref(t)), "mcrt_results_begin")
+        return (t.value, r, keep)
+
+    def results_wait(self, handle):
+        t, r, (c, eps, bufs) = handle
+        self._check(lib().mcrt_results_wait(self.h, t), "mcrt_results_wait")
+        out = dict(bufs)
+        out["counters"] = {n: int(getattr(c, n)) for n, _ in _Counters._fields_}
+        out["eps"] = eps.value
+        return out
+
+    def get_results(self, bufs):
+        """Everything in one call and one synchronisation."""
+        return self.results_wait(self.results_begin(bufs))
+
     def _out(self, shape, np_dtype, device, out=None):
         """Output buffer: a torch CUDA tensor (device=True), the caller's `out` (a C-contiguous
         numpy array of the right shape and dtype -- e.g. a view of pinned memory, reused from

@@ -2,13 +2,15 @@
 
 Within a batch packets are independent (temperatures frozen, per-packet Philox streams), so a
 batch [first, first+n) is dealt to the ranks in contiguous ranges; every rank transports its
-own range (`transport_batch`), the ranks sum their cumulative integer tallies with ONE
-all-reduce, and every rank runs the same temperature update on the sum with the global
-package count (`update_temperature`).  Integer sums commute, so tallies and temperatures are
-bit-identical to a single-rank run over the same packet ids.
+own range, tallying the batch's absorptions into a per-batch uint32 array
+(`transport_batch_delta`), the ranks sum those arrays with ONE all-reduce (4 bytes per storage
+slot, in the library's storage order: no layout conversion, no allocation), and every rank adds
+the sum to its cumulative tally and updates the temperatures with the global package count
+(`accumulate_update`).  Integer sums commute, so tallies and temperatures are bit-identical
+to a single-rank run over the same packet ids, and every rank ends up with the global tally.
 
-The engine is anything with the binding's three calls (mcrt.Context on a GPU); torch is used
-for the collective only.
+The engine is anything with the binding's calls (mcrt.Context on a GPU); torch is used for the
+collective only.
 """
 from __future__ import annotations
 
@@ -39,10 +41,9 @@ class ShardedRunner:
         if self.world == 1:
             self.engine.run_batch(seed, f, c, stream)
             return f, c
-        self.engine.transport_batch(seed, f, c, stream)
-        tally, _ = self.engine.get_cell_energy(device=True)     # this rank's cumulative counts
-        self.dist.all_reduce(tally, op=self.dist.ReduceOp.SUM, group=self.group)
-        self.engine.update_temperature(tally, self.n_cum, stream)
+        delta = self.engine.transport_batch_delta(seed, f, c, stream)   # this rank's counts of this batch
+        self.dist.all_reduce(delta, op=self.dist.ReduceOp.SUM, group=self.group)
+        self.engine.accumulate_update(delta, self.n_cum, stream)
         return f, c
 
     def reduce_counts(self, t):

@@ -527,3 +527,97 @@ def test_two_level_bricked_root_bit_identical_to_x_fastest(M, maker):
         done += cnt
         c.update_temperature(tally, done)
     _assert_identical(a, c)
+
+
+# ---- packet-sharded batches on the real kernels, and the combined read-out ------
+@pytest.mark.parametrize("maker,layout", [
+    (lambda: W.tiny_random(n_root=13, seed=6, tau_cell=0.3, n_packets=40_000, batch=10_000), 1),
+    (lambda: W.tiny_random(n_root=13, seed=6, tau_cell=0.3, n_packets=40_000, batch=10_000), 2),
+    (lambda: W.c3(n_root=32, n_packets=60_000, batch=20_000), 0),
+    (lambda: W.c3(n_root=32, n_packets=60_000, batch=20_000), 2)])
+def test_two_emulated_ranks_equal_one(M, maker, layout):
+    """Two contexts play two ranks on one GPU: each transports its contiguous half of every batch
+    into its own per-batch uint32 delta array (storage order), the arrays are summed (what the
+    NCCL all-reduce does), and both add the sum and update T with the global package count.
+    Tallies and temperatures of BOTH equal the single-context run bit for bit; SEDs and counters
+    add up to it."""
+    from paper_1201_3588_b200.sharding import rank_range
+    wl = maker()
+    one = _run_layout(M, wl, layout)
+    ranks = [M.from_workload(wl, layout=layout) for _ in range(2)]
+    done = 0
+    for first, cnt in wl.batches():
+        deltas = []
+        for r, ctx in enumerate(ranks):
+            f, c = rank_range(first, cnt, 2, r)
+            deltas.append(ctx.transport_batch_delta(wl.seed, f, c))
+        total = deltas[0] + deltas[1]
+        done += cnt
+        for ctx in ranks:
+            ctx.accumulate_update(total, done)
+    for ctx in ranks:
+        assert np.array_equal(ctx.get_cell_energy()[0], one.get_cell_energy()[0])
+        assert np.array_equal(ctx.get_cell_temperature(), one.get_cell_temperature())
+        assert ctx.get_cell_energy()[1] == one.get_cell_energy()[1]       # eps = L / packages of ALL ranks
+    assert np.array_equal(ranks[0].get_sed() + ranks[1].get_sed(), one.get_sed())
+    ca, cb, c1 = ranks[0].get_counters(), ranks[1].get_counters(), one.get_counters()
+    for k in c1:
+        assert np.array_equal(ca[k] + cb[k], c1[k]), k
+
+
+@pytest.mark.parametrize("maker", [W.c0, lambda: W.c2(n_root=20, n_packets=60_000, batch=20_000),
+                                   lambda: W.c4(n_root=24, n_packets=60_000, batch=20_000, corr_cells=3.0)])
+def test_combined_and_overlapped_read_out(M, maker):
+    """mcrt_get_results = the four getters in one call; mcrt_results_begin / _wait deliver the state
+    of the batch they were queued behind even though the next batch is already running."""
+    import torch
+    wl = maker()
+    batches = list(wl.batches())
+    ref = M.from_workload(wl, layout=2 if wl.n_root == 24 else 0)
+    ctx = M.from_workload(wl, layout=2 if wl.n_root == 24 else 0)
+    pin = lambda shape, dt: torch.empty(shape, dtype=dt).pin_memory().numpy()
+    mk = lambda: dict(n_abs=pin((ctx.slots,), torch.int64).view(np.uint64), T=pin((ctx.slots,), torch.float32),
+                      sed=pin((3, wl.n_bins), torch.int64).view(np.uint64),
+                      emitted_per_bin=pin((wl.n_bins,), torch.int64).view(np.uint64))
+    bufs = [mk(), mk()]
+    handles, snaps = [], []
+    for i, (first, cnt) in enumerate(batches):
+        ref.run_batch(wl.seed, first, cnt)
+        snaps.append((ref.get_cell_energy()[0].copy(), ref.get_cell_temperature().copy(), ref.get_sed().copy(),
+                      ref.get_counters()))
+        ctx.run_batch(wl.seed, first, cnt)
+        handles.append(ctx.results_begin(bufs[i % 2]))          # the next batch is issued before this is read
+        if i > 0:
+            out = ctx.results_wait(handles[i - 1])
+            n_abs, T, sed, c = snaps[i - 1]
+            assert np.array_equal(out["n_abs"], n_abs) and np.array_equal(out["T"], T)
+            assert np.array_equal(out["sed"], sed)
+            assert np.array_equal(out["emitted_per_bin"], c["emitted_per_bin"])
+            assert all(out["counters"][k] == c[k] for k in out["counters"])
+    out = ctx.results_wait(handles[-1])
+    assert np.array_equal(out["n_abs"], snaps[-1][0]) and out["eps"] == ref.get_cell_energy()[1]
+    # one call, device buffers
+    dev = dict(n_abs=torch.empty(ctx.slots, dtype=torch.int64, device="cuda"),
+               T=torch.empty(ctx.slots, dtype=torch.float32, device="cuda"),
+               sed=torch.empty((3, wl.n_bins), dtype=torch.int64, device="cuda"))
+    out = ctx.get_results(dev)
+    assert np.array_equal(dev["n_abs"].cpu().numpy().astype(np.uint64), snaps[-1][0])
+    assert np.array_equal(dev["T"].cpu().numpy(), snaps[-1][1])
+    assert np.array_equal(dev["sed"].cpu().numpy().astype(np.uint64), snaps[-1][2])
+    assert out["counters"]["emitted"] == wl.n_packets
+    with pytest.raises(M.McrtError):                           # a third ticket while two are in flight
+        h1, h2 = ctx.results_begin(bufs[0]), ctx.results_begin(bufs[1])
+        ctx.results_begin(bufs[0])
+    ctx.results_wait(h1), ctx.results_wait(h2)
+
+
+def test_automatic_walk_quorum_does_not_change_results(M):
+    """quorum 0 = chosen by the kernel from the job's crossings per flight."""
+    wl = W.c2(n_root=32, n_packets=3 << 17, batch=1 << 17)
+    a = M.from_workload(wl)
+    a.set_walk_quorum(16)
+    b = M.from_workload(wl)                                     # automatic
+    for first, cnt in wl.batches():
+        a.run_batch(wl.seed, first, cnt)
+        b.run_batch(wl.seed, first, cnt)
+    _assert_identical(a, b)

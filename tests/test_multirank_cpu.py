@@ -24,25 +24,34 @@ BATCHES = [(0, 5001), (5001, 4000), (9001, 2999)]       # odd sizes: ragged spli
 
 
 class OracleEngine:
-    """Adapter with the binding's call names (run_batch / transport_batch / get_cell_energy /
-    update_temperature)."""
+    """Adapter with the binding's call names (run_batch / transport_batch_delta /
+    accumulate_update / get_cell_energy).  Like the library after a sharded batch, it keeps the
+    GLOBAL cumulative tally (`glob`): the oracle's own tally holds this rank's packets only."""
 
     def __init__(self, wl):
         from oracle import oracle as O
         self.o = O.Oracle(wl)
+        self.glob = np.zeros(self.o.slots, dtype=np.uint64)
+        self.sharded = False
 
     def run_batch(self, seed, first, n, stream=None):
         self.o.run_batch(seed, first, n, 1)
 
-    def transport_batch(self, seed, first, n, stream=None):
+    def transport_batch_delta(self, seed, first, n, stream=None):
+        before = self.o.cell_energy()[0]
         self.o.transport_batch(seed, first, n, 1)
+        delta = self.o.cell_energy()[0] - before
+        assert delta.max(initial=0) < 2 ** 31
+        return torch.from_numpy(delta.astype(np.int32))
+
+    def accumulate_update(self, delta_sum, n_cum, stream=None):
+        self.sharded = True
+        self.glob += delta_sum.numpy().astype(np.uint64)
+        self.o.update_temperature(self.glob, n_cum)
 
     def get_cell_energy(self, device=False):
         n, eps = self.o.cell_energy()
-        return torch.from_numpy(n.astype(np.int64)), eps
-
-    def update_temperature(self, tally, n_cum, stream=None):
-        self.o.update_temperature(tally.numpy().astype(np.uint64), n_cum)
+        return torch.from_numpy((self.glob if self.sharded else n).astype(np.int64)), eps
 
 
 def _free_port():
@@ -64,8 +73,7 @@ def _worker(rank, world, port, out_dir):
         mine = []
         for first, n in BATCHES:
             mine.append(run.run_batch(wl.seed, first, n))
-        tally, _ = eng.get_cell_energy()
-        run.reduce_counts(tally)
+        tally, _ = eng.get_cell_energy()                 # already the global tally on every rank
         sed = run.reduce_counts(torch.from_numpy(eng.o.sed().astype(np.int64)))
         c = eng.o.counters()
         cnt = run.reduce_counts(torch.tensor([c[k] for k in ("emitted", "escaped", "lost",
