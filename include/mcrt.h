@@ -253,6 +253,16 @@ mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t bl
  * (long free flights -> keep more lanes walking).  A scheduling knob only: results do not depend
  * on it. */
 mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum);
+/* Density kept in shared memory (single-level grids): a density array of at most 40 KB is copied
+ * into every block's shared memory by one bulk copy (cp.async.bulk) and a crossing reads shared
+ * memory instead of the L2 (C0: -10 % per launch).  mode 0 = automatic (the default), 1 = off
+ * (always gather from global memory), 2 = automatic, and additionally a larger grid that holds
+ * only two distinct densities (a uniform sphere in vacuum) is staged as ONE BIT per cell if the
+ * bits fit in 40 KB -- kept for measurement: on the 64^3 sphere it is 3 % slower than global
+ * gathers (profiles/r02_summary.md).  Results do not depend on it.  mcrt_density_staging returns
+ * what the next batch will use: 0 none, 1 the fp32 array, 2 one bit per cell (-1: NULL). */
+mcrt_status mcrt_set_density_staging(mcrt_ctx* ctx, int32_t mode);
+int32_t mcrt_density_staging(const mcrt_ctx* ctx);
 /* Hand the packages of a batch to the lanes grouped by where they start (a pre-pass evaluates the
  * first decisions of every package's emission and groups the package numbers), so that the
  * packages in flight share a neighbourhood and the L2 serves more of their gathers.  mode 1 =

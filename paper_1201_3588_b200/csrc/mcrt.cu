@@ -63,6 +63,11 @@ struct mcrt_ctx {
   int order_by_source = -1;               // -1 automatic, 0 off, 1 by source, 2 by source and start direction
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 0;                         // 0 = automatic (from the job's crossings per flight so far)
+  // density staged in shared memory (single-level grids): 0 none, 1 the fp32 array itself, 2 one bit per slot
+  int dens_mode = 0, dens_off = 0;        // dens_off: the caller switched staging off (mcrt_set_density_staging)
+  uint32_t* d_bits = nullptr;
+  unsigned stage_bytes = 0;
+  float pal0 = 0.f, pal1 = 0.f;
   int threads = 256, blocks_per_sm = 0;   // 0 = automatic (5; 4 on HBM-resident single-level grids)
   long long launches = 0;
   // observer (O9 / R34): escape-direction tallies, off by default
@@ -114,9 +119,18 @@ static void free_sources(mcrt_ctx* c) {
 
 // dynamic shared memory of the transport kernel: opacity float4[nb], SED u32[3 nb], emitted u32[nb], then at
 // a 64-byte boundary the root delta tables int[6 N] (+ the subcube rows int[6][16] on two-level grids)
+// what the next launch uses: the one-bit form only on request (it measured 3 % SLOWER than global gathers on
+// the 64^3 sphere: the walk is bound by instruction issue, not by the gathers; profiles/r02_summary.md)
+static int staging_mode(const mcrt_ctx* ctx) {
+  if (ctx->dens_off == 1) return 0;
+  if (ctx->dens_mode == 2 && ctx->dens_off != 2) return 0;
+  return ctx->dens_mode;
+}
 static size_t transport_smem_bytes(const mcrt_ctx* ctx) {
   const size_t n_lut = ctx->uni ? 6 * (size_t)ctx->N : (size_t)lut_sub_offset(ctx->N) + 6 * kSubStride;
-  return ((32 * (size_t)ctx->nb + 63) & ~(size_t)63) + sizeof(int) * n_lut;
+  size_t b = ((32 * (size_t)ctx->nb + 63) & ~(size_t)63) + sizeof(int) * n_lut;
+  if (staging_mode(ctx)) b = ((b + 127) & ~(size_t)127) + ctx->stage_bytes + 16;   // staged density + its mbarrier
+  return b;
 }
 constexpr size_t kMaxSmemPerBlock = 227u << 10;              // B200: opt-in limit of dynamic shared memory
 
@@ -249,6 +263,45 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
   }
   CUG(cudaGetLastError());
   CUG(cudaDeviceSynchronize());
+  // Small single-level problems keep their density in shared memory (transport_u.cuh, DENS): the array itself
+  // if it is at most 40 KB, or one bit per slot if it holds only two distinct values and the bits fit.
+  if (ctx->uni) {
+    const size_t kStageMax = 40u << 10;
+    if ((size_t)ctx->store_slots * 4 <= kStageMax) {
+      ctx->dens_mode = 1;
+      ctx->stage_bytes = (unsigned)(((size_t)ctx->store_slots * 4 + 15) & ~(size_t)15);
+      if (ctx->stage_bytes > (size_t)ctx->store_slots * 4) {   // the bulk copy reads whole 16-byte units
+        float* padded = nullptr;
+        CUG(cudaMalloc(&padded, ctx->stage_bytes));
+        CUG(cudaMemset(padded, 0, ctx->stage_bytes));
+        CUG(cudaMemcpy(padded, ctx->d_rho, (size_t)ctx->store_slots * 4, cudaMemcpyDeviceToDevice));
+        cudaFree(ctx->d_rho);
+        ctx->d_rho = padded;
+      }
+    } else if ((size_t)(ctx->store_slots + 7) / 8 <= kStageMax) {
+      std::vector<float> h((size_t)ctx->store_slots);
+      CUG(cudaMemcpy(h.data(), ctx->d_rho, 4 * h.size(), cudaMemcpyDeviceToHost));
+      float v0 = h[0], v1 = h[0];
+      bool two = true, have1 = false;
+      for (float v : h) {
+        if (v == v0 || (have1 && v == v1)) continue;
+        if (!have1) { v1 = v; have1 = true; continue; }
+        two = false;
+        break;
+      }
+      if (two) {
+        const size_t words = (((size_t)ctx->store_slots + 31) / 32 + 3) & ~(size_t)3;   // 16-byte units
+        std::vector<uint32_t> bits(words, 0u);
+        for (size_t i = 0; i < h.size(); ++i)
+          if (have1 && h[i] == v1) bits[i >> 5] |= 1u << (i & 31);
+        CUG(cudaMalloc(&ctx->d_bits, 4 * words));
+        CUG(cudaMemcpy(ctx->d_bits, bits.data(), 4 * words, cudaMemcpyHostToDevice));
+        ctx->dens_mode = 2;
+        ctx->stage_bytes = (unsigned)(4 * words);
+        ctx->pal0 = v0; ctx->pal1 = v1;
+      }
+    }
+  }
   guard.c = nullptr;
   *out = ctx;
   return MCRT_OK;
@@ -270,7 +323,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_sources(ctx);
   free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
-  cudaFree(ctx->d_lut); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
+  cudaFree(ctx->d_lut); cudaFree(ctx->d_bits); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -455,10 +508,17 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   const size_t smem = transport_smem_bytes(ctx);
   TransportParamsU PU;
   PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
+  const int dens = staging_mode(ctx);
+  PU.stage = dens == 1 ? (const void*)ctx->d_rho : (const void*)ctx->d_bits;
+  PU.stage_bytes = ctx->stage_bytes; PU.pal0 = ctx->pal0; PU.pal1 = ctx->pal1;
   const bool five = bps * threads > 1024;                    // 48-register build (5 blocks of 256) or 64-register build
-  void (*kern)(TransportParamsU) = ctx->uni ? (five ? k_transport_u<5, false> : k_transport_u<4, false>)
-                                            : (five ? k_transport_u<5, true> : k_transport_u<4, true>);
+  void (*kern)(TransportParamsU) =
+      !ctx->uni ? (five ? k_transport_u<5, true, 0> : k_transport_u<4, true, 0>)
+      : dens == 1 ? k_transport_u<5, false, 1>
+      : dens == 2 ? k_transport_u<5, false, 2>
+                  : (five ? k_transport_u<5, false, 0> : k_transport_u<4, false, 0>);
   if (smem > (48u << 10)) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (dens) CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   int resident = 0;                                          // large tables (many bins) lower the residency:
   CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem));   // size the grid to what fits
   if (resident < 1) return fail(ctx, MCRT_EINVAL, "mcrt_run_batch: the transport kernel does not fit on an SM with these tables");
@@ -870,6 +930,15 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
   ctx->quorum = quorum;
   return MCRT_OK;
 }
+
+mcrt_status mcrt_set_density_staging(mcrt_ctx* ctx, int32_t mode) {
+  if (!ctx) return MCRT_EINVAL;
+  if (mode < 0 || mode > 2) return fail(ctx, MCRT_EINVAL, "mcrt_set_density_staging: mode must be 0 (automatic), 1 (off) or 2 (also one bit per cell)");
+  ctx->dens_off = mode;
+  return MCRT_OK;
+}
+
+int32_t mcrt_density_staging(const mcrt_ctx* ctx) { return ctx ? staging_mode(ctx) : -1; }
 
 mcrt_status mcrt_set_source_order(mcrt_ctx* ctx, int32_t mode) {
   if (!ctx) return MCRT_EINVAL;

@@ -30,6 +30,12 @@
 //    cost a handful of predicated instructions, only entering / leaving the refined REGION diverges.
 //  * The density of the NEXT leaf is requested before the optical-depth test of the current one
 //    (the geometric walk does not depend on rho), taking the gather latency off the dependent chain.
+//  * Small problems keep their density ON CHIP (template DENS): a single-level grid of up to 40 KB
+//    is copied into every block's shared memory as it is (DENS = 1: C0's 16^3), a grid with only
+//    two distinct densities as ONE BIT per cell (DENS = 2: the uniform spheres, 64^3 = 32 KB), by
+//    one cp.async.bulk (TMA) per block.  A crossing then costs a shared-memory read instead of an
+//    L1TEX wavefront and an L2 round trip: this lifts the scattered-gather ceiling and shortens the
+//    end-of-batch tail, where a lone package's crossing latency is all there is.
 //  * The walk loop runs until fewer than `quorum` lanes of the warp are still walking; then all
 //    stopped lanes go through ONE event pass (escape tally -> refill from the work queue ->
 //    emission / scattering / absorption+re-emission -> new flight).  Emission and re-emission
@@ -95,7 +101,32 @@ struct TransportParamsU {
                                  // (2*axis+1)*N; two-level grids: [6][kSubStride] sub-cell rows from lut_sub_offset(N)
   LayoutU lay;
   int quorum;                    // leave the walk loop when fewer lanes than this are walking; 0 = automatic
+  // density staged in shared memory (kernel template DENS = 1 / 2): what every block copies in
+  const void* __restrict__ stage;   // DENS 1: the fp32 density array itself; DENS 2: one bit per storage slot
+  unsigned stage_bytes;             // multiple of 16
+  float pal0, pal1;                 // DENS 2: the two densities (bit 0 / bit 1)
 };
+
+// where a kernel instance reads densities from
+struct DensU {
+  const float* __restrict__ rho;  // DENS 0: global gathers
+  uint32_t base;                  // DENS 1, 2: shared-memory byte address of the staged array
+  float v0, v1;                   // DENS 2
+};
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+template <int DENS>
+__device__ __forceinline__ float density_at(const DensU& D, int slot) {
+  if (DENS == 1) return __uint_as_float(lds_u32(D.base + 4u * (uint32_t)slot));
+  if (DENS == 2) {
+    const uint32_t w = lds_u32(D.base + (((uint32_t)slot >> 3) & ~3u));
+    return ((w >> ((uint32_t)slot & 31u)) & 1u) ? D.v1 : D.v0;
+  }
+  return __ldg(D.rho + slot);
+}
 
 // Automatic walk quorum.  A warp that walks until w lanes are left and then spends E instructions on
 // one event pass does about L (32 - w) crossings in c L ln(32/w) + E instructions (L = mean crossings
@@ -270,9 +301,9 @@ __device__ __forceinline__ void root_entry(const TransportParams& P, PacketU& p,
 // alternate the two registers and no instruction waits on the gather except its real use.
 // tau_rem > 0 always (u01 < 1, and a - b > 0 for a > b in IEEE arithmetic), so dtau >= tau_rem
 // implies rho*kappa > 0: no interaction in an empty leaf (R14).
-template <bool TL>
-__device__ __forceinline__ void walk_step_u(const TransportParams& P, PacketU& p, float& cur, float& nxt,
-                                            float kx, uint32_t sublut, int& state, uint32_t& crossings) {
+template <bool TL, int DENS>
+__device__ __forceinline__ void walk_step_u(const TransportParams& P, const DensU& D, PacketU& p, float& cur,
+                                            float& nxt, float kx, uint32_t sublut, int& state, uint32_t& crossings) {
   if (TL) {
     if ((p.cb | __float_as_int(cur)) < 0) root_entry(P, p, sublut, cur);
   }
@@ -292,7 +323,7 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, PacketU& p
   }
   const bool esc = dl == kLutEscape;
   const int nslot = from + dl;
-  if (!esc) { MCRT_CHECK_SLOT(nslot); nxt = __ldg(P.rho + nslot); }
+  if (!esc) { MCRT_CHECK_SLOT(nslot); nxt = density_at<DENS>(D, nslot); }
   const float dtau = cur * kx * (tnext - p.tcur);
   if (dtau >= p.tau_rem) {                                   // interaction inside this leaf
     state = SU_INTERACT;
@@ -371,7 +402,7 @@ __device__ __forceinline__ void emit_position_u(const TransportParams& P, const 
 // MINBLOCKS = resident blocks per SM the kernel is compiled for: 4 (64 registers) or 5 (48
 // registers).  Five blocks hide more of the L2 latency on cache-resident grids; on HBM-resident
 // grids the extra threads thrash the L1, so the host picks per grid (profiles/).
-template <int MINBLOCKS, bool TL>
+template <int MINBLOCKS, bool TL, int DENS>
 __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportParamsU PU) {
   const TransportParams& P = PU.base;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -387,6 +418,25 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   for (int i = threadIdx.x; i < P.nb; i += blockDim.x) { s_opac[i] = P.opac[i]; s_emit[i] = 0; }
   for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x) s_sed[i] = 0;
   for (int i = threadIdx.x; i < n_lut; i += blockDim.x) s_lut[i] = PU.lut[i];
+  DensU D;
+  D.rho = P.rho; D.base = 0; D.v0 = PU.pal0; D.v1 = PU.pal1;
+  if (DENS != 0) {
+    // the staged density array behind the tables (128-byte aligned), then the mbarrier of its bulk copy
+    const uint32_t off = (uint32_t)(((32u * (unsigned)P.nb + 63u) & ~63u) + 4u * (unsigned)n_lut + 127u) & ~127u;
+    D.base = (uint32_t)__cvta_generic_to_shared(smem_raw) + off;
+    const uint32_t bar = D.base + PU.stage_bytes;
+    if (threadIdx.x == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(PU.stage_bytes) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(D.base), "l"(PU.stage), "r"(PU.stage_bytes), "r"(bar) : "memory");
+    }
+    __syncthreads();                                         // the barrier is initialised for everyone
+    asm volatile("{\n.reg .pred p;\nMCRT_STAGE_WAIT:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n"
+                 "@p bra MCRT_STAGE_DONE;\nbra MCRT_STAGE_WAIT;\nMCRT_STAGE_DONE:\n}" ::"r"(bar) : "memory");
+  }
   __syncthreads();
 
   const unsigned lane = threadIdx.x & 31;
@@ -524,7 +574,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
           }
           p.slot = (int)slot_of(PU.lay, ix, iy, iz);
           MCRT_CHECK_SLOT(p.slot);
-          p.rho = __ldg(P.rho + p.slot);
+          p.rho = density_at<DENS>(D, p.slot);
           if (TL && P.src[s].type == 0) {
             if (__float_as_int(p.rho) < 0) {                 // the source sits in a refined cube
               const int S = P.S;
@@ -567,9 +617,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
     // ---- a3: cell walk until fewer than `quorum` lanes are walking ----
 #pragma unroll 1
     for (;;) {
-      if (state == SU_WALK) walk_step_u<TL>(P, p, p.rho, rho_b, kx, sublut, state, n_cross);
+      if (state == SU_WALK) walk_step_u<TL, DENS>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
       if (state == SU_WALK) {
-        walk_step_u<TL>(P, p, rho_b, p.rho, kx, sublut, state, n_cross);
+        walk_step_u<TL, DENS>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);
         if (state == SU_INTERACT) state = SU_INTERACT_B;
       }
       if (__popc(__ballot_sync(kFull, state == SU_WALK)) < quorum) break;

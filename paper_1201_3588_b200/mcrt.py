@@ -63,6 +63,7 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_observer",
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
+           "mcrt_set_density_staging", "mcrt_density_staging",
            "mcrt_get_batch_times", "mcrt_get_tables",
            "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_uniforms", "mcrt_gather_calibrate", "mcrt_last_error")
 
@@ -104,6 +105,10 @@ def lib():
         L.mcrt_set_launch.argtypes = [vp, i32, i32]
         L.mcrt_set_walk_quorum.argtypes = [vp, i32]
         L.mcrt_set_source_order.argtypes = [vp, i32]
+        L.mcrt_set_density_staging.argtypes = [vp, i32]
+        L.mcrt_set_density_staging.restype = C.c_int
+        L.mcrt_density_staging.argtypes = [vp]
+        L.mcrt_density_staging.restype = i32
         L.mcrt_get_batch_times.argtypes = [vp, vp, vp, i32, C.POINTER(i32)]
         L.mcrt_get_tables.argtypes = [vp, vp, vp, vp]
         L.mcrt_kernel_launches.restype = i64
@@ -373,6 +378,12 @@ class Context:
 
     def set_walk_quorum(self, quorum):
         self._check(lib().mcrt_set_walk_quorum(self.h, int(quorum)), "mcrt_set_walk_quorum")
+
+    def set_density_staging(self, mode):
+        self._check(lib().mcrt_set_density_staging(self.h, int(mode)), "mcrt_set_density_staging")
+
+    def density_staging(self):
+        return int(lib().mcrt_density_staging(self.h))
 
     def set_source_order(self, mode):
         self._check(lib().mcrt_set_source_order(self.h, int(mode)), "mcrt_set_source_order")

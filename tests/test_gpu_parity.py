@@ -621,3 +621,31 @@ def test_automatic_walk_quorum_does_not_change_results(M):
         a.run_batch(wl.seed, first, cnt)
         b.run_batch(wl.seed, first, cnt)
     _assert_identical(a, b)
+
+
+def test_density_staged_in_shared_memory_does_not_change_results(M):
+    """Small single-level problems keep their density in shared memory (one cp.async.bulk per
+    block): the fp32 array itself up to 40 KB (C0), one bit per cell for a two-valued grid (the
+    64^3 sphere of C1).  Every count must equal the global-gather path's; grids that qualify for
+    neither (three densities, > 40 KB) stay on global gathers."""
+    three = W.c1(n_packets=50_000, batch=25_000)
+    three.rho_root = three.rho_root.copy()
+    three.rho_root[::7] *= np.float32(0.5)                     # a third distinct density
+    for wl, mode in ((W.c0(), 1),
+                     (W.tiny_random(n_root=3, seed=4, external=True, n_packets=40_000, batch=10_000), 1),
+                     (W.c1(n_packets=300_000, batch=100_000), 2),
+                     (W.c1(tau_v=100.0, n_packets=20_000, batch=10_000), 2),
+                     (W.sphere(n_root=40, albedo=1.0, gval=0.4, n_packets=100_000, batch=50_000), 2),
+                     (three, 0)):
+        a = M.from_workload(wl)
+        assert a.density_staging() == (mode if mode == 1 else 0)   # the one-bit form is opt-in (measured slower)
+        a.set_density_staging(2)
+        assert a.density_staging() == mode, (wl.name, a.density_staging())
+        b = M.from_workload(wl)
+        b.set_density_staging(1)
+        assert b.density_staging() == 0
+        for first, cnt in wl.batches():
+            a.run_batch(wl.seed, first, cnt)
+            b.run_batch(wl.seed, first, cnt)
+        _assert_identical(a, b)
+        assert a.get_counters()["emitted"] == wl.n_packets
