@@ -72,10 +72,14 @@ typedef struct {
   const float* rho_sub;  /* [n_ref*S^3]; NULL iff no cube is refined                          */
   mcrt_mem mem;          /* where refine / rho_root / rho_sub live                            */
   int32_t layout;        /* device storage order of the root grid (never visible in the getters,
-                            which always use the slot order above): 0 = automatic (bricked for
-                            a single-level grid larger than the L2, else x-fastest), 1 =
-                            x-fastest, 2 = 8^3 bricks in Morton order.  Subcubes always follow
-                            the root grid as blocks of sub^3.                                  */
+                            which always use the slot order above): 0 = automatic, 1 =
+                            x-fastest, 2 = 8^3 bricks in Morton order (automatic for a
+                            single-level grid larger than the L2), 3 / 4 = macro cubes of 4^3 /
+                            8^3 cells: a single-level grid run internally as a two-level one in
+                            which a cube of cells that all hold the same density is crossed in
+                            one step (automatic, 4^3, when n_root is a multiple of 4 and at
+                            least 30 % of the cubes are uniform: a sphere or slab in vacuum).
+                            Subcubes always follow the root grid as blocks of sub^3.           */
 } mcrt_grid_desc;
 
 /* Creates a context on the current CUDA device and uploads the grid. */

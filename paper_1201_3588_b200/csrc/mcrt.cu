@@ -53,7 +53,13 @@ struct mcrt_ctx {
   std::vector<BatchEvents> pending, spare;
   // single-level grids: storage layout (transport_u.cuh); `slots` stays the caller-visible count
   bool uni = false;
-  LayoutU lay = {0, 0, 0};
+  LayoutU lay = {0, 0, 0, 0};
+  // Macro cubes (single-level grids whose density is piecewise uniform): internally the grid is run as a
+  // two-level one -- N/M macro cubes per axis, each with its M^3 cells behind the macro array; a macro cube
+  // whose cells all hold the same density is walked in ONE step (transport_u.cuh, MACRO).  N, S, root_size
+  // then describe the macro grid; n_fine / lay_fine the caller's grid (the getters' slot order, R22).
+  int macro = 0, n_fine = 0;
+  LayoutU lay_fine = {0, 0, 0, 0};
   long long store_slots = 0;
   int* d_lut = nullptr;
   unsigned long long* d_tally_scratch = nullptr;
@@ -115,6 +121,56 @@ static void free_observer(mcrt_ctx* c) {
 static void free_sources(mcrt_ctx* c) {
   cudaFree(c->d_src); cudaFree(c->d_csrc); cudaFree(c->d_csrc32);
   c->d_src = nullptr; c->d_csrc = nullptr; c->d_csrc32 = nullptr;
+}
+
+// ---- storage order <-> the caller's slot order (R22) ---------------------------------------------
+// root part through the root layout, sub-cells (contiguous behind it) copied; macro-cube grids: the
+// caller's slots are the N^3 cells, stored cube by cube behind the macro array.
+static bool needs_reorder(const mcrt_ctx* ctx) { return ctx->macro || ctx->lay.bricked; }
+
+static mcrt_status store_to_api_u64(mcrt_ctx* ctx, const unsigned long long* store, unsigned long long* out, cudaStream_t st) {
+  if (ctx->macro) {
+    const long long nf3 = ctx->slots;
+    k_store_to_ext<unsigned long long><<<(unsigned)((nf3 + 255) / 256), 256, 0, st>>>(store + ctx->store_n3, out, ctx->lay_fine, nf3);
+    ctx->launches++;
+    return MCRT_OK;
+  }
+  k_store_to_ext<unsigned long long><<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(store, out, ctx->lay, ctx->n3);
+  ctx->launches++;
+  if (ctx->slots > ctx->n3)
+    CU(cudaMemcpyAsync(out + ctx->n3, store + ctx->store_n3, 8 * (size_t)(ctx->slots - ctx->n3), cudaMemcpyDeviceToDevice, st));
+  return MCRT_OK;
+}
+static mcrt_status api_to_store_u64(mcrt_ctx* ctx, const unsigned long long* in, unsigned long long* store, cudaStream_t st) {
+  if (ctx->macro) {
+    const long long nf3 = ctx->slots;
+    CU(cudaMemsetAsync(store, 0, 8 * (size_t)ctx->store_n3, st));
+    k_ext_to_store_u64<<<(unsigned)((nf3 + 255) / 256), 256, 0, st>>>(in, store + ctx->store_n3, ctx->lay_fine, nf3);
+    ctx->launches++;
+    return MCRT_OK;
+  }
+  k_ext_to_store_u64<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(in, store, ctx->lay, ctx->n3);
+  ctx->launches++;
+  if (ctx->slots > ctx->n3)
+    CU(cudaMemcpyAsync(store + ctx->store_n3, in + ctx->n3, 8 * (size_t)(ctx->slots - ctx->n3), cudaMemcpyDeviceToDevice, st));
+  return MCRT_OK;
+}
+static mcrt_status trow_to_api_T(mcrt_ctx* ctx, float* out, cudaStream_t st) {
+  const float lnTmin = (float)std::log(ctx->Tmin), dlnT = (float)ctx->dlnT;
+  if (ctx->macro) {
+    const long long nf3 = ctx->slots;
+    k_trow_to_T_u<<<(unsigned)((nf3 + 255) / 256), 256, 0, st>>>(ctx->d_trow + ctx->store_n3, out, ctx->lay_fine, nf3, lnTmin, dlnT);
+    ctx->launches++;
+    return MCRT_OK;
+  }
+  k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(ctx->d_trow, out, ctx->lay, ctx->n3, lnTmin, dlnT);
+  ctx->launches++;
+  if (ctx->slots > ctx->n3) {                                // sub-cells: same order in storage and in the getter
+    const long long ns = ctx->slots - ctx->n3;
+    k_trow_to_T<<<(unsigned)((ns + 255) / 256), 256, 0, st>>>(ctx->d_trow + ctx->store_n3, out + ctx->n3, ns, lnTmin, dlnT);
+    ctx->launches++;
+  }
+  return MCRT_OK;
 }
 
 // dynamic shared memory of the transport kernel: opacity float4[nb], SED u32[3 nb], emitted u32[nb], then at
@@ -186,7 +242,7 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
   if (ctx->slots >= (1ll << 31)) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: more than 2^31-1 leaf slots"));
   if (k > 0 && !d->rho_sub) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: rho_sub is NULL but cubes are refined"));
   // storage order of the root grid (both kinds of grid; sub-cells always follow as blocks of S^3)
-  if (d->layout < 0 || d->layout > 2) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: layout must be 0, 1 or 2"));
+  if (d->layout < 0 || d->layout > 4) return bail(fail(ctx, MCRT_EINVAL, "mcrt_grid_create: layout must be 0..4"));
   ctx->uni = k == 0;
   ctx->lay.N = d->n_root;
   ctx->lay.nbk = (d->n_root + 7) / 8;
@@ -199,11 +255,6 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     ctx->store_n3 = n3;
   }
   ctx->store_slots = ctx->store_n3 + k * s3;
-  CUG(cudaMalloc(&ctx->d_rho, sizeof(float) * ctx->store_slots));
-  CUG(cudaMalloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->store_slots));
-  CUG(cudaMalloc(&ctx->d_trow, sizeof(float) * ctx->store_slots));
-  CUG(cudaMemset(ctx->d_tally, 0, sizeof(unsigned long long) * ctx->store_slots));
-  CUG(cudaMemset(ctx->d_trow, 0, sizeof(float) * ctx->store_slots));
   // staging copies of caller data (freed before returning)
   float *st_root = nullptr, *st_sub = nullptr;
   int* d_refidx = nullptr;
@@ -219,6 +270,41 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
       src_sub = st_sub;
     }
   }
+  // ---- macro cubes: a single-level grid in which enough 4^3 (8^3) blocks of cells hold ONE density ----
+  if (k == 0 && (d->layout == 0 || d->layout >= 3)) {
+    const int M = d->layout == 4 ? 8 : 4;
+    if (d->n_root % M == 0 && d->n_root / M >= 2 && n3 + n3 / (M * M * M) < (1ll << 31)) {
+      const int Nm = d->n_root / M;
+      const long long nm3 = (long long)Nm * Nm * Nm;
+      unsigned int* d_cnt = nullptr;
+      CUG(cudaMalloc(&d_cnt, sizeof(unsigned int)));
+      CUG(cudaMemset(d_cnt, 0, sizeof(unsigned int)));
+      k_count_uniform_macros<<<(unsigned)((nm3 + 127) / 128), 128>>>(src_root, d->n_root, M, nm3, d_cnt);
+      unsigned int n_uniform = 0;
+      cudaError_t e1 = cudaMemcpy(&n_uniform, d_cnt, sizeof(unsigned int), cudaMemcpyDeviceToHost);
+      cudaFree(d_cnt);
+      if (e1 != cudaSuccess) return bail(fail(ctx, MCRT_ECUDA, std::string("macro count: ") + cudaGetErrorString(e1)));
+      ctx->launches++;
+      // automatic: when at least 30 % of the macro cubes are uniform (a sphere or a slab in vacuum; not a
+      // turbulent field) and the grid is not one the brick layout is meant for
+      if (d->layout >= 3 || ((double)n_uniform >= 0.3 * (double)nm3 && !ctx->lay.bricked)) {
+        ctx->macro = M;
+        ctx->n_fine = d->n_root;
+        ctx->lay_fine.N = d->n_root; ctx->lay_fine.bricked = 2; ctx->lay_fine.nbk = Nm; ctx->lay_fine.bm = M;
+        ctx->N = Nm; ctx->S = M; ctx->root_size = d->root_size * M;
+        ctx->lay.N = Nm; ctx->lay.bricked = 0; ctx->lay.nbk = (Nm + 7) / 8;
+        ctx->uni = false;                                      // the two-level kernel runs it
+        ctx->n3 = nm3; ctx->store_n3 = nm3;
+        ctx->store_slots = nm3 + n3;                           // macro array, then the cells cube by cube
+        ctx->slots = n3;                                       // the caller's leaf slots stay the N^3 cells
+      }
+    }
+  }
+  CUG(cudaMalloc(&ctx->d_rho, sizeof(float) * ctx->store_slots));
+  CUG(cudaMalloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->store_slots));
+  CUG(cudaMalloc(&ctx->d_trow, sizeof(float) * ctx->store_slots));
+  CUG(cudaMemset(ctx->d_tally, 0, sizeof(unsigned long long) * ctx->store_slots));
+  CUG(cudaMemset(ctx->d_trow, 0, sizeof(float) * ctx->store_slots));
   if (k > 0) {
     CUG(cudaMalloc(&d_refidx, sizeof(int) * n3));
     CUG(cudaMemcpy(d_refidx, refidx.data(), sizeof(int) * n3, cudaMemcpyHostToDevice));
@@ -253,7 +339,14 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     CUG(cudaMalloc(&ctx->d_lut, sizeof(int) * lut.size()));
     CUG(cudaMemcpy(ctx->d_lut, lut.data(), sizeof(int) * lut.size(), cudaMemcpyHostToDevice));
     CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
-    if (ctx->uni) k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho, ctx->lay, n3);
+    if (ctx->macro) {
+      // the cells cube by cube behind the macro array; then one entry per macro cube: its density if all
+      // its cells hold the same one, else the marker (sign bit | cube number) that sends the walk to the cells
+      k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho + ctx->store_n3, ctx->lay_fine, n3);
+      k_macro_entries<<<(unsigned)((ctx->n3 + 127) / 128), 128>>>(ctx->d_rho + ctx->store_n3, ctx->d_rho, ctx->n3,
+                                                                ctx->macro * ctx->macro * ctx->macro);
+      ctx->launches++;
+    } else if (ctx->uni) k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho, ctx->lay, n3);
     else k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, ctx->lay, n3);
   }
   ctx->launches++;
@@ -501,7 +594,8 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   const int threads = ctx->threads;
   // resident blocks per SM: the caller's choice, else 5 (48-register kernels), except 4 for the
   // single-level kernel on HBM-resident grids (bricked storage), where more threads thrash the L1
-  const int bps = ctx->blocks_per_sm ? ctx->blocks_per_sm : (ctx->uni && ctx->lay.bricked ? 4 : 5);
+  // (and 4 for macro-cube grids: the 48-register build of that instance spills in the walk, c1_tau1 0.337 vs 0.329 ms)
+  const int bps = ctx->blocks_per_sm ? ctx->blocks_per_sm : ((ctx->uni && ctx->lay.bricked) || ctx->macro ? 4 : 5);
   long long want = ((long long)n + threads - 1) / threads;
   long long grid = (long long)ctx->sm_count * bps;
   if (want < grid) grid = want;
@@ -513,10 +607,11 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   PU.stage_bytes = ctx->stage_bytes; PU.pal0 = ctx->pal0; PU.pal1 = ctx->pal1;
   const bool five = bps * threads > 1024;                    // 48-register build (5 blocks of 256) or 64-register build
   void (*kern)(TransportParamsU) =
-      !ctx->uni ? (five ? k_transport_u<5, true, 0> : k_transport_u<4, true, 0>)
-      : dens == 1 ? k_transport_u<5, false, 1>
-      : dens == 2 ? k_transport_u<5, false, 2>
-                  : (five ? k_transport_u<5, false, 0> : k_transport_u<4, false, 0>);
+      ctx->macro ? (five ? k_transport_u<5, true, 0, true> : k_transport_u<4, true, 0, true>)
+      : !ctx->uni ? (five ? k_transport_u<5, true, 0, false> : k_transport_u<4, true, 0, false>)
+      : dens == 1 ? k_transport_u<5, false, 1, false>
+      : dens == 2 ? k_transport_u<5, false, 2, false>
+                  : (five ? k_transport_u<5, false, 0, false> : k_transport_u<4, false, 0, false>);
   if (smem > (48u << 10)) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   if (dens) CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   int resident = 0;                                          // large tables (many bins) lower the residency:
@@ -539,16 +634,13 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
   double V = ctx->root_size * ctx->root_size * ctx->root_size;
   float ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)n_cum) - std::log(4.0 * PI) - std::log(V));
   float ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
-  if (tally != ctx->d_tally && ctx->lay.bricked) {                 // caller's sum is in slot order (R22)
+  if (tally != ctx->d_tally && needs_reorder(ctx)) {               // caller's sum is in slot order (R22)
     if (!ctx->d_tally_scratch) {
       CU(cudaMalloc(&ctx->d_tally_scratch, 8 * (size_t)ctx->store_slots));
       CU(cudaMemsetAsync(ctx->d_tally_scratch, 0, 8 * (size_t)ctx->store_slots, st));
     }
-    k_ext_to_store_u64<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(tally, ctx->d_tally_scratch, ctx->lay, ctx->n3);
-    ctx->launches++;
-    if (ctx->slots > ctx->n3)                                // sub-cells keep their order behind the root grid
-      CU(cudaMemcpyAsync(ctx->d_tally_scratch + ctx->store_n3, tally + ctx->n3, 8 * (size_t)(ctx->slots - ctx->n3),
-                         cudaMemcpyDeviceToDevice, st));
+    mcrt_status rc = api_to_store_u64(ctx, tally, ctx->d_tally_scratch, st);
+    if (rc != MCRT_OK) return rc;
     tally = ctx->d_tally_scratch;
   }
   long long blocks = (ctx->store_slots / 2 + 256) / 256;     // two leaves per thread and turn
@@ -680,20 +772,16 @@ mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps
     const unsigned long long n_eps = ctx->Nglobal > ctx->Ncum ? ctx->Nglobal : ctx->Ncum;
     if (eps_out) *eps_out = n_eps ? ctx->Ltot / (double)n_eps : 0.0;
   }
-  if (ctx->lay.bricked) {                                    // storage order -> slot order (R22)
+  if (needs_reorder(ctx)) {                                  // storage order -> slot order (R22)
     unsigned long long* d_out = (unsigned long long*)n_abs_out;
     unsigned long long* tmp = nullptr;
     if (mem == MCRT_HOST) {
       if (!ctx->d_out_scratch) CU(cudaMalloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
       tmp = (unsigned long long*)ctx->d_out_scratch; d_out = tmp;
     }
-    k_store_to_ext<unsigned long long><<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
-        ctx->d_tally, d_out, ctx->lay, ctx->n3);
-    ctx->launches++;
+    mcrt_status rc = store_to_api_u64(ctx, ctx->d_tally, d_out, ctx->last_stream);
+    if (rc != MCRT_OK) return rc;
     CU(cudaGetLastError());
-    if (ctx->slots > ctx->n3)
-      CU(cudaMemcpyAsync(d_out + ctx->n3, ctx->d_tally + ctx->store_n3, 8 * (size_t)(ctx->slots - ctx->n3),
-                         cudaMemcpyDeviceToDevice, ctx->last_stream));
     if (mem == MCRT_HOST) return copy_out(ctx, n_abs_out, tmp, 8 * (size_t)ctx->slots, MCRT_HOST);
     return sync_last(ctx);
   }
@@ -710,14 +798,9 @@ mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem)
     if (!ctx->d_out_scratch) CU(cudaMalloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
     tmp = (float*)ctx->d_out_scratch; d_T = tmp;
   }
-  k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, ctx->last_stream>>>(
-      ctx->d_trow, d_T, ctx->lay, ctx->n3, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
-  ctx->launches++;
-  if (ctx->slots > ctx->n3) {                                // sub-cells: same order in storage and in the getter
-    const long long ns = ctx->slots - ctx->n3;
-    k_trow_to_T<<<(unsigned)((ns + 255) / 256), 256, 0, ctx->last_stream>>>(
-        ctx->d_trow + ctx->store_n3, d_T + ctx->n3, ns, (float)std::log(ctx->Tmin), (float)ctx->dlnT);
-    ctx->launches++;
+  {
+    mcrt_status rc = trow_to_api_T(ctx, d_T, ctx->last_stream);
+    if (rc != MCRT_OK) return rc;
   }
   CU(cudaGetLastError());
   if (mem == MCRT_HOST) return copy_out(ctx, T_out, tmp, 4 * (size_t)ctx->slots, MCRT_HOST);
@@ -750,11 +833,9 @@ mcrt_status mcrt_results_begin(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem 
   if (out->n_abs) {
     if (host && !t.snap_abs) CU(cudaMalloc(&t.snap_abs, 8 * (size_t)ctx->slots));
     abs_dst = host ? t.snap_abs : (unsigned long long*)out->n_abs;
-    if (ctx->lay.bricked) {
-      k_store_to_ext<unsigned long long><<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(ctx->d_tally, abs_dst, ctx->lay, ctx->n3);
-      ctx->launches++;
-      if (ctx->slots > ctx->n3)
-        CU(cudaMemcpyAsync(abs_dst + ctx->n3, ctx->d_tally + ctx->store_n3, 8 * (size_t)(ctx->slots - ctx->n3), cudaMemcpyDeviceToDevice, st));
+    if (needs_reorder(ctx)) {
+      mcrt_status rc = store_to_api_u64(ctx, ctx->d_tally, abs_dst, st);
+      if (rc != MCRT_OK) return rc;
     } else {
       CU(cudaMemcpyAsync(abs_dst, ctx->d_tally, 8 * (size_t)ctx->slots, cudaMemcpyDeviceToDevice, st));
     }
@@ -762,15 +843,8 @@ mcrt_status mcrt_results_begin(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem 
   if (out->T) {
     if (host && !t.snap_T) CU(cudaMalloc(&t.snap_T, 4 * (size_t)ctx->slots));
     T_dst = host ? t.snap_T : out->T;
-    k_trow_to_T_u<<<(unsigned)((ctx->n3 + 255) / 256), 256, 0, st>>>(ctx->d_trow, T_dst, ctx->lay, ctx->n3,
-                                                                     (float)std::log(ctx->Tmin), (float)ctx->dlnT);
-    ctx->launches++;
-    if (ctx->slots > ctx->n3) {
-      const long long ns = ctx->slots - ctx->n3;
-      k_trow_to_T<<<(unsigned)((ns + 255) / 256), 256, 0, st>>>(ctx->d_trow + ctx->store_n3, T_dst + ctx->n3, ns,
-                                                                (float)std::log(ctx->Tmin), (float)ctx->dlnT);
-      ctx->launches++;
-    }
+    mcrt_status rc = trow_to_api_T(ctx, T_dst, st);
+    if (rc != MCRT_OK) return rc;
   }
   if (!t.snap_small) { CU(cudaMalloc(&t.snap_small, 8 * n_small)); }
   CU(cudaMemcpyAsync(t.snap_small, ctx->d_small, 8 * n_small, cudaMemcpyDeviceToDevice, st));

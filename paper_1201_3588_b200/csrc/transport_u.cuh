@@ -36,6 +36,16 @@
 //    one cp.async.bulk (TMA) per block.  A crossing then costs a shared-memory read instead of an
 //    L1TEX wavefront and an L2 round trip: this lifts the scattered-gather ceiling and shortens the
 //    end-of-batch tail, where a lone package's crossing latency is all there is.
+//  * MACRO: a single-level grid whose density is piecewise uniform (a sphere in vacuum) is run as a
+//    two-level one: N/M macro cubes per axis, the M^3 cells of each behind the macro array.  A macro
+//    cube whose cells all hold the same density is crossed in ONE step (the sum of equal per-cell
+//    optical depths is the optical depth of the whole chord; empty space is skipped the same way);
+//    a mixed cube carries the marker and is walked cell by cell.  Tallies and temperatures stay per
+//    cell: an absorption inside a uniform cube is booked on the cell the interaction point lies in.
+//    Cell crossings are not counted step by step there but from the cell coordinates at the two
+//    ends of every flight (motion is monotonic per axis, so a flight crosses |F_end - F_start|
+//    cell faces on each axis): "a kernel that skips empty space must add the skipped leaf count
+//    arithmetically".
 //  * The walk loop runs until fewer than `quorum` lanes of the warp are still walking; then all
 //    stopped lanes go through ONE event pass (escape tally -> refill from the work queue ->
 //    emission / scattering / absorption+re-emission -> new flight).  Emission and re-emission
@@ -46,11 +56,13 @@
 
 namespace mcrt {
 
-// ---- storage layout of the root grid (host and device) ----------------------------------------
+// ---- storage layouts of a cubic array of N^3 cells (host and device) ----------------------------
 struct LayoutU {
-  int N;          // root cells per axis
-  int bricked;    // 0: x-fastest;  1: 8^3 bricks (x-fastest over bricks), Morton order inside
+  int N;          // cells per axis
+  int bricked;    // 0: x-fastest;  1: 8^3 bricks (x-fastest over bricks), Morton order inside;
+                  // 2: bm^3 bricks (x-fastest over bricks), x-fastest inside (the cells of a macro cube)
   int nbk;        // bricks per axis (bricked)
+  int bm;         // brick edge (bricked = 2)
 };
 __host__ __device__ __forceinline__ unsigned dil3(unsigned v) {      // 3 bits -> every third bit
   return (v & 1u) | ((v & 2u) << 2) | ((v & 4u) << 4);
@@ -60,9 +72,14 @@ __host__ __device__ __forceinline__ unsigned undil3(unsigned m) {
 }
 // contribution of coordinate i on axis a to the storage slot
 __host__ __device__ __forceinline__ long long axis_term(const LayoutU& L, int a, int i) {
-  if (L.bricked) {
+  if (L.bricked == 1) {
     long long bs = a == 0 ? 1 : (a == 1 ? L.nbk : (long long)L.nbk * L.nbk);
     return (long long)(dil3((unsigned)i & 7u) << a) + 512ll * (i >> 3) * bs;
+  }
+  if (L.bricked == 2) {
+    long long bs = a == 0 ? 1 : (a == 1 ? L.nbk : (long long)L.nbk * L.nbk);
+    long long is = a == 0 ? 1 : (a == 1 ? L.bm : (long long)L.bm * L.bm);
+    return (long long)(i % L.bm) * is + (long long)L.bm * L.bm * L.bm * (i / L.bm) * bs;
   }
   long long s = a == 0 ? 1 : (a == 1 ? L.N : (long long)L.N * L.N);
   return s * i;
@@ -71,11 +88,20 @@ __host__ __device__ __forceinline__ long long slot_of(const LayoutU& L, int ix, 
   return axis_term(L, 0, ix) + axis_term(L, 1, iy) + axis_term(L, 2, iz);
 }
 __host__ __device__ __forceinline__ long long slots_of(const LayoutU& L) {
-  return L.bricked ? 512ll * L.nbk * L.nbk * L.nbk : (long long)L.N * L.N * L.N;
+  if (L.bricked == 1) return 512ll * L.nbk * L.nbk * L.nbk;
+  return (long long)L.N * L.N * L.N;                                  // bricked = 2 needs N = nbk * bm: no padding
 }
 // storage slot -> x-fastest cell number (R22), or -1 for a padding slot
 __host__ __device__ __forceinline__ long long ext_of_slot(const LayoutU& L, long long s) {
   if (!L.bricked) return s;
+  if (L.bricked == 2) {
+    const long long b3 = (long long)L.bm * L.bm * L.bm;
+    long long b = s / b3;
+    int m = (int)(s % b3);
+    int bx = (int)(b % L.nbk), by = (int)((b / L.nbk) % L.nbk), bz = (int)(b / ((long long)L.nbk * L.nbk));
+    int ix = bx * L.bm + m % L.bm, iy = by * L.bm + (m / L.bm) % L.bm, iz = bz * L.bm + m / (L.bm * L.bm);
+    return ix + (long long)L.N * (iy + (long long)L.N * iz);
+  }
   unsigned m = (unsigned)(s & 511);
   long long b = s >> 9;
   int bx = (int)(b % L.nbk), by = (int)((b / L.nbk) % L.nbk), bz = (int)(b / ((long long)L.nbk * L.nbk));
@@ -301,7 +327,7 @@ __device__ __forceinline__ void root_entry(const TransportParams& P, PacketU& p,
 // alternate the two registers and no instruction waits on the gather except its real use.
 // tau_rem > 0 always (u01 < 1, and a - b > 0 for a > b in IEEE arithmetic), so dtau >= tau_rem
 // implies rho*kappa > 0: no interaction in an empty leaf (R14).
-template <bool TL, int DENS>
+template <bool TL, int DENS, bool MACRO>
 __device__ __forceinline__ void walk_step_u(const TransportParams& P, const DensU& D, PacketU& p, float& cur,
                                             float& nxt, float kx, uint32_t sublut, int& state, uint32_t& crossings) {
   if (TL) {
@@ -330,7 +356,7 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, const Dens
   } else {
     p.tau_rem -= dtau;
     p.tcur = tnext;
-    ++crossings;
+    if (!MACRO) ++crossings;                                 // MACRO: counted from the ends of the flight
     if (TL) {
       uint32_t cnew = csel + 4u;
       if (leave) {
@@ -402,7 +428,13 @@ __device__ __forceinline__ void emit_position_u(const TransportParams& P, const 
 // MINBLOCKS = resident blocks per SM the kernel is compiled for: 4 (64 registers) or 5 (48
 // registers).  Five blocks hide more of the L2 latency on cache-resident grids; on HBM-resident
 // grids the extra threads thrash the L1, so the host picks per grid (profiles/).
-template <int MINBLOCKS, bool TL, int DENS>
+// signed sum of the cell coordinates along the direction of flight: a flight from cell F to cell F' crosses
+// sum_a sign(d_a) (F'_a - F_a) cell faces (per axis the motion is monotonic)
+__device__ __forceinline__ uint32_t along(const PacketU& p, int f0, int f1, int f2) {
+  return (uint32_t)((p.d0 > 0.f ? f0 : -f0) + (p.d1 > 0.f ? f1 : -f1) + (p.d2 > 0.f ? f2 : -f2));
+}
+
+template <int MINBLOCKS, bool TL, int DENS, bool MACRO>
 __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportParamsU PU) {
   const TransportParams& P = PU.base;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -459,14 +491,22 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   for (;;) {
     // ---- a7: escaped packages -> SED; a8: refill from the work queue (one atomic per warp) ----
     if (state == SU_ESCAPE) {
-      if (P.obs.n_mu | P.obs.n_pix) {                        // exit point: cube from the cursors, offset from the t's
+      if (MACRO || (P.obs.n_mu | P.obs.n_pix)) {             // exit point: cube from the cursors, offset from the t's
         int ix, iy, iz;                                      // (a package always leaves the grid at the root level)
         cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
         const float w0 = fminf(1.f, fmaxf(0.f, (p.t0 - p.tcur) * fabsf(p.d0)));
         const float w1 = fminf(1.f, fmaxf(0.f, (p.t1 - p.tcur) * fabsf(p.d1)));
         const float w2 = fminf(1.f, fmaxf(0.f, (p.t2 - p.tcur) * fabsf(p.d2)));
-        tally_observer(P, (float)ix + (p.d0 > 0.f ? 1.f - w0 : w0), (float)iy + (p.d1 > 0.f ? 1.f - w1 : w1),
-                       (float)iz + (p.d2 > 0.f ? 1.f - w2 : w2), p.d0, p.d1, p.d2, p.cb & 0xffff, p.cb >> 16);
+        const float ex = p.d0 > 0.f ? 1.f - w0 : w0, ey = p.d1 > 0.f ? 1.f - w1 : w1, ez = p.d2 > 0.f ? 1.f - w2 : w2;
+        if (MACRO) {                                         // cell coordinates where the flight ends: beyond the box on the exit axis
+          const int S = P.S;
+          const int f0 = ix >= N ? N * S : (ix < 0 ? -1 : ix * S + min(S - 1, (int)(ex * (float)S)));
+          const int f1 = iy >= N ? N * S : (iy < 0 ? -1 : iy * S + min(S - 1, (int)(ey * (float)S)));
+          const int f2 = iz >= N ? N * S : (iz < 0 ? -1 : iz * S + min(S - 1, (int)(ez * (float)S)));
+          n_cross += along(p, f0, f1, f2);
+        }
+        if (P.obs.n_mu | P.obs.n_pix)
+          tally_observer(P, (float)ix + ex, (float)iy + ey, (float)iz + ez, p.d0, p.d1, p.d2, p.cb & 0xffff, p.cb >> 16);
       }
       atomicAdd(&s_sed[(p.cb >> 16) * P.nb + (p.cb & 0xffff)], 1u);
       state = SU_FETCH;
@@ -516,7 +556,12 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
           sz = p.d2 > 0.f ? j2 : S - 1 - j2;
         } else {
           cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
+          if (MACRO) {                                       // the cell of the uniform macro cube the point lies in
+            const int S = P.S;
+            sx = min(S - 1, (int)(ux * (float)S)); sy = min(S - 1, (int)(uy * (float)S)); sz = min(S - 1, (int)(uz * (float)S));
+          }
         }
+        if (MACRO) n_cross += along(p, ix * P.S + sx, iy * P.S + sy, iz * P.S + sz);   // this flight ends here
         scatter = p.u1 < s_opac[bin].y;                      // a4 (R16)
       }
       if (scatter) {                                         // a5
@@ -540,13 +585,15 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         } else {
           ++n_abs;
           // warp-aggregated integer tally: one atomic per distinct cell per warp
-          MCRT_CHECK_SLOT(p.slot);
-          unsigned peers = __match_any_sync(__activemask(), p.slot);
+          int tslot = p.slot;
+          if (MACRO && !in_sub) tslot = P.n3 + p.slot * (P.S * P.S * P.S) + sx + P.S * (sy + P.S * sz);
+          MCRT_CHECK_SLOT(tslot);
+          unsigned peers = __match_any_sync(__activemask(), tslot);
           if ((int)lane == __ffs(peers) - 1) {
-            if (P.tally32) atomicAdd(P.tally32 + p.slot, (uint32_t)__popc(peers));
-            else atomicAdd(P.tally + p.slot, (unsigned long long)__popc(peers));
+            if (P.tally32) atomicAdd(P.tally32 + tslot, (uint32_t)__popc(peers));
+            else atomicAdd(P.tally + tslot, (unsigned long long)__popc(peers));
           }
-          float tr = __ldg(P.trow + p.slot);                 // T frozen = T before absorption
+          float tr = __ldg(P.trow + tslot);                  // T frozen = T before absorption
           int k0 = min(P.nT - 1, (int)tr);
           float w = tr - (float)k0;
           int rw = (u01(xw[1]) < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
@@ -588,6 +635,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
               const float hs = 1.f / (float)P.S;
               ux = ((float)sx + ux) * hs; uy = ((float)sy + uy) * hs; uz = ((float)sz + uz) * hs;
             }
+          } else if (MACRO) {                                // external field: the cell the entry point lies in
+            const int S = P.S;
+            sx = min(S - 1, (int)(ux * (float)S)); sy = min(S - 1, (int)(uy * (float)S)); sz = min(S - 1, (int)(uz * (float)S));
           }
           comp = 0; p.k = 0;
           atomicAdd(&s_emit[bin], 1u);
@@ -603,6 +653,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         state = SU_FETCH;
       } else {
         set_direction(p, a, b, c);
+        if (MACRO) n_cross -= along(p, ix * P.S + sx, iy * P.S + sy, iz * P.S + sz);   // ... and the next one starts here
         if (TL && in_sub) begin_flight_sub(p, lut, sublut, N, P.S, ix, iy, iz, sx, sy, sz, ux, uy, uz);
         else begin_flight(p, lut, N, ix, iy, iz, ux, uy, uz);
         float u[4];
@@ -617,9 +668,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
     // ---- a3: cell walk until fewer than `quorum` lanes are walking ----
 #pragma unroll 1
     for (;;) {
-      if (state == SU_WALK) walk_step_u<TL, DENS>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
+      if (state == SU_WALK) walk_step_u<TL, DENS, MACRO>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
       if (state == SU_WALK) {
-        walk_step_u<TL, DENS>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);
+        walk_step_u<TL, DENS, MACRO>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);
         if (state == SU_INTERACT) state = SU_INTERACT_B;
       }
       if (__popc(__ballot_sync(kFull, state == SU_WALK)) < quorum) break;
@@ -674,6 +725,37 @@ __global__ void k_encode_root(const float* __restrict__ rho_root, const int* __r
   float v = rho_root[e];
   v = (v > 0.f) ? v : 0.f;
   out[slot_of(lay, ix, iy, iz)] = k >= 0 ? __int_as_float((int)(0x80000000u | (unsigned)k)) : v;
+}
+// Macro cubes (single-level grids run as two-level ones, see MACRO in the kernel): how many M^3 blocks of
+// the caller's x-fastest density array hold one single (sanitised) value ...
+__global__ void k_count_uniform_macros(const float* __restrict__ rho_ext, int N, int M, long long nm3,
+                                       unsigned int* __restrict__ count) {
+  long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= nm3) return;
+  const int Nm = N / M;
+  const int mx = (int)(m % Nm), my = (int)((m / Nm) % Nm), mz = (int)(m / ((long long)Nm * Nm));
+  float v0 = rho_ext[(long long)mx * M + (long long)N * ((long long)my * M + (long long)N * mz * M)];
+  v0 = v0 > 0.f ? v0 : 0.f;
+  bool same = true;
+  for (int z = 0; z < M && same; ++z)
+    for (int y = 0; y < M && same; ++y)
+      for (int x = 0; x < M; ++x) {
+        float v = rho_ext[(long long)(mx * M + x) + (long long)N * ((long long)(my * M + y) + (long long)N * (mz * M + z))];
+        v = v > 0.f ? v : 0.f;
+        if (v != v0) { same = false; break; }
+      }
+  if (same) atomicAdd(count, 1u);
+}
+// ... and the macro array itself from the cells stored cube by cube: the common density, or the marker
+// (sign bit | cube number) that sends the walk down to the cells.
+__global__ void k_macro_entries(const float* __restrict__ cells, float* __restrict__ macro, long long nm3, int m3) {
+  long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= nm3) return;
+  const float* c = cells + m * m3;
+  const float v0 = c[0];
+  bool same = true;
+  for (int i = 1; i < m3; ++i) if (c[i] != v0) { same = false; break; }
+  macro[m] = same ? v0 : __int_as_float((int)(0x80000000u | (unsigned)m));
 }
 // storage order -> x-fastest output
 template <typename T>

@@ -637,11 +637,11 @@ def test_density_staged_in_shared_memory_does_not_change_results(M):
                      (W.c1(tau_v=100.0, n_packets=20_000, batch=10_000), 2),
                      (W.sphere(n_root=40, albedo=1.0, gval=0.4, n_packets=100_000, batch=50_000), 2),
                      (three, 0)):
-        a = M.from_workload(wl)
+        a = M.from_workload(wl, layout=1)                       # plain x-fastest grid (no macro cubes)
         assert a.density_staging() == (mode if mode == 1 else 0)   # the one-bit form is opt-in (measured slower)
         a.set_density_staging(2)
         assert a.density_staging() == mode, (wl.name, a.density_staging())
-        b = M.from_workload(wl)
+        b = M.from_workload(wl, layout=1)
         b.set_density_staging(1)
         assert b.density_staging() == 0
         for first, cnt in wl.batches():
@@ -649,3 +649,54 @@ def test_density_staged_in_shared_memory_does_not_change_results(M):
             b.run_batch(wl.seed, first, cnt)
         _assert_identical(a, b)
         assert a.get_counters()["emitted"] == wl.n_packets
+
+
+# ---- macro cubes: uniform blocks of cells crossed in one step --------------------
+def _blocky(n_root, block, seed, external=True, n_packets=300_000, batch=100_000):
+    """A single-level grid whose density is constant on block^3 blocks (a few of them empty), point
+    source off-centre + external field."""
+    wl = W.tiny_random(n_root=n_root, seed=seed, external=external, tau_cell=0.25, n_packets=n_packets, batch=batch)
+    rng = np.random.default_rng(seed)
+    nb = n_root // block
+    coarse = rng.random((nb, nb, nb)) * (rng.random((nb, nb, nb)) > 0.3)
+    fine = np.kron(coarse, np.ones((block, block, block)))
+    if n_root > 8:                                              # ... and one block with structure inside
+        fine[:block, :block, :block] = rng.random((block, block, block))
+    wl.rho_root = (fine.ravel() * wl.rho_root.max()).astype(np.float32)
+    return wl
+
+
+@pytest.mark.parametrize("maker,layout", [
+    (lambda: W.c1(tau_v=1.0, n_packets=600_000, batch=200_000), 0),      # automatic: 4^3 macro cubes
+    (lambda: W.c1(tau_v=10.0, n_packets=200_000, batch=50_000), 4),
+    (lambda: W.sphere(n_root=32, tau_v=3.0, gval=0.3, n_packets=400_000, batch=100_000), 3),
+    (lambda: _blocky(16, 4, 3), 3),
+    (lambda: _blocky(24, 8, 5), 4),
+    (lambda: _blocky(24, 4, 6, external=False), 3)])
+def test_macro_cubes_against_oracle_and_plain_walk(M, oracle_mod, maker, layout):
+    """Single-level grids run with macro cubes (uniform cubes of cells crossed in one step, empty space
+    skipped, crossings counted from the ends of each flight): full parity rules against the oracle,
+    and against the plain cell-by-cell walk of the same kernel the histories coincide except at
+    rounding level -- event totals within 1e-3, including the arithmetic crossings count."""
+    wl = maker()
+    a = _run_layout(M, wl, 1)                                    # plain x-fastest walk
+    b = _run_layout(M, wl, layout)
+    ca, cb = a.get_counters(), b.get_counters()
+    assert cb["emitted"] == cb["escaped"] == wl.n_packets and cb["lost"] == 0
+    assert np.array_equal(ca["emitted_per_bin"], cb["emitted_per_bin"])
+    for k in ("crossings", "absorptions", "scatterings", "flights"):
+        assert abs(ca[k] - cb[k]) <= 1e-3 * ca[k] + 20, (k, ca[k], cb[k])
+    na, nb_ = a.get_cell_energy()[0].astype(np.int64), b.get_cell_energy()[0].astype(np.int64)
+    assert len(nb_) == wl.n_root ** 3 and np.abs(na - nb_).sum() <= 2e-3 * na.sum() + 50
+    orc = oracle_mod.Oracle(wl).run()
+    _compare(b, orc, groups=PR.super_blocks(wl.n_root, 4), min_count=300)
+
+
+def test_macro_cubes_are_chosen_automatically_only_where_they_pay(M):
+    import ctypes
+    sphere = M.from_workload(W.c1(n_packets=10, batch=10))       # 64^3 sphere: 16^3 macro cubes
+    assert sphere.slots == 64 ** 3 and int(M.lib().mcrt_store_slots(sphere.h)) == 64 ** 3 + 16 ** 3
+    clumpy = M.from_workload(W.c4(n_root=24, n_packets=10, batch=10, corr_cells=3.0))
+    assert int(M.lib().mcrt_store_slots(clumpy.h)) == 24 ** 3   # no uniform cubes: plain grid
+    small = M.from_workload(W.c0(n_packets=10, batch=10))        # 16^3: 12 % uniform cubes: plain + staged
+    assert int(M.lib().mcrt_store_slots(small.h)) == 16 ** 3 and small.density_staging() == 1
