@@ -492,6 +492,8 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
     ctx.grid_create(wl.n_root, wl.sub, wl.origin, wl.root_size, wl.refine, rho, wl.rho_sub)
     ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g)
     ctx.set_source(wl.sources)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t0
     from paper_1201_3588_b200.sharding import ShardedRunner
     runner = ShardedRunner(ctx, dist if world > 1 else None)
     pending, n_read = None, 0
@@ -516,6 +518,8 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
     ctx.destroy()
     return {"value": steps * batch * world / dt, "unit": UNIT,
             "h2d_bytes_per_step": h2d_job / steps, "d2h_bytes_per_step": d2h,
+            "job_ms": 1e3 * dt, "setup_ms": 1e3 * t_setup, "steps_ms": 1e3 * (dt - t_setup),
+            "value_steps_only": steps * batch * world / (dt - t_setup),
             "what": f"one job of {steps} batches from host arrays: grid/opacity/source set-up "
                     "(H2D) + run_batch + host read-back of SED, counters, cell energy and "
                     "temperature after EVERY batch (pinned buffers; the read-out of batch k "

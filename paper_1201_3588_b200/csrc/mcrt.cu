@@ -214,11 +214,11 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
                        std::string(#call) + ": " + cudaGetErrorString(e_)));              \
   } while (0)
   CUG(cudaGetDevice(&ctx->device));
-  cudaDeviceProp prop;
-  CUG(cudaGetDeviceProperties(&prop, ctx->device));
-  if (prop.major < 10)
+  int cc_major = 0;                                          // (attributes: cudaGetDeviceProperties costs ~1 ms)
+  CUG(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, ctx->device));
+  if (cc_major < 10)
     return bail(fail(ctx, MCRT_ECUDA, "mcrt_grid_create: device is not sm_100 class (built for sm_100a only)"));
-  ctx->sm_count = prop.multiProcessorCount;
+  CUG(cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device));
   ctx->N = d->n_root;
   ctx->S = d->sub > 1 ? d->sub : 1;
   ctx->root_size = d->root_size;
