@@ -32,6 +32,11 @@
 // tests/test_oracle_observer.py): sum identity, isotropy in mu, cone fraction, hand-computed
 // projection geometry, symmetry.  O10 (serial Bjorkman-Wood scheme, tests/test_oracle_bw.py):
 // telescoping of the corrected emission to the Planck spectrum at the final temperature.
+// O11..O13 (transiently heated PAH, PAPER.md L23/L45/L49; DESIGN.md readings
+// R35..R40; tests/test_oracle_pah.py): the temperature distribution P(T) is pinned by its two
+// physical limits (strong heating -> a narrow peak at the equilibrium temperature; rare hard
+// photons -> the cooling-curve distribution C(T)/Lambda(T)), by the balance of mean heating and
+// mean cooling, and by the exact split of absorptions between PAH and equilibrium grains.
 // PARITY UNPINNED: the full multi-scattering + re-emission SED and temperatures at
 // tau_V >= 1 have no closed form and the paper's benchmarks are not
 // available; they are held only by the component pins above.
@@ -58,7 +63,8 @@ const double C_LIGHT = 2.99792458e10;
 const double K_BOLTZ = 1.380649e-16;
 const double PI = 3.14159265358979323846;
 
-const uint32_t TAG_EMIT = 0, TAG_FLIGHT = 1, TAG_REEMIT = 2;
+const uint32_t TAG_EMIT = 0, TAG_FLIGHT = 1, TAG_REEMIT = 2, TAG_PAH = 4;
+const double M_CARBON = 1.99264687992e-23;   // g, 12 amu (CODATA 2018 atomic mass constant x 12)
 const uint32_t K_MAX_FLIGHTS = 10000000u;   // R20
 const int COMP_DIRECT = 0, COMP_SCATTERED = 1, COMP_THERMAL = 2;
 
@@ -154,6 +160,17 @@ struct Ctx {
   int n_pix = 0; double obs[3] = {0, 0, 1}, e1[3] = {1, 0, 0}, e2[3] = {0, 1, 0};
   double cos_alpha = 1, half_width = 1; int img_lo = 0, img_hi = -1;
   std::vector<uint64_t> image;                              // [n_pix][n_pix], row = e2, column = e1
+  // O11..O13 (f2): transiently heated PAH, one kind per context
+  bool pah = false;
+  int nC = 0, KP = 0;                   // carbon atoms per molecule; temperature bins of P(T)
+  double fP = 0, thetaP = 0;            // mass fraction of the dust in PAH; Debye-like temperature of the enthalpy law
+  std::vector<double> kabs_all;         // [nb] absorption of the whole mix (kabs then holds the equilibrium grains only)
+  std::vector<double> kP, qP, CP, EP;   // [nb] PAH absorption per g of mix; kP / kabs_all; per molecule; photon energy
+  std::vector<double> TP, UP, LamP;     // [KP] temperature grid, enthalpy U(T_k), cooling power of one molecule
+  std::vector<double> WP;               // [KP][nb] C_j dnu_j B_j(T_k): emission of one molecule at T_k into bin j
+  std::vector<uint64_t> cumP;           // [slots][nb] PAH absorptions per leaf and bin, cumulative
+  std::vector<double> EcdfP;            // [slots][nb] emission CDF of the PAH of each leaf (frozen within a batch)
+  uint64_t pah_absorptions = 0;
   bool have_opacity = false, have_source = false;
 };
 
@@ -451,10 +468,23 @@ void run_packet(Ctx& c, uint64_t seed, uint64_t pid, std::vector<uint64_t>& batc
       rec(1, slot);
     } else {                                                     // absorb + re-emit
       loc.absorptions++;
-#pragma omp atomic
-      batch[slot] += 1;
       double r[4];
       draw4(seed, pid, k, TAG_REEMIT, r);
+      bool by_pah = false;
+      double v[4] = {0, 0, 0, 0};
+      if (c.pah) {                                               // O11 (R36): which grain absorbed the package
+        draw4(seed, pid, k, TAG_PAH, v);
+        by_pah = v[0] < c.qP[p.bin];
+      }
+      if (by_pah) {
+#pragma omp atomic
+        c.cumP[(size_t)slot * c.nb + p.bin] += 1;
+#pragma omp atomic
+        c.pah_absorptions += 1;
+        p.bin = search_cdf(&c.EcdfP[(size_t)slot * c.nb], c.nb, v[1]);   // from the leaf's P(T), frozen in the batch
+      } else {
+#pragma omp atomic
+      batch[slot] += 1;
       if (c.bw_mode) {                                             // O10: serial only
         double T_old = c.T[slot];
         c.cum[slot] += 1;
@@ -464,6 +494,7 @@ void run_packet(Ctx& c, uint64_t seed, uint64_t pid, std::vector<uint64_t>& batc
         p.bin = sample_bw_bin(c, T_old, T_new, r[0]);
       } else
       p.bin = sample_emission_bin(c, c.T[slot], r[0], r[1]);     // T frozen = T before absorption
+      }
       isotropic_dir(r[2], r[3], p.d);
       p.comp = COMP_THERMAL;
       rec(2, slot);
@@ -509,9 +540,119 @@ void update_temperatures(Ctx& c, const uint64_t* cum, uint64_t n_cum) {
     }
   }
 }
+void pah_update(Ctx& c, const uint64_t* counts, uint64_t n_cum);
 void batch_end(Ctx& c, const std::vector<uint64_t>& batch, uint64_t n_packets) {
   merge_tally(c, batch, n_packets);
   update_temperatures(c, c.cum.data(), c.Ncum);
+  if (c.pah) pah_update(c, c.cumP.data(), c.Ncum);
+}
+
+// O2: Q(T_k) and the emission CDF rows C_k[j] from c.kabs (midpoint rule R5, R11)
+void build_emission_tables(Ctx& c) {
+  const int nT = c.nT, n_bins = c.nb;
+  c.Q.assign(nT, 0); c.C.assign((size_t)nT * n_bins, 0);
+  for (int k = 0; k < nT; ++k) {
+    double T = c.Tmin * std::pow(c.Tmax / c.Tmin, (double)k / (nT - 1));
+    double acc = 0;
+    for (int j = 0; j < n_bins; ++j) {
+      acc += c.kabs[j] * planck_nu(c.nu[j], T) * c.dnu[j];
+      c.C[(size_t)k * n_bins + j] = acc;
+    }
+    c.Q[k] = acc;
+    for (int j = 0; j < n_bins; ++j)
+      c.C[(size_t)k * n_bins + j] = acc > 0 ? c.C[(size_t)k * n_bins + j] / acc : 1.0;
+    c.C[(size_t)k * n_bins + n_bins - 1] = 1.0;
+  }
+}
+
+// ---- O11 (R37): synthetic enthalpy law of a PAH with N carbon atoms.  Heat capacity
+// C(T) = 3 N k x^2/(1+x^2), x = T/Theta (quadratic at low T as for graphitic sheets, 3Nk at high T);
+// enthalpy U(T) = integral_0^T C = 3 N k Theta (x - atan x).
+double pah_heat_capacity(const Ctx& c, double T) {
+  double x = T / c.thetaP;
+  return 3.0 * c.nC * K_BOLTZ * x * x / (1.0 + x * x);
+}
+double pah_enthalpy(const Ctx& c, double T) {
+  double x = T / c.thetaP;
+  return 3.0 * c.nC * K_BOLTZ * c.thetaP * (x - std::atan(x));
+}
+
+// ---- O12 (R38): stationary temperature distribution of one PAH molecule that absorbs photons of
+// bin j at the rate R[j] (1/s).  States k = 0..K-1 with enthalpies U_k = U(T_k).
+//  * heating: a photon of energy E takes state i to the enthalpy U* = U_i + E, shared between the two
+//    states that bracket U* in proportion to the distance (mean enthalpy conserved); beyond the last
+//    state everything lands in it.  The rate from i into states >= f is therefore
+//        B(f,i) = sum_j R_j clamp((U_i + E_j - U_{f-1}) / (U_f - U_{f-1}), 0, 1)        (f > i);
+//    photons too soft to reach the next state act as continuous heating (the same formula).
+//  * cooling: only to the next lower state, A(f-1,f) = Lambda(T_f) / (U_f - U_{f-1})
+//    ("thermal continuous" cooling of Guhathakurta & Draine 1989, as in Kruegel's treatment).
+//  * stationarity in that case is the recursion X_0 = 1, X_f = sum_{i<f} B(f,i) X_i / A(f-1,f),
+//    P = X / sum X (all terms positive; X is rescaled when it grows large).
+void pah_temperature_distribution(const Ctx& c, const double* R, double* P) {
+  const int K = c.KP, nb = c.nb;
+  std::vector<double> X(K, 0.0);
+  X[0] = 1.0;
+  for (int f = 1; f < K; ++f) {
+    const double dU = c.UP[f] - c.UP[f - 1];
+    double sum = 0;
+    for (int i = 0; i < f; ++i) {
+      if (X[i] == 0) continue;
+      double B = 0;
+      for (int j = 0; j < nb; ++j) {
+        if (R[j] == 0) continue;
+        double w = (c.UP[i] + c.EP[j] - c.UP[f - 1]) / dU;
+        B += R[j] * std::min(1.0, std::max(0.0, w));
+      }
+      sum += B * X[i];
+    }
+    X[f] = sum / (c.LamP[f] / dU);
+    if (X[f] > 1e200) for (int i = 0; i <= f; ++i) X[i] *= 1e-200;
+  }
+  double tot = 0;
+  for (int k = 0; k < K; ++k) tot += X[k];
+  for (int k = 0; k < K; ++k) P[k] = X[k] / tot;
+}
+
+// photon absorption rates (1/s) of one PAH molecule of leaf `slot` from cumulative counts (R40):
+// counts_j * (L_tot / N_cum) / (h nu_j) / (number of molecules in the leaf)
+bool pah_rates(const Ctx& c, int64_t slot, const uint64_t* counts, uint64_t n_cum, double* R) {
+  double m = leaf_mass(c, slot);
+  bool any = false;
+  for (int j = 0; j < c.nb; ++j) { R[j] = 0; any = any || counts[j] > 0; }
+  if (!(m > 0) || !any || n_cum == 0) return false;
+  double n_mol = c.fP * m / (c.nC * M_CARBON);
+  for (int j = 0; j < c.nb; ++j)
+    R[j] = (double)counts[j] * c.Ltot / ((double)n_cum * c.EP[j] * n_mol);
+  return true;
+}
+
+// ---- O13 (R39): emission CDF of the PAH of a leaf from P(T): E_j = sum_k P_k C_j dnu_j B_j(T_k)
+void pah_emission_cdf(const Ctx& c, const double* P, double* cdf) {
+  const int K = c.KP, nb = c.nb;
+  double acc = 0;
+  for (int j = 0; j < nb; ++j) {
+    double e = 0;
+    for (int k = 0; k < K; ++k) e += P[k] * c.WP[(size_t)k * nb + j];
+    acc += e;
+    cdf[j] = acc;
+  }
+  for (int j = 0; j < nb; ++j) cdf[j] = acc > 0 ? cdf[j] / acc : 1.0;
+  cdf[nb - 1] = 1.0;
+}
+
+// batch end for the PAH: P(T) and emission CDF of every leaf from counts after n_cum packages
+void pah_update(Ctx& c, const uint64_t* counts, uint64_t n_cum) {
+  const int nb = c.nb, K = c.KP;
+#pragma omp parallel
+  {
+    std::vector<double> R(nb), P(K);
+#pragma omp for schedule(dynamic, 64)
+    for (int64_t i = 0; i < c.slots; ++i) {
+      if (!pah_rates(c, i, counts + (size_t)i * nb, n_cum, R.data())) continue;   // cold row stays
+      pah_temperature_distribution(c, R.data(), P.data());
+      pah_emission_cdf(c, P.data(), &c.EcdfP[(size_t)i * nb]);
+    }
+  }
 }
 
 }  // namespace
@@ -576,19 +717,7 @@ int orc_set_opacity(void* h, int n_bins, const double* lambda_edges_um, int n_sp
     c.alb[j] = c.kext[j] > 0 ? c.ksca[j] / c.kext[j] : 0.0;
     c.g[j] = c.ksca[j] > 0 ? gs / c.ksca[j] : 0.0;
   }
-  c.Q.assign(nT, 0); c.C.assign((size_t)nT * n_bins, 0);
-  for (int k = 0; k < nT; ++k) {
-    double T = Tmin * std::pow(Tmax / Tmin, (double)k / (nT - 1));
-    double acc = 0;
-    for (int j = 0; j < n_bins; ++j) {
-      acc += c.kabs[j] * planck_nu(c.nu[j], T) * c.dnu[j];
-      c.C[(size_t)k * n_bins + j] = acc;
-    }
-    c.Q[k] = acc;
-    for (int j = 0; j < n_bins; ++j)
-      c.C[(size_t)k * n_bins + j] = acc > 0 ? c.C[(size_t)k * n_bins + j] / acc : 1.0;
-    c.C[(size_t)k * n_bins + n_bins - 1] = 1.0;
-  }
+  build_emission_tables(c);
   c.sed.assign((size_t)3 * n_bins, 0);
   c.emitted_per_bin.assign(n_bins, 0);
   c.have_opacity = true;
@@ -658,6 +787,83 @@ int orc_update_temperature(void* h, const uint64_t* tally_sum, uint64_t n_cum) {
   if (!c.have_source || !tally_sum || n_cum == 0) return -2;
   update_temperatures(c, tally_sum, n_cum);
   return 0;
+}
+
+// O11: declare the PAH (one kind per context).  kabs_pah[nb] = absorption of the PAH per gram of the dust MIX
+// (it must be part of the mix given to orc_set_opacity: clipped to the mix's kappa_abs).  The equilibrium
+// tables Q(T), C_k are rebuilt from what is left for the grains in equilibrium.  Temperature grid of P(T):
+// K log-spaced values T_lo..T_hi.
+void pah_cold_rows(Ctx& c) {
+  std::vector<double> P(c.KP, 0.0), row(c.nb);
+  P[0] = 1.0;
+  pah_emission_cdf(c, P.data(), row.data());
+  c.EcdfP.assign((size_t)c.slots * c.nb, 0.0);
+  for (int64_t i = 0; i < c.slots; ++i) std::copy(row.begin(), row.end(), c.EcdfP.begin() + (size_t)i * c.nb);
+}
+int orc_set_pah(void* h, int n_C, double mass_fraction, double theta_K, const float* kabs_pah, double T_lo,
+                double T_hi, int K) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.have_opacity || n_C < 1 || !(mass_fraction > 0) || !(theta_K > 0) || K < 4 || !(T_lo > 0) || !(T_hi > T_lo))
+    return -1;
+  const int nb = c.nb;
+  if (c.kabs_all.empty()) c.kabs_all = c.kabs;
+  c.pah = true; c.nC = n_C; c.fP = mass_fraction; c.thetaP = theta_K; c.KP = K;
+  c.kP.assign(nb, 0); c.qP.assign(nb, 0); c.CP.assign(nb, 0); c.EP.assign(nb, 0);
+  for (int j = 0; j < nb; ++j) {
+    c.kP[j] = std::min((double)kabs_pah[j], c.kabs_all[j]);
+    if (!(c.kP[j] > 0)) c.kP[j] = 0;
+    c.kabs[j] = c.kabs_all[j] - c.kP[j];                       // grains in equilibrium
+    c.qP[j] = c.kabs_all[j] > 0 ? c.kP[j] / c.kabs_all[j] : 0.0;
+    c.CP[j] = c.kP[j] * n_C * M_CARBON / mass_fraction;        // cm^2 per molecule
+    c.EP[j] = H_PLANCK * c.nu[j];
+  }
+  build_emission_tables(c);
+  c.TP.resize(K); c.UP.resize(K); c.LamP.resize(K); c.WP.assign((size_t)K * nb, 0);
+  for (int k = 0; k < K; ++k) {
+    c.TP[k] = T_lo * std::pow(T_hi / T_lo, (double)k / (K - 1));
+    c.UP[k] = pah_enthalpy(c, c.TP[k]);
+    double lam = 0;
+    for (int j = 0; j < nb; ++j) {
+      double w = c.CP[j] * planck_nu(c.nu[j], c.TP[k]) * c.dnu[j];
+      c.WP[(size_t)k * nb + j] = w;
+      lam += w;
+    }
+    c.LamP[k] = 4.0 * PI * lam;
+  }
+  c.cumP.assign((size_t)c.slots * nb, 0);
+  c.pah_absorptions = 0;
+  pah_cold_rows(c);
+  return 0;
+}
+void orc_get_pah_grid(void* h, double* T, double* U, double* Lam, double* Cmol, double* q) {
+  Ctx& c = *(Ctx*)h;
+  for (int k = 0; k < c.KP; ++k) { T[k] = c.TP[k]; U[k] = c.UP[k]; Lam[k] = c.LamP[k]; }
+  for (int j = 0; j < c.nb; ++j) { Cmol[j] = c.CP[j]; q[j] = c.qP[j]; }
+}
+// O12 / O13 as component entry points (pins), and for the tallies of another implementation (parity)
+void orc_pah_solve(void* h, const double* R, double* P, double* cdf) {
+  Ctx& c = *(Ctx*)h;
+  pah_temperature_distribution(c, R, P);
+  if (cdf) pah_emission_cdf(c, P, cdf);
+}
+int orc_pah_rates(void* h, int64_t slot, const uint64_t* counts, uint64_t n_cum, double* R) {
+  return pah_rates(*(Ctx*)h, slot, counts, n_cum, R) ? 1 : 0;
+}
+void orc_pah_update(void* h, const uint64_t* counts, uint64_t n_cum) {
+  Ctx& c = *(Ctx*)h;
+  pah_cold_rows(c);
+  pah_update(c, counts, n_cum);
+}
+double orc_pah_enthalpy(void* h, double T) { return pah_enthalpy(*(Ctx*)h, T); }
+double orc_pah_heat_capacity(void* h, double T) { return pah_heat_capacity(*(Ctx*)h, T); }
+void orc_get_pah_absorbed(void* h, uint64_t* out, uint64_t* total) {
+  Ctx& c = *(Ctx*)h;
+  std::memcpy(out, c.cumP.data(), sizeof(uint64_t) * c.cumP.size());
+  if (total) *total = c.pah_absorptions;
+}
+void orc_get_pah_cdf(void* h, double* out) {
+  Ctx& c = *(Ctx*)h;
+  std::memcpy(out, c.EcdfP.data(), sizeof(double) * c.EcdfP.size());
 }
 
 // O9: observer set-up.  dir need not be normalised; half_width in cm; n_mu = 0 / n_pix = 0 switch
@@ -775,7 +981,8 @@ void orc_reset_tallies(void* h, int what) {
                   std::fill(c.emitted_per_bin.begin(), c.emitted_per_bin.end(), 0); c.cnt = Counters{};
                   std::fill(c.sed_mu.begin(), c.sed_mu.end(), 0); std::fill(c.image.begin(), c.image.end(), 0); }
   if (what & 2) { std::fill(c.cum.begin(), c.cum.end(), 0); std::fill(c.T.begin(), c.T.end(), c.Tmin);
-                  c.Ncum = 0; }
+                  c.Ncum = 0;
+                  if (c.pah) { std::fill(c.cumP.begin(), c.cumP.end(), 0); c.pah_absorptions = 0; pah_cold_rows(c); } }
 }
 void orc_get_tables(void* h, double* nu, double* dnu, double* kabs, double* kext, double* alb,
                     double* g, double* Q, double* C) {

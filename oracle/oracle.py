@@ -91,6 +91,18 @@ def lib():
         L.orc_emit.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64] + [C.c_void_p] * 4
         L.orc_walk.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int,
                                C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_set_pah.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_double,
+                                  C.c_double, C.c_int]
+        L.orc_get_pah_grid.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+        L.orc_pah_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_pah_rates.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_uint64, C.c_void_p]
+        L.orc_pah_update.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
+        L.orc_pah_enthalpy.restype = C.c_double
+        L.orc_pah_enthalpy.argtypes = [C.c_void_p, C.c_double]
+        L.orc_pah_heat_capacity.restype = C.c_double
+        L.orc_pah_heat_capacity.argtypes = [C.c_void_p, C.c_double]
+        L.orc_get_pah_absorbed.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_get_pah_cdf.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_max_threads.restype = C.c_int
     return _lib
 
@@ -140,6 +152,55 @@ class Oracle:
         if getattr(self, "h", None):
             lib().orc_destroy(self.h)
             self.h = None
+
+    # ---- O11..O13: transiently heated PAH ----
+    def set_pah(self, n_C, mass_fraction, kabs_pah, theta_K=500.0, T_lo=5.0, T_hi=1.0e4, n_Tp=128):
+        k = np.ascontiguousarray(kabs_pah, dtype=np.float32)
+        assert k.shape == (self.nb,)
+        rc = lib().orc_set_pah(self.h, int(n_C), float(mass_fraction), float(theta_K), _p(k), float(T_lo),
+                               float(T_hi), int(n_Tp))
+        assert rc == 0
+        self.n_Tp = int(n_Tp)
+
+    def pah_grid(self):
+        T, U, Lam = np.zeros(self.n_Tp), np.zeros(self.n_Tp), np.zeros(self.n_Tp)
+        Cmol, q = np.zeros(self.nb), np.zeros(self.nb)
+        lib().orc_get_pah_grid(self.h, _p(T), _p(U), _p(Lam), _p(Cmol), _p(q))
+        return dict(T=T, U=U, Lam=Lam, Cmol=Cmol, q=q)
+
+    def pah_solve(self, R):
+        R = np.ascontiguousarray(R, dtype=np.float64)
+        P, cdf = np.zeros(self.n_Tp), np.zeros(self.nb)
+        lib().orc_pah_solve(self.h, _p(R), _p(P), _p(cdf))
+        return P, cdf
+
+    def pah_rates(self, slot, counts, n_cum):
+        c = np.ascontiguousarray(counts, dtype=np.uint64)
+        R = np.zeros(self.nb)
+        ok = lib().orc_pah_rates(self.h, int(slot), _p(c), int(n_cum), _p(R))
+        return R if ok else None
+
+    def pah_update(self, counts, n_cum):
+        c = np.ascontiguousarray(counts, dtype=np.uint64)
+        assert c.size == self.slots * self.nb
+        lib().orc_pah_update(self.h, _p(c), int(n_cum))
+
+    def pah_enthalpy(self, T):
+        return lib().orc_pah_enthalpy(self.h, float(T))
+
+    def pah_heat_capacity(self, T):
+        return lib().orc_pah_heat_capacity(self.h, float(T))
+
+    def pah_absorbed(self):
+        out = np.zeros((self.slots, self.nb), dtype=np.uint64)
+        tot = C.c_uint64(0)
+        lib().orc_get_pah_absorbed(self.h, _p(out), C.byref(tot))
+        return out, tot.value
+
+    def pah_cdf(self):
+        out = np.zeros((self.slots, self.nb))
+        lib().orc_get_pah_cdf(self.h, _p(out))
+        return out
 
     def set_walker(self, w: int):
         lib().orc_set_walker(self.h, w)

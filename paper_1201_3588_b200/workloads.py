@@ -351,3 +351,31 @@ def tiny_random(n_root=2, sub=0, n_refined=0, seed=0, tau_cell=0.7, albedo=0.5, 
                     root_size=h, refine=refine, rho_root=rho_root, rho_sub=rho_sub,
                     lambda_edges_um=edges, weight=w, kabs=kabs, ksca=ksca, g=g, sources=srcs,
                     n_packets=n_packets, batch=batch, seed=seed + 1)
+
+
+# ---------------------------------------------------------------------------------------
+# transiently heated PAH: input description only
+# ---------------------------------------------------------------------------------------
+@dataclass
+class Pah:
+    n_C: int                 # carbon atoms per molecule
+    mass_fraction: float     # of the dust mass
+    kabs: np.ndarray         # float32 [n_bins] absorption of the PAH per gram of the dust MIX (part of the mix's kappa_abs)
+    theta_K: float = 500.0   # temperature scale of the synthetic enthalpy law (R37)
+    T_lo: float = 5.0
+    T_hi: float = 1.0e4
+    n_Tp: int = 128
+
+
+def pah_share(wl: Workload, n_C=100, mass_fraction=0.05, uv_share=0.4, band_share=0.2) -> Pah:
+    """A synthetic PAH living inside the workload's dust mix: it takes `uv_share` of the mix's
+    absorption below 0.4 micron, falling off towards the visible, plus `band_share` in 17
+    Lorentzian bands between 3.3 and 20 micron (the shape of BASELINE.json configs[2]; the real
+    cross-sections and band table are not available)."""
+    lam = lambda_centres(wl.lambda_edges_um)
+    kmix = (np.asarray(wl.weight, np.float64)[:, None] * wl.kabs.astype(np.float64)).sum(axis=0)
+    bands = 3.3 * (20.0 / 3.3) ** (np.arange(17) / 16.0)
+    share = uv_share / (1.0 + (lam / 0.4) ** 4) + band_share * np.clip(
+        sum(lorentz(lam, lk, 0.03 * lk) for lk in bands), 0.0, 1.0)
+    return Pah(n_C=n_C, mass_fraction=mass_fraction,
+               kabs=(np.clip(share, 0.0, 1.0) * kmix).astype(np.float32))
