@@ -246,6 +246,45 @@ mcrt_status mcrt_set_observer(mcrt_ctx* ctx, const mcrt_observer_desc* desc);
 mcrt_status mcrt_get_sed_mu(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
 mcrt_status mcrt_get_image(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
 
+/* ---- transiently heated PAH (the method is "extended to the treatment of transiently
+ * heated PAHs"; L45 Fig. 3: their temperature distribution P(T); L49: "P(T) depends strongly on the
+ * hardness and spectral shape of the exciting radiation field"; DESIGN.md
+ * readings R35..R40 -- the paper prints no formula, the cited book and the PAH data are not
+ * available) ------------------------------------------------------------------------------------
+ * One PAH kind per context, declared AFTER mcrt_set_opacity as a part of that dust mix:
+ * kabs_pah[n_bins] = absorption of the PAH in cm^2 per gram of the MIX (clipped to the mix's
+ * kappa_abs).  The grains in equilibrium keep the rest: Q(T) and the emission rows are rebuilt
+ * from it.  From then on an absorbed package is taken by the PAH with probability kappa_PAH,j /
+ * kappa_abs,j (R36); it is booked on the leaf's absorbed spectrum (per leaf and bin) and
+ * re-emitted from the leaf's PAH emission spectrum.  After every batch each leaf's absorbed
+ * spectrum gives the photon absorption rates of one molecule (R40: counts * L_tot / N_cum / h nu /
+ * molecules in the leaf, a molecule = n_C carbon atoms, the PAH hold mass_fraction of the dust
+ * mass), its stationary temperature distribution P(T_k) on n_Tp log-spaced temperatures (R38:
+ * enthalpy U(T) = 3 n_C k theta (x - atan x), x = T/theta (R37); photon jumps shared linearly
+ * between the two bracketing states; cooling to the next lower state at the rate
+ * 4 pi sum_j C_j B_j(T) dnu_j / (U_k - U_k-1)), and the emission CDF sum_k P_k C_j B_j(T_k) dnu_j
+ * (R39).  n_Tp = 0 takes the defaults 128 states, 5 K .. 1e4 K; theta_K <= 0 takes 500 K.
+ * Calling mcrt_set_opacity again drops the PAH; mcrt_reset_tallies(bit 1) zeroes its tallies.
+ * Host pointers.  Not combined with mcrt_transport_batch_delta yet (MCRT_ESTATE). */
+typedef struct {
+  int32_t n_C;            /* carbon atoms per molecule, >= 1                                    */
+  double mass_fraction;   /* of the dust mass, (0, 1]                                           */
+  const float* kabs_pah;  /* [n_bins] cm^2 per gram of the dust mix                             */
+  double theta_K;         /* temperature scale of the enthalpy law                              */
+  double T_lo, T_hi;      /* K: range of the states                                             */
+  int32_t n_Tp;           /* number of states, 4..1024 (0 = defaults)                           */
+} mcrt_pah_desc;
+mcrt_status mcrt_set_pah(mcrt_ctx* ctx, const mcrt_pah_desc* desc);
+/* counts_out[leaf slots][n_bins]: packages absorbed by the PAH per leaf and bin, cumulative (they
+ * are NOT in mcrt_get_cell_energy, which counts the grains in equilibrium; the counter
+ * `absorptions` counts both). */
+mcrt_status mcrt_get_pah_absorbed(mcrt_ctx* ctx, uint32_t* counts_out, mcrt_mem mem);
+/* cdf_out[leaf slots][n_bins]: the emission CDF the PAH of each leaf re-emits from in the next batch. */
+mcrt_status mcrt_get_pah_emission_cdf(mcrt_ctx* ctx, float* cdf_out, mcrt_mem mem);
+/* P(T) of the PAH of one leaf from its tallies so far: P_out[n_Tp] on the temperatures T_out[n_Tp]
+ * (host pointers; T_out may be NULL). */
+mcrt_status mcrt_get_pah_temperature_distribution(mcrt_ctx* ctx, int64_t leaf_slot, double* T_out, double* P_out);
+
 /* ---- tuning and introspection (do not change results) ---------------------------------------
  * Launch shape of the transport kernel: threads per block (multiple of 32, <= 256; 0 keeps the
  * current value) and resident blocks per SM (0 = automatic: 5, or 4 for a single-level grid larger

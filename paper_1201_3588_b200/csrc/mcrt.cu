@@ -18,6 +18,7 @@
 #include "tables.cuh"
 #include "transport.cuh"
 #include "transport_u.cuh"
+#include "pah.cuh"
 
 using namespace mcrt;
 
@@ -89,6 +90,14 @@ struct mcrt_ctx {
   } tickets[2];
   int next_ticket = 0;
   cudaStream_t copy_stream = nullptr;
+  // transiently heated PAH (row f2, pah.cuh): tables and the per-leaf, per-bin tallies / emission CDFs
+  bool pah = false;
+  PahDev pahd = {};
+  double *d_kabs_eq = nullptr, *d_pah_C = nullptr, *d_pah_E = nullptr, *d_pah_T = nullptr, *d_pah_U = nullptr,
+         *d_pah_Lam = nullptr, *d_pah_W = nullptr, *d_pah_P = nullptr;
+  int* d_pah_J = nullptr;
+  float *d_pah_q = nullptr, *d_pah_cdf = nullptr, *d_pah_cold = nullptr;
+  uint32_t* d_pah_cnt = nullptr;
   bool have_opacity = false, have_source = false;
   std::string err;
 };
@@ -112,6 +121,14 @@ static void free_opacity(mcrt_ctx* c) {
   cudaFree(c->d_lnQ); cudaFree(c->d_cdf); cudaFree(c->d_small); cudaFree(c->d_guide);
   c->d_nu = c->d_dnu = c->d_kabs = nullptr; c->d_opac = nullptr; c->d_lnQ = c->d_cdf = nullptr; c->d_guide = nullptr;
   c->d_small = nullptr;
+}
+static void free_pah(mcrt_ctx* c) {
+  cudaFree(c->d_kabs_eq); cudaFree(c->d_pah_C); cudaFree(c->d_pah_E); cudaFree(c->d_pah_T); cudaFree(c->d_pah_U);
+  cudaFree(c->d_pah_Lam); cudaFree(c->d_pah_W); cudaFree(c->d_pah_P); cudaFree(c->d_pah_J); cudaFree(c->d_pah_q);
+  cudaFree(c->d_pah_cdf); cudaFree(c->d_pah_cold); cudaFree(c->d_pah_cnt);
+  c->d_kabs_eq = c->d_pah_C = c->d_pah_E = c->d_pah_T = c->d_pah_U = c->d_pah_Lam = c->d_pah_W = c->d_pah_P = nullptr;
+  c->d_pah_J = nullptr; c->d_pah_q = c->d_pah_cdf = c->d_pah_cold = nullptr; c->d_pah_cnt = nullptr;
+  c->pah = false;
 }
 static void free_observer(mcrt_ctx* c) {
   cudaFree(c->obs.sed_mu); cudaFree(c->obs.image);
@@ -413,6 +430,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   }
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   free_opacity(ctx);
+  free_pah(ctx);
   free_sources(ctx);
   free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
@@ -445,6 +463,7 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
     return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: bad temperature table");
   CU(cudaDeviceSynchronize());
   free_opacity(ctx);
+  free_pah(ctx);                                            // a PAH is declared against an opacity set
   free_sources(ctx);
   free_observer(ctx);                                       // its tallies are sized by n_bins
   ctx->have_opacity = ctx->have_source = false;
@@ -562,6 +581,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
   P.seed = seed; P.first = first; P.count = n;
   P.obs = ctx->obs;
+  P.pah_q = ctx->pah ? ctx->d_pah_q : nullptr; P.pah_cnt = ctx->d_pah_cnt; P.pah_cdf = ctx->d_pah_cdf;
   P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->store_n3;
 #ifdef MCRT_CHECKS
   CU(cudaMemcpyToSymbolAsync(g_mcrt_nstore, &ctx->store_slots, sizeof(long long), 0, cudaMemcpyHostToDevice, st));
@@ -624,6 +644,29 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   return MCRT_OK;
 }
 
+// a9 for the PAH (pah.cuh): P(T) and emission CDF of every leaf from its absorbed spectrum
+static size_t pah_smem_bytes(const mcrt_ctx* ctx, int warps) {
+  return sizeof(double) * (size_t)warps * (2 * (size_t)ctx->nb + ctx->pahd.K);
+}
+static mcrt_status launch_pah_update(mcrt_ctx* ctx, uint64_t n_cum, cudaStream_t st, long long only_slot) {
+  if (n_cum == 0) return MCRT_OK;
+  int warps = 4;
+  while (warps > 1 && pah_smem_bytes(ctx, warps) > (96u << 10)) warps >>= 1;
+  const size_t smem = pah_smem_bytes(ctx, warps);
+  if (smem > (48u << 10)) CU(cudaFuncSetAttribute(k_pah_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const double V = ctx->root_size * ctx->root_size * ctx->root_size;
+  const double s3 = (double)ctx->S * ctx->S * ctx->S;
+  long long blocks = only_slot >= 0 ? 1 : (ctx->store_slots + warps - 1) / warps;
+  const long long cap = (long long)ctx->sm_count * 16;
+  if (blocks > cap) blocks = cap;
+  k_pah_update<<<(unsigned)blocks, 32 * (only_slot >= 0 ? 1 : warps), smem, st>>>(
+      ctx->pahd, ctx->d_rho, ctx->d_pah_cnt, ctx->d_pah_cdf, ctx->store_slots,
+      ctx->uni ? ctx->store_slots : ctx->store_n3, ctx->Ltot / (double)n_cum, V, 1.0 / s3, only_slot, ctx->d_pah_P);
+  ctx->launches++;
+  CU(cudaGetLastError());
+  return MCRT_OK;
+}
+
 // a9: T from `tally` (the context's own cumulative tally, or a caller's device array that
 // holds the sum over ranks) and n_cum packages emitted so far in the whole job.
 // delta != NULL: first add the batch's counts (u32, storage order, summed over ranks) to the context's tally.
@@ -657,6 +700,7 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
                                                                      ctx->store_slots, n3, ln_coef, ln_sub3);
   ctx->launches++;
   CU(cudaGetLastError());
+  if (ctx->pah) return launch_pah_update(ctx, n_cum, st, -1);
   return MCRT_OK;
 }
 
@@ -726,6 +770,7 @@ mcrt_status mcrt_transport_batch_delta(mcrt_ctx* ctx, uint64_t seed, uint64_t fi
   if (!ctx) return MCRT_EINVAL;
   if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_transport_batch_delta: grid, opacity and sources must be set first");
   if (!delta_dev) return fail(ctx, MCRT_EINVAL, "mcrt_transport_batch_delta: NULL delta buffer");
+  if (ctx->pah) return fail(ctx, MCRT_ESTATE, "mcrt_transport_batch_delta: packet-sharded batches do not carry the PAH tallies yet");
   cudaStream_t st = (cudaStream_t)stream_;
   BatchEvents ev;
   mcrt_status rc = begin_batch(ctx, &ev);
@@ -812,6 +857,143 @@ mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem) {
   if (!counts_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_sed: NULL output");
   if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_sed: opacity not set");
   return copy_out(ctx, counts_out, ctx->d_small + 1 + CNT_N, 8 * 3 * (size_t)ctx->nb, mem);
+}
+
+// ---- transiently heated PAH (row f2) --------------------------------------------------------------
+static mcrt_status pah_reset_rows(mcrt_ctx* ctx) {
+  const long long n = ctx->store_slots * (long long)ctx->nb;
+  CU(cudaMemset(ctx->d_pah_cnt, 0, sizeof(uint32_t) * (size_t)n));
+  k_pah_fill_rows<<<(unsigned)((n + 255) / 256), 256>>>(ctx->d_pah_cold, ctx->d_pah_cdf, ctx->store_slots, ctx->nb);
+  ctx->launches++;
+  CU(cudaGetLastError());
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_set_pah(mcrt_ctx* ctx, const mcrt_pah_desc* d) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!d || !d->kabs_pah) return fail(ctx, MCRT_EINVAL, "mcrt_set_pah: NULL argument");
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_set_pah: call mcrt_set_opacity first");
+  int K = d->n_Tp;
+  double T_lo = d->T_lo, T_hi = d->T_hi, theta = d->theta_K;
+  if (K == 0) { K = 128; T_lo = 5.0; T_hi = 1.0e4; }
+  if (!(theta > 0)) theta = 500.0;
+  if (d->n_C < 1 || !(d->mass_fraction > 0) || d->mass_fraction > 1 || K < 4 || K > 1024 || !(T_lo > 0) || !(T_hi > T_lo))
+    return fail(ctx, MCRT_EINVAL, "mcrt_set_pah: n_C >= 1, 0 < mass_fraction <= 1, 4 <= n_Tp <= 1024, 0 < T_lo < T_hi");
+  if ((double)ctx->store_slots * ctx->nb >= 4.0e9)
+    return fail(ctx, MCRT_EINVAL, "mcrt_set_pah: leaf slots x n_bins must stay below 4e9 (per-leaf spectra)");
+  CU(cudaDeviceSynchronize());
+  free_pah(ctx);
+  const int nb = ctx->nb;
+  float* d_in = nullptr;
+  struct Tmp { float*& a; ~Tmp() { cudaFree(a); } } tmp{d_in};
+  CU(cudaMalloc(&d_in, 4 * (size_t)nb));
+  CU(cudaMemcpy(d_in, d->kabs_pah, 4 * (size_t)nb, cudaMemcpyHostToDevice));
+  CU(cudaMalloc(&ctx->d_kabs_eq, 8 * (size_t)nb)); CU(cudaMalloc(&ctx->d_pah_q, 4 * (size_t)nb));
+  CU(cudaMalloc(&ctx->d_pah_C, 8 * (size_t)nb)); CU(cudaMalloc(&ctx->d_pah_E, 8 * (size_t)nb));
+  CU(cudaMalloc(&ctx->d_pah_T, 8 * (size_t)K)); CU(cudaMalloc(&ctx->d_pah_U, 8 * (size_t)K));
+  CU(cudaMalloc(&ctx->d_pah_Lam, 8 * (size_t)K)); CU(cudaMalloc(&ctx->d_pah_P, 8 * (size_t)K));
+  CU(cudaMalloc(&ctx->d_pah_W, 8 * (size_t)K * nb)); CU(cudaMalloc(&ctx->d_pah_J, sizeof(int) * (size_t)K * K));
+  CU(cudaMalloc(&ctx->d_pah_cold, 4 * (size_t)nb));
+  CU(cudaMalloc(&ctx->d_pah_cnt, sizeof(uint32_t) * (size_t)ctx->store_slots * nb));
+  CU(cudaMalloc(&ctx->d_pah_cdf, sizeof(float) * (size_t)ctx->store_slots * nb));
+  k_pah_split<<<(nb + 127) / 128, 128>>>(nb, ctx->d_kabs, d_in, ctx->d_nu, d->n_C, d->mass_fraction, ctx->d_kabs_eq,
+                                         ctx->d_pah_q, ctx->d_pah_C, ctx->d_pah_E);
+  // the equilibrium tables from what is left for the grains in equilibrium (R35)
+  k_build_emission_rows<<<ctx->nT, 128, 8 * (nb + 1)>>>(nb, ctx->nT, ctx->Tmin, ctx->Tmax, ctx->d_nu, ctx->d_dnu,
+                                                        ctx->d_kabs_eq, ctx->d_lnQ, ctx->d_cdf);
+  k_build_guide<<<kGuide / 256, 256>>>(ctx->d_lnQ, ctx->nT, ctx->d_guide);
+  k_pah_states<<<K, 128>>>(nb, K, T_lo, T_hi, d->n_C, theta, ctx->d_nu, ctx->d_dnu, ctx->d_pah_C, ctx->d_pah_T,
+                           ctx->d_pah_U, ctx->d_pah_Lam, ctx->d_pah_W);
+  k_pah_thresholds<<<(K * K + 255) / 256, 256>>>(nb, K, ctx->d_pah_E, ctx->d_pah_U, ctx->d_pah_J);
+  k_pah_cold_row<<<1, 32>>>(nb, ctx->d_pah_W, ctx->d_pah_cold);
+  ctx->launches += 6;
+  CU(cudaGetLastError());
+  ctx->pahd.nC = d->n_C; ctx->pahd.K = K; ctx->pahd.nb = nb; ctx->pahd.fP = d->mass_fraction; ctx->pahd.theta = theta;
+  ctx->pahd.E = ctx->d_pah_E; ctx->pahd.U = ctx->d_pah_U; ctx->pahd.Lam = ctx->d_pah_Lam; ctx->pahd.W = ctx->d_pah_W;
+  ctx->pahd.J = ctx->d_pah_J;
+  mcrt_status rc = pah_reset_rows(ctx);
+  if (rc != MCRT_OK) return rc;
+  CU(cudaDeviceSynchronize());
+  ctx->pah = true;
+  return MCRT_OK;
+}
+
+}  // extern "C" (templates follow)
+
+// per-leaf rows of n_bins values: storage order -> the caller's slot order
+template <typename T>
+static mcrt_status rows_to_api(mcrt_ctx* ctx, const T* store, T* out, cudaStream_t st) {
+  const int nb = ctx->nb;
+  if (ctx->macro) {
+    const long long nf3 = ctx->slots;
+    k_rows_store_to_ext<T><<<(unsigned)((nf3 * nb + 255) / 256), 256, 0, st>>>(store + (size_t)ctx->store_n3 * nb, out, ctx->lay_fine, nf3, nb);
+  } else {
+    k_rows_store_to_ext<T><<<(unsigned)((ctx->n3 * nb + 255) / 256), 256, 0, st>>>(store, out, ctx->lay, ctx->n3, nb);
+    if (ctx->slots > ctx->n3)
+      CU(cudaMemcpyAsync(out + (size_t)ctx->n3 * nb, store + (size_t)ctx->store_n3 * nb,
+                         sizeof(T) * (size_t)(ctx->slots - ctx->n3) * nb, cudaMemcpyDeviceToDevice, st));
+  }
+  ctx->launches++;
+  CU(cudaGetLastError());
+  return MCRT_OK;
+}
+template <typename T>
+static mcrt_status get_rows(mcrt_ctx* ctx, const T* store, T* out, mcrt_mem mem) {
+  const size_t bytes = sizeof(T) * (size_t)ctx->slots * ctx->nb;
+  T* d_out = out;
+  T* tmp = nullptr;
+  struct Tmp { T*& a; ~Tmp() { cudaFree(a); } } guard{tmp};
+  if (mem == MCRT_HOST) { CU(cudaMalloc(&tmp, bytes)); d_out = tmp; }
+  mcrt_status rc = rows_to_api<T>(ctx, store, d_out, ctx->last_stream);
+  if (rc != MCRT_OK) return rc;
+  if (mem == MCRT_HOST) return copy_out(ctx, out, tmp, bytes, MCRT_HOST);
+  return sync_last(ctx);
+}
+
+extern "C" {
+
+mcrt_status mcrt_get_pah_absorbed(mcrt_ctx* ctx, uint32_t* counts_out, mcrt_mem mem) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!counts_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_pah_absorbed: NULL output");
+  if (!ctx->pah) return fail(ctx, MCRT_ESTATE, "mcrt_get_pah_absorbed: no PAH declared (mcrt_set_pah)");
+  return get_rows<uint32_t>(ctx, ctx->d_pah_cnt, counts_out, mem);
+}
+
+mcrt_status mcrt_get_pah_emission_cdf(mcrt_ctx* ctx, float* cdf_out, mcrt_mem mem) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!cdf_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_pah_emission_cdf: NULL output");
+  if (!ctx->pah) return fail(ctx, MCRT_ESTATE, "mcrt_get_pah_emission_cdf: no PAH declared (mcrt_set_pah)");
+  return get_rows<float>(ctx, ctx->d_pah_cdf, cdf_out, mem);
+}
+
+// storage slot of a leaf slot of the caller's order (R22)
+static long long storage_slot_of(const mcrt_ctx* ctx, long long api) {
+  if (ctx->macro) {
+    const int N = ctx->n_fine;
+    return ctx->store_n3 + slot_of(ctx->lay_fine, (int)(api % N), (int)((api / N) % N), (int)(api / ((long long)N * N)));
+  }
+  if (api >= ctx->n3) return ctx->store_n3 + (api - ctx->n3);
+  const int N = ctx->N;
+  return slot_of(ctx->lay, (int)(api % N), (int)((api / N) % N), (int)(api / ((long long)N * N)));
+}
+
+mcrt_status mcrt_get_pah_temperature_distribution(mcrt_ctx* ctx, int64_t leaf_slot, double* T_out, double* P_out) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!ctx->pah) return fail(ctx, MCRT_ESTATE, "mcrt_get_pah_temperature_distribution: no PAH declared (mcrt_set_pah)");
+  if (leaf_slot < 0 || leaf_slot >= ctx->slots || !P_out) return fail(ctx, MCRT_EINVAL, "mcrt_get_pah_temperature_distribution: bad slot / NULL");
+  const int K = ctx->pahd.K;
+  const unsigned long long n_cum = ctx->Nglobal > ctx->Ncum ? ctx->Nglobal : ctx->Ncum;
+  std::vector<double> P(K, 0.0);
+  P[0] = 1.0;                                                // nothing absorbed yet: the ground state
+  CU(cudaMemcpyAsync(ctx->d_pah_P, P.data(), 8 * (size_t)K, cudaMemcpyHostToDevice, ctx->last_stream));
+  if (n_cum) {
+    mcrt_status rc = launch_pah_update(ctx, n_cum, ctx->last_stream, storage_slot_of(ctx, leaf_slot));
+    if (rc != MCRT_OK) return rc;
+  }
+  mcrt_status rc = copy_out(ctx, P_out, ctx->d_pah_P, 8 * (size_t)K, MCRT_HOST);
+  if (rc != MCRT_OK) return rc;
+  if (T_out) return copy_out(ctx, T_out, ctx->d_pah_T, 8 * (size_t)K, MCRT_HOST);
+  return MCRT_OK;
 }
 
 // ---- combined / asynchronous read-out ----------------------------------------------------------
@@ -985,6 +1167,7 @@ mcrt_status mcrt_reset_tallies(mcrt_ctx* ctx, int32_t what) {
     CU(cudaMemset(ctx->d_trow, 0, 4 * (size_t)ctx->store_slots));
     ctx->Ncum = 0;
     ctx->Nglobal = 0;
+    if (ctx->pah) { mcrt_status rc = pah_reset_rows(ctx); if (rc != MCRT_OK) return rc; CU(cudaDeviceSynchronize()); }
   }
   return MCRT_OK;
 }

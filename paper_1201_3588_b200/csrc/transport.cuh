@@ -24,7 +24,7 @@ __device__ long long g_mcrt_nstore = 0;
 #define MCRT_CHECK_SLOT(s) do { } while (0)
 #endif
 
-constexpr uint32_t kTagEmit = 0, kTagFlight = 1, kTagReemit = 2;
+constexpr uint32_t kTagEmit = 0, kTagFlight = 1, kTagReemit = 2, kTagPah = 4;
 constexpr uint32_t kMaxFlights = 10000000u;          // R20
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -59,6 +59,10 @@ struct TransportParams {
                                                // instruction stream as the re-emission rows ...
   const double* __restrict__ csrc64;           // ... and the fp64 table that settles the bin exactly
   const SrcDev* __restrict__ src;              // [nsrc]
+  // transiently heated PAH (row f2, pah.cuh); pah_q = NULL: no PAH declared
+  const float* __restrict__ pah_q;             // [nb] share of an absorption taken by the PAH (R36)
+  uint32_t* __restrict__ pah_cnt;              // [slots][nb] packages absorbed by the PAH, per leaf and bin
+  const float* __restrict__ pah_cdf;           // [slots][nb] emission CDF of each leaf's PAH (frozen in a batch)
   unsigned long long* next;                    // work-queue head (packet offset within the batch)
   const uint32_t* __restrict__ perm;           // NULL, or the batch's package numbers grouped by source
   unsigned long long* sed;                     // [3][nb]

@@ -584,21 +584,34 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
           us = (float)u01d(xw[1]);
         } else {
           ++n_abs;
-          // warp-aggregated integer tally: one atomic per distinct cell per warp
           int tslot = p.slot;
           if (MACRO && !in_sub) tslot = P.n3 + p.slot * (P.S * P.S * P.S) + sx + P.S * (sy + P.S * sz);
           MCRT_CHECK_SLOT(tslot);
-          unsigned peers = __match_any_sync(__activemask(), tslot);
-          if ((int)lane == __ffs(peers) - 1) {
-            if (P.tally32) atomicAdd(P.tally32 + tslot, (uint32_t)__popc(peers));
-            else atomicAdd(P.tally + tslot, (unsigned long long)__popc(peers));
+          bool by_pah = false;
+          if (P.pah_q) {                                     // R36: which grain took the package
+            uint32_t vw[4];
+            draw4w(P.seed, pid, p.k, kTagPah, vw);
+            by_pah = u01(vw[0]) < __ldg(P.pah_q + bin);
+            if (by_pah) {                                    // booked on the leaf's absorbed spectrum; re-emitted
+              atomicAdd(P.pah_cnt + (size_t)tslot * P.nb + bin, 1u);      // from the leaf's P(T) (frozen)
+              row = P.pah_cdf + (size_t)tslot * P.nb;
+              us = u01(vw[1]);
+            }
           }
-          float tr = __ldg(P.trow + tslot);                  // T frozen = T before absorption
-          int k0 = min(P.nT - 1, (int)tr);
-          float w = tr - (float)k0;
-          int rw = (u01(xw[1]) < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
-          row = P.cdf + (size_t)rw * P.nb;
-          us = u01(xw[0]);
+          if (!by_pah) {
+            // warp-aggregated integer tally: one atomic per distinct cell per warp
+            unsigned peers = __match_any_sync(__activemask(), tslot);
+            if ((int)lane == __ffs(peers) - 1) {
+              if (P.tally32) atomicAdd(P.tally32 + tslot, (uint32_t)__popc(peers));
+              else atomicAdd(P.tally + tslot, (unsigned long long)__popc(peers));
+            }
+            float tr = __ldg(P.trow + tslot);                // T frozen = T before absorption
+            int k0 = min(P.nT - 1, (int)tr);
+            float w = tr - (float)k0;
+            int rw = (u01(xw[1]) < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
+            row = P.cdf + (size_t)rw * P.nb;
+            us = u01(xw[0]);
+          }
         }
         bin = search_cdf<float>(row, P.nb, us);              // one search loop for emission and re-emission
         if (is_new) {

@@ -48,6 +48,11 @@ class _Counters(C.Structure):
                                           "scatterings", "flights", "crossings")]
 
 
+class _PahDesc(C.Structure):
+    _fields_ = [("n_C", C.c_int32), ("mass_fraction", C.c_double), ("kabs_pah", C.c_void_p),
+                ("theta_K", C.c_double), ("T_lo", C.c_double), ("T_hi", C.c_double), ("n_Tp", C.c_int32)]
+
+
 class _Results(C.Structure):
     _fields_ = [("n_abs", C.c_void_p), ("T", C.c_void_p), ("sed", C.c_void_p),
                 ("emitted_per_bin", C.c_void_p), ("counters", C.POINTER(_Counters)),
@@ -60,7 +65,8 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_update_temperature", "mcrt_store_slots", "mcrt_transport_batch_delta",
            "mcrt_accumulate_update", "mcrt_get_results", "mcrt_results_begin", "mcrt_results_wait",
            "mcrt_get_cell_energy",
-           "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_observer",
+           "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_pah", "mcrt_get_pah_absorbed",
+           "mcrt_get_pah_emission_cdf", "mcrt_get_pah_temperature_distribution", "mcrt_set_observer",
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
            "mcrt_set_density_staging", "mcrt_density_staging",
@@ -97,6 +103,10 @@ def lib():
         L.mcrt_get_cell_energy.argtypes = [vp, vp, C.POINTER(C.c_double), C.c_int]
         L.mcrt_get_cell_temperature.argtypes = [vp, vp, C.c_int]
         L.mcrt_get_sed.argtypes = [vp, vp, C.c_int]
+        L.mcrt_set_pah.argtypes = [vp, C.POINTER(_PahDesc)]
+        L.mcrt_get_pah_absorbed.argtypes = [vp, vp, C.c_int]
+        L.mcrt_get_pah_emission_cdf.argtypes = [vp, vp, C.c_int]
+        L.mcrt_get_pah_temperature_distribution.argtypes = [vp, i64, vp, vp]
         L.mcrt_set_observer.argtypes = [vp, C.POINTER(_ObserverDesc)]
         L.mcrt_get_sed_mu.argtypes = [vp, vp, C.c_int]
         L.mcrt_get_image.argtypes = [vp, vp, C.c_int]
@@ -124,7 +134,9 @@ def lib():
         for name in ("mcrt_grid_create", "mcrt_destroy", "mcrt_set_opacity", "mcrt_set_source",
                      "mcrt_run_batch", "mcrt_transport_batch", "mcrt_update_temperature",
                      "mcrt_transport_batch_delta", "mcrt_accumulate_update", "mcrt_get_results",
-                     "mcrt_results_begin", "mcrt_results_wait", "mcrt_get_cell_energy", "mcrt_get_cell_temperature",
+                     "mcrt_results_begin", "mcrt_results_wait", "mcrt_get_cell_energy", "mcrt_set_pah",
+                     "mcrt_get_pah_absorbed", "mcrt_get_pah_emission_cdf",
+                     "mcrt_get_pah_temperature_distribution", "mcrt_get_cell_temperature",
                      "mcrt_get_sed", "mcrt_set_observer", "mcrt_get_sed_mu", "mcrt_get_image",
                      "mcrt_get_counters", "mcrt_reset_tallies",
                      "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
@@ -214,6 +226,32 @@ class Context:
         self.n_bins = d.n_bins
         self.n_T = n_T if n_T > 0 else 801
         return self
+
+    def set_pah(self, n_C, mass_fraction, kabs_pah, theta_K=500.0, T_lo=5.0, T_hi=1.0e4, n_Tp=128):
+        """Declare the transiently heated PAH (after set_opacity)."""
+        k = np.ascontiguousarray(kabs_pah, dtype=np.float32)
+        d = _PahDesc()
+        d.n_C, d.mass_fraction, d.kabs_pah = int(n_C), float(mass_fraction), _np_ptr(k)
+        d.theta_K, d.T_lo, d.T_hi, d.n_Tp = float(theta_K), float(T_lo), float(T_hi), int(n_Tp)
+        self._check(lib().mcrt_set_pah(self.h, C.byref(d)), "mcrt_set_pah")
+        self.n_Tp = int(n_Tp) if n_Tp else 128
+        return self
+
+    def get_pah_absorbed(self, device=False):
+        out, p, mem = self._out((self.slots, self.n_bins), np.uint32, device)
+        self._check(lib().mcrt_get_pah_absorbed(self.h, p, mem), "mcrt_get_pah_absorbed")
+        return out
+
+    def get_pah_emission_cdf(self, device=False):
+        out, p, mem = self._out((self.slots, self.n_bins), np.float32, device)
+        self._check(lib().mcrt_get_pah_emission_cdf(self.h, p, mem), "mcrt_get_pah_emission_cdf")
+        return out
+
+    def get_pah_temperature_distribution(self, leaf_slot):
+        T, P = np.zeros(self.n_Tp), np.zeros(self.n_Tp)
+        self._check(lib().mcrt_get_pah_temperature_distribution(self.h, int(leaf_slot), _np_ptr(T), _np_ptr(P)),
+                    "mcrt_get_pah_temperature_distribution")
+        return T, P
 
     def set_source(self, sources):
         arr = (_Source * len(sources))()
@@ -312,7 +350,8 @@ class Context:
         if device:
             import torch
             t = torch.empty(shape, dtype=getattr(torch, np.dtype(np_dtype).name
-                                                 .replace("uint64", "int64")), device="cuda")
+                                                 .replace("uint64", "int64").replace("uint32", "int32")),
+                            device="cuda")
             return t, C.c_void_p(t.data_ptr()), MCRT_DEVICE
         if out is not None:
             if out.shape != tuple(shape) or out.dtype != np.dtype(np_dtype) or not out.flags.c_contiguous:
