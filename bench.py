@@ -112,15 +112,32 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def ncu_traffic(name):
-    """DRAM bytes per k_transport launch from the committed ncu capture of this workload."""
+def ncu_capture(name):
+    """What the committed ncu --set full capture of this workload says about one k_transport_u launch
+    (profiles/traffic.json): DRAM bytes, warp instructions, lanes per instruction; {} if none."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(p):
         with open(p) as f:
             t = json.load(f).get(name)
-        if t:
-            return float(t["bytes_per_launch"])
-    return None
+        if isinstance(t, dict):
+            return t
+    return {}
+
+
+def ncu_traffic(name):
+    t = ncu_capture(name).get("bytes_per_launch")
+    return float(t) if t else None
+
+
+def issue_peak():
+    """Issue-slot ceiling of the GPU in warp instructions per second: SMs x 4 warp schedulers x 1
+    instruction per clock x the maximum SM clock (B200_PROFILING.md: 148 SMs, 1965 MHz)."""
+    mhz = 1965.0
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            mhz = float(json.load(f).get("sm_max_mhz", mhz))
+    return 148 * 4 * mhz * 1e6
 
 
 def measured_peaks():
@@ -292,8 +309,22 @@ def rooflines(wl, name, d, tr_s, steps, gather_peak):
                           "of k_transport_u.  A fraction above 1 means the walk's locality (bricks, grouped "
                           "hand-out) lets one sector serve several crossings: then it is no ceiling and the "
                           "hbm figures are the ones that bound"}
+    cap = ncu_capture(name)
     resident = foot <= 0.75 * L2_BYTES
-    if resident and gather:
+    if cap.get("warp_instructions_per_launch") and name != "c4":
+        # The committed capture of this workload shows what binds it: the issue slots (75-85 % busy, DRAM at
+        # a few per cent, L1TEX wavefronts well below their peak).  achieved = the capture's warp instructions
+        # per launch / the kernel time measured HERE; peak = SMs x 4 schedulers x max clock.
+        ipl = float(cap["warp_instructions_per_launch"])
+        ach = ipl / (tr_s / steps) / 1e9 if tr_s > 0 else 0.0
+        pk = issue_peak() / 1e9
+        roof = {"bound": "alu", "kernel": "k_transport_u", "achieved": ach, "peak": pk, "unit": "G warp instructions/s",
+                "frac": ach / pk, "traffic": hbm["traffic"],
+                "peak_source": "148 SMs x 4 warp schedulers x 1 instruction/clock x sm_max_mhz (MEASURED_PEAKS.json)",
+                "instructions_per_launch_from_capture": ipl, "lanes_per_instruction": cap.get("lanes_per_instruction"),
+                "useful_lane_frac": (ach / pk) * float(cap.get("lanes_per_instruction", 32.0)) / 32.0,
+                "kernel_ms": 1e3 * tr_s / steps, "hbm": hbm}
+    elif resident and gather:
         roof = {"bound": "l1tex-gather", "kernel": "k_transport_u", "achieved": 4e-9 * gather["achieved_gathers_per_s"],
                 "peak": 4e-9 * gather_peak, "unit": "GB/s", "frac": gather["frac"], "traffic": hbm["traffic"],
                 "peak_source": "calibrated live: scattered 4-byte gathers over the density footprint x 4 B "
