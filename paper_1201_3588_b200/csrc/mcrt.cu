@@ -195,7 +195,7 @@ static mcrt_status trow_to_api_T(mcrt_ctx* ctx, float* out, cudaStream_t st) {
 // what the next launch uses: the one-bit form only on request (it measured 3 % SLOWER than global gathers on
 // the 64^3 sphere: the walk is bound by instruction issue, not by the gathers; profiles/r02_summary.md)
 static int staging_mode(const mcrt_ctx* ctx) {
-  if (ctx->dens_off == 1) return 0;
+  if (ctx->dens_off == 1 || ctx->pah) return 0;              // (the PAH instances of the kernel gather from global memory)
   if (ctx->dens_mode == 2 && ctx->dens_off != 2) return 0;
   return ctx->dens_mode;
 }
@@ -625,13 +625,16 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   const int dens = staging_mode(ctx);
   PU.stage = dens == 1 ? (const void*)ctx->d_rho : (const void*)ctx->d_bits;
   PU.stage_bytes = ctx->stage_bytes; PU.pal0 = ctx->pal0; PU.pal1 = ctx->pal1;
-  const bool five = bps * threads > 1024;                    // 48-register build (5 blocks of 256) or 64-register build
+  const bool five = bps * threads > 1024 && !ctx->pah;      // 48-register build (5 blocks of 256) or 64-register build
   void (*kern)(TransportParamsU) =
-      ctx->macro ? (five ? k_transport_u<5, true, 0, true> : k_transport_u<4, true, 0, true>)
-      : !ctx->uni ? (five ? k_transport_u<5, true, 0, false> : k_transport_u<4, true, 0, false>)
-      : dens == 1 ? k_transport_u<5, false, 1, false>
-      : dens == 2 ? k_transport_u<5, false, 2, false>
-                  : (five ? k_transport_u<5, false, 0, false> : k_transport_u<4, false, 0, false>);
+      ctx->pah ? (ctx->macro ? k_transport_u<4, true, 0, true, true>              // PAH instances: 64-register builds,
+                  : !ctx->uni ? k_transport_u<4, true, 0, false, true>            // global gathers
+                              : k_transport_u<4, false, 0, false, true>)
+      : ctx->macro ? (five ? k_transport_u<5, true, 0, true, false> : k_transport_u<4, true, 0, true, false>)
+      : !ctx->uni ? (five ? k_transport_u<5, true, 0, false, false> : k_transport_u<4, true, 0, false, false>)
+      : dens == 1 ? k_transport_u<5, false, 1, false, false>
+      : dens == 2 ? k_transport_u<5, false, 2, false, false>
+                  : (five ? k_transport_u<5, false, 0, false, false> : k_transport_u<4, false, 0, false, false>);
   if (smem > (48u << 10)) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   if (dens) CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   int resident = 0;                                          // large tables (many bins) lower the residency:

@@ -434,7 +434,10 @@ __device__ __forceinline__ uint32_t along(const PacketU& p, int f0, int f1, int 
   return (uint32_t)((p.d0 > 0.f ? f0 : -f0) + (p.d1 > 0.f ? f1 : -f1) + (p.d2 > 0.f ? f2 : -f2));
 }
 
-template <int MINBLOCKS, bool TL, int DENS, bool MACRO>
+// PAH: the instance that knows the transiently heated PAH (row f2).  A template parameter, not a run-time
+// branch: the third Philox block in the event pass costs registers and spills in every instance that
+// contains it (C2 3.38 -> 3.52 ms per launch when it was compiled into all of them).
+template <int MINBLOCKS, bool TL, int DENS, bool MACRO, bool PAH>
 __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportParamsU PU) {
   const TransportParams& P = PU.base;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -588,7 +591,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
           if (MACRO && !in_sub) tslot = P.n3 + p.slot * (P.S * P.S * P.S) + sx + P.S * (sy + P.S * sz);
           MCRT_CHECK_SLOT(tslot);
           bool by_pah = false;
-          if (P.pah_q) {                                     // R36: which grain took the package
+          if (PAH) {                                         // R36: which grain took the package
             uint32_t vw[4];
             draw4w(P.seed, pid, p.k, kTagPah, vw);
             by_pah = u01(vw[0]) < __ldg(P.pah_q + bin);
