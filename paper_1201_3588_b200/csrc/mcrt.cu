@@ -96,7 +96,7 @@ struct mcrt_ctx {
   double *d_kabs_eq = nullptr, *d_pah_C = nullptr, *d_pah_E = nullptr, *d_pah_T = nullptr, *d_pah_U = nullptr,
          *d_pah_Lam = nullptr, *d_pah_W = nullptr, *d_pah_P = nullptr;
   int* d_pah_J = nullptr;
-  float *d_pah_q = nullptr, *d_pah_cdf = nullptr, *d_pah_cold = nullptr;
+  float *d_pah_q = nullptr, *d_pah_cdf = nullptr, *d_pah_cold = nullptr, *d_pah_W32 = nullptr;
   uint32_t* d_pah_cnt = nullptr;
   bool have_opacity = false, have_source = false;
   std::string err;
@@ -125,7 +125,8 @@ static void free_opacity(mcrt_ctx* c) {
 static void free_pah(mcrt_ctx* c) {
   cudaFree(c->d_kabs_eq); cudaFree(c->d_pah_C); cudaFree(c->d_pah_E); cudaFree(c->d_pah_T); cudaFree(c->d_pah_U);
   cudaFree(c->d_pah_Lam); cudaFree(c->d_pah_W); cudaFree(c->d_pah_P); cudaFree(c->d_pah_J); cudaFree(c->d_pah_q);
-  cudaFree(c->d_pah_cdf); cudaFree(c->d_pah_cold); cudaFree(c->d_pah_cnt);
+  cudaFree(c->d_pah_cdf); cudaFree(c->d_pah_cold); cudaFree(c->d_pah_cnt); cudaFree(c->d_pah_W32);
+  c->d_pah_W32 = nullptr;
   c->d_kabs_eq = c->d_pah_C = c->d_pah_E = c->d_pah_T = c->d_pah_U = c->d_pah_Lam = c->d_pah_W = c->d_pah_P = nullptr;
   c->d_pah_J = nullptr; c->d_pah_q = c->d_pah_cdf = c->d_pah_cold = nullptr; c->d_pah_cnt = nullptr;
   c->pah = false;
@@ -896,6 +897,7 @@ mcrt_status mcrt_set_pah(mcrt_ctx* ctx, const mcrt_pah_desc* d) {
   CU(cudaMalloc(&ctx->d_pah_T, 8 * (size_t)K)); CU(cudaMalloc(&ctx->d_pah_U, 8 * (size_t)K));
   CU(cudaMalloc(&ctx->d_pah_Lam, 8 * (size_t)K)); CU(cudaMalloc(&ctx->d_pah_P, 8 * (size_t)K));
   CU(cudaMalloc(&ctx->d_pah_W, 8 * (size_t)K * nb)); CU(cudaMalloc(&ctx->d_pah_J, sizeof(int) * (size_t)K * K));
+  CU(cudaMalloc(&ctx->d_pah_W32, 4 * (size_t)K * nb));
   CU(cudaMalloc(&ctx->d_pah_cold, 4 * (size_t)nb));
   CU(cudaMalloc(&ctx->d_pah_cnt, sizeof(uint32_t) * (size_t)ctx->store_slots * nb));
   CU(cudaMalloc(&ctx->d_pah_cdf, sizeof(float) * (size_t)ctx->store_slots * nb));
@@ -906,14 +908,14 @@ mcrt_status mcrt_set_pah(mcrt_ctx* ctx, const mcrt_pah_desc* d) {
                                                         ctx->d_kabs_eq, ctx->d_lnQ, ctx->d_cdf);
   k_build_guide<<<kGuide / 256, 256>>>(ctx->d_lnQ, ctx->nT, ctx->d_guide);
   k_pah_states<<<K, 128>>>(nb, K, T_lo, T_hi, d->n_C, theta, ctx->d_nu, ctx->d_dnu, ctx->d_pah_C, ctx->d_pah_T,
-                           ctx->d_pah_U, ctx->d_pah_Lam, ctx->d_pah_W);
+                           ctx->d_pah_U, ctx->d_pah_Lam, ctx->d_pah_W, ctx->d_pah_W32);
   k_pah_thresholds<<<(K * K + 255) / 256, 256>>>(nb, K, ctx->d_pah_E, ctx->d_pah_U, ctx->d_pah_J);
   k_pah_cold_row<<<1, 32>>>(nb, ctx->d_pah_W, ctx->d_pah_cold);
   ctx->launches += 6;
   CU(cudaGetLastError());
   ctx->pahd.nC = d->n_C; ctx->pahd.K = K; ctx->pahd.nb = nb; ctx->pahd.fP = d->mass_fraction; ctx->pahd.theta = theta;
   ctx->pahd.E = ctx->d_pah_E; ctx->pahd.U = ctx->d_pah_U; ctx->pahd.Lam = ctx->d_pah_Lam; ctx->pahd.W = ctx->d_pah_W;
-  ctx->pahd.J = ctx->d_pah_J;
+  ctx->pahd.J = ctx->d_pah_J; ctx->pahd.W32 = ctx->d_pah_W32;
   mcrt_status rc = pah_reset_rows(ctx);
   if (rc != MCRT_OK) return rc;
   CU(cudaDeviceSynchronize());

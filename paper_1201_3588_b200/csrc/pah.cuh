@@ -27,6 +27,7 @@ struct PahDev {
   const double* __restrict__ U;       // [K] enthalpy of state k
   const double* __restrict__ Lam;     // [K] cooling power of one molecule in state k
   const double* __restrict__ W;       // [K][nb] C_j dnu_j B_j(T_k)
+  const float* __restrict__ W32;      // the same rounded to fp32 (emission sums of the fast kernel: 6e-8 relative)
   const int* __restrict__ J;          // [K][K] J[f][i] = number of bins with E_j >= U_f - U_i (f > i)
 };
 
@@ -54,10 +55,14 @@ __global__ void k_pah_split(int nb, const double* __restrict__ kabs_all, const f
 __global__ void k_pah_states(int nb, int K, double T_lo, double T_hi, int nC, double theta,
                              const double* __restrict__ nu, const double* __restrict__ dnu,
                              const double* __restrict__ Cmol, double* __restrict__ Tk, double* __restrict__ U,
-                             double* __restrict__ Lam, double* __restrict__ W) {
+                             double* __restrict__ Lam, double* __restrict__ W, float* __restrict__ W32) {
   const int k = blockIdx.x;
   const double T = T_lo * pow(T_hi / T_lo, (double)k / (double)(K - 1));
-  for (int j = threadIdx.x; j < nb; j += blockDim.x) W[(size_t)k * nb + j] = Cmol[j] * planck_nu(nu[j], T) * dnu[j];
+  for (int j = threadIdx.x; j < nb; j += blockDim.x) {
+    const double w = Cmol[j] * planck_nu(nu[j], T) * dnu[j];
+    W[(size_t)k * nb + j] = w;
+    W32[(size_t)k * nb + j] = (float)w;
+  }
   __syncthreads();
   if (threadIdx.x == 0) {
     double acc = 0;
@@ -174,11 +179,24 @@ __global__ void __launch_bounds__(128) k_pah_update(const PahDev D, const float*
     __syncwarp();
     float* row = cdf + (size_t)s * nb;
     double etot = 0;
-    for (int j = lane; j < nb; j += 32) {
-      double e = 0;
-      for (int k = 0; k < K; ++k) e += X[k] * D.W[(size_t)k * nb + j];
-      cumN[j] = e;
-      etot += e;
+    for (int j0 = 4 * lane; j0 < nb; j0 += 128) {            // W rounded to fp32 (L1-resident), four bins per lane and turn
+      double e0 = 0, e1 = 0, e2 = 0, e3 = 0;
+      if (j0 + 3 < nb && (nb & 3) == 0) {
+        for (int k = 0; k < K; ++k) {
+          const double pk = X[k];
+          const float4 w = __ldg(reinterpret_cast<const float4*>(D.W32 + (size_t)k * nb + j0));
+          e0 += pk * (double)w.x; e1 += pk * (double)w.y; e2 += pk * (double)w.z; e3 += pk * (double)w.w;
+        }
+        cumN[j0] = e0; cumN[j0 + 1] = e1; cumN[j0 + 2] = e2; cumN[j0 + 3] = e3;
+        etot += (e0 + e1) + (e2 + e3);
+      } else {
+        for (int j = j0; j < min(nb, j0 + 4); ++j) {
+          double e = 0;
+          for (int k = 0; k < K; ++k) e += X[k] * (double)__ldg(D.W32 + (size_t)k * nb + j);
+          cumN[j] = e;
+          etot += e;
+        }
+      }
     }
     etot = warp_sum(etot);
     __syncwarp();
