@@ -296,6 +296,13 @@ mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t bl
  * (long free flights -> keep more lanes walking).  A scheduling knob only: results do not depend
  * on it. */
 mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum);
+/* Region sweeps (single-level grids of at least 256^3 cells in the brick layout, batches of at least 2^20
+ * packages): the batch is transported in `sweeps` + 1 passes; in all but the last a package that crosses
+ * into another region of 128^3 cells is suspended (48 bytes of state) and continues in the next pass,
+ * where the waiting packages are handed out region by region, so that the cells the packages in flight
+ * visit stay in the L2; the last pass finishes whatever is left.  -1 = automatic (the default: 6), 0 =
+ * off, 1..30.  Results do not depend on it (integer tallies, the state is restored exactly). */
+mcrt_status mcrt_set_region_sweeps(mcrt_ctx* ctx, int32_t sweeps);
 /* Density kept in shared memory (single-level grids): a density array of at most 40 KB is copied
  * into every block's shared memory by one bulk copy (cp.async.bulk) and a crossing reads shared
  * memory instead of the L2 (C0: -10 % per launch).  mode 0 = automatic (the default), 1 = off

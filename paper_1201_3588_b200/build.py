@@ -16,7 +16,11 @@ INCLUDE = os.path.join(_ROOT, "include")
 LIB_PATH = os.path.join(_HERE, "libmcrt.so")
 CHECKS_LIB_PATH = os.path.join(_HERE, "libmcrt_checks.so")      # same sources with -DMCRT_CHECKS
 
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+# -fmad=false: no implicit contraction of a*b+c into FMA.  Which products the compiler fuses differs from one
+# template instance of the transport kernel to the next (it did between the swept and the unswept instance:
+# one crossing in 2.3e8), and every knob of the library promises bit-identical results; the fused operations
+# the kernels want are written as fmaf().
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
               "-Xcompiler", "-fPIC", "-shared"]
 
 

@@ -70,6 +70,14 @@ struct mcrt_ctx {
   int order_by_source = -1;               // -1 automatic, 0 off, 1 by source, 2 by source and start direction
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 0;                         // 0 = automatic (from the job's crossings per flight so far)
+  // region sweeps (transport_u.cuh, REGION): single-level bricked grids far larger than the L2
+  int region_cells = 0, region_sweeps = -1;   // cells per region edge (0: grid does not qualify); -1 automatic, 0 off
+  int *d_lut_marked = nullptr, *d_lut_plain2 = nullptr;     // [12 N]: marked | plain root tables; plain | plain
+  float4* d_rec = nullptr;                // [perm_cap][3] suspended packages
+  unsigned long long* d_list[2] = {nullptr, nullptr};       // suspended packages of a sweep: region << 32 | number
+  unsigned int* d_swcnt = nullptr;        // [kMaxSweeps + 2] packages suspended in each sweep
+  unsigned int* d_regcnt = nullptr;       // [2][regions] histogram, cursors
+  unsigned long long rec_cap = 0;
   // density staged in shared memory (single-level grids): 0 none, 1 the fp32 array itself, 2 one bit per slot
   int dens_mode = 0, dens_off = 0;        // dens_off: the caller switched staging off (mcrt_set_density_staging)
   uint32_t* d_bits = nullptr;
@@ -200,8 +208,8 @@ static int staging_mode(const mcrt_ctx* ctx) {
   if (ctx->dens_mode == 2 && ctx->dens_off != 2) return 0;
   return ctx->dens_mode;
 }
-static size_t transport_smem_bytes(const mcrt_ctx* ctx) {
-  const size_t n_lut = ctx->uni ? 6 * (size_t)ctx->N : (size_t)lut_sub_offset(ctx->N) + 6 * kSubStride;
+static size_t transport_smem_bytes(const mcrt_ctx* ctx, bool region = false) {
+  const size_t n_lut = ctx->uni ? (region ? 12 : 6) * (size_t)ctx->N : (size_t)lut_sub_offset(ctx->N) + 6 * kSubStride;
   size_t b = ((32 * (size_t)ctx->nb + 63) & ~(size_t)63) + sizeof(int) * n_lut;
   if (staging_mode(ctx)) b = ((b + 127) & ~(size_t)127) + ctx->stage_bytes + 16;   // staged density + its mbarrier
   return b;
@@ -356,6 +364,24 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     }
     CUG(cudaMalloc(&ctx->d_lut, sizeof(int) * lut.size()));
     CUG(cudaMemcpy(ctx->d_lut, lut.data(), sizeof(int) * lut.size(), cudaMemcpyHostToDevice));
+    // Region sweeps for single-level bricked grids of at least 256^3 cells (four times the L2 and more): the root
+    // tables once more with a marker on every step that crosses a boundary between regions of 128^3 cells.
+    constexpr int kRegionCells = 128;
+    if (ctx->uni && ctx->lay.bricked == 1 && N >= 2 * kRegionCells && N % kRegionCells == 0) {
+      ctx->region_cells = kRegionCells;
+      std::vector<int> marked(12 * (size_t)N), plain2(12 * (size_t)N);
+      for (size_t i = 0; i < 6 * (size_t)N; ++i) { marked[i] = lut[i]; marked[6 * (size_t)N + i] = lut[i]; plain2[i] = lut[i]; plain2[6 * (size_t)N + i] = lut[i]; }
+      for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < N; ++i) {
+          if (i != N - 1 && (i + 1) % kRegionCells == 0) marked[(size_t)(2 * a) * N + i] = kLutRegion;      // i -> i+1
+          const int ir = N - 1 - i;
+          if (ir != 0 && ir % kRegionCells == 0) marked[(size_t)(2 * a + 1) * N + i] = kLutRegion;          // ir -> ir-1
+        }
+      CUG(cudaMalloc(&ctx->d_lut_marked, sizeof(int) * marked.size()));
+      CUG(cudaMalloc(&ctx->d_lut_plain2, sizeof(int) * plain2.size()));
+      CUG(cudaMemcpy(ctx->d_lut_marked, marked.data(), sizeof(int) * marked.size(), cudaMemcpyHostToDevice));
+      CUG(cudaMemcpy(ctx->d_lut_plain2, plain2.data(), sizeof(int) * plain2.size(), cudaMemcpyHostToDevice));
+    }
     CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
     if (ctx->macro) {
       // the cells cube by cube behind the macro array; then one entry per macro cube: its density if all
@@ -435,7 +461,9 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_sources(ctx);
   free_observer(ctx);
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
-  cudaFree(ctx->d_lut); cudaFree(ctx->d_bits); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
+  cudaFree(ctx->d_lut); cudaFree(ctx->d_lut_marked); cudaFree(ctx->d_lut_plain2); cudaFree(ctx->d_rec);
+  cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]); cudaFree(ctx->d_swcnt); cudaFree(ctx->d_regcnt);
+  cudaFree(ctx->d_bits); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -565,6 +593,8 @@ static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
   return MCRT_OK;
 }
 
+static bool tally32_is_unsupported(const uint32_t*) { return false; }   // (sweeps work with either tally)
+
 static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st,
                                     uint32_t* tally32 = nullptr) {
   if (n == 0) return MCRT_OK;
@@ -620,22 +650,54 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   long long want = ((long long)n + threads - 1) / threads;
   long long grid = (long long)ctx->sm_count * bps;
   if (want < grid) grid = want;
-  const size_t smem = transport_smem_bytes(ctx);
+  // region sweeps: automatic for qualifying grids and batches of at least 2^20 packages
+  constexpr int kMaxSweeps = 30;
+  int sweeps = 0;
+  if (ctx->region_cells && !ctx->pah && !tally32_is_unsupported(tally32)) {
+    if (ctx->region_sweeps < 0) sweeps = n >= (1ull << 20) ? 8 : 0;          // automatic
+    else sweeps = ctx->region_sweeps > kMaxSweeps ? kMaxSweeps : ctx->region_sweeps;   // forced: any batch size
+  }
+  const bool region = sweeps > 0;
+  const size_t smem = transport_smem_bytes(ctx, region);
   TransportParamsU PU;
   PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
+  PU.rec = nullptr; PU.list_out = nullptr; PU.list_out_count = nullptr; PU.count_dev = nullptr; PU.resume = 0;
+  PU.region_cells = ctx->region_cells; PU.regions_per_axis = ctx->region_cells ? ctx->N / ctx->region_cells : 0; PU.lut2 = 0;
+  if (region) {
+    if (ctx->rec_cap < n) {
+      cudaFree(ctx->d_rec); cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]);
+      ctx->d_rec = nullptr; ctx->d_list[0] = ctx->d_list[1] = nullptr; ctx->rec_cap = 0;
+      CU(cudaMalloc(&ctx->d_rec, sizeof(float4) * 3 * (size_t)n));
+      CU(cudaMalloc(&ctx->d_list[0], 8 * (size_t)n));
+      CU(cudaMalloc(&ctx->d_list[1], 8 * (size_t)n));
+      ctx->rec_cap = n;
+    }
+    if (ctx->perm_cap < n) {
+      cudaFree(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
+      CU(cudaMalloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
+      ctx->perm_cap = n;
+    }
+    const int nreg = PU.regions_per_axis * PU.regions_per_axis * PU.regions_per_axis;
+    if (!ctx->d_swcnt) CU(cudaMalloc(&ctx->d_swcnt, sizeof(unsigned int) * (kMaxSweeps + 2)));
+    if (!ctx->d_regcnt) CU(cudaMalloc(&ctx->d_regcnt, sizeof(unsigned int) * 2 * (size_t)nreg));
+    CU(cudaMemsetAsync(ctx->d_swcnt, 0, sizeof(unsigned int) * (kMaxSweeps + 2), st));
+    PU.rec = ctx->d_rec; PU.lut = ctx->d_lut_marked;
+    PU.list_out = ctx->d_list[0]; PU.list_out_count = ctx->d_swcnt;
+  }
   const int dens = staging_mode(ctx);
   PU.stage = dens == 1 ? (const void*)ctx->d_rho : (const void*)ctx->d_bits;
   PU.stage_bytes = ctx->stage_bytes; PU.pal0 = ctx->pal0; PU.pal1 = ctx->pal1;
   const bool five = bps * threads > 1024 && !ctx->pah;      // 48-register build (5 blocks of 256) or 64-register build
   void (*kern)(TransportParamsU) =
-      ctx->pah ? (ctx->macro ? k_transport_u<4, true, 0, true, true>              // PAH instances: 64-register builds,
-                  : !ctx->uni ? k_transport_u<4, true, 0, false, true>            // global gathers
-                              : k_transport_u<4, false, 0, false, true>)
-      : ctx->macro ? (five ? k_transport_u<5, true, 0, true, false> : k_transport_u<4, true, 0, true, false>)
-      : !ctx->uni ? (five ? k_transport_u<5, true, 0, false, false> : k_transport_u<4, true, 0, false, false>)
-      : dens == 1 ? k_transport_u<5, false, 1, false, false>
-      : dens == 2 ? k_transport_u<5, false, 2, false, false>
-                  : (five ? k_transport_u<5, false, 0, false, false> : k_transport_u<4, false, 0, false, false>);
+      ctx->pah ? (ctx->macro ? k_transport_u<4, true, 0, true, true, false>       // PAH instances: 64-register builds,
+                  : !ctx->uni ? k_transport_u<4, true, 0, false, true, false>     // global gathers
+                              : k_transport_u<4, false, 0, false, true, false>)
+      : ctx->macro ? (five ? k_transport_u<5, true, 0, true, false, false> : k_transport_u<4, true, 0, true, false, false>)
+      : !ctx->uni ? (five ? k_transport_u<5, true, 0, false, false, false> : k_transport_u<4, true, 0, false, false, false>)
+      : region ? k_transport_u<4, false, 0, false, false, true>
+      : dens == 1 ? k_transport_u<5, false, 1, false, false, false>
+      : dens == 2 ? k_transport_u<5, false, 2, false, false, false>
+                  : (five ? k_transport_u<5, false, 0, false, false, false> : k_transport_u<4, false, 0, false, false, false>);
   if (smem > (48u << 10)) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   if (dens) CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   int resident = 0;                                          // large tables (many bins) lower the residency:
@@ -645,6 +707,30 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   kern<<<(unsigned)grid, threads, smem, st>>>(PU);
   ctx->launches++;
   CU(cudaGetLastError());
+  if (region) {
+    // sweeps 1..sweeps: the packages suspended in the previous sweep, grouped by the region they wait in; the last
+    // one runs on plain tables (no markers) and finishes every package that is left
+    const int nreg = PU.regions_per_axis * PU.regions_per_axis * PU.regions_per_axis;
+    const long long full = (long long)ctx->sm_count * resident < (long long)ctx->sm_count * bps
+                               ? (long long)ctx->sm_count * resident : (long long)ctx->sm_count * bps;
+    for (int sw = 1; sw <= sweeps; ++sw) {
+      const unsigned long long* list_in = ctx->d_list[(sw - 1) & 1];
+      const unsigned int* n_in = ctx->d_swcnt + (sw - 1);
+      CU(cudaMemsetAsync(ctx->d_regcnt, 0, sizeof(unsigned int) * 2 * (size_t)nreg, st));
+      const unsigned gblocks = (unsigned)ctx->sm_count * 4u;
+      k_region_hist<<<gblocks, 256, sizeof(unsigned int) * nreg, st>>>(list_in, n_in, nreg, ctx->d_regcnt);
+      k_scan_sources<<<1, 32, 0, st>>>(ctx->d_regcnt, ctx->d_regcnt + nreg, nreg);
+      k_region_scatter<<<gblocks, 256, sizeof(unsigned int) * 2 * nreg, st>>>(list_in, n_in, nreg, ctx->d_regcnt + nreg, ctx->d_perm);
+      CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
+      PU.base.perm = ctx->d_perm;
+      PU.resume = 1; PU.count_dev = n_in;
+      PU.lut = sw == sweeps ? ctx->d_lut_plain2 : ctx->d_lut_marked;
+      PU.list_out = ctx->d_list[sw & 1]; PU.list_out_count = ctx->d_swcnt + sw;
+      kern<<<(unsigned)full, threads, smem, st>>>(PU);
+      ctx->launches += 4;
+      CU(cudaGetLastError());
+    }
+  }
   return MCRT_OK;
 }
 
@@ -1190,6 +1276,13 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
   if (!ctx) return MCRT_EINVAL;
   if (quorum < 0 || quorum > 32) return fail(ctx, MCRT_EINVAL, "mcrt_set_walk_quorum: quorum must be 0..32");
   ctx->quorum = quorum;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_set_region_sweeps(mcrt_ctx* ctx, int32_t sweeps) {
+  if (!ctx) return MCRT_EINVAL;
+  if (sweeps < -1 || sweeps > 30) return fail(ctx, MCRT_EINVAL, "mcrt_set_region_sweeps: -1 (automatic), 0 (off) or 1..30");
+  ctx->region_sweeps = sweeps;
   return MCRT_OK;
 }
 

@@ -46,6 +46,14 @@
 //    ends of every flight (motion is monotonic per axis, so a flight crosses |F_end - F_start|
 //    cell faces on each axis): "a kernel that skips empty space must add the skipped leaf count
 //    arithmetically".
+//  * REGION: grids far larger than the L2 (C4's 512^3) are swept region by region.  The root delta tables
+//    carry a marker (kLutRegion) on every step that crosses a region boundary (regions of 128^3 cells);
+//    a package that takes such a step is SUSPENDED: its state (48 bytes) goes to a record indexed by its
+//    package number and the number is appended, with the region it entered, to the list of the next sweep.
+//    Between sweeps the list is grouped by region, so the packages in flight at any time sit in one or two
+//    regions whose density the L2 holds: the walk's gathers become L2 hits instead of DRAM bursts.  After a
+//    few sweeps the stragglers are finished by one sweep without markers.  Integer tallies and exact
+//    restoration of the state make the result identical to the unswept run.
 //  * The walk loop runs until fewer than `quorum` lanes of the warp are still walking; then all
 //    stopped lanes go through ONE event pass (escape tally -> refill from the work queue ->
 //    emission / scattering / absorption+re-emission -> new flight).  Emission and re-emission
@@ -112,6 +120,8 @@ __host__ __device__ __forceinline__ long long ext_of_slot(const LayoutU& L, long
 
 constexpr int kLutEscape = INT_MIN;       // root table: the step leaves the grid
 constexpr int kLutLeave = INT_MIN + 1;    // sub table: the step leaves the refined root cube
+constexpr int kLutRegion = INT_MIN + 2;   // root table of a swept grid: the step crosses a region boundary (the
+                                          // delta itself is in the second copy of the tables)
 constexpr int kSubStride = 16;            // ints per (axis, direction) row of the sub table (64-byte rows, S <= 8):
                                           // [0..S-1] slot deltas (+-S^a, the last one kLutLeave), [15] = -(S-1) * delta
 constexpr int kPending = (int)0x80000000u; // PacketU::cb: the package crossed into a new root cube at the sub level
@@ -127,6 +137,14 @@ struct TransportParamsU {
                                  // (2*axis+1)*N; two-level grids: [6][kSubStride] sub-cell rows from lut_sub_offset(N)
   LayoutU lay;
   int quorum;                    // leave the walk loop when fewer lanes than this are walking; 0 = automatic
+  // region sweeps (kernel template REGION)
+  float4* rec;                            // [packages of the batch][3] state of a suspended package
+  unsigned long long* list_out;           // packages suspended in this sweep: (region << 32 | package number) ...
+  unsigned int* list_out_count;           // ... and how many
+  const unsigned int* count_dev;          // NULL: base.count items; else the number of items of this sweep (device)
+  int resume;                             // the items are suspended packages (records), not new package numbers
+  int region_cells, regions_per_axis;
+  int lut2;                               // byte offset from the marked tables to the plain ones in shared memory
   // density staged in shared memory (kernel template DENS = 1 / 2): what every block copies in
   const void* __restrict__ stage;   // DENS 1: the fp32 density array itself; DENS 2: one bit per storage slot
   unsigned stage_bytes;             // multiple of 16
@@ -170,7 +188,7 @@ __device__ __forceinline__ int auto_quorum(const unsigned long long* __restrict_
 // SU_INTERACT_B: interaction found in the second step of a pair -> the cell's density is in the
 // alternate register (moved back in the event pass, never inside the walk loop where the move
 // would wait for the gather in flight).
-enum : int { SU_WALK = 0, SU_INTERACT = 1, SU_ESCAPE = 2, SU_FETCH = 3, SU_DONE = 4, SU_INTERACT_B = 5 };
+enum : int { SU_WALK = 0, SU_INTERACT = 1, SU_ESCAPE = 2, SU_FETCH = 3, SU_DONE = 4, SU_INTERACT_B = 5, SU_SUSPEND = 6 };
 
 struct PacketU {
   float d0, d1, d2;          // direction
@@ -327,7 +345,7 @@ __device__ __forceinline__ void root_entry(const TransportParams& P, PacketU& p,
 // alternate the two registers and no instruction waits on the gather except its real use.
 // tau_rem > 0 always (u01 < 1, and a - b > 0 for a > b in IEEE arithmetic), so dtau >= tau_rem
 // implies rho*kappa > 0: no interaction in an empty leaf (R14).
-template <bool TL, int DENS, bool MACRO>
+template <bool TL, int DENS, bool MACRO, bool REGION>
 __device__ __forceinline__ void walk_step_u(const TransportParams& P, const DensU& D, PacketU& p, float& cur,
                                             float& nxt, float kx, uint32_t sublut, int& state, uint32_t& crossings) {
   if (TL) {
@@ -340,6 +358,11 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, const Dens
   int dl = lds_s32(csel);
   int from = p.slot;
   bool leave = false;
+  bool cross = false;                                        // REGION: the step crosses a region boundary
+  if (REGION) {
+    cross = dl == kLutRegion;
+    if (cross) dl = lds_s32(csel + sublut);                  // (sublut = offset to the plain tables here)
+  }
   if (TL) {
     leave = dl == kLutLeave;
     if (leave) {                                             // the step leaves the refined cube: root table
@@ -349,7 +372,7 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, const Dens
   }
   const bool esc = dl == kLutEscape;
   const int nslot = from + dl;
-  if (!esc) { MCRT_CHECK_SLOT(nslot); nxt = density_at<DENS>(D, nslot); }
+  if (!esc && !(REGION && cross)) { MCRT_CHECK_SLOT(nslot); nxt = density_at<DENS>(D, nslot); }
   const float dtau = cur * kx * (tnext - p.tcur);
   if (dtau >= p.tau_rem) {                                   // interaction inside this leaf
     state = SU_INTERACT;
@@ -382,6 +405,7 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, const Dens
       if (a0) { p.t0 += p.dt0; p.p0 += 4u; } else if (a1) { p.t1 += p.dt1; p.p1 += 4u; } else { p.t2 += p.dt2; p.p2 += 4u; }
       p.slot = nslot;
       if (esc) state = SU_ESCAPE;
+      else if (REGION && cross) state = SU_SUSPEND;          // it now sits in the first cell of the next region
     }
   }
 }
@@ -437,7 +461,7 @@ __device__ __forceinline__ uint32_t along(const PacketU& p, int f0, int f1, int 
 // PAH: the instance that knows the transiently heated PAH (row f2).  A template parameter, not a run-time
 // branch: the third Philox block in the event pass costs registers and spills in every instance that
 // contains it (C2 3.38 -> 3.52 ms per launch when it was compiled into all of them).
-template <int MINBLOCKS, bool TL, int DENS, bool MACRO, bool PAH>
+template <int MINBLOCKS, bool TL, int DENS, bool MACRO, bool PAH, bool REGION>
 __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportParamsU PU) {
   const TransportParams& P = PU.base;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -448,8 +472,10 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   int* s_lut = reinterpret_cast<int*>(smem_raw + ((32u * (unsigned)P.nb + 63u) & ~63u));
   const uint32_t lut = (uint32_t)__cvta_generic_to_shared(s_lut);
   const int N = P.N;
-  const uint32_t sublut = lut + 4u * (uint32_t)lut_sub_offset(N);
-  const int n_lut = TL ? lut_sub_offset(N) + 6 * kSubStride : 6 * N;
+  // two-level grids: address of the subcube rows; swept grids: byte OFFSET from the marked to the plain root tables
+  const uint32_t sublut = REGION ? 4u * (uint32_t)(6 * N) : lut + 4u * (uint32_t)lut_sub_offset(N);
+  const int n_lut = TL ? lut_sub_offset(N) + 6 * kSubStride : (REGION ? 12 * N : 6 * N);
+  const unsigned long long n_items = REGION && PU.count_dev ? (unsigned long long)*PU.count_dev : P.count;
   for (int i = threadIdx.x; i < P.nb; i += blockDim.x) { s_opac[i] = P.opac[i]; s_emit[i] = 0; }
   for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x) s_sed[i] = 0;
   for (int i = threadIdx.x; i < n_lut; i += blockDim.x) s_lut[i] = PU.lut[i];
@@ -514,17 +540,60 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       atomicAdd(&s_sed[(p.cb >> 16) * P.nb + (p.cb & 0xffff)], 1u);
       state = SU_FETCH;
     }
+    if (REGION) {                                            // packages that crossed into another region wait for its sweep
+      const unsigned sm = __ballot_sync(kFull, state == SU_SUSPEND);
+      if (state == SU_SUSPEND) {
+        int ix, iy, iz;
+        cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
+        const int R = PU.region_cells, nR = PU.regions_per_axis;
+        const unsigned key = (unsigned)(ix / R + nR * (iy / R + nR * (iz / R)));
+        float4* r = PU.rec + 3 * (size_t)p.off;
+        r[0] = make_float4(p.d0, p.d1, p.d2, p.tcur);
+        r[1] = make_float4(p.t0, p.t1, p.t2, p.tau_rem);
+        r[2] = make_float4(__int_as_float(ix | (iy << 16)), __int_as_float(iz), __int_as_float(p.cb),
+                           __int_as_float((int)p.k));
+        const int leader = __ffs(sm) - 1;
+        unsigned base = 0;
+        if ((int)lane == leader) base = atomicAdd(PU.list_out_count, (unsigned)__popc(sm));
+        base = __shfl_sync(sm, base, leader);
+        PU.list_out[base + __popc(sm & lt_mask)] = ((unsigned long long)key << 32) | p.off;
+        state = SU_FETCH;
+      }
+    }
     bool is_new = false;
     const unsigned need = __ballot_sync(kFull, state == SU_FETCH);
     if (need) {
       unsigned long long base = 0;
       if (lane == 0) base = atomicAdd(P.next, (unsigned long long)__popc(need));
       base = __shfl_sync(kFull, base, 0);
-      if (base + 32ull > P.count) quorum = 1;                // queue (nearly) empty: no more refills
+      if (base + 32ull > n_items) quorum = 1;                // queue (nearly) empty: no more refills
       if (state == SU_FETCH) {
         unsigned long long my = base + (unsigned long long)__popc(need & lt_mask);
-        if (my < P.count) { p.off = P.perm ? __ldg(P.perm + my) : (uint32_t)my; is_new = true; }
-        else state = SU_DONE;
+        if (my < n_items) {
+          p.off = P.perm ? __ldg(P.perm + my) : (uint32_t)my;
+          if (REGION && PU.resume) {                         // a suspended package: restore it exactly
+            const float4* r = PU.rec + 3 * (size_t)p.off;
+            const float4 ra = r[0], rb = r[1], rc = r[2];
+            p.d0 = ra.x; p.d1 = ra.y; p.d2 = ra.z; p.tcur = ra.w;
+            p.dt0 = __frcp_rn(fabsf(p.d0)); p.dt1 = __frcp_rn(fabsf(p.d1)); p.dt2 = __frcp_rn(fabsf(p.d2));
+            p.t0 = rb.x; p.t1 = rb.y; p.t2 = rb.z; p.tau_rem = rb.w;
+            const int cxy = __float_as_int(rc.x), ix = cxy & 0xffff, iy = cxy >> 16, iz = __float_as_int(rc.y);
+            p.cb = __float_as_int(rc.z); p.k = (uint32_t)__float_as_int(rc.w);
+            root_cursors(p, lut, N, ix, iy, iz, p.p0, p.p1, p.p2);
+            p.slot = (int)slot_of(PU.lay, ix, iy, iz);
+            MCRT_CHECK_SLOT(p.slot);
+            p.rho = density_at<DENS>(D, p.slot);
+            kx = s_opac[p.cb & 0xffff].x;
+            float u[4];                                      // the flight's uniforms again (R18: fixed slots)
+            draw4(P.seed, P.first + p.off, p.k, kTagFlight, u);
+            p.u1 = u[1]; p.u2 = u[2]; p.u3 = u[3];
+            state = SU_WALK;
+          } else {
+            is_new = true;
+          }
+        } else {
+          state = SU_DONE;
+        }
       }
     }
     if (__all_sync(kFull, state == SU_DONE)) break;
@@ -684,9 +753,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
     // ---- a3: cell walk until fewer than `quorum` lanes are walking ----
 #pragma unroll 1
     for (;;) {
-      if (state == SU_WALK) walk_step_u<TL, DENS, MACRO>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
+      if (state == SU_WALK) walk_step_u<TL, DENS, MACRO, REGION>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
       if (state == SU_WALK) {
-        walk_step_u<TL, DENS, MACRO>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);
+        walk_step_u<TL, DENS, MACRO, REGION>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);
         if (state == SU_INTERACT) state = SU_INTERACT_B;
       }
       if (__popc(__ballot_sync(kFull, state == SU_WALK)) < quorum) break;
@@ -718,6 +787,43 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   }
   if (lane == 0 && esc) atomicAdd(P.counters + CNT_ESCAPED, esc);
   if (lane == 0 && emi) atomicAdd(P.counters + CNT_EMITTED, emi);
+}
+
+// ---- region sweeps: group the suspended packages of a sweep by the region they wait in ----------
+// list[i] = region << 32 | package number (i < *n_dev).  Same three steps as the grouped hand-out: histogram,
+// exclusive scan, scatter with a per-block reservation (the order inside a region is arbitrary).
+__global__ void k_region_hist(const unsigned long long* __restrict__ list, const unsigned int* __restrict__ n_dev,
+                              int nreg, unsigned int* __restrict__ counts) {
+  extern __shared__ unsigned int s_cnt[];
+  for (int i = threadIdx.x; i < nreg; i += blockDim.x) s_cnt[i] = 0;
+  __syncthreads();
+  const unsigned n = *n_dev;
+  for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    atomicAdd(&s_cnt[(unsigned)(list[i] >> 32)], 1u);
+  __syncthreads();
+  for (int i = threadIdx.x; i < nreg; i += blockDim.x)
+    if (s_cnt[i]) atomicAdd(&counts[i], s_cnt[i]);
+}
+__global__ void k_region_scatter(const unsigned long long* __restrict__ list, const unsigned int* __restrict__ n_dev,
+                                 int nreg, unsigned int* __restrict__ cursor, uint32_t* __restrict__ perm) {
+  extern __shared__ unsigned int s_cnt[];                    // [2 * nreg]: block histogram, block bases
+  for (int i = threadIdx.x; i < 2 * nreg; i += blockDim.x) s_cnt[i] = 0;
+  __syncthreads();
+  const unsigned n = *n_dev;
+  const unsigned per_block = (n + gridDim.x - 1) / gridDim.x;
+  const unsigned lo = per_block * blockIdx.x, hi = min(n, lo + per_block);
+  for (unsigned i = lo + threadIdx.x; i < hi; i += blockDim.x) atomicAdd(&s_cnt[(unsigned)(list[i] >> 32)], 1u);
+  __syncthreads();
+  for (int i = threadIdx.x; i < nreg; i += blockDim.x) {
+    s_cnt[nreg + i] = s_cnt[i] ? atomicAdd(&cursor[i], s_cnt[i]) : 0u;
+    s_cnt[i] = 0;
+  }
+  __syncthreads();
+  for (unsigned i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+    const unsigned long long e = list[i];
+    const unsigned g = (unsigned)(e >> 32);
+    perm[s_cnt[nreg + g] + atomicAdd(&s_cnt[g], 1u)] = (uint32_t)e;
+  }
 }
 
 // ---- layout conversion (set-up and read-out; storage order never shows at the C ABI, R22) ----

@@ -700,3 +700,22 @@ def test_macro_cubes_are_chosen_automatically_only_where_they_pay(M):
     assert int(M.lib().mcrt_store_slots(clumpy.h)) == 24 ** 3   # no uniform cubes: plain grid
     small = M.from_workload(W.c0(n_packets=10, batch=10))        # 16^3: 12 % uniform cubes: plain + staged
     assert int(M.lib().mcrt_store_slots(small.h)) == 16 ** 3 and small.density_staging() == 1
+
+
+def test_region_sweeps_do_not_change_results(M):
+    """Grids far larger than the L2 are swept region by region (packages that cross a region boundary are
+    suspended and continue in the next sweep, restored exactly): every count must equal the unswept run's,
+    for any number of sweeps.  256^3 clumpy cube (8 regions of 128^3), 11 sources, batches of 2^20."""
+    wl = W.c4(n_root=256, n_packets=(1 << 21) + 12345, batch=1 << 20)
+    runs = []
+    for sweeps in (0, -1, 1, 3):
+        ctx = M.from_workload(wl)
+        ctx.set_region_sweeps(sweeps)
+        for first, cnt in wl.batches():
+            ctx.run_batch(wl.seed, first, cnt)                   # the last batch (12345 packages) is never swept
+        runs.append(ctx)
+    for other in runs[1:]:
+        _assert_identical(runs[0], other)
+    c = runs[1].get_counters()
+    assert c["emitted"] == c["escaped"] == wl.n_packets and c["lost"] == 0
+    assert runs[1].kernel_launches() > runs[0].kernel_launches() + 2 * 6 * 4
