@@ -311,10 +311,11 @@ def rooflines(wl, name, d, tr_s, steps, gather_peak):
                           "hbm figures are the ones that bound"}
     cap = ncu_capture(name)
     resident = foot <= 0.75 * L2_BYTES
-    if cap.get("warp_instructions_per_launch") and name != "c4":
-        # The committed capture of this workload shows what binds it: the issue slots (75-85 % busy, DRAM at
-        # a few per cent, L1TEX wavefronts well below their peak).  achieved = the capture's warp instructions
-        # per launch / the kernel time measured HERE; peak = SMs x 4 schedulers x max clock.
+    if cap.get("warp_instructions_per_launch"):
+        # The committed capture of this workload shows what binds it: the issue slots (65-85 % busy, DRAM at
+        # a few per cent of its peak -- C4 too since it is swept region by region --, L1TEX wavefronts well
+        # below their peak).  achieved = the capture's warp instructions per step (all launches of the
+        # transport kernel in a batch) / the kernel time measured HERE; peak = SMs x 4 schedulers x max clock.
         ipl = float(cap["warp_instructions_per_launch"])
         ach = ipl / (tr_s / steps) / 1e9 if tr_s > 0 else 0.0
         pk = issue_peak() / 1e9

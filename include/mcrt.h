@@ -298,11 +298,16 @@ mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t bl
 mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum);
 /* Region sweeps (single-level grids of at least 256^3 cells in the brick layout, batches of at least 2^20
  * packages): the batch is transported in `sweeps` + 1 passes; in all but the last a package that crosses
- * into another region of 128^3 cells is suspended (48 bytes of state) and continues in the next pass,
+ * into another region (256 x 128 x 128 cells by default, 128^3 on a 256^3 grid) is suspended (48 bytes of state) and continues in the next pass,
  * where the waiting packages are handed out region by region, so that the cells the packages in flight
- * visit stay in the L2; the last pass finishes whatever is left.  -1 = automatic (the default: 6), 0 =
- * off, 1..30.  Results do not depend on it (integer tallies, the state is restored exactly). */
-mcrt_status mcrt_set_region_sweeps(mcrt_ctx* ctx, int32_t sweeps);
+ * visit stay in the L2; the last pass finishes whatever is left.  sweeps: -1 = automatic (the default: 6
+ * for batches of at least 2^20 packages), 0 = off, 1..30 (then for any batch size).  rx, ry, rz: region
+ * edges in cells (multiples of 8 that divide n_root, 2..4096 regions), 0 0 0 = keep.  Results do not
+ * depend on any of it (integer tallies, the state is restored exactly). */
+mcrt_status mcrt_set_region_sweeps(mcrt_ctx* ctx, int32_t sweeps, int32_t rx, int32_t ry, int32_t rz);
+/* Packages suspended in sweep 0, 1, ... of the LAST swept batch (host array of `cap` entries, at most 32
+ * are written; *n_out = number written, 0 if no batch was swept yet). */
+mcrt_status mcrt_get_region_sweep_counts(mcrt_ctx* ctx, uint32_t* suspended_out, int32_t cap, int32_t* n_out);
 /* Density kept in shared memory (single-level grids): a density array of at most 40 KB is copied
  * into every block's shared memory by one bulk copy (cp.async.bulk) and a crossing reads shared
  * memory instead of the L2 (C0: -10 % per launch).  mode 0 = automatic (the default), 1 = off

@@ -71,7 +71,8 @@ struct mcrt_ctx {
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 0;                         // 0 = automatic (from the job's crossings per flight so far)
   // region sweeps (transport_u.cuh, REGION): single-level bricked grids far larger than the L2
-  int region_cells = 0, region_sweeps = -1;   // cells per region edge (0: grid does not qualify); -1 automatic, 0 off
+  int region_cells[3] = {0, 0, 0};        // cells per region along x, y, z (0: the grid does not qualify)
+  int region_sweeps = -1;                 // -1 automatic, 0 off
   int *d_lut_marked = nullptr, *d_lut_plain2 = nullptr;     // [12 N]: marked | plain root tables; plain | plain
   float4* d_rec = nullptr;                // [perm_cap][3] suspended packages
   unsigned long long* d_list[2] = {nullptr, nullptr};       // suspended packages of a sweep: region << 32 | number
@@ -147,6 +148,26 @@ static void free_observer(mcrt_ctx* c) {
 static void free_sources(mcrt_ctx* c) {
   cudaFree(c->d_src); cudaFree(c->d_csrc); cudaFree(c->d_csrc32);
   c->d_src = nullptr; c->d_csrc = nullptr; c->d_csrc32 = nullptr;
+}
+
+// Root delta tables of a swept grid: [12 N] = the tables with kLutRegion on every step that crosses a region
+// boundary, followed by the plain tables; and plain | plain for the last sweep.
+static mcrt_status build_region_tables(mcrt_ctx* ctx, const int* lut6N, const int shape[3]) {
+  const int N = ctx->N;
+  std::vector<int> marked(12 * (size_t)N), plain2(12 * (size_t)N);
+  for (size_t i = 0; i < 6 * (size_t)N; ++i) { marked[i] = marked[6 * (size_t)N + i] = plain2[i] = plain2[6 * (size_t)N + i] = lut6N[i]; }
+  for (int a = 0; a < 3; ++a)
+    for (int i = 0; i < N; ++i) {
+      if (i != N - 1 && (i + 1) % shape[a] == 0) marked[(size_t)(2 * a) * N + i] = kLutRegion;          // i -> i+1
+      const int ir = N - 1 - i;
+      if (ir != 0 && ir % shape[a] == 0) marked[(size_t)(2 * a + 1) * N + i] = kLutRegion;              // ir -> ir-1
+    }
+  if (!ctx->d_lut_marked) CU(cudaMalloc(&ctx->d_lut_marked, sizeof(int) * marked.size()));
+  if (!ctx->d_lut_plain2) CU(cudaMalloc(&ctx->d_lut_plain2, sizeof(int) * plain2.size()));
+  CU(cudaMemcpy(ctx->d_lut_marked, marked.data(), sizeof(int) * marked.size(), cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_lut_plain2, plain2.data(), sizeof(int) * plain2.size(), cudaMemcpyHostToDevice));
+  for (int a = 0; a < 3; ++a) ctx->region_cells[a] = shape[a];
+  return MCRT_OK;
 }
 
 // ---- storage order <-> the caller's slot order (R22) ---------------------------------------------
@@ -364,23 +385,14 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     }
     CUG(cudaMalloc(&ctx->d_lut, sizeof(int) * lut.size()));
     CUG(cudaMemcpy(ctx->d_lut, lut.data(), sizeof(int) * lut.size(), cudaMemcpyHostToDevice));
-    // Region sweeps for single-level bricked grids of at least 256^3 cells (four times the L2 and more): the root
-    // tables once more with a marker on every step that crosses a boundary between regions of 128^3 cells.
+    // Region sweeps for single-level bricked grids of at least 256^3 cells (the L2 and more): the root tables once
+    // more with a marker on every step that crosses a boundary between regions of 256 x 128 x 128 cells (17 MB of
+    // density: two of them in flight stay L2-resident; measured best on the 512^3 cube, profiles/r02_summary.md).
     constexpr int kRegionCells = 128;
     if (ctx->uni && ctx->lay.bricked == 1 && N >= 2 * kRegionCells && N % kRegionCells == 0) {
-      ctx->region_cells = kRegionCells;
-      std::vector<int> marked(12 * (size_t)N), plain2(12 * (size_t)N);
-      for (size_t i = 0; i < 6 * (size_t)N; ++i) { marked[i] = lut[i]; marked[6 * (size_t)N + i] = lut[i]; plain2[i] = lut[i]; plain2[6 * (size_t)N + i] = lut[i]; }
-      for (int a = 0; a < 3; ++a)
-        for (int i = 0; i < N; ++i) {
-          if (i != N - 1 && (i + 1) % kRegionCells == 0) marked[(size_t)(2 * a) * N + i] = kLutRegion;      // i -> i+1
-          const int ir = N - 1 - i;
-          if (ir != 0 && ir % kRegionCells == 0) marked[(size_t)(2 * a + 1) * N + i] = kLutRegion;          // ir -> ir-1
-        }
-      CUG(cudaMalloc(&ctx->d_lut_marked, sizeof(int) * marked.size()));
-      CUG(cudaMalloc(&ctx->d_lut_plain2, sizeof(int) * plain2.size()));
-      CUG(cudaMemcpy(ctx->d_lut_marked, marked.data(), sizeof(int) * marked.size(), cudaMemcpyHostToDevice));
-      CUG(cudaMemcpy(ctx->d_lut_plain2, plain2.data(), sizeof(int) * plain2.size(), cudaMemcpyHostToDevice));
+      const int shape[3] = {N % (2 * kRegionCells) == 0 && N >= 4 * kRegionCells ? 2 * kRegionCells : kRegionCells,
+                            kRegionCells, kRegionCells};
+      if (build_region_tables(ctx, lut.data(), shape) != MCRT_OK) return bail(MCRT_ECUDA);
     }
     CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
     if (ctx->macro) {
@@ -653,8 +665,8 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   // region sweeps: automatic for qualifying grids and batches of at least 2^20 packages
   constexpr int kMaxSweeps = 30;
   int sweeps = 0;
-  if (ctx->region_cells && !ctx->pah && !tally32_is_unsupported(tally32)) {
-    if (ctx->region_sweeps < 0) sweeps = n >= (1ull << 20) ? 8 : 0;          // automatic
+  if (ctx->region_cells[0] && !ctx->pah && !tally32_is_unsupported(tally32)) {
+    if (ctx->region_sweeps < 0) sweeps = n >= (1ull << 20) ? 6 : 0;          // automatic
     else sweeps = ctx->region_sweeps > kMaxSweeps ? kMaxSweeps : ctx->region_sweeps;   // forced: any batch size
   }
   const bool region = sweeps > 0;
@@ -662,7 +674,11 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   TransportParamsU PU;
   PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
   PU.rec = nullptr; PU.list_out = nullptr; PU.list_out_count = nullptr; PU.count_dev = nullptr; PU.resume = 0;
-  PU.region_cells = ctx->region_cells; PU.regions_per_axis = ctx->region_cells ? ctx->N / ctx->region_cells : 0; PU.lut2 = 0;
+  for (int a = 0; a < 3; ++a) {
+    PU.region_cells[a] = ctx->region_cells[a] ? ctx->region_cells[a] : 1;
+    PU.regions_per_axis[a] = ctx->region_cells[a] ? ctx->N / ctx->region_cells[a] : 1;
+  }
+  PU.lut2 = 0;
   if (region) {
     if (ctx->rec_cap < n) {
       cudaFree(ctx->d_rec); cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]);
@@ -677,7 +693,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
       CU(cudaMalloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
       ctx->perm_cap = n;
     }
-    const int nreg = PU.regions_per_axis * PU.regions_per_axis * PU.regions_per_axis;
+    const int nreg = 4096;                                   // capacity of the histogram (regions <= 4096)
     if (!ctx->d_swcnt) CU(cudaMalloc(&ctx->d_swcnt, sizeof(unsigned int) * (kMaxSweeps + 2)));
     if (!ctx->d_regcnt) CU(cudaMalloc(&ctx->d_regcnt, sizeof(unsigned int) * 2 * (size_t)nreg));
     CU(cudaMemsetAsync(ctx->d_swcnt, 0, sizeof(unsigned int) * (kMaxSweeps + 2), st));
@@ -710,7 +726,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   if (region) {
     // sweeps 1..sweeps: the packages suspended in the previous sweep, grouped by the region they wait in; the last
     // one runs on plain tables (no markers) and finishes every package that is left
-    const int nreg = PU.regions_per_axis * PU.regions_per_axis * PU.regions_per_axis;
+    const int nreg = PU.regions_per_axis[0] * PU.regions_per_axis[1] * PU.regions_per_axis[2];
     const long long full = (long long)ctx->sm_count * resident < (long long)ctx->sm_count * bps
                                ? (long long)ctx->sm_count * resident : (long long)ctx->sm_count * bps;
     for (int sw = 1; sw <= sweeps; ++sw) {
@@ -1279,10 +1295,37 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
   return MCRT_OK;
 }
 
-mcrt_status mcrt_set_region_sweeps(mcrt_ctx* ctx, int32_t sweeps) {
+mcrt_status mcrt_set_region_sweeps(mcrt_ctx* ctx, int32_t sweeps, int32_t rx, int32_t ry, int32_t rz) {
   if (!ctx) return MCRT_EINVAL;
   if (sweeps < -1 || sweeps > 30) return fail(ctx, MCRT_EINVAL, "mcrt_set_region_sweeps: -1 (automatic), 0 (off) or 1..30");
+  if (rx | ry | rz) {                                        // a new region shape: the marked tables are rebuilt
+    const int shape[3] = {rx, ry, rz};
+    if (!ctx->region_cells[0]) return fail(ctx, MCRT_ESTATE, "mcrt_set_region_sweeps: this grid is not swept (single-level, brick layout, >= 256^3)");
+    long long nreg = 1;
+    for (int a = 0; a < 3; ++a) {
+      if (shape[a] < 8 || shape[a] % 8 || ctx->N % shape[a]) return fail(ctx, MCRT_EINVAL, "mcrt_set_region_sweeps: region edges must be multiples of 8 that divide n_root");
+      nreg *= ctx->N / shape[a];
+    }
+    if (nreg < 2 || nreg > 4096) return fail(ctx, MCRT_EINVAL, "mcrt_set_region_sweeps: 2..4096 regions");
+    CU(cudaDeviceSynchronize());
+    std::vector<int> lut(6 * (size_t)ctx->N);
+    CU(cudaMemcpy(lut.data(), ctx->d_lut, sizeof(int) * lut.size(), cudaMemcpyDeviceToHost));
+    mcrt_status rc = build_region_tables(ctx, lut.data(), shape);
+    if (rc != MCRT_OK) return rc;
+  }
   ctx->region_sweeps = sweeps;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_get_region_sweep_counts(mcrt_ctx* ctx, uint32_t* suspended_out, int32_t cap, int32_t* n_out) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!suspended_out || !n_out || cap < 0) return fail(ctx, MCRT_EINVAL, "mcrt_get_region_sweep_counts: bad arguments");
+  *n_out = 0;
+  if (!ctx->d_swcnt) return MCRT_OK;                         // no batch was swept yet
+  const int n = cap < 32 ? cap : 32;
+  mcrt_status rc = copy_out(ctx, suspended_out, ctx->d_swcnt, sizeof(uint32_t) * (size_t)n, MCRT_HOST);
+  if (rc != MCRT_OK) return rc;
+  *n_out = n;
   return MCRT_OK;
 }
 

@@ -47,7 +47,8 @@
 //    cell faces on each axis): "a kernel that skips empty space must add the skipped leaf count
 //    arithmetically".
 //  * REGION: grids far larger than the L2 (C4's 512^3) are swept region by region.  The root delta tables
-//    carry a marker (kLutRegion) on every step that crosses a region boundary (regions of 128^3 cells);
+//    carry a marker (kLutRegion) on every step that crosses a region boundary (regions of 128 x 128 x 128 cells
+//    by default);
 //    a package that takes such a step is SUSPENDED: its state (48 bytes) goes to a record indexed by its
 //    package number and the number is appended, with the region it entered, to the list of the next sweep.
 //    Between sweeps the list is grouped by region, so the packages in flight at any time sit in one or two
@@ -143,7 +144,7 @@ struct TransportParamsU {
   unsigned int* list_out_count;           // ... and how many
   const unsigned int* count_dev;          // NULL: base.count items; else the number of items of this sweep (device)
   int resume;                             // the items are suspended packages (records), not new package numbers
-  int region_cells, regions_per_axis;
+  int region_cells[3], regions_per_axis[3];
   int lut2;                               // byte offset from the marked tables to the plain ones in shared memory
   // density staged in shared memory (kernel template DENS = 1 / 2): what every block copies in
   const void* __restrict__ stage;   // DENS 1: the fp32 density array itself; DENS 2: one bit per storage slot
@@ -545,8 +546,8 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       if (state == SU_SUSPEND) {
         int ix, iy, iz;
         cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
-        const int R = PU.region_cells, nR = PU.regions_per_axis;
-        const unsigned key = (unsigned)(ix / R + nR * (iy / R + nR * (iz / R)));
+        const unsigned key = (unsigned)(ix / PU.region_cells[0] + PU.regions_per_axis[0] *
+                                        (iy / PU.region_cells[1] + PU.regions_per_axis[1] * (iz / PU.region_cells[2])));
         float4* r = PU.rec + 3 * (size_t)p.off;
         r[0] = make_float4(p.d0, p.d1, p.d2, p.tcur);
         r[1] = make_float4(p.t0, p.t1, p.t2, p.tau_rem);

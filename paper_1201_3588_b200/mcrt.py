@@ -69,7 +69,7 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_get_pah_emission_cdf", "mcrt_get_pah_temperature_distribution", "mcrt_set_observer",
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
-           "mcrt_set_density_staging", "mcrt_density_staging", "mcrt_set_region_sweeps",
+           "mcrt_set_density_staging", "mcrt_density_staging", "mcrt_set_region_sweeps", "mcrt_get_region_sweep_counts",
            "mcrt_get_batch_times", "mcrt_get_tables",
            "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_uniforms", "mcrt_gather_calibrate", "mcrt_last_error")
 
@@ -115,8 +115,10 @@ def lib():
         L.mcrt_set_launch.argtypes = [vp, i32, i32]
         L.mcrt_set_walk_quorum.argtypes = [vp, i32]
         L.mcrt_set_source_order.argtypes = [vp, i32]
-        L.mcrt_set_region_sweeps.argtypes = [vp, i32]
+        L.mcrt_set_region_sweeps.argtypes = [vp, i32, i32, i32, i32]
         L.mcrt_set_region_sweeps.restype = C.c_int
+        L.mcrt_get_region_sweep_counts.argtypes = [vp, vp, i32, C.POINTER(i32)]
+        L.mcrt_get_region_sweep_counts.restype = C.c_int
         L.mcrt_set_density_staging.argtypes = [vp, i32]
         L.mcrt_set_density_staging.restype = C.c_int
         L.mcrt_density_staging.argtypes = [vp]
@@ -420,8 +422,16 @@ class Context:
     def set_walk_quorum(self, quorum):
         self._check(lib().mcrt_set_walk_quorum(self.h, int(quorum)), "mcrt_set_walk_quorum")
 
-    def set_region_sweeps(self, sweeps):
-        self._check(lib().mcrt_set_region_sweeps(self.h, int(sweeps)), "mcrt_set_region_sweeps")
+    def set_region_sweeps(self, sweeps, shape=(0, 0, 0)):
+        self._check(lib().mcrt_set_region_sweeps(self.h, int(sweeps), *[int(v) for v in shape]),
+                    "mcrt_set_region_sweeps")
+
+    def get_region_sweep_counts(self):
+        out = np.zeros(32, dtype=np.uint32)
+        n = C.c_int32(0)
+        self._check(lib().mcrt_get_region_sweep_counts(self.h, _np_ptr(out), 32, C.byref(n)),
+                    "mcrt_get_region_sweep_counts")
+        return out[:n.value].copy()
 
     def set_density_staging(self, mode):
         self._check(lib().mcrt_set_density_staging(self.h, int(mode)), "mcrt_set_density_staging")

@@ -708,9 +708,10 @@ def test_region_sweeps_do_not_change_results(M):
     for any number of sweeps.  256^3 clumpy cube (8 regions of 128^3), 11 sources, batches of 2^20."""
     wl = W.c4(n_root=256, n_packets=(1 << 21) + 12345, batch=1 << 20)
     runs = []
-    for sweeps in (0, -1, 1, 3):
+    for sweeps, shape in ((0, (0, 0, 0)), (-1, (0, 0, 0)), (1, (0, 0, 0)), (3, (0, 0, 0)),
+                          (2, (256, 128, 64)), (4, (64, 32, 128))):      # region shapes per axis
         ctx = M.from_workload(wl)
-        ctx.set_region_sweeps(sweeps)
+        ctx.set_region_sweeps(sweeps, shape)
         for first, cnt in wl.batches():
             ctx.run_batch(wl.seed, first, cnt)                   # the last batch (12345 packages) is never swept
         runs.append(ctx)
@@ -718,4 +719,13 @@ def test_region_sweeps_do_not_change_results(M):
         _assert_identical(runs[0], other)
     c = runs[1].get_counters()
     assert c["emitted"] == c["escaped"] == wl.n_packets and c["lost"] == 0
-    assert runs[1].kernel_launches() > runs[0].kernel_launches() + 2 * 6 * 4
+    assert runs[1].kernel_launches() >= runs[0].kernel_launches() + 2 * 6 * 3     # two batches of six sweeps
+    # packages suspended at the end of each sweep of the last batch (a forced sweep count applies to batches of any
+    # size: here the 12345 left over): fewer every sweep, never more than the batch
+    assert runs[0].get_region_sweep_counts().size == 0
+    susp = runs[3].get_region_sweep_counts()[:3].astype(np.int64)
+    assert 12345 > susp[0] > susp[1] > susp[2] > 0
+    with pytest.raises(M.McrtError):
+        runs[1].set_region_sweeps(2, (100, 128, 128))            # edges: multiples of 8 that divide n_root
+    with pytest.raises(M.McrtError):
+        runs[1].set_region_sweeps(2, (256, 256, 256))            # at least two regions
