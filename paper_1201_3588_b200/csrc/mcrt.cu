@@ -605,8 +605,6 @@ static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
   return MCRT_OK;
 }
 
-static bool tally32_is_unsupported(const uint32_t*) { return false; }   // (sweeps work with either tally)
-
 static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st,
                                     uint32_t* tally32 = nullptr) {
   if (n == 0) return MCRT_OK;
@@ -665,7 +663,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   // region sweeps: automatic for qualifying grids and batches of at least 2^20 packages
   constexpr int kMaxSweeps = 30;
   int sweeps = 0;
-  if (ctx->region_cells[0] && !ctx->pah && !tally32_is_unsupported(tally32)) {
+  if (ctx->region_cells[0] && !ctx->pah) {                   // (either tally; the PAH split is not carried in a record)
     if (ctx->region_sweeps < 0) sweeps = n >= (1ull << 20) ? 6 : 0;          // automatic
     else sweeps = ctx->region_sweeps > kMaxSweeps ? kMaxSweeps : ctx->region_sweeps;   // forced: any batch size
   }

@@ -702,6 +702,43 @@ def test_macro_cubes_are_chosen_automatically_only_where_they_pay(M):
     assert int(M.lib().mcrt_store_slots(small.h)) == 16 ** 3 and small.density_staging() == 1
 
 
+def test_region_sweeps_with_sharded_batches_and_observer(M):
+    """Swept batches under the packet-sharded pair of calls (uint32 per-batch tally) and with the direction-resolved
+    tallies switched on: two emulated ranks, swept, against ONE unswept context, bit for bit; the inclination-binned
+    SEDs and images add up."""
+    from paper_1201_3588_b200.sharding import rank_range
+    wl = W.c4(n_root=256, n_packets=3 * (1 << 19), batch=1 << 20)
+    obs = dict(n_mu=6, n_pix=16, direction=(0.3, -0.5, 0.81), half_angle_deg=12.0, half_width_cm=128 * wl.root_size)
+    one = M.from_workload(wl)
+    one.set_region_sweeps(0)
+    one.set_observer(**obs)
+    for first, cnt in wl.batches():
+        one.run_batch(wl.seed, first, cnt)
+    ranks = [M.from_workload(wl) for _ in range(2)]
+    for ctx, sweeps in zip(ranks, (2, 5)):
+        ctx.set_region_sweeps(sweeps, (128, 256, 128))
+        ctx.set_observer(**obs)
+    done = 0
+    for first, cnt in wl.batches():
+        deltas = []
+        for r, ctx in enumerate(ranks):
+            f, c = rank_range(first, cnt, 2, r)
+            deltas.append(ctx.transport_batch_delta(wl.seed, f, c))
+        done += cnt
+        for ctx in ranks:
+            ctx.accumulate_update(deltas[0] + deltas[1], done)
+    for ctx in ranks:
+        assert np.array_equal(ctx.get_cell_energy()[0], one.get_cell_energy()[0])
+        assert np.array_equal(ctx.get_cell_temperature(), one.get_cell_temperature())
+        assert ctx.get_region_sweep_counts()[0] > 0
+    assert np.array_equal(ranks[0].get_sed() + ranks[1].get_sed(), one.get_sed())
+    assert np.array_equal(ranks[0].get_sed_mu() + ranks[1].get_sed_mu(), one.get_sed_mu())
+    assert np.array_equal(ranks[0].get_image() + ranks[1].get_image(), one.get_image())
+    ca, cb, c1 = ranks[0].get_counters(), ranks[1].get_counters(), one.get_counters()
+    for k in c1:
+        assert np.array_equal(ca[k] + cb[k], c1[k]), k
+
+
 def test_region_sweeps_do_not_change_results(M):
     """Grids far larger than the L2 are swept region by region (packages that cross a region boundary are
     suspended and continue in the next sweep, restored exactly): every count must equal the unswept run's,
