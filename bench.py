@@ -392,6 +392,8 @@ def run_gpu(args, wl, name):
         ctx.set_walk_quorum(args.quorum)
     if args.source_order is not None:
         ctx.set_source_order(args.source_order)
+    if args.tail_mode is not None:
+        ctx.set_tail_mode(args.tail_mode)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
     from paper_1201_3588_b200.sharding import ShardedRunner
@@ -585,6 +587,7 @@ def main():
     ap.add_argument("--quorum", type=int, default=0, help="walk-loop quorum (0 = automatic)")
     ap.add_argument("--source-order", type=int, default=None,
                     help="hand packages out grouped by source: 1 on, 0 off (default: automatic)")
+    ap.add_argument("--tail-mode", type=int, default=None, help="end of a batch: -1 auto, 0 quorum drops to 1, 1 quorum follows the live lanes")
     ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 x-fastest, 2 bricked")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")

@@ -70,6 +70,7 @@ struct mcrt_ctx {
   int order_by_source = -1;               // -1 automatic, 0 off, 1 by source, 2 by source and start direction
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 0;                         // 0 = automatic (from the job's crossings per flight so far)
+  int tail_mode = -1;                     // end of a batch: -1 automatic, 1 the quorum follows the live lanes, 0 it drops to 1
   // region sweeps (transport_u.cuh, REGION): single-level bricked grids far larger than the L2
   int region_cells[3] = {0, 0, 0};        // cells per region along x, y, z (0: the grid does not qualify)
   int region_sweeps = -1;                 // -1 automatic, 0 off
@@ -235,6 +236,7 @@ static size_t transport_smem_bytes(const mcrt_ctx* ctx, bool region = false) {
   if (staging_mode(ctx)) b = ((b + 127) & ~(size_t)127) + ctx->stage_bytes + 16;   // staged density + its mbarrier
   return b;
 }
+
 constexpr size_t kMaxSmemPerBlock = 227u << 10;              // B200: opt-in limit of dynamic shared memory
 
 extern "C" {
@@ -670,6 +672,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   const bool region = sweeps > 0;
   const size_t smem = transport_smem_bytes(ctx, region);
   TransportParamsU PU;
+  PU.tail = ctx->tail_mode < 0 ? 1 : ctx->tail_mode;
   PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
   PU.rec = nullptr; PU.list_out = nullptr; PU.list_out_count = nullptr; PU.count_dev = nullptr; PU.resume = 0;
   for (int a = 0; a < 3; ++a) {
@@ -1290,6 +1293,13 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
   if (!ctx) return MCRT_EINVAL;
   if (quorum < 0 || quorum > 32) return fail(ctx, MCRT_EINVAL, "mcrt_set_walk_quorum: quorum must be 0..32");
   ctx->quorum = quorum;
+  return MCRT_OK;
+}
+
+mcrt_status mcrt_set_tail_mode(mcrt_ctx* ctx, int32_t mode) {
+  if (!ctx) return MCRT_EINVAL;
+  if (mode < -1 || mode > 1) return fail(ctx, MCRT_EINVAL, "mcrt_set_tail_mode: -1 (automatic), 0 or 1");
+  ctx->tail_mode = mode;
   return MCRT_OK;
 }
 

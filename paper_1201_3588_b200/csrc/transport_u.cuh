@@ -146,6 +146,8 @@ struct TransportParamsU {
   int resume;                             // the items are suspended packages (records), not new package numbers
   int region_cells[3], regions_per_axis[3];
   int lut2;                               // byte offset from the marked tables to the plain ones in shared memory
+  int tail;                               // end of a batch: 1 = once the work queue is empty the walk quorum follows the
+                                          // number of packages the warp still holds (0: it drops to 1)
   // density staged in shared memory (kernel template DENS = 1 / 2): what every block copies in
   const void* __restrict__ stage;   // DENS 1: the fp32 density array itself; DENS 2: one bit per storage slot
   unsigned stage_bytes;             // multiple of 16
@@ -516,7 +518,9 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   p.cb = 0; p.k = 0; p.off = 0; p.u1 = p.u2 = p.u3 = 0.f;
   float kx = 0.f;
   int state = SU_FETCH;
-  int quorum = PU.quorum > 0 ? PU.quorum : auto_quorum(P.counters);
+  const int quorum0 = PU.quorum > 0 ? PU.quorum : auto_quorum(P.counters);
+  int quorum = quorum0;
+  bool tail = false;                                         // the work queue is (nearly) empty
 
   for (;;) {
     // ---- a7: escaped packages -> SED; a8: refill from the work queue (one atomic per warp) ----
@@ -567,7 +571,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       unsigned long long base = 0;
       if (lane == 0) base = atomicAdd(P.next, (unsigned long long)__popc(need));
       base = __shfl_sync(kFull, base, 0);
-      if (base + 32ull > n_items) quorum = 1;                // queue (nearly) empty: no more refills
+      if (base + 32ull > n_items) { quorum = 1; tail = PU.tail != 0; }   // queue (nearly) empty: no more refills
       if (state == SU_FETCH) {
         unsigned long long my = base + (unsigned long long)__popc(need & lt_mask);
         if (my < n_items) {
@@ -750,6 +754,11 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         state = SU_WALK;
       }
     }
+
+    // End of the batch: without refills the lanes of a warp run dry one by one.  The warp keeps the rhythm of
+    // the steady state -- it leaves the walk loop when the share `quorum0 / 32` of the lanes that still walk has
+    // stopped -- instead of waiting for its last walker before every event pass.
+    if (tail) quorum = max(1, (__popc(__ballot_sync(kFull, state == SU_WALK)) * quorum0) >> 5);
 
     // ---- a3: cell walk until fewer than `quorum` lanes are walking ----
 #pragma unroll 1

@@ -68,7 +68,7 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_pah", "mcrt_get_pah_absorbed",
            "mcrt_get_pah_emission_cdf", "mcrt_get_pah_temperature_distribution", "mcrt_set_observer",
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
-           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
+           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_tail_mode", "mcrt_set_source_order",
            "mcrt_set_density_staging", "mcrt_density_staging", "mcrt_set_region_sweeps", "mcrt_get_region_sweep_counts",
            "mcrt_get_batch_times", "mcrt_get_tables",
            "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_uniforms", "mcrt_gather_calibrate", "mcrt_last_error")
@@ -114,6 +114,7 @@ def lib():
         L.mcrt_reset_tallies.argtypes = [vp, i32]
         L.mcrt_set_launch.argtypes = [vp, i32, i32]
         L.mcrt_set_walk_quorum.argtypes = [vp, i32]
+        L.mcrt_set_tail_mode.argtypes = [vp, i32]
         L.mcrt_set_source_order.argtypes = [vp, i32]
         L.mcrt_set_region_sweeps.argtypes = [vp, i32, i32, i32, i32]
         L.mcrt_set_region_sweeps.restype = C.c_int
@@ -143,7 +144,7 @@ def lib():
                      "mcrt_get_pah_temperature_distribution", "mcrt_get_cell_temperature",
                      "mcrt_get_sed", "mcrt_set_observer", "mcrt_get_sed_mu", "mcrt_get_image",
                      "mcrt_get_counters", "mcrt_reset_tallies",
-                     "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_source_order",
+                     "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_tail_mode", "mcrt_set_source_order",
                      "mcrt_get_batch_times",
                      "mcrt_get_tables",
                      "mcrt_philox_blocks", "mcrt_uniforms"):
@@ -421,6 +422,9 @@ class Context:
 
     def set_walk_quorum(self, quorum):
         self._check(lib().mcrt_set_walk_quorum(self.h, int(quorum)), "mcrt_set_walk_quorum")
+
+    def set_tail_mode(self, mode):
+        self._check(lib().mcrt_set_tail_mode(self.h, int(mode)), "mcrt_set_tail_mode")
 
     def set_region_sweeps(self, sweeps, shape=(0, 0, 0)):
         self._check(lib().mcrt_set_region_sweeps(self.h, int(sweeps), *[int(v) for v in shape]),

@@ -356,6 +356,29 @@ def test_walk_quorum_does_not_change_results(M):
     _assert_identical(a, c)
 
 
+@pytest.mark.parametrize("maker", [
+    lambda: W.c0(),                                                         # density staged in shared memory
+    lambda: W.c1(tau_v=10.0, n_packets=300_000, batch=100_000),            # macro cubes
+    lambda: W.c2(n_root=32, n_packets=300_000, batch=100_000),             # cubes and subcubes
+    lambda: W.c4(n_root=24, n_packets=90_000, batch=30_000, corr_cells=3.0),
+    lambda: W.tiny_random(n_root=3, sub=8, n_refined=5, seed=11, external=True, n_packets=40_000, batch=10_000)])
+def test_end_of_batch_modes_do_not_change_results(M, maker):
+    """mcrt_set_tail_mode: how a warp schedules its last packages once the work queue is empty is
+    scheduling only -- tallies, SED, temperatures and every counter stay bit-identical."""
+    wl = maker()
+    runs = []
+    for mode in (0, 1, -1):
+        ctx = M.from_workload(wl)
+        ctx.set_tail_mode(mode)
+        for first, cnt in wl.batches():
+            ctx.run_batch(wl.seed, first, cnt)
+        runs.append(ctx)
+    for r in runs[1:]:
+        _assert_identical(runs[0], r)
+    c = runs[1].get_counters()
+    assert c["emitted"] == c["escaped"] == wl.n_packets and c["lost"] == 0
+
+
 @pytest.mark.parametrize("layout", [1, 2])
 def test_split_batch_halves_equal_run_batch(M, layout):
     """transport_batch + update_temperature(sum in slot order) == run_batch (multi-GPU path,
