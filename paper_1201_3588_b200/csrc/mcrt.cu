@@ -48,6 +48,11 @@ struct mcrt_ctx {
   double Ltot = 0;
   // tallies: [0] work-queue head, [1..CNT_N] counters, then sed[3*nb], emit_bin[nb]
   unsigned long long* d_small = nullptr;
+  unsigned long long* d_heads = nullptr;  // two work-queue heads used in turn: a launch zeroes the one its successor takes
+  int head = 0;
+  const void* occ_kern = nullptr;         // launch set-up of the transport kernel done for this (kernel, threads, bytes)
+  int occ_threads = 0, occ_resident = 0;
+  size_t occ_smem = 0;
   unsigned long long Ncum = 0;            // packages this context has transported since the last reset
   unsigned long long Nglobal = 0;         // packages of ALL ranks behind the temperatures (= Ncum on one GPU)
   cudaStream_t last_stream = nullptr;
@@ -477,6 +482,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
   cudaFree(ctx->d_lut); cudaFree(ctx->d_lut_marked); cudaFree(ctx->d_lut_plain2); cudaFree(ctx->d_rec);
   cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]); cudaFree(ctx->d_swcnt); cudaFree(ctx->d_regcnt);
+  cudaFree(ctx->d_heads);
   cudaFree(ctx->d_bits); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
@@ -620,7 +626,12 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   TransportParams P;
   P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.tally32 = tally32; P.trow = ctx->d_trow;
   P.opac = ctx->d_opac; P.cdf = ctx->d_cdf; P.csrc = ctx->d_csrc32; P.csrc64 = ctx->d_csrc; P.src = ctx->d_src;
-  P.next = ctx->d_small; P.counters = ctx->d_small + 1;
+  if (!ctx->d_heads) {
+    CU(cudaMalloc(&ctx->d_heads, 16));
+    CU(cudaMemset(ctx->d_heads, 0, 16));
+  }
+  P.next = nullptr; P.next_reset = nullptr;                  // (set at each launch, below)
+  P.counters = ctx->d_small + 1;
   P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
   P.seed = seed; P.first = first; P.count = n;
   P.obs = ctx->obs;
@@ -653,7 +664,6 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
     ctx->launches += 3;
     P.perm = ctx->d_perm;
   }
-  CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
   const int threads = ctx->threads;
   // resident blocks per SM: the caller's choice, else 5 (48-register kernels), except 4 for the
   // single-level kernel on HBM-resident grids (bricked storage), where more threads thrash the L1
@@ -715,12 +725,17 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
       : dens == 1 ? k_transport_u<5, false, 1, false, false, false>
       : dens == 2 ? k_transport_u<5, false, 2, false, false, false>
                   : (five ? k_transport_u<5, false, 0, false, false, false> : k_transport_u<4, false, 0, false, false, false>);
-  if (smem > (48u << 10)) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  if (dens) CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-  int resident = 0;                                          // large tables (many bins) lower the residency:
-  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem));   // size the grid to what fits
+  int resident = ctx->occ_resident;                          // large tables (many bins) lower the residency:
+  if (ctx->occ_kern != (const void*)kern || ctx->occ_threads != threads || ctx->occ_smem != smem) {
+    if (smem > (48u << 10)) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (dens) CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem));   // size the grid to what fits
+    ctx->occ_kern = (const void*)kern; ctx->occ_threads = threads; ctx->occ_smem = smem; ctx->occ_resident = resident;
+  }
   if (resident < 1) return fail(ctx, MCRT_EINVAL, "mcrt_run_batch: the transport kernel does not fit on an SM with these tables");
   if ((long long)ctx->sm_count * resident < grid) grid = (long long)ctx->sm_count * resident;
+  PU.base.next = ctx->d_heads + ctx->head; PU.base.next_reset = ctx->d_heads + (ctx->head ^ 1);
+  ctx->head ^= 1;
   kern<<<(unsigned)grid, threads, smem, st>>>(PU);
   ctx->launches++;
   CU(cudaGetLastError());
@@ -738,7 +753,8 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
       k_region_hist<<<gblocks, 256, sizeof(unsigned int) * nreg, st>>>(list_in, n_in, nreg, ctx->d_regcnt);
       k_scan_sources<<<1, 32, 0, st>>>(ctx->d_regcnt, ctx->d_regcnt + nreg, nreg);
       k_region_scatter<<<gblocks, 256, sizeof(unsigned int) * 2 * nreg, st>>>(list_in, n_in, nreg, ctx->d_regcnt + nreg, ctx->d_perm);
-      CU(cudaMemsetAsync(ctx->d_small, 0, 8, st));
+      PU.base.next = ctx->d_heads + ctx->head; PU.base.next_reset = ctx->d_heads + (ctx->head ^ 1);
+      ctx->head ^= 1;
       PU.base.perm = ctx->d_perm;
       PU.resume = 1; PU.count_dev = n_in;
       PU.lut = sw == sweeps ? ctx->d_lut_plain2 : ctx->d_lut_marked;

@@ -64,6 +64,8 @@ struct TransportParams {
   uint32_t* __restrict__ pah_cnt;              // [slots][nb] packages absorbed by the PAH, per leaf and bin
   const float* __restrict__ pah_cdf;           // [slots][nb] emission CDF of each leaf's PAH (frozen in a batch)
   unsigned long long* next;                    // work-queue head (packet offset within the batch)
+  unsigned long long* next_reset;              // the head the NEXT launch will use: set to 0 by this one (two heads
+                                               // alternate, so no launch needs a memset of its own in front of it)
   const uint32_t* __restrict__ perm;           // NULL, or the batch's package numbers grouped by source
   unsigned long long* sed;                     // [3][nb]
   unsigned long long* emit_bin;                // [nb]

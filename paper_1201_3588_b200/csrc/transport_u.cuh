@@ -482,6 +482,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   for (int i = threadIdx.x; i < P.nb; i += blockDim.x) { s_opac[i] = P.opac[i]; s_emit[i] = 0; }
   for (int i = threadIdx.x; i < 3 * P.nb; i += blockDim.x) s_sed[i] = 0;
   for (int i = threadIdx.x; i < n_lut; i += blockDim.x) s_lut[i] = PU.lut[i];
+  if (blockIdx.x == 0 && threadIdx.x == 0) *P.next_reset = 0ull;
   DensU D;
   D.rho = P.rho; D.base = 0; D.v0 = PU.pal0; D.v1 = PU.pal1;
   if (DENS != 0) {
