@@ -151,8 +151,10 @@ mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, ui
                                     void* cuda_stream);
 
 /* The same exchange with HALF the bytes and no layout conversion (what sharding.ShardedRunner uses):
- * mcrt_transport_batch_delta zeroes `delta_dev` (DEVICE, uint32[mcrt_store_slots], owned by the
- * caller, e.g. a torch int32 tensor), then transports this rank's packets tallying the batch's
+ * mcrt_transport_batch_delta zeroes `delta_dev` (DEVICE, uint32[mcrt_delta_words], owned by the
+ * caller, e.g. a torch int32 tensor: mcrt_store_slots words for the grains in equilibrium, followed --
+ * once a PAH is declared (mcrt_set_pah) -- by mcrt_store_slots x n_bins words for the PAH's absorbed
+ * spectrum of every leaf), then transports this rank's packets tallying the batch's
  * absorptions into it instead of into the cumulative tally; the ranks all-reduce (sum) their delta
  * arrays; mcrt_accumulate_update adds the summed delta to the context's cumulative tally and
  * updates the temperatures with n_cum = packages emitted so far by ALL ranks (one kernel).  The
@@ -160,6 +162,7 @@ mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, ui
  * subcubes behind it): opaque to the caller, identical on every rank that created the same grid.
  * After the call every rank's mcrt_get_cell_energy returns the global cumulative counts. */
 int64_t mcrt_store_slots(const mcrt_ctx* ctx);
+int64_t mcrt_delta_words(const mcrt_ctx* ctx);
 mcrt_status mcrt_transport_batch_delta(mcrt_ctx* ctx, uint64_t seed, uint64_t first_packet_id,
                                        uint64_t n_packets, uint32_t* delta_dev, void* cuda_stream);
 mcrt_status mcrt_accumulate_update(mcrt_ctx* ctx, const uint32_t* delta_sum_dev, uint64_t n_cum,
@@ -265,7 +268,7 @@ mcrt_status mcrt_get_image(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);
  * 4 pi sum_j C_j B_j(T) dnu_j / (U_k - U_k-1)), and the emission CDF sum_k P_k C_j B_j(T_k) dnu_j
  * (R39).  n_Tp = 0 takes the defaults 128 states, 5 K .. 1e4 K; theta_K <= 0 takes 500 K.
  * Calling mcrt_set_opacity again drops the PAH; mcrt_reset_tallies(bit 1) zeroes its tallies.
- * Host pointers.  Not combined with mcrt_transport_batch_delta yet (MCRT_ESTATE). */
+ * Host pointers.  Packet-sharded batches carry the PAH's tallies in the same delta array (mcrt_delta_words). */
 typedef struct {
   int32_t n_C;            /* carbon atoms per molecule, >= 1                                    */
   double mass_fraction;   /* of the dust mass, (0, 1]                                           */

@@ -613,6 +613,8 @@ static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
   return MCRT_OK;
 }
 
+// tally32 != NULL (packet-sharded batch): uint32[store slots] for the equilibrium grains, followed -- when a PAH is
+// declared -- by uint32[store slots][n_bins] for the PAH's absorbed spectrum; this batch's counts only.
 static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st,
                                     uint32_t* tally32 = nullptr) {
   if (n == 0) return MCRT_OK;
@@ -635,7 +637,8 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   P.sed = ctx->d_small + 1 + CNT_N; P.emit_bin = P.sed + 3 * (size_t)nb;
   P.seed = seed; P.first = first; P.count = n;
   P.obs = ctx->obs;
-  P.pah_q = ctx->pah ? ctx->d_pah_q : nullptr; P.pah_cnt = ctx->d_pah_cnt; P.pah_cdf = ctx->d_pah_cdf;
+  P.pah_q = ctx->pah ? ctx->d_pah_q : nullptr; P.pah_cdf = ctx->d_pah_cdf;
+  P.pah_cnt = (ctx->pah && tally32) ? tally32 + ctx->store_slots : ctx->d_pah_cnt;
   P.N = ctx->N; P.S = ctx->S; P.nb = nb; P.nT = ctx->nT; P.nsrc = ctx->nsrc; P.n3 = (int)ctx->store_n3;
 #ifdef MCRT_CHECKS
   CU(cudaMemcpyToSymbolAsync(g_mcrt_nstore, &ctx->store_slots, sizeof(long long), 0, cudaMemcpyHostToDevice, st));
@@ -887,19 +890,22 @@ mcrt_status mcrt_update_temperature(mcrt_ctx* ctx, const uint64_t* tally_sum, ui
 }
 
 int64_t mcrt_store_slots(const mcrt_ctx* ctx) { return ctx ? ctx->store_slots : -1; }
+int64_t mcrt_delta_words(const mcrt_ctx* ctx) {
+  if (!ctx) return -1;
+  return ctx->store_slots * (ctx->pah ? 1 + (int64_t)ctx->nb : 1);
+}
 
 mcrt_status mcrt_transport_batch_delta(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, uint32_t* delta_dev,
                                        void* stream_) {
   if (!ctx) return MCRT_EINVAL;
   if (!ctx->have_source) return fail(ctx, MCRT_ESTATE, "mcrt_transport_batch_delta: grid, opacity and sources must be set first");
   if (!delta_dev) return fail(ctx, MCRT_EINVAL, "mcrt_transport_batch_delta: NULL delta buffer");
-  if (ctx->pah) return fail(ctx, MCRT_ESTATE, "mcrt_transport_batch_delta: packet-sharded batches do not carry the PAH tallies yet");
   cudaStream_t st = (cudaStream_t)stream_;
   BatchEvents ev;
   mcrt_status rc = begin_batch(ctx, &ev);
   if (rc != MCRT_OK) return rc;
   CU(cudaEventRecord(ev.e0, st));
-  CU(cudaMemsetAsync(delta_dev, 0, sizeof(uint32_t) * (size_t)ctx->store_slots, st));
+  CU(cudaMemsetAsync(delta_dev, 0, sizeof(uint32_t) * (size_t)mcrt_delta_words(ctx), st));
   rc = launch_transport(ctx, seed, first, n, st, delta_dev);
   if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
   CU(cudaEventRecord(ev.e1, st));
@@ -916,6 +922,13 @@ mcrt_status mcrt_accumulate_update(mcrt_ctx* ctx, const uint32_t* delta_sum_dev,
   if (!delta_sum_dev || n_cum == 0) return fail(ctx, MCRT_EINVAL, "mcrt_accumulate_update: NULL delta / n_cum = 0");
   cudaStream_t st = (cudaStream_t)stream_;
   ctx->Nglobal = n_cum;
+  if (ctx->pah) {                                            // the PAH's absorbed spectra of the batch, all ranks
+    const long long nw = (long long)ctx->store_slots * ctx->nb;
+    k_add_u32<<<(unsigned)std::min<long long>((nw + 1023) / 1024, (long long)ctx->sm_count * 16), 256, 0, st>>>(
+        ctx->d_pah_cnt, delta_sum_dev + ctx->store_slots, nw);
+    ctx->launches++;
+    CU(cudaGetLastError());
+  }
   mcrt_status rc = launch_update(ctx, ctx->d_tally, n_cum, st, delta_sum_dev);
   ctx->last_stream = st;
   return rc;

@@ -227,4 +227,13 @@ __global__ void k_rows_store_to_ext(const T* __restrict__ store, T* __restrict__
   ext[e] = store[(size_t)slot_of(lay, ix, iy, iz) * nb + j];
 }
 
+// packet-sharded batches: the PAH counts of one batch (summed over ranks) join the cumulative ones
+__global__ void k_add_u32(uint32_t* __restrict__ acc, const uint32_t* __restrict__ delta, long long n) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const uint32_t d = delta[i];
+    if (d) acc[i] += d;
+  }
+}
+
 }  // namespace mcrt

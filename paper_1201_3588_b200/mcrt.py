@@ -62,7 +62,7 @@ class _Results(C.Structure):
 # every symbol include/mcrt.h declares
 SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opacity",
            "mcrt_set_source", "mcrt_run_batch", "mcrt_transport_batch",
-           "mcrt_update_temperature", "mcrt_store_slots", "mcrt_transport_batch_delta",
+           "mcrt_update_temperature", "mcrt_store_slots", "mcrt_delta_words", "mcrt_transport_batch_delta",
            "mcrt_accumulate_update", "mcrt_get_results", "mcrt_results_begin", "mcrt_results_wait",
            "mcrt_get_cell_energy",
            "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_pah", "mcrt_get_pah_absorbed",
@@ -95,6 +95,8 @@ def lib():
         L.mcrt_update_temperature.argtypes = [vp, vp, u64, vp]
         L.mcrt_store_slots.restype = i64
         L.mcrt_store_slots.argtypes = [vp]
+        L.mcrt_delta_words.restype = i64
+        L.mcrt_delta_words.argtypes = [vp]
         L.mcrt_transport_batch_delta.argtypes = [vp, u64, u64, u64, vp, vp]
         L.mcrt_accumulate_update.argtypes = [vp, vp, u64, vp]
         L.mcrt_get_results.argtypes = [vp, C.POINTER(_Results), C.c_int]
@@ -299,8 +301,9 @@ class Context:
         import torch
         if stream is None:
             stream = torch.cuda.current_stream().cuda_stream
-        if getattr(self, "_delta", None) is None:
-            self._delta = torch.empty(int(lib().mcrt_store_slots(self.h)), dtype=torch.int32, device="cuda")
+        words = int(lib().mcrt_delta_words(self.h))                # (grows when a PAH is declared)
+        if getattr(self, "_delta", None) is None or self._delta.numel() != words:
+            self._delta = torch.empty(words, dtype=torch.int32, device="cuda")
         self._check(lib().mcrt_transport_batch_delta(self.h, int(seed), int(first_packet_id), int(n_packets),
                                                      C.c_void_p(self._delta.data_ptr()), C.c_void_p(stream)),
                     "mcrt_transport_batch_delta")

@@ -138,8 +138,6 @@ def test_pah_reset_and_states(M):
         ctx.run_batch(wl.seed, f, c)
     first = (ctx.get_pah_absorbed().copy(), ctx.get_sed().copy(), ctx.get_pah_emission_cdf().copy())
     assert first[0].sum() > 500 and not np.array_equal(first[2], cold)
-    with pytest.raises(M.McrtError):
-        ctx.transport_batch_delta(wl.seed, 0, 10)                        # not combined with sharded batches yet
     ctx.reset_tallies(3)
     assert ctx.get_pah_absorbed().sum() == 0 and np.array_equal(ctx.get_pah_emission_cdf(), cold)
     for f, c in wl.batches():
@@ -149,3 +147,57 @@ def test_pah_reset_and_states(M):
     ctx.set_opacity(wl.lambda_edges_um, wl.weight, wl.kabs, wl.ksca, wl.g)   # a new opacity set drops the PAH
     with pytest.raises(M.McrtError):
         ctx.get_pah_absorbed()
+
+
+@pytest.mark.parametrize("maker,layout", [
+    (lambda: W.sphere(n_root=16, tau_v=2.0, gval=0.3, n_bins=32, n_packets=120_000, batch=40_000), 1),
+    (lambda: W.sphere(n_root=16, tau_v=2.0, gval=0.3, n_bins=32, n_packets=120_000, batch=40_000), 3),
+    (lambda: W.c2(n_root=24, n_packets=150_000, batch=50_000), 0)])
+def test_pah_two_emulated_ranks_equal_one(M, maker, layout):
+    """Packet-sharded batches with a PAH: the per-batch delta array carries the PAH's
+    absorbed spectrum of every leaf behind the equilibrium counts; two contexts playing two ranks end up with
+    the tallies, temperatures, P(T) and emission CDFs of the single-context run, bit for bit."""
+    from paper_1201_3588_b200.sharding import rank_range
+    wl = maker()
+    if wl.n_ref:
+        mix = (np.asarray(wl.weight)[:, None] * wl.kabs.astype(np.float64)).sum(axis=0)
+        kp = (np.asarray(wl.weight)[3:, None] * wl.kabs[3:].astype(np.float64)).sum(axis=0)
+        pah = W.Pah(n_C=100, mass_fraction=float(np.asarray(wl.weight)[3:].sum()),
+                    kabs=np.minimum(kp, mix).astype(np.float32), n_Tp=32)
+    else:
+        pah = W.pah_share(wl, n_C=100, mass_fraction=0.04)
+        pah.n_Tp = 32
+
+    def make():
+        ctx = M.from_workload(wl, layout=layout)
+        ctx.set_pah(pah.n_C, pah.mass_fraction, pah.kabs, n_Tp=pah.n_Tp)
+        return ctx
+
+    one = make()
+    for f, c in wl.batches():
+        one.run_batch(wl.seed, f, c)
+    ranks = [make(), make()]
+    words = int(M.lib().mcrt_delta_words(ranks[0].h))
+    assert words == int(M.lib().mcrt_store_slots(ranks[0].h)) * (1 + wl.n_bins)
+    done = 0
+    for first, cnt in wl.batches():
+        deltas = []
+        for r, ctx in enumerate(ranks):
+            f, c = rank_range(first, cnt, 2, r)
+            d = ctx.transport_batch_delta(wl.seed, f, c)
+            assert d.numel() == words
+            deltas.append(d)
+        total = deltas[0] + deltas[1]
+        done += cnt
+        for ctx in ranks:
+            ctx.accumulate_update(total, done)
+    assert one.get_pah_absorbed().sum() > 100
+    for ctx in ranks:
+        assert np.array_equal(ctx.get_cell_energy()[0], one.get_cell_energy()[0])
+        assert np.array_equal(ctx.get_cell_temperature(), one.get_cell_temperature())
+        assert np.array_equal(ctx.get_pah_absorbed(), one.get_pah_absorbed())
+        assert np.array_equal(ctx.get_pah_emission_cdf(), one.get_pah_emission_cdf())
+    assert np.array_equal(ranks[0].get_sed() + ranks[1].get_sed(), one.get_sed())
+    ca, cb, c1 = ranks[0].get_counters(), ranks[1].get_counters(), one.get_counters()
+    for k in c1:
+        assert np.array_equal(ca[k] + cb[k], c1[k]), k
