@@ -348,7 +348,7 @@ __device__ __forceinline__ void root_entry(const TransportParams& P, PacketU& p,
 // alternate the two registers and no instruction waits on the gather except its real use.
 // tau_rem > 0 always (u01 < 1, and a - b > 0 for a > b in IEEE arithmetic), so dtau >= tau_rem
 // implies rho*kappa > 0: no interaction in an empty leaf (R14).
-template <bool TL, int DENS, bool MACRO, bool REGION>
+template <bool TL, int DENS, bool MACRO, bool REGION, int INTERACT = SU_INTERACT>
 __device__ __forceinline__ void walk_step_u(const TransportParams& P, const DensU& D, PacketU& p, float& cur,
                                             float& nxt, float kx, uint32_t sublut, int& state, uint32_t& crossings) {
   if (TL) {
@@ -378,11 +378,12 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, const Dens
   if (!esc && !(REGION && cross)) { MCRT_CHECK_SLOT(nslot); nxt = density_at<DENS>(D, nslot); }
   const float dtau = cur * kx * (tnext - p.tcur);
   if (dtau >= p.tau_rem) {                                   // interaction inside this leaf
-    state = SU_INTERACT;
+    state = INTERACT;
   } else {
     p.tau_rem -= dtau;
     p.tcur = tnext;
-    if (!MACRO) ++crossings;                                 // MACRO: counted from the ends of the flight
+    if (TL && !MACRO) ++crossings;                           // MACRO: counted from the ends of the flight; single-level
+                                                             // grids: from the table cursors at the ends of the flight
     if (TL) {
       uint32_t cnew = csel + 4u;
       if (leave) {
@@ -392,20 +393,24 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, const Dens
         cnew = csel & ~63u;
         p.slot += lds_s32(cnew + 4u * (uint32_t)(kSubStride - 1));
         p.rslot = nslot;
-        if (a0) p.r0 += 4u; else if (a1) p.r1 += 4u; else p.r2 += 4u;
+        p.r0 = a0 ? p.r0 + 4u : p.r0; p.r1 = a1 ? p.r1 + 4u : p.r1; p.r2 = (!a0 && !a1) ? p.r2 + 4u : p.r2;
         p.cb |= kPending;
       } else {
         p.slot = nslot;
       }
-      if (a0) { p.t0 = fmaf(p.dt0, p.hs, p.t0); p.p0 = cnew; }
-      else if (a1) { p.t1 = fmaf(p.dt1, p.hs, p.t1); p.p1 = cnew; }
-      else { p.t2 = fmaf(p.dt2, p.hs, p.t2); p.p2 = cnew; }
+      const bool a2 = !a0 && !a1;
+      p.t0 = a0 ? fmaf(p.dt0, p.hs, p.t0) : p.t0; p.p0 = a0 ? cnew : p.p0;
+      p.t1 = a1 ? fmaf(p.dt1, p.hs, p.t1) : p.t1; p.p1 = a1 ? cnew : p.p1;
+      p.t2 = a2 ? fmaf(p.dt2, p.hs, p.t2) : p.t2; p.p2 = a2 ? cnew : p.p2;
       if (esc) {
         if (leave) { p.cb &= ~kPending; to_root_level(P, p); }   // left the grid from a subcube (rare)
         state = SU_ESCAPE;
       }
     } else {
-      if (a0) { p.t0 += p.dt0; p.p0 += 4u; } else if (a1) { p.t1 += p.dt1; p.p1 += 4u; } else { p.t2 += p.dt2; p.p2 += 4u; }
+      const bool a2 = !a0 && !a1;
+      p.t0 = a0 ? p.t0 + p.dt0 : p.t0; p.p0 = a0 ? p.p0 + 4u : p.p0;
+      p.t1 = a1 ? p.t1 + p.dt1 : p.t1; p.p1 = a1 ? p.p1 + 4u : p.p1;
+      p.t2 = a2 ? p.t2 + p.dt2 : p.t2; p.p2 = a2 ? p.p2 + 4u : p.p2;
       p.slot = nslot;
       if (esc) state = SU_ESCAPE;
       else if (REGION && cross) state = SU_SUSPEND;          // it now sits in the first cell of the next region
@@ -460,6 +465,10 @@ __device__ __forceinline__ void emit_position_u(const TransportParams& P, const 
 __device__ __forceinline__ uint32_t along(const PacketU& p, int f0, int f1, int f2) {
   return (uint32_t)((p.d0 > 0.f ? f0 : -f0) + (p.d1 > 0.f ? f1 : -f1) + (p.d2 > 0.f ? f2 : -f2));
 }
+
+// Single-level grids: every crossing moves exactly one of the three table cursors on by one entry, so the crossings
+// of a flight are the difference of this sum between its end and its start (R27; no counter in the walk loop).
+__device__ __forceinline__ uint32_t cursor_sum(const PacketU& p) { return (p.p0 + p.p1 + p.p2) >> 2; }
 
 // PAH: the instance that knows the transiently heated PAH (row f2).  A template parameter, not a run-time
 // branch: the third Philox block in the event pass costs registers and spills in every instance that
@@ -526,6 +535,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   for (;;) {
     // ---- a7: escaped packages -> SED; a8: refill from the work queue (one atomic per warp) ----
     if (state == SU_ESCAPE) {
+      if (!TL) n_cross += cursor_sum(p);
       if (MACRO || (P.obs.n_mu | P.obs.n_pix)) {             // exit point: cube from the cursors, offset from the t's
         int ix, iy, iz;                                      // (a package always leaves the grid at the root level)
         cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
@@ -550,6 +560,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       const unsigned sm = __ballot_sync(kFull, state == SU_SUSPEND);
       if (state == SU_SUSPEND) {
         int ix, iy, iz;
+        n_cross += cursor_sum(p);
         cell_of(p, p.p0, p.p1, p.p2, lut, N, ix, iy, iz);
         const unsigned key = (unsigned)(ix / PU.region_cells[0] + PU.regions_per_axis[0] *
                                         (iy / PU.region_cells[1] + PU.regions_per_axis[1] * (iz / PU.region_cells[2])));
@@ -586,6 +597,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
             const int cxy = __float_as_int(rc.x), ix = cxy & 0xffff, iy = cxy >> 16, iz = __float_as_int(rc.y);
             p.cb = __float_as_int(rc.z); p.k = (uint32_t)__float_as_int(rc.w);
             root_cursors(p, lut, N, ix, iy, iz, p.p0, p.p1, p.p2);
+            n_cross -= cursor_sum(p);
             p.slot = (int)slot_of(PU.lay, ix, iy, iz);
             MCRT_CHECK_SLOT(p.slot);
             p.rho = density_at<DENS>(D, p.slot);
@@ -614,6 +626,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       bool scatter = false;
       bool in_sub = TL && !is_new && p.hs < 1.f;             // the package sits in a subcube
       if (!is_new) {                                         // where the interaction happened
+        if (!TL) n_cross += cursor_sum(p);
         // it lies tau_rem / (rho kappa) further along this leaf's segment (rho kappa > 0 here)
         const float seg = fminf(p.t0, fminf(p.t1, p.t2)) - p.tcur;
         const float ak = p.rho * kx;
@@ -747,6 +760,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         if (MACRO) n_cross -= along(p, ix * P.S + sx, iy * P.S + sy, iz * P.S + sz);   // ... and the next one starts here
         if (TL && in_sub) begin_flight_sub(p, lut, sublut, N, P.S, ix, iy, iz, sx, sy, sz, ux, uy, uz);
         else begin_flight(p, lut, N, ix, iy, iz, ux, uy, uz);
+        if (!TL) n_cross -= cursor_sum(p);
         float u[4];
         draw4(P.seed, pid, p.k, kTagFlight, u);
         p.tau_rem = -logf(u[0]);
@@ -764,10 +778,13 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
     // ---- a3: cell walk until fewer than `quorum` lanes are walking ----
 #pragma unroll 1
     for (;;) {
-      if (state == SU_WALK) walk_step_u<TL, DENS, MACRO, REGION>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
-      if (state == SU_WALK) {
-        walk_step_u<TL, DENS, MACRO, REGION>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);
-        if (state == SU_INTERACT) state = SU_INTERACT_B;
+      // (pairs of steps per ballot: two on swept grids, where flights are long -- c4 32.5 -> 31.5 ms per batch;
+      // one elsewhere -- c1_tau1 0.325 -> 0.343 ms with two, c2 / c3 within 1 %)
+#pragma unroll
+      for (int rep = 0; rep < (REGION ? 2 : 1); ++rep) {
+        if (state == SU_WALK) walk_step_u<TL, DENS, MACRO, REGION>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
+        if (state == SU_WALK)
+          walk_step_u<TL, DENS, MACRO, REGION, SU_INTERACT_B>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);
       }
       if (__popc(__ballot_sync(kFull, state == SU_WALK)) < quorum) break;
     }
