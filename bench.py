@@ -502,7 +502,7 @@ def ctx_launch_desc(args):
             f"quorum={args.quorum or 'auto'} layout={args.layout or 'auto'}")
 
 
-def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
+def run_e2e_job(args, wl, mcrt, torch, dist, rank, world, stream):
     """End to end through the public API with HOST buffers: the job starts from host arrays
     (grid_create/set_opacity/set_source copy them H2D inside the timed region) and every step
     ends with a device->host read of that step's results (SED, counters, cell energies, cell
@@ -558,6 +558,18 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream):
                     "(H2D) + run_batch + host read-back of SED, counters, cell energy and "
                     "temperature after EVERY batch (pinned buffers; the read-out of batch k "
                     "overlaps batch k+1); wall clock, device-synchronised"}
+
+
+def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream, repeats=3):
+    """The whole job `repeats` times, each from scratch (new context, host arrays in, host results out); the
+    MEDIAN job is reported and every job's wall time is listed.  A ~10 ms job timed by wall clock once is at the
+    mercy of one slow cudaMalloc / cudaMallocHost (jobs of 13, 33 and 145 ms were seen back to back)."""
+    jobs = [run_e2e_job(args, wl, mcrt, torch, dist, rank, world, stream) for _ in range(repeats)]
+    order = sorted(range(repeats), key=lambda i: jobs[i]["job_ms"])
+    out = dict(jobs[order[repeats // 2]])
+    out["job_ms_all"] = [j["job_ms"] for j in jobs]
+    out["what"] += f"; the job is run {repeats} times from scratch, the median job is reported"
+    return out
 
 
 def relaunch_under_torchrun(args):

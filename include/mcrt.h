@@ -77,8 +77,9 @@ typedef struct {
                             single-level grid larger than the L2), 3 / 4 = macro cubes of 4^3 /
                             8^3 cells: a single-level grid run internally as a two-level one in
                             which a cube of cells that all hold the same density is crossed in
-                            one step (automatic, 4^3, when n_root is a multiple of 4 and at
-                            least 30 % of the cubes are uniform: a sphere or slab in vacuum).
+                            one step (on request only; n_root must be a multiple of 4 / 8: it
+                            pays where flights cross many uniform cubes, e.g. an optically thin
+                            sphere in vacuum -- DESIGN.md section 6).
                             Subcubes always follow the root grid as blocks of sub^3.           */
 } mcrt_grid_desc;
 

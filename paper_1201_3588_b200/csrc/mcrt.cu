@@ -324,24 +324,17 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
       src_sub = st_sub;
     }
   }
-  // ---- macro cubes: a single-level grid in which enough 4^3 (8^3) blocks of cells hold ONE density ----
-  if (k == 0 && (d->layout == 0 || d->layout >= 3)) {
+  // ---- macro cubes (on request: layout 3 / 4): a single-level grid run as a two-level one, 4^3 (8^3) blocks of
+  // cells that hold ONE density are crossed in one step.  Not automatic any more: since the plain walk takes 35
+  // instead of 42 instructions per crossing it is ahead on the 64^3 sphere for tau_V >= 1 (0.308 vs 0.316 ms per
+  // 2^20 packages at tau_V = 1, 0.603 vs 0.627 at 100); the macro cubes still win where flights are long and
+  // cross many uniform cubes (tau_V = 0.1: 0.212 vs 0.228 ms).  profiles/r02_summary.md
+  if (k == 0 && d->layout >= 3) {
     const int M = d->layout == 4 ? 8 : 4;
     if (d->n_root % M == 0 && d->n_root / M >= 2 && n3 + n3 / (M * M * M) < (1ll << 31)) {
       const int Nm = d->n_root / M;
       const long long nm3 = (long long)Nm * Nm * Nm;
-      unsigned int* d_cnt = nullptr;
-      CUG(cudaMalloc(&d_cnt, sizeof(unsigned int)));
-      CUG(cudaMemset(d_cnt, 0, sizeof(unsigned int)));
-      k_count_uniform_macros<<<(unsigned)((nm3 + 127) / 128), 128>>>(src_root, d->n_root, M, nm3, d_cnt);
-      unsigned int n_uniform = 0;
-      cudaError_t e1 = cudaMemcpy(&n_uniform, d_cnt, sizeof(unsigned int), cudaMemcpyDeviceToHost);
-      cudaFree(d_cnt);
-      if (e1 != cudaSuccess) return bail(fail(ctx, MCRT_ECUDA, std::string("macro count: ") + cudaGetErrorString(e1)));
-      ctx->launches++;
-      // automatic: when at least 30 % of the macro cubes are uniform (a sphere or a slab in vacuum; not a
-      // turbulent field) and the grid is not one the brick layout is meant for
-      if (d->layout >= 3 || ((double)n_uniform >= 0.3 * (double)nm3 && !ctx->lay.bricked)) {
+      {
         ctx->macro = M;
         ctx->n_fine = d->n_root;
         ctx->lay_fine.N = d->n_root; ctx->lay_fine.bricked = 2; ctx->lay_fine.nbk = Nm; ctx->lay_fine.bm = M;
@@ -404,13 +397,13 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     CUG(cudaMemset(ctx->d_rho, 0, sizeof(float) * ctx->store_slots));
     if (ctx->macro) {
       // the cells cube by cube behind the macro array; then one entry per macro cube: its density if all
-      // its cells hold the same one, else the marker (sign bit | cube number) that sends the walk to the cells
+      // its cells hold the same one, else the marker (sign bit | slot of its first cell) that sends the walk to the cells
       k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho + ctx->store_n3, ctx->lay_fine, n3);
       k_macro_entries<<<(unsigned)((ctx->n3 + 127) / 128), 128>>>(ctx->d_rho + ctx->store_n3, ctx->d_rho, ctx->n3,
-                                                                ctx->macro * ctx->macro * ctx->macro);
+                                                                ctx->macro * ctx->macro * ctx->macro, ctx->store_n3);
       ctx->launches++;
     } else if (ctx->uni) k_encode_uniform<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, ctx->d_rho, ctx->lay, n3);
-    else k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, ctx->lay, n3);
+    else k_encode_root<<<(unsigned)((n3 + 255) / 256), 256>>>(src_root, d_refidx, ctx->d_rho, ctx->lay, n3, ctx->store_n3, (int)s3);
   }
   ctx->launches++;
   if (k > 0) {

@@ -22,7 +22,7 @@
 //    cube's entry and keeps walking at the sub level (the subcube index on the exit axis wraps,
 //    the other two carry over: the faces of neighbouring refined cubes line up).  The density array
 //    doubles as the two-level index: if the entry that comes back has its
-//    sign bit set it is the number of a refined cube and the leaf slot just moves to that cube
+//    sign bit set it names a refined cube (by its first leaf slot) and the leaf slot just moves to that cube
 //    (integer arithmetic only); if not, the package has left the refined region and its exits move
 //    out to the faces of the root cube.  A package that meets a marker at the root level descends
 //    into the subcube its remaining distances to the root faces select.  Root-level and sub-level
@@ -207,7 +207,7 @@ struct PacketU {
   // two-level grids only (dead registers otherwise): state of a package inside a refined cube
   uint32_t r0, r1, r2;       // the root-level cursors while p0..p2 walk the sub table
   int rslot;                 // storage slot of the refined root cube
-  int kref;                  // its refined-cube number
+  int kref;                  // its first leaf slot (what the cube's marker in the root array holds)
   float hs;                  // leaf edge in root-cube edges: 1, or 1/S inside a refined cube
 };
 
@@ -276,7 +276,7 @@ __device__ __forceinline__ int sub_j(uint32_t cursor) {
 }
 
 // A package at the root level whose gathered "density" is the marker of a refined cube (sign bit
-// | refined-cube number k): descend into the subcube it is in.  Per axis the remaining distance to
+// | storage slot of its first subcube): descend into the subcube it is in.  Per axis the remaining distance to
 // the cube's exit face, in subcube edges, W = (t_a - tcur)|d_a| S, selects the subcube: m =
 // ceil(W) - 1 whole subcubes lie between the package's subcube and that face (a package exactly on
 // a subcube face belongs to the subcube it flies into: direction-aware as R7; the entry axis has
@@ -284,7 +284,7 @@ __device__ __forceinline__ int sub_j(uint32_t cursor) {
 __device__ __forceinline__ void descend(const TransportParams& P, PacketU& p, uint32_t sublut, float& cur) {
   const int S = P.S;
   const float fS = (float)S, hs = 1.f / fS;
-  const int kref = __float_as_int(cur) & 0x7fffffff;
+  const int kref = __float_as_int(cur) & 0x7fffffff;        // first leaf slot of the refined cube
   const int m0 = min(S - 1, max(0, (int)ceilf((p.t0 - p.tcur) * fabsf(p.d0) * fS) - 1));
   const int m1 = min(S - 1, max(0, (int)ceilf((p.t1 - p.tcur) * fabsf(p.d1) * fS) - 1));
   const int m2 = min(S - 1, max(0, (int)ceilf((p.t2 - p.tcur) * fabsf(p.d2) * fS) - 1));
@@ -298,7 +298,7 @@ __device__ __forceinline__ void descend(const TransportParams& P, PacketU& p, ui
   p.p1 = sub_cursor(sublut, 1, p.d1, j1);
   p.p2 = sub_cursor(sublut, 2, p.d2, j2);
   const int sx = p.d0 > 0.f ? j0 : m0, sy = p.d1 > 0.f ? j1 : m1, sz = p.d2 > 0.f ? j2 : m2;
-  p.slot = P.n3 + kref * (S * S * S) + sx + S * (sy + S * sz);
+  p.slot = kref + sx + S * (sy + S * sz);
   p.kref = kref;
   p.hs = hs;
   MCRT_CHECK_SLOT(p.slot);
@@ -331,7 +331,7 @@ __device__ __forceinline__ void root_entry(const TransportParams& P, PacketU& p,
     p.cb &= ~kPending;
     if (bits < 0) {
       const int kref = bits & 0x7fffffff;
-      p.slot += (kref - p.kref) * (P.S * P.S * P.S);
+      p.slot += kref - p.kref;
       p.kref = kref;
       MCRT_CHECK_SLOT(p.slot);
       cur = __ldg(P.rho + p.slot);
@@ -731,7 +731,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
               const int S = P.S;
               p.rslot = p.slot;
               p.kref = __float_as_int(p.rho) & 0x7fffffff;
-              p.slot = P.n3 + p.kref * (S * S * S) + sx + S * (sy + S * sz);
+              p.slot = p.kref + sx + S * (sy + S * sz);
               MCRT_CHECK_SLOT(p.slot);
               p.rho = __ldg(P.rho + p.slot);
               in_sub = true;
@@ -864,48 +864,30 @@ __global__ void k_encode_uniform(const float* __restrict__ rho_ext, float* __res
   float v = rho_ext[e];
   rho_store[slot_of(lay, ix, iy, iz)] = (v > 0.f) ? v : 0.f;
 }
-// Two-level grids: root array in storage order; density >= 0, or (sign bit | k) for the k-th
-// refined root cube (negative / NaN densities -> 0; padding slots stay 0)
+// Two-level grids: root array in storage order; density >= 0, or (sign bit | storage slot of its first subcube)
+// for a refined root cube (negative / NaN densities -> 0; padding slots stay 0)
 __global__ void k_encode_root(const float* __restrict__ rho_root, const int* __restrict__ refidx,
-                              float* __restrict__ out, LayoutU lay, long long n3) {
+                              float* __restrict__ out, LayoutU lay, long long n3, long long first_sub, int s3) {
   long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n3) return;
   int ix = (int)(e % lay.N), iy = (int)((e / lay.N) % lay.N), iz = (int)(e / ((long long)lay.N * lay.N));
   int k = refidx ? refidx[e] : -1;
   float v = rho_root[e];
   v = (v > 0.f) ? v : 0.f;
-  out[slot_of(lay, ix, iy, iz)] = k >= 0 ? __int_as_float((int)(0x80000000u | (unsigned)k)) : v;
+  out[slot_of(lay, ix, iy, iz)] = k >= 0 ? __int_as_float((int)(0x80000000u | (unsigned)(first_sub + (long long)k * s3))) : v;
 }
-// Macro cubes (single-level grids run as two-level ones, see MACRO in the kernel): how many M^3 blocks of
-// the caller's x-fastest density array hold one single (sanitised) value ...
-__global__ void k_count_uniform_macros(const float* __restrict__ rho_ext, int N, int M, long long nm3,
-                                       unsigned int* __restrict__ count) {
-  long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (m >= nm3) return;
-  const int Nm = N / M;
-  const int mx = (int)(m % Nm), my = (int)((m / Nm) % Nm), mz = (int)(m / ((long long)Nm * Nm));
-  float v0 = rho_ext[(long long)mx * M + (long long)N * ((long long)my * M + (long long)N * mz * M)];
-  v0 = v0 > 0.f ? v0 : 0.f;
-  bool same = true;
-  for (int z = 0; z < M && same; ++z)
-    for (int y = 0; y < M && same; ++y)
-      for (int x = 0; x < M; ++x) {
-        float v = rho_ext[(long long)(mx * M + x) + (long long)N * ((long long)(my * M + y) + (long long)N * (mz * M + z))];
-        v = v > 0.f ? v : 0.f;
-        if (v != v0) { same = false; break; }
-      }
-  if (same) atomicAdd(count, 1u);
-}
-// ... and the macro array itself from the cells stored cube by cube: the common density, or the marker
-// (sign bit | cube number) that sends the walk down to the cells.
-__global__ void k_macro_entries(const float* __restrict__ cells, float* __restrict__ macro, long long nm3, int m3) {
+// Macro cubes (single-level grids run as two-level ones, see MACRO in the kernel):
+// the macro array from the cells stored cube by cube: the common density, or the marker
+// (sign bit | storage slot of the cube's first cell) that sends the walk down to the cells.
+__global__ void k_macro_entries(const float* __restrict__ cells, float* __restrict__ macro, long long nm3, int m3,
+                                long long first_cell) {
   long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= nm3) return;
   const float* c = cells + m * m3;
   const float v0 = c[0];
   bool same = true;
   for (int i = 1; i < m3; ++i) if (c[i] != v0) { same = false; break; }
-  macro[m] = same ? v0 : __int_as_float((int)(0x80000000u | (unsigned)m));
+  macro[m] = same ? v0 : __int_as_float((int)(0x80000000u | (unsigned)(first_cell + m * m3)));
 }
 // storage order -> x-fastest output
 template <typename T>

@@ -356,19 +356,20 @@ def test_walk_quorum_does_not_change_results(M):
     _assert_identical(a, c)
 
 
-@pytest.mark.parametrize("maker", [
-    lambda: W.c0(),                                                         # density staged in shared memory
-    lambda: W.c1(tau_v=10.0, n_packets=300_000, batch=100_000),            # macro cubes
-    lambda: W.c2(n_root=32, n_packets=300_000, batch=100_000),             # cubes and subcubes
-    lambda: W.c4(n_root=24, n_packets=90_000, batch=30_000, corr_cells=3.0),
-    lambda: W.tiny_random(n_root=3, sub=8, n_refined=5, seed=11, external=True, n_packets=40_000, batch=10_000)])
-def test_end_of_batch_modes_do_not_change_results(M, maker):
+@pytest.mark.parametrize("maker,layout", [
+    (lambda: W.c0(), 0),                                                    # density staged in shared memory
+    (lambda: W.c1(tau_v=10.0, n_packets=300_000, batch=100_000), 0),       # plain single-level walk
+    (lambda: W.c1(tau_v=10.0, n_packets=300_000, batch=100_000), 3),       # macro cubes
+    (lambda: W.c2(n_root=32, n_packets=300_000, batch=100_000), 0),        # cubes and subcubes
+    (lambda: W.c4(n_root=24, n_packets=90_000, batch=30_000, corr_cells=3.0), 2),
+    (lambda: W.tiny_random(n_root=3, sub=8, n_refined=5, seed=11, external=True, n_packets=40_000, batch=10_000), 0)])
+def test_end_of_batch_modes_do_not_change_results(M, maker, layout):
     """mcrt_set_tail_mode: how a warp schedules its last packages once the work queue is empty is
     scheduling only -- tallies, SED, temperatures and every counter stay bit-identical."""
     wl = maker()
     runs = []
     for mode in (0, 1, -1):
-        ctx = M.from_workload(wl)
+        ctx = M.from_workload(wl, layout=layout)
         ctx.set_tail_mode(mode)
         for first, cnt in wl.batches():
             ctx.run_batch(wl.seed, first, cnt)
@@ -690,7 +691,7 @@ def _blocky(n_root, block, seed, external=True, n_packets=300_000, batch=100_000
 
 
 @pytest.mark.parametrize("maker,layout", [
-    (lambda: W.c1(tau_v=1.0, n_packets=600_000, batch=200_000), 0),      # automatic: 4^3 macro cubes
+    (lambda: W.c1(tau_v=1.0, n_packets=600_000, batch=200_000), 3),      # 4^3 macro cubes
     (lambda: W.c1(tau_v=10.0, n_packets=200_000, batch=50_000), 4),
     (lambda: W.sphere(n_root=32, tau_v=3.0, gval=0.3, n_packets=400_000, batch=100_000), 3),
     (lambda: _blocky(16, 4, 3), 3),
@@ -715,14 +716,11 @@ def test_macro_cubes_against_oracle_and_plain_walk(M, oracle_mod, maker, layout)
     _compare(b, orc, groups=PR.super_blocks(wl.n_root, 4), min_count=300)
 
 
-def test_macro_cubes_are_chosen_automatically_only_where_they_pay(M):
-    import ctypes
-    sphere = M.from_workload(W.c1(n_packets=10, batch=10))       # 64^3 sphere: 16^3 macro cubes
-    assert sphere.slots == 64 ** 3 and int(M.lib().mcrt_store_slots(sphere.h)) == 64 ** 3 + 16 ** 3
-    clumpy = M.from_workload(W.c4(n_root=24, n_packets=10, batch=10, corr_cells=3.0))
-    assert int(M.lib().mcrt_store_slots(clumpy.h)) == 24 ** 3   # no uniform cubes: plain grid
-    small = M.from_workload(W.c0(n_packets=10, batch=10))        # 16^3: 12 % uniform cubes: plain + staged
-    assert int(M.lib().mcrt_store_slots(small.h)) == 16 ** 3 and small.density_staging() == 1
+def test_macro_cubes_are_a_storage_layout_on_request(M):
+    sphere = M.from_workload(W.c1(n_packets=10, batch=10))       # 64^3 sphere, automatic layout: the plain grid
+    assert sphere.slots == 64 ** 3 and int(M.lib().mcrt_store_slots(sphere.h)) == 64 ** 3
+    macro = M.from_workload(W.c1(n_packets=10, batch=10), layout=3)      # 16^3 macro cubes in front of the cells
+    assert macro.slots == 64 ** 3 and int(M.lib().mcrt_store_slots(macro.h)) == 64 ** 3 + 16 ** 3
 
 
 def test_region_sweeps_with_sharded_batches_and_observer(M):
