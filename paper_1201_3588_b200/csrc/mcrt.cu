@@ -111,6 +111,7 @@ struct mcrt_ctx {
   double *d_kabs_eq = nullptr, *d_pah_C = nullptr, *d_pah_E = nullptr, *d_pah_T = nullptr, *d_pah_U = nullptr,
          *d_pah_Lam = nullptr, *d_pah_W = nullptr, *d_pah_P = nullptr;
   int* d_pah_J = nullptr;
+  unsigned long long* d_pah_next = nullptr;   // work-queue head of k_pah_update
   float *d_pah_q = nullptr, *d_pah_cdf = nullptr, *d_pah_cold = nullptr, *d_pah_W32 = nullptr;
   uint32_t* d_pah_cnt = nullptr;
   bool have_opacity = false, have_source = false;
@@ -139,11 +140,11 @@ static void free_opacity(mcrt_ctx* c) {
 }
 static void free_pah(mcrt_ctx* c) {
   cudaFree(c->d_kabs_eq); cudaFree(c->d_pah_C); cudaFree(c->d_pah_E); cudaFree(c->d_pah_T); cudaFree(c->d_pah_U);
-  cudaFree(c->d_pah_Lam); cudaFree(c->d_pah_W); cudaFree(c->d_pah_P); cudaFree(c->d_pah_J); cudaFree(c->d_pah_q);
+  cudaFree(c->d_pah_Lam); cudaFree(c->d_pah_W); cudaFree(c->d_pah_P); cudaFree(c->d_pah_J); cudaFree(c->d_pah_next); cudaFree(c->d_pah_q);
   cudaFree(c->d_pah_cdf); cudaFree(c->d_pah_cold); cudaFree(c->d_pah_cnt); cudaFree(c->d_pah_W32);
   c->d_pah_W32 = nullptr;
   c->d_kabs_eq = c->d_pah_C = c->d_pah_E = c->d_pah_T = c->d_pah_U = c->d_pah_Lam = c->d_pah_W = c->d_pah_P = nullptr;
-  c->d_pah_J = nullptr; c->d_pah_q = c->d_pah_cdf = c->d_pah_cold = nullptr; c->d_pah_cnt = nullptr;
+  c->d_pah_J = nullptr; c->d_pah_next = nullptr; c->d_pah_q = c->d_pah_cdf = c->d_pah_cold = nullptr; c->d_pah_cnt = nullptr;
   c->pah = false;
 }
 static void free_observer(mcrt_ctx* c) {
@@ -765,7 +766,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
 
 // a9 for the PAH (pah.cuh): P(T) and emission CDF of every leaf from its absorbed spectrum
 static size_t pah_smem_bytes(const mcrt_ctx* ctx, int warps) {
-  return sizeof(double) * (size_t)warps * (2 * (size_t)ctx->nb + ctx->pahd.K);
+  return sizeof(double) * (size_t)warps * (size_t)pah_warp_doubles(ctx->nb, ctx->pahd.K);
 }
 static mcrt_status launch_pah_update(mcrt_ctx* ctx, uint64_t n_cum, cudaStream_t st, long long only_slot) {
   if (n_cum == 0) return MCRT_OK;
@@ -778,9 +779,12 @@ static mcrt_status launch_pah_update(mcrt_ctx* ctx, uint64_t n_cum, cudaStream_t
   long long blocks = only_slot >= 0 ? 1 : (ctx->store_slots + warps - 1) / warps;
   const long long cap = (long long)ctx->sm_count * 16;
   if (blocks > cap) blocks = cap;
+  if (!ctx->d_pah_next) CU(cudaMalloc(&ctx->d_pah_next, 8));
+  CU(cudaMemsetAsync(ctx->d_pah_next, 0, 8, st));            // work queue of leaves
   k_pah_update<<<(unsigned)blocks, 32 * (only_slot >= 0 ? 1 : warps), smem, st>>>(
       ctx->pahd, ctx->d_rho, ctx->d_pah_cnt, ctx->d_pah_cdf, ctx->store_slots,
-      ctx->uni ? ctx->store_slots : ctx->store_n3, ctx->Ltot / (double)n_cum, V, 1.0 / s3, only_slot, ctx->d_pah_P);
+      ctx->uni ? ctx->store_slots : ctx->store_n3, ctx->Ltot / (double)n_cum, V, 1.0 / s3, only_slot, ctx->d_pah_P,
+      ctx->d_pah_next);
   ctx->launches++;
   CU(cudaGetLastError());
   return MCRT_OK;
