@@ -33,6 +33,8 @@ UNIT = "packets/s"
 def make_workload(name: str):
     """Bench workloads.  c1_tau1 = BASELINE.json configs[1] at tau_V = 1 (the configuration the
     10^8 packets/s target is quoted on)."""
+    if name == "c1_tau1_pah":                                # row f2: the tau_V = 1 sphere with a transiently heated PAH
+        return W.c1(tau_v=1.0)
     if name.startswith("c1_tau"):
         return W.c1(tau_v=float(name[6:]))
     if name == "c0":
@@ -341,6 +343,9 @@ def measure_workload(torch, mcrt, wl, name, steps, warmup, stream, flush, args, 
     """One entry of per_config: a fresh context, `warmup` + `steps` batches on this GPU."""
     from paper_1201_3588_b200.sharding import ShardedRunner
     ctx = mcrt.from_workload(wl)
+    if name.endswith("_pah"):       # a 100-C PAH holding 5 % of the dust mass (workloads.pah_share), 128 temperature states
+        pah = W.pah_share(wl, n_C=100, mass_fraction=0.05)
+        ctx.set_pah(pah.n_C, pah.mass_fraction, pah.kabs, n_Tp=128)
     runner = ShardedRunner(ctx, None)
     r = time_steps(torch, ctx, wl, runner, stream, 1, steps, warmup, flush, torch.cuda.synchronize)
     secs = float(sum(r["step_ms"])) * 1e-3
@@ -361,7 +366,8 @@ def measure_workload(torch, mcrt, wl, name, steps, warmup, stream, flush, args, 
     return out
 
 
-PER_CONFIG = (("c0", 6), ("c1_tau0.1", 4), ("c1_tau10", 4), ("c1_tau100", 4), ("c2", 3), ("c3", 3), ("c4", 3))
+PER_CONFIG = (("c0", 6), ("c1_tau0.1", 4), ("c1_tau10", 4), ("c1_tau100", 4), ("c2", 3), ("c3", 3), ("c4", 3),
+              ("c1_tau1_pah", 4))
 
 
 def run_gpu(args, wl, name):
