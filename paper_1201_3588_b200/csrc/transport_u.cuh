@@ -418,6 +418,180 @@ __device__ __forceinline__ void walk_step_u(const TransportParams& P, const Dens
   }
 }
 
+// The same two steps for single-level grids with global gathers, written in PTX as ONE block: the axis update stays
+// predicated, nothing is recomputed, and a package that stops in the first step leaves without a second test.
+// Same operations in the same order as walk_step_u (so the results are bit-identical; the checked build keeps the
+// C++ form).  States: 1 = SU_INTERACT, 5 = SU_INTERACT_B (the leaf's density is in the second register), 2 =
+// SU_ESCAPE, 6 = SU_SUSPEND; table marks: INT_MIN = kLutEscape, INT_MIN + 2 = kLutRegion.
+static_assert(SU_WALK == 0 && SU_INTERACT == 1 && SU_ESCAPE == 2 && SU_INTERACT_B == 5 && SU_SUSPEND == 6, "walk_pair_ptx");
+static_assert(kLutEscape == -2147483647 - 1 && kLutRegion == -2147483646, "walk_pair_ptx");
+template <bool REGION>
+__device__ __forceinline__ void walk_pair_ptx(const float* __restrict__ rho, PacketU& p, float& rho_a, float& rho_b,
+                                              const float kx, const uint32_t lut2, int& state) {
+  if (REGION) {
+    asm volatile(
+        "{\n"
+        ".reg .pred a0, a01, na0, a1, ne, hit, rg, ldp, stop;\n"
+        ".reg .f32 tn, ds, s, dtau;\n"
+        ".reg .u32 c, c2;\n"
+        ".reg .s32 dl, ns;\n"
+        ".reg .u64 ad;\n"
+        "min.f32 tn, %1, %2;\n"
+        "min.f32 tn, %0, tn;\n"
+        "setp.eq.f32 a0, %0, tn;\n"
+        "setp.eq.or.f32 a01, %1, tn, a0;\n"
+        "selp.u32 c, %5, %6, a0;\n"
+        "selp.u32 c, c, %7, a01;\n"
+        "ld.shared.s32 dl, [c];\n"
+        "setp.eq.s32 rg, dl, -2147483646;\n"
+        "add.u32 c2, c, %17;\n"
+        "@rg ld.shared.s32 dl, [c2];\n"
+        "setp.ne.s32 ne, dl, -2147483648;\n"
+        "add.s32 ns, %8, dl;\n"
+        "mul.wide.s32 ad, ns, 4;\n"
+        "add.u64 ad, ad, %16;\n"
+        "and.pred ldp, ne, !rg;\n"
+        "@ldp ld.global.nc.f32 %11, [ad];\n"
+        "sub.f32 ds, tn, %3;\n"
+        "mul.f32 s, %10, %15;\n"
+        "mul.f32 dtau, s, ds;\n"
+        "setp.ge.f32 hit, dtau, %4;\n"
+        "@hit mov.s32 %9, 1;\n"
+        "@hit bra MCRT_PAIR_DONE;\n"
+        "sub.f32 %4, %4, dtau;\n"
+        "mov.f32 %3, tn;\n"
+        "mov.s32 %8, ns;\n"
+        "not.pred na0, a0;\n"
+        "and.pred a1, a01, na0;\n"
+        "@a0 add.f32 %0, %0, %12;\n"
+        "@a0 add.u32 %5, %5, 4;\n"
+        "@a1 add.f32 %1, %1, %13;\n"
+        "@a1 add.u32 %6, %6, 4;\n"
+        "@!a01 add.f32 %2, %2, %14;\n"
+        "@!a01 add.u32 %7, %7, 4;\n"
+        "@rg mov.s32 %9, 6;\n"
+        "@!ne mov.s32 %9, 2;\n"
+        "or.pred stop, rg, !ne;\n"
+        "@stop bra MCRT_PAIR_DONE;\n"
+        "min.f32 tn, %1, %2;\n"
+        "min.f32 tn, %0, tn;\n"
+        "setp.eq.f32 a0, %0, tn;\n"
+        "setp.eq.or.f32 a01, %1, tn, a0;\n"
+        "selp.u32 c, %5, %6, a0;\n"
+        "selp.u32 c, c, %7, a01;\n"
+        "ld.shared.s32 dl, [c];\n"
+        "setp.eq.s32 rg, dl, -2147483646;\n"
+        "add.u32 c2, c, %17;\n"
+        "@rg ld.shared.s32 dl, [c2];\n"
+        "setp.ne.s32 ne, dl, -2147483648;\n"
+        "add.s32 ns, %8, dl;\n"
+        "mul.wide.s32 ad, ns, 4;\n"
+        "add.u64 ad, ad, %16;\n"
+        "and.pred ldp, ne, !rg;\n"
+        "@ldp ld.global.nc.f32 %10, [ad];\n"
+        "sub.f32 ds, tn, %3;\n"
+        "mul.f32 s, %11, %15;\n"
+        "mul.f32 dtau, s, ds;\n"
+        "setp.ge.f32 hit, dtau, %4;\n"
+        "@hit mov.s32 %9, 5;\n"
+        "@hit bra MCRT_PAIR_DONE;\n"
+        "sub.f32 %4, %4, dtau;\n"
+        "mov.f32 %3, tn;\n"
+        "mov.s32 %8, ns;\n"
+        "not.pred na0, a0;\n"
+        "and.pred a1, a01, na0;\n"
+        "@a0 add.f32 %0, %0, %12;\n"
+        "@a0 add.u32 %5, %5, 4;\n"
+        "@a1 add.f32 %1, %1, %13;\n"
+        "@a1 add.u32 %6, %6, 4;\n"
+        "@!a01 add.f32 %2, %2, %14;\n"
+        "@!a01 add.u32 %7, %7, 4;\n"
+        "@rg mov.s32 %9, 6;\n"
+        "@!ne mov.s32 %9, 2;\n"
+        "MCRT_PAIR_DONE:\n"
+        "}\n"
+        : "+f"(p.t0), "+f"(p.t1), "+f"(p.t2), "+f"(p.tcur), "+f"(p.tau_rem), "+r"(p.p0), "+r"(p.p1), "+r"(p.p2),
+          "+r"(p.slot), "+r"(state), "+f"(rho_a), "+f"(rho_b)
+        : "f"(p.dt0), "f"(p.dt1), "f"(p.dt2), "f"(kx), "l"(rho), "r"(lut2)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n"
+        ".reg .pred a0, a01, na0, a1, ne, hit, rg, ldp, stop;\n"
+        ".reg .f32 tn, ds, s, dtau;\n"
+        ".reg .u32 c, c2;\n"
+        ".reg .s32 dl, ns;\n"
+        ".reg .u64 ad;\n"
+        "min.f32 tn, %1, %2;\n"
+        "min.f32 tn, %0, tn;\n"
+        "setp.eq.f32 a0, %0, tn;\n"
+        "setp.eq.or.f32 a01, %1, tn, a0;\n"
+        "selp.u32 c, %5, %6, a0;\n"
+        "selp.u32 c, c, %7, a01;\n"
+        "ld.shared.s32 dl, [c];\n"
+        "setp.ne.s32 ne, dl, -2147483648;\n"
+        "add.s32 ns, %8, dl;\n"
+        "mul.wide.s32 ad, ns, 4;\n"
+        "add.u64 ad, ad, %16;\n"
+        "@ne ld.global.nc.f32 %11, [ad];\n"
+        "sub.f32 ds, tn, %3;\n"
+        "mul.f32 s, %10, %15;\n"
+        "mul.f32 dtau, s, ds;\n"
+        "setp.ge.f32 hit, dtau, %4;\n"
+        "@hit mov.s32 %9, 1;\n"
+        "@hit bra MCRT_PAIR_DONE;\n"
+        "sub.f32 %4, %4, dtau;\n"
+        "mov.f32 %3, tn;\n"
+        "mov.s32 %8, ns;\n"
+        "not.pred na0, a0;\n"
+        "and.pred a1, a01, na0;\n"
+        "@a0 add.f32 %0, %0, %12;\n"
+        "@a0 add.u32 %5, %5, 4;\n"
+        "@a1 add.f32 %1, %1, %13;\n"
+        "@a1 add.u32 %6, %6, 4;\n"
+        "@!a01 add.f32 %2, %2, %14;\n"
+        "@!a01 add.u32 %7, %7, 4;\n"
+        "@!ne mov.s32 %9, 2;\n"
+        "@!ne bra MCRT_PAIR_DONE;\n"
+        "min.f32 tn, %1, %2;\n"
+        "min.f32 tn, %0, tn;\n"
+        "setp.eq.f32 a0, %0, tn;\n"
+        "setp.eq.or.f32 a01, %1, tn, a0;\n"
+        "selp.u32 c, %5, %6, a0;\n"
+        "selp.u32 c, c, %7, a01;\n"
+        "ld.shared.s32 dl, [c];\n"
+        "setp.ne.s32 ne, dl, -2147483648;\n"
+        "add.s32 ns, %8, dl;\n"
+        "mul.wide.s32 ad, ns, 4;\n"
+        "add.u64 ad, ad, %16;\n"
+        "@ne ld.global.nc.f32 %10, [ad];\n"
+        "sub.f32 ds, tn, %3;\n"
+        "mul.f32 s, %11, %15;\n"
+        "mul.f32 dtau, s, ds;\n"
+        "setp.ge.f32 hit, dtau, %4;\n"
+        "@hit mov.s32 %9, 5;\n"
+        "@hit bra MCRT_PAIR_DONE;\n"
+        "sub.f32 %4, %4, dtau;\n"
+        "mov.f32 %3, tn;\n"
+        "mov.s32 %8, ns;\n"
+        "not.pred na0, a0;\n"
+        "and.pred a1, a01, na0;\n"
+        "@a0 add.f32 %0, %0, %12;\n"
+        "@a0 add.u32 %5, %5, 4;\n"
+        "@a1 add.f32 %1, %1, %13;\n"
+        "@a1 add.u32 %6, %6, 4;\n"
+        "@!a01 add.f32 %2, %2, %14;\n"
+        "@!a01 add.u32 %7, %7, 4;\n"
+        "@!ne mov.s32 %9, 2;\n"
+        "MCRT_PAIR_DONE:\n"
+        "}\n"
+        : "+f"(p.t0), "+f"(p.t1), "+f"(p.t2), "+f"(p.tcur), "+f"(p.tau_rem), "+r"(p.p0), "+r"(p.p1), "+r"(p.p2),
+          "+r"(p.slot), "+r"(state), "+f"(rho_a), "+f"(rho_b)
+        : "f"(p.dt0), "f"(p.dt1), "f"(p.dt2), "f"(kx), "l"(rho), "r"(lut2)
+        : "memory");
+  }
+}
+
 // O4: where a new package starts.  Point source: finest-level cell fx.. and fractional position
 // in it (direction-aware on a face, R7).  External field (R25): a point on one of the six box
 // faces and an inward cosine-law direction; returns the ROOT cube and cube-local position.
@@ -782,6 +956,12 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
       // one elsewhere -- c1_tau1 0.325 -> 0.343 ms with two, c2 / c3 within 1 %)
 #pragma unroll
       for (int rep = 0; rep < (REGION ? 2 : 1); ++rep) {
+#ifndef MCRT_CHECKS
+        if (!TL && DENS == 0) {                              // (compile-time choice)
+          if (state == SU_WALK) walk_pair_ptx<REGION>(P.rho, p, p.rho, rho_b, kx, sublut, state);
+          continue;
+        }
+#endif
         if (state == SU_WALK) walk_step_u<TL, DENS, MACRO, REGION>(P, D, p, p.rho, rho_b, kx, sublut, state, n_cross);
         if (state == SU_WALK)
           walk_step_u<TL, DENS, MACRO, REGION, SU_INTERACT_B>(P, D, p, rho_b, p.rho, kx, sublut, state, n_cross);

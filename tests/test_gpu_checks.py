@@ -53,3 +53,40 @@ def test_production_build_has_no_checks():
     from paper_1201_3588_b200 import build, mcrt
     build.build_library()
     assert mcrt.debug_violations() == -1
+
+
+DIGEST = r"""
+import hashlib
+import numpy as np
+from paper_1201_3588_b200 import mcrt, workloads as W
+h = hashlib.sha256()
+for wl, layout, sweeps in [(W.c1(tau_v=3.0, n_packets=200000, batch=100000), 1, 0),
+                           (W.tiny_random(n_root=13, seed=5, external=True, tau_cell=0.2, n_packets=60000, batch=20000), 2, 0),
+                           (W.c4(n_root=256, n_packets=400000, batch=200000), 0, 3)]:
+    ctx = mcrt.from_workload(wl, layout=layout)
+    if sweeps:
+        ctx.set_region_sweeps(sweeps, (64, 128, 64))
+    for f, c in wl.batches():
+        ctx.run_batch(wl.seed, f, c)
+    cn = ctx.get_counters()
+    for a in (ctx.get_cell_energy()[0], ctx.get_sed(), ctx.get_cell_temperature(), cn["emitted_per_bin"]):
+        h.update(np.ascontiguousarray(a).tobytes())
+    h.update(repr(sorted((k, int(v)) for k, v in cn.items() if np.ndim(v) == 0)).encode())
+    ctx.destroy()
+print("DIGEST", h.hexdigest())
+"""
+
+
+def test_ptx_walk_equals_the_checked_build():
+    """Single-level grids walk through a PTX block in the production build (transport_u.cuh walk_pair_ptx) and
+    through the C++ step in the checked build: same operations in the same order, so tallies, SEDs, temperatures
+    and counters must be identical bit for bit (plain walk, brick layout, swept regions)."""
+    from paper_1201_3588_b200 import build
+    out = []
+    for lib in (build.build_library(), build.build_library(checks=True)):
+        env = dict(os.environ, MCRT_LIBRARY=lib, PYTHONPATH=ROOT + os.pathsep + os.environ.get("PYTHONPATH", ""))
+        r = subprocess.run([sys.executable, "-c", DIGEST], env=env, cwd=ROOT, capture_output=True, text=True,
+                           timeout=600)
+        assert r.returncode == 0, r.stdout + r.stderr
+        out.append([l for l in r.stdout.splitlines() if l.startswith("DIGEST")][-1])
+    assert out[0] == out[1], out
