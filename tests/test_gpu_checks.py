@@ -62,6 +62,10 @@ from paper_1201_3588_b200 import mcrt, workloads as W
 h = hashlib.sha256()
 for wl, layout, sweeps in [(W.c1(tau_v=3.0, n_packets=200000, batch=100000), 1, 0),
                            (W.tiny_random(n_root=13, seed=5, external=True, tau_cell=0.2, n_packets=60000, batch=20000), 2, 0),
+                           (W.c2(n_root=32, n_packets=300000, batch=100000), 0, 0),
+                           (W.c3(n_root=32, n_packets=200000, batch=100000), 2, 0),
+                           (W.tiny_random(n_root=3, sub=3, n_refined=7, seed=8, external=True, n_packets=40000, batch=10000), 0, 0),
+                           (W.c1(tau_v=3.0, n_packets=200000, batch=100000), 3, 0),
                            (W.c4(n_root=256, n_packets=400000, batch=200000), 0, 3)]:
     ctx = mcrt.from_workload(wl, layout=layout)
     if sweeps:
@@ -78,9 +82,10 @@ print("DIGEST", h.hexdigest())
 
 
 def test_ptx_walk_equals_the_checked_build():
-    """Single-level grids walk through a PTX block in the production build (transport_u.cuh walk_pair_ptx) and
-    through the C++ step in the checked build: same operations in the same order, so tallies, SEDs, temperatures
-    and counters must be identical bit for bit (plain walk, brick layout, swept regions)."""
+    """The production build walks through PTX blocks (transport_u.cuh walk_pair_ptx, walk_step_tl_ptx), the checked
+    build through the C++ step: same operations in the same order, so tallies, SEDs, temperatures and counters
+    must be identical bit for bit (plain walk, brick layout, cubes and subcubes with S = 3 and 4, bricked root,
+    macro cubes, swept regions)."""
     from paper_1201_3588_b200 import build
     out = []
     for lib in (build.build_library(), build.build_library(checks=True)):
