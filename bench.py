@@ -392,6 +392,9 @@ def run_gpu(args, wl, name):
 
     stream = torch.cuda.current_stream().cuda_stream
     ctx = mcrt.from_workload(wl, layout=args.layout)
+    if name.endswith("_pah"):                                # row f2 as the headline workload (--workload c1_tau1_pah)
+        pah = W.pah_share(wl, n_C=100, mass_fraction=0.05)
+        ctx.set_pah(pah.n_C, pah.mass_fraction, pah.kabs, n_Tp=128)
     if args.threads or args.blocks_per_sm:
         ctx.set_launch(args.threads, args.blocks_per_sm)
     if args.quorum:
