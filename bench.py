@@ -608,7 +608,7 @@ def main():
     ap.add_argument("--quorum", type=int, default=0, help="walk-loop quorum (0 = automatic)")
     ap.add_argument("--source-order", type=int, default=None,
                     help="hand packages out grouped by source: 1 on, 0 off (default: automatic)")
-    ap.add_argument("--tail-mode", type=int, default=None, help="end of a batch: -1 auto, 0 quorum drops to 1, 1 quorum follows the live lanes")
+    ap.add_argument("--tail-mode", type=int, default=None, help="end of a batch: -1 auto; bit 0: quorum follows the live lanes; bit 1: temperature update fused into the transport launch")
     ap.add_argument("--layout", type=int, default=0, help="0 auto, 1 x-fastest, 2 bricked")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")

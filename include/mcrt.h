@@ -300,11 +300,15 @@ mcrt_status mcrt_set_launch(mcrt_ctx* ctx, int32_t threads_per_block, int32_t bl
  * (long free flights -> keep more lanes walking).  A scheduling knob only: results do not depend
  * on it. */
 mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum);
-/* End of a batch.  When the work queue is empty every warp still holds up to 32 packages (PAPER.md L25:
- * the packages of a batch fly together, and the batch is over when the last one has left).  mode 1: the
- * walk quorum then follows the number of packages the warp still holds (the same share of them as in the
- * steady state); mode 0: it drops to 1 (the warp waits for its last walker before every event pass).
- * -1 = automatic (the default: 1).  A scheduling knob only: results do not depend on it. */
+/* End of a batch.  mode bit 0: when the work queue is empty every warp still holds up to 32 packages (PAPER.md
+ * L25: the packages of a batch fly together, and the batch is over when the last one has left); the walk quorum
+ * then follows the number of packages the warp still holds (the same share of them as in the steady state)
+ * instead of dropping to 1.  mode bit 1: mcrt_run_batch runs the temperature update (the cell's
+ * energy "and accordingly its temperature") at the end of the transport launch itself, behind a grid-wide
+ * barrier (cooperative launch), instead of in a launch of its own -- not on swept grids, with a PAH declared or
+ * for packet-sharded batches.  -1 = automatic (the default: bit 0, and bit 1 on grids of at most 65536 leaf
+ * slots, where a second launch costs as much as the whole batch: the 16^3 sphere's 10^4-package batches).
+ * Scheduling only: results do not depend on it. */
 mcrt_status mcrt_set_tail_mode(mcrt_ctx* ctx, int32_t mode);
 /* Region sweeps (single-level grids of at least 256^3 cells in the brick layout, batches of at least 2^20
  * packages): the batch is transported in `sweeps` + 1 passes; in all but the last a package that crosses

@@ -75,7 +75,9 @@ struct mcrt_ctx {
   int order_by_source = -1;               // -1 automatic, 0 off, 1 by source, 2 by source and start direction
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
   int quorum = 0;                         // 0 = automatic (from the job's crossings per flight so far)
-  int tail_mode = -1;                     // end of a batch: -1 automatic, 1 the quorum follows the live lanes, 0 it drops to 1
+  int tail_mode = -1;                     // end of a batch: -1 automatic (= 3); bit 0: the quorum follows the live lanes;
+                                          // bit 1: the temperature update runs at the end of the transport launch
+  int coop_launch = 0;                    // the device launches kernels cooperatively (grid-wide barrier)
   // region sweeps (transport_u.cuh, REGION): single-level bricked grids far larger than the L2
   int region_cells[3] = {0, 0, 0};        // cells per region along x, y, z (0: the grid does not qualify)
   int region_sweeps = -1;                 // -1 automatic, 0 off
@@ -274,6 +276,7 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
   if (cc_major < 10)
     return bail(fail(ctx, MCRT_ECUDA, "mcrt_grid_create: device is not sm_100 class (built for sm_100a only)"));
   CUG(cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device));
+  CUG(cudaDeviceGetAttribute(&ctx->coop_launch, cudaDevAttrCooperativeLaunch, ctx->device));
   ctx->N = d->n_root;
   ctx->S = d->sub > 1 ? d->sub : 1;
   ctx->root_size = d->root_size;
@@ -609,8 +612,12 @@ static mcrt_status take_events(mcrt_ctx* ctx, BatchEvents* b) {
 
 // tally32 != NULL (packet-sharded batch): uint32[store slots] for the equilibrium grains, followed -- when a PAH is
 // declared -- by uint32[store slots][n_bins] for the PAH's absorbed spectrum; this batch's counts only.
+// fused != NULL: the caller wants the temperature update (a9) of THIS batch (n_cum = ctx->Ncum + n) at the end of the
+// same launch; *fused says whether that was done (one cooperative launch; not on swept grids, with a PAH, for
+// sharded batches or when the device cannot launch cooperatively -- then the caller launches k_update_temperature).
 static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_t n, cudaStream_t st,
-                                    uint32_t* tally32 = nullptr) {
+                                    uint32_t* tally32 = nullptr, bool* fused = nullptr) {
+  if (fused) *fused = false;
   if (n == 0) return MCRT_OK;
   const uint64_t kMaxLaunch = 1ull << 31;                    // the kernels number packages within a launch in 32 bits
   if (n > kMaxLaunch) {
@@ -679,7 +686,8 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   const bool region = sweeps > 0;
   const size_t smem = transport_smem_bytes(ctx, region);
   TransportParamsU PU;
-  PU.tail = ctx->tail_mode < 0 ? 1 : ctx->tail_mode;
+  const int tail_mode = ctx->tail_mode < 0 ? 3 : ctx->tail_mode;
+  PU.tail = tail_mode & 1;
   PU.base = P; PU.lut = ctx->d_lut; PU.lay = ctx->lay; PU.quorum = ctx->quorum;
   PU.rec = nullptr; PU.list_out = nullptr; PU.list_out_count = nullptr; PU.count_dev = nullptr; PU.resume = 0;
   for (int a = 0; a < 3; ++a) {
@@ -733,7 +741,26 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   if ((long long)ctx->sm_count * resident < grid) grid = (long long)ctx->sm_count * resident;
   PU.base.next = ctx->d_heads + ctx->head; PU.base.next_reset = ctx->d_heads + (ctx->head ^ 1);
   ctx->head ^= 1;
-  kern<<<(unsigned)grid, threads, smem, st>>>(PU);
+  PU.upd_nT = 0;
+  // (it pays on small grids only: C0's 10^4-package batches 0.052 -> 0.048 ms per step; at 2.7e5 leaves (C1) the
+  // barrier and the update inside the kernel cost what the second launch did, from 3e6 leaves on (C2, C3) more: the
+  // kernel of its own reads the tables from shared memory and two leaves per thread)
+  constexpr long long kFuseUpdateMaxSlots = 65536;
+  if (fused && !region && !ctx->pah && !tally32 && (tail_mode & 2) && ctx->coop_launch &&
+      (ctx->store_slots <= kFuseUpdateMaxSlots || ctx->tail_mode == 2 || ctx->tail_mode == 3)) {
+    const double PI = 3.14159265358979323846;
+    const double V = ctx->root_size * ctx->root_size * ctx->root_size;
+    PU.upd_nT = ctx->nT;
+    PU.upd_ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)(ctx->Ncum + n)) - std::log(4.0 * PI) - std::log(V));
+    PU.upd_ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
+    PU.upd_lnQ = ctx->d_lnQ; PU.upd_guide = ctx->d_guide; PU.upd_trow = ctx->d_trow;
+    PU.upd_slots = ctx->store_slots; PU.upd_n3 = ctx->uni ? ctx->store_slots : ctx->store_n3;
+    void* args[] = {(void*)&PU};
+    CU(cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3((unsigned)threads), args, smem, st));
+    *fused = true;
+  } else {
+    kern<<<(unsigned)grid, threads, smem, st>>>(PU);
+  }
   ctx->launches++;
   CU(cudaGetLastError());
   if (region) {
@@ -844,12 +871,13 @@ mcrt_status mcrt_run_batch(mcrt_ctx* ctx, uint64_t seed, uint64_t first, uint64_
   mcrt_status rc = begin_batch(ctx, &ev);
   if (rc != MCRT_OK) return rc;
   CU(cudaEventRecord(ev.e0, st));
-  rc = launch_transport(ctx, seed, first, n, st);
+  bool fused = false;                                        // a9 at the end of the transport launch (when it can be)
+  rc = launch_transport(ctx, seed, first, n, st, nullptr, n <= (1ull << 31) ? &fused : nullptr);
   if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
   CU(cudaEventRecord(ev.e1, st));
   ctx->Ncum += n;
   ctx->Nglobal = ctx->Ncum;
-  rc = launch_update(ctx, ctx->d_tally, ctx->Ncum, st);
+  if (!fused) rc = launch_update(ctx, ctx->d_tally, ctx->Ncum, st);
   if (rc != MCRT_OK) { ctx->spare.push_back(ev); return rc; }
   CU(cudaEventRecord(ev.e2, st));
   ctx->pending.push_back(ev);
@@ -1324,7 +1352,7 @@ mcrt_status mcrt_set_walk_quorum(mcrt_ctx* ctx, int32_t quorum) {
 
 mcrt_status mcrt_set_tail_mode(mcrt_ctx* ctx, int32_t mode) {
   if (!ctx) return MCRT_EINVAL;
-  if (mode < -1 || mode > 1) return fail(ctx, MCRT_EINVAL, "mcrt_set_tail_mode: -1 (automatic), 0 or 1");
+  if (mode < -1 || mode > 3) return fail(ctx, MCRT_EINVAL, "mcrt_set_tail_mode: -1 (automatic) or a combination of bits 0 and 1");
   ctx->tail_mode = mode;
   return MCRT_OK;
 }

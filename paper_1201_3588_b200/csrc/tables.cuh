@@ -137,6 +137,15 @@ __device__ __forceinline__ float row_of_lnq(float lq, const float* s_lnQ, const 
   return (float)lo + (lq - s_lnQ[lo]) / (s_lnQ[lo + 1] - s_lnQ[lo]);
 }
 
+// O7 for one leaf: table row coordinate of its temperature from its cumulative count c and density r
+__device__ __forceinline__ float trow_of_leaf(unsigned long long c, float r, bool is_sub, float ln_coef, float ln_sub3,
+                                              const float* lnQ, const int* guide, int nT, float lq0, float inv_w,
+                                              bool use_guide) {
+  if (c == 0 || !(r > 0.f)) return 0.f;                       // refined-root markers have r < 0
+  const float lq = logf((float)c) + ln_coef - logf(r) + (is_sub ? ln_sub3 : 0.f);
+  return row_of_lnq(lq, lnQ, guide, nT, lq0, inv_w, use_guide);
+}
+
 // ADD: first add the batch's absorbed-package counts `delta` (u32, the sum over all ranks of a
 // packet-sharded run) to the cumulative tally, then update (one pass over the leaves).
 template <bool ADD>
@@ -153,9 +162,7 @@ __global__ void __launch_bounds__(256) k_update_temperature(const float* __restr
   const float lq0 = s_lnQ[0], inv_w = (float)kGuide / (s_lnQ[nT - 1] - s_lnQ[0]);
   const bool use_guide = lq0 > -1e29f && s_lnQ[nT - 1] > lq0;
   auto one = [&](unsigned long long c, float r, long long i) -> float {
-    if (c == 0 || !(r > 0.f)) return 0.f;                     // refined-root markers have r < 0
-    const float lq = logf((float)c) + ln_coef - logf(r) + (i >= n3 ? ln_sub3 : 0.f);
-    return row_of_lnq(lq, s_lnQ, s_guide, nT, lq0, inv_w, use_guide);
+    return trow_of_leaf(c, r, i >= n3, ln_coef, ln_sub3, s_lnQ, s_guide, nT, lq0, inv_w, use_guide);
   };
   const long long stride = 2ll * gridDim.x * blockDim.x;
   for (long long i = 2ll * ((long long)blockIdx.x * blockDim.x + threadIdx.x); i < slots; i += stride) {

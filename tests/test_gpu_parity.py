@@ -364,11 +364,12 @@ def test_walk_quorum_does_not_change_results(M):
     (lambda: W.c4(n_root=24, n_packets=90_000, batch=30_000, corr_cells=3.0), 2),
     (lambda: W.tiny_random(n_root=3, sub=8, n_refined=5, seed=11, external=True, n_packets=40_000, batch=10_000), 0)])
 def test_end_of_batch_modes_do_not_change_results(M, maker, layout):
-    """mcrt_set_tail_mode: how a warp schedules its last packages once the work queue is empty is
+    """mcrt_set_tail_mode: how a warp schedules its last packages once the work queue is empty, and whether the
+    temperature update runs at the end of the transport launch (grid-wide barrier) or in a launch of its own, is
     scheduling only -- tallies, SED, temperatures and every counter stay bit-identical."""
     wl = maker()
     runs = []
-    for mode in (0, 1, -1):
+    for mode in (0, 1, 2, 3, -1):
         ctx = M.from_workload(wl, layout=layout)
         ctx.set_tail_mode(mode)
         for first, cnt in wl.batches():
