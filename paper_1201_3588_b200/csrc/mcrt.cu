@@ -71,6 +71,8 @@ struct mcrt_ctx {
   unsigned long long* d_tally_scratch = nullptr;
   uint32_t* d_perm = nullptr;             // package numbers of a batch grouped by source
   unsigned long long perm_cap = 0;
+  uint16_t* d_keys = nullptr;             // group of every package of the batch (kept between the two grouping passes)
+  unsigned long long keys_cap = 0;
   unsigned int* d_srccnt = nullptr;       // [2][nsrc] counts, cursors
   int order_by_source = -1;               // -1 automatic, 0 off, 1 by source, 2 by source and start direction
   void* d_out_scratch = nullptr;          // staging for host read-outs that need a conversion kernel (8 B x slots)
@@ -463,7 +465,7 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
 
 mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   if (!ctx) return MCRT_EINVAL;
-  if (ctx->last_stream || true) cudaDeviceSynchronize();
+  cudaDeviceSynchronize();                                   // nothing of this context may still be running
   for (auto& b : ctx->pending) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& b : ctx->spare) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& t : ctx->tickets) {
@@ -480,7 +482,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   cudaFree(ctx->d_lut); cudaFree(ctx->d_lut_marked); cudaFree(ctx->d_lut_plain2); cudaFree(ctx->d_rec);
   cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]); cudaFree(ctx->d_swcnt); cudaFree(ctx->d_regcnt);
   cudaFree(ctx->d_heads);
-  cudaFree(ctx->d_bits); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
+  cudaFree(ctx->d_bits); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_keys); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -658,13 +660,18 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
       CU(cudaMalloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
       ctx->perm_cap = n;
     }
+    if (ctx->keys_cap < n) {
+      cudaFree(ctx->d_keys); ctx->d_keys = nullptr; ctx->keys_cap = 0;
+      CU(cudaMalloc(&ctx->d_keys, sizeof(uint16_t) * (size_t)n));
+      ctx->keys_cap = n;
+    }
     if (!ctx->d_srccnt) CU(cudaMalloc(&ctx->d_srccnt, sizeof(unsigned int) * 2 * kMaxOrderedSources));
     CU(cudaMemsetAsync(ctx->d_srccnt, 0, sizeof(unsigned int) * 2 * kMaxOrderedSources, st));
     const unsigned gblocks = (unsigned)ctx->sm_count * 8u;
     const size_t gsmem = sizeof(unsigned int) * 2 * (size_t)ctx->nsrc * sub;
-    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, nullptr, nullptr);
+    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, nullptr, nullptr, ctx->d_keys);
     k_scan_sources<<<1, 32, 0, st>>>(ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->nsrc * sub);
-    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->d_perm);
+    k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->d_perm, ctx->d_keys);
     ctx->launches += 3;
     P.perm = ctx->d_perm;
   }

@@ -226,30 +226,37 @@ __device__ __forceinline__ int group_of(const TransportParams& P, unsigned long 
   return s * sub + b;
 }
 
-// counts[g] += packages of group g (cursor == NULL), or perm[cursor[g]++] = package number
+// counts[g] += packages of group g (cursor == NULL: the group of every package is also kept in keys[], so that
+// the second pass need not repeat its Philox block), or perm[cursor[g]++] = package number
 __global__ void k_group_by_source(const TransportParams P, const int sub, unsigned int* __restrict__ counts,
-                                  unsigned int* __restrict__ cursor, uint32_t* __restrict__ perm) {
+                                  unsigned int* __restrict__ cursor, uint32_t* __restrict__ perm,
+                                  uint16_t* __restrict__ keys) {
   extern __shared__ unsigned int s_cnt[];                    // [2 * ngroups]: block histogram, block bases
   const int ng = P.nsrc * sub;
   for (int i = threadIdx.x; i < 2 * ng; i += blockDim.x) s_cnt[i] = 0;
   __syncthreads();
   const unsigned long long per_block = (P.count + gridDim.x - 1) / gridDim.x;
   const unsigned long long lo = per_block * blockIdx.x, hi = min(P.count, lo + per_block);
-  for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x)
-    atomicAdd(&s_cnt[group_of(P, P.first + i, sub)], 1u);
-  __syncthreads();
   if (!cursor) {
+    for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+      const int g = group_of(P, P.first + i, sub);
+      keys[i] = (uint16_t)g;
+      atomicAdd(&s_cnt[g], 1u);
+    }
+    __syncthreads();
     for (int i = threadIdx.x; i < ng; i += blockDim.x)
       if (s_cnt[i]) atomicAdd(&counts[i], s_cnt[i]);
     return;
   }
+  for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x) atomicAdd(&s_cnt[keys[i]], 1u);
+  __syncthreads();
   for (int i = threadIdx.x; i < ng; i += blockDim.x) {       // reserve this block's range in every group
     s_cnt[ng + i] = s_cnt[i] ? atomicAdd(&cursor[i], s_cnt[i]) : 0u;
     s_cnt[i] = 0;
   }
   __syncthreads();
   for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
-    const int g = group_of(P, P.first + i, sub);
+    const int g = keys[i];
     perm[s_cnt[ng + g] + atomicAdd(&s_cnt[g], 1u)] = (uint32_t)i;
   }
 }
