@@ -31,6 +31,7 @@ struct mcrt_ctx {
   long long store_n3 = 0;                 // storage slots of the root grid (sub-cells follow it)
   double origin[3] = {0, 0, 0}, root_size = 1;
   float* d_rho = nullptr;
+  float* d_lnrho = nullptr;               // ln of d_rho (-inf: empty leaf / refined-cube marker), for the temperature update
   unsigned long long* d_tally = nullptr;
   float* d_trow = nullptr;
   // opacity
@@ -416,6 +417,9 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     k_sanitize<<<(unsigned)((k * s3 + 255) / 256), 256>>>(src_sub, ctx->d_rho + ctx->store_n3, k * s3);
     ctx->launches++;
   }
+  CUG(cudaMalloc(&ctx->d_lnrho, sizeof(float) * ctx->store_slots));
+  k_ln_density<<<(unsigned)((ctx->store_slots + 255) / 256), 256>>>(ctx->d_rho, ctx->d_lnrho, ctx->store_slots);
+  ctx->launches++;
   CUG(cudaGetLastError());
   CUG(cudaDeviceSynchronize());
   // Small single-level problems keep their density in shared memory (transport_u.cuh, DENS): the array itself
@@ -478,7 +482,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_pah(ctx);
   free_sources(ctx);
   free_observer(ctx);
-  cudaFree(ctx->d_rho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
+  cudaFree(ctx->d_rho); cudaFree(ctx->d_lnrho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
   cudaFree(ctx->d_lut); cudaFree(ctx->d_lut_marked); cudaFree(ctx->d_lut_plain2); cudaFree(ctx->d_rec);
   cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]); cudaFree(ctx->d_swcnt); cudaFree(ctx->d_regcnt);
   cudaFree(ctx->d_heads);
@@ -760,7 +764,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
     PU.upd_nT = ctx->nT;
     PU.upd_ln_coef = (float)(std::log(ctx->Ltot) - std::log((double)(ctx->Ncum + n)) - std::log(4.0 * PI) - std::log(V));
     PU.upd_ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
-    PU.upd_lnQ = ctx->d_lnQ; PU.upd_guide = ctx->d_guide; PU.upd_trow = ctx->d_trow;
+    PU.upd_lnQ = ctx->d_lnQ; PU.upd_guide = ctx->d_guide; PU.upd_trow = ctx->d_trow; PU.upd_lnrho = ctx->d_lnrho;
     PU.upd_slots = ctx->store_slots; PU.upd_n3 = ctx->uni ? ctx->store_slots : ctx->store_n3;
     void* args[] = {(void*)&PU};
     CU(cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3((unsigned)threads), args, smem, st));
@@ -849,10 +853,10 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
   const size_t smem = 4 * (size_t)ctx->nT + sizeof(int) * kGuide;
   const long long n3 = ctx->uni ? ctx->store_slots : ctx->store_n3;
   if (delta)
-    k_update_temperature<true><<<(unsigned)blocks, 256, smem, st>>>(ctx->d_rho, ctx->d_tally, delta, ctx->d_trow, ctx->d_lnQ,
+    k_update_temperature<true><<<(unsigned)blocks, 256, smem, st>>>(ctx->d_lnrho, ctx->d_tally, delta, ctx->d_trow, ctx->d_lnQ,
                                                                     ctx->d_guide, ctx->nT, ctx->store_slots, n3, ln_coef, ln_sub3);
   else
-    k_update_temperature<false><<<(unsigned)blocks, 256, smem, st>>>(ctx->d_rho, const_cast<unsigned long long*>(tally), nullptr,
+    k_update_temperature<false><<<(unsigned)blocks, 256, smem, st>>>(ctx->d_lnrho, const_cast<unsigned long long*>(tally), nullptr,
                                                                      ctx->d_trow, ctx->d_lnQ, ctx->d_guide, ctx->nT,
                                                                      ctx->store_slots, n3, ln_coef, ln_sub3);
   ctx->launches++;

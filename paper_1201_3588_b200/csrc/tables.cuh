@@ -134,22 +134,32 @@ __device__ __forceinline__ float row_of_lnq(float lq, const float* s_lnQ, const 
     lo = 0;
     while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (s_lnQ[mid] <= lq) lo = mid; else hi = mid; }
   }
-  return (float)lo + (lq - s_lnQ[lo]) / (s_lnQ[lo + 1] - s_lnQ[lo]);
+  return (float)lo + __fdividef(lq - s_lnQ[lo], s_lnQ[lo + 1] - s_lnQ[lo]);
 }
 
-// O7 for one leaf: table row coordinate of its temperature from its cumulative count c and density r
-__device__ __forceinline__ float trow_of_leaf(unsigned long long c, float r, bool is_sub, float ln_coef, float ln_sub3,
+// ln of the density of every storage slot, once per grid (-inf for empty leaves and for the markers of refined
+// cubes): the update kernel then takes one logarithm per leaf instead of two
+__global__ void k_ln_density(const float* __restrict__ rho, float* __restrict__ lnrho, long long slots) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= slots) return;
+  const float r = rho[i];
+  lnrho[i] = r > 0.f ? logf(r) : -INFINITY;
+}
+
+// O7 for one leaf: table row coordinate of its temperature from its cumulative count c and ln(density) lnr.
+// ln c through the special-function unit (__logf: absolute error < 1e-6 on ln q, i.e. < 3e-7 relative on T).
+__device__ __forceinline__ float trow_of_leaf(unsigned long long c, float lnr, bool is_sub, float ln_coef, float ln_sub3,
                                               const float* lnQ, const int* guide, int nT, float lq0, float inv_w,
                                               bool use_guide) {
-  if (c == 0 || !(r > 0.f)) return 0.f;                       // refined-root markers have r < 0
-  const float lq = logf((float)c) + ln_coef - logf(r) + (is_sub ? ln_sub3 : 0.f);
+  if (c == 0 || !(lnr > -1e30f)) return 0.f;                  // nothing absorbed; empty leaf or refined-cube marker
+  const float lq = __logf((float)c) + ln_coef - lnr + (is_sub ? ln_sub3 : 0.f);
   return row_of_lnq(lq, lnQ, guide, nT, lq0, inv_w, use_guide);
 }
 
 // ADD: first add the batch's absorbed-package counts `delta` (u32, the sum over all ranks of a
 // packet-sharded run) to the cumulative tally, then update (one pass over the leaves).
 template <bool ADD>
-__global__ void __launch_bounds__(256) k_update_temperature(const float* __restrict__ rho,
+__global__ void __launch_bounds__(256) k_update_temperature(const float* __restrict__ lnrho,
                                      unsigned long long* __restrict__ tally, const uint32_t* __restrict__ delta,
                                      float* __restrict__ trow, const float* __restrict__ lnQ,
                                      const int* __restrict__ guide, int nT, long long slots, long long n3,
@@ -168,7 +178,7 @@ __global__ void __launch_bounds__(256) k_update_temperature(const float* __restr
   for (long long i = 2ll * ((long long)blockIdx.x * blockDim.x + threadIdx.x); i < slots; i += stride) {
     if (i + 1 < slots) {                                      // two leaves per turn: 16-byte tally, 8-byte rho / trow accesses
       ulonglong2 c = *reinterpret_cast<const ulonglong2*>(tally + i);
-      const float2 r = *reinterpret_cast<const float2*>(rho + i);
+      const float2 r = *reinterpret_cast<const float2*>(lnrho + i);
       if (ADD) {
         const uint2 d = *reinterpret_cast<const uint2*>(delta + i);
         c.x += d.x; c.y += d.y;
@@ -178,7 +188,7 @@ __global__ void __launch_bounds__(256) k_update_temperature(const float* __restr
     } else {
       unsigned long long c = tally[i];
       if (ADD) { c += delta[i]; tally[i] = c; }
-      trow[i] = one(c, rho[i], i);
+      trow[i] = one(c, lnrho[i], i);
     }
   }
 }

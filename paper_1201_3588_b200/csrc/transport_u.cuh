@@ -156,6 +156,7 @@ struct TransportParamsU {
   float upd_ln_coef, upd_ln_sub3;
   const float* upd_lnQ;                   // [nT]
   const int* upd_guide;                   // [kGuide]
+  const float* upd_lnrho;                 // [slots] ln of the density (k_ln_density)
   float* upd_trow;                        // = base.trow (written here, read-only above)
   long long upd_slots, upd_n3;
   // density staged in shared memory (kernel template DENS = 1 / 2): what every block copies in
@@ -1021,7 +1022,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < PU.upd_slots; i += stride) {
       const unsigned long long c = __ldcg(P.tally + i);            // (tallied by every block: read from the L2)
-      PU.upd_trow[i] = trow_of_leaf(c, P.rho[i], i >= PU.upd_n3, PU.upd_ln_coef, PU.upd_ln_sub3, PU.upd_lnQ, PU.upd_guide,
+      PU.upd_trow[i] = trow_of_leaf(c, __ldg(PU.upd_lnrho + i), i >= PU.upd_n3, PU.upd_ln_coef, PU.upd_ln_sub3, PU.upd_lnQ, PU.upd_guide,
                                     nT, lq0, inv_w, use_guide);
     }
   }
