@@ -250,6 +250,37 @@ static size_t transport_smem_bytes(const mcrt_ctx* ctx, bool region = false) {
 
 constexpr size_t kMaxSmemPerBlock = 227u << 10;              // B200: opt-in limit of dynamic shared memory
 
+// One bit per cell for a single-level grid that holds only two distinct densities and whose bits fit into shared
+// memory (mcrt_set_density_staging(2); measured slower than global gathers, so it is prepared only on request: the
+// scan of the density array costs a device-to-host copy that mcrt_grid_create should not pay -- 0.8 of its 2.2 ms
+// on the 64^3 sphere).
+static mcrt_status prepare_density_bits(mcrt_ctx* ctx) {
+  const size_t kStageMax = 40u << 10;
+  if (ctx->dens_mode != 0 || !ctx->uni || ctx->d_bits || (size_t)(ctx->store_slots + 7) / 8 > kStageMax) return MCRT_OK;
+  CU(cudaDeviceSynchronize());
+  std::vector<float> h((size_t)ctx->store_slots);
+  CU(cudaMemcpy(h.data(), ctx->d_rho, 4 * h.size(), cudaMemcpyDeviceToHost));
+  float v0 = h[0], v1 = h[0];
+  bool two = true, have1 = false;
+  for (float v : h) {
+    if (v == v0 || (have1 && v == v1)) continue;
+    if (!have1) { v1 = v; have1 = true; continue; }
+    two = false;
+    break;
+  }
+  if (!two) return MCRT_OK;
+  const size_t words = (((size_t)ctx->store_slots + 31) / 32 + 3) & ~(size_t)3;   // 16-byte units
+  std::vector<uint32_t> bits(words, 0u);
+  for (size_t i = 0; i < h.size(); ++i)
+    if (have1 && h[i] == v1) bits[i >> 5] |= 1u << (i & 31);
+  CU(cudaMalloc(&ctx->d_bits, 4 * words));
+  CU(cudaMemcpy(ctx->d_bits, bits.data(), 4 * words, cudaMemcpyHostToDevice));
+  ctx->dens_mode = 2;
+  ctx->stage_bytes = (unsigned)(4 * words);
+  ctx->pal0 = v0; ctx->pal1 = v1;
+  return MCRT_OK;
+}
+
 extern "C" {
 
 mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
@@ -436,28 +467,6 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
         CUG(cudaMemcpy(padded, ctx->d_rho, (size_t)ctx->store_slots * 4, cudaMemcpyDeviceToDevice));
         cudaFree(ctx->d_rho);
         ctx->d_rho = padded;
-      }
-    } else if ((size_t)(ctx->store_slots + 7) / 8 <= kStageMax) {
-      std::vector<float> h((size_t)ctx->store_slots);
-      CUG(cudaMemcpy(h.data(), ctx->d_rho, 4 * h.size(), cudaMemcpyDeviceToHost));
-      float v0 = h[0], v1 = h[0];
-      bool two = true, have1 = false;
-      for (float v : h) {
-        if (v == v0 || (have1 && v == v1)) continue;
-        if (!have1) { v1 = v; have1 = true; continue; }
-        two = false;
-        break;
-      }
-      if (two) {
-        const size_t words = (((size_t)ctx->store_slots + 31) / 32 + 3) & ~(size_t)3;   // 16-byte units
-        std::vector<uint32_t> bits(words, 0u);
-        for (size_t i = 0; i < h.size(); ++i)
-          if (have1 && h[i] == v1) bits[i >> 5] |= 1u << (i & 31);
-        CUG(cudaMalloc(&ctx->d_bits, 4 * words));
-        CUG(cudaMemcpy(ctx->d_bits, bits.data(), 4 * words, cudaMemcpyHostToDevice));
-        ctx->dens_mode = 2;
-        ctx->stage_bytes = (unsigned)(4 * words);
-        ctx->pal0 = v0; ctx->pal1 = v1;
       }
     }
   }
@@ -1406,6 +1415,7 @@ mcrt_status mcrt_set_density_staging(mcrt_ctx* ctx, int32_t mode) {
   if (!ctx) return MCRT_EINVAL;
   if (mode < 0 || mode > 2) return fail(ctx, MCRT_EINVAL, "mcrt_set_density_staging: mode must be 0 (automatic), 1 (off) or 2 (also one bit per cell)");
   ctx->dens_off = mode;
+  if (mode == 2) return prepare_density_bits(ctx);
   return MCRT_OK;
 }
 
