@@ -189,14 +189,16 @@ __device__ __forceinline__ float density_at(const DensU& D, int slot) {
 // Automatic walk quorum.  A warp that walks until w lanes are left and then spends E instructions on
 // one event pass does about L (32 - w) crossings in c L ln(32/w) + E instructions (L = mean crossings
 // per flight, c = instructions per step), so the best w grows with L.  Measured optima (profiles/):
-// 12-16 at L = 38 (c1), ~19 at L = 160 (c2), 20-24 at L = 320 (c3): w = 14 + 2 log2(L / 24), 8..24.
+// 12-16 at L = 38 (c1); on the two-level disks 17-18 both at L = 160 (c2) and at L = 320 (c3), with a cliff
+// below 17 (c2: 16 -> 3.67, 17 -> 3.16, 18 -> 3.13, 20 -> 3.23, 22 -> 3.41 ms; c3: 16 -> 7.60, 18 -> 6.57, 21 -> 6.80):
+// w = 14 + 2 log2(L / 24), at least 8 and at most 24 (18 on two-level grids).
 // L is taken from the job's own cumulative counters (crossings / flights so far; the first batch
 // starts at 16).  A scheduling knob only: results do not depend on it.
-__device__ __forceinline__ int auto_quorum(const unsigned long long* __restrict__ counters) {
+__device__ __forceinline__ int auto_quorum(const unsigned long long* __restrict__ counters, int q_max) {
   const float cr = (float)counters[CNT_CROSS], fl = (float)counters[CNT_FLIGHTS];
   if (fl < 1024.f) return 16;
   const int q = 14 + (int)rintf(2.f * log2f(fmaxf(cr / fl, 1.f) * (1.f / 24.f)));
-  return min(24, max(8, q));
+  return min(q_max, max(8, q));
 }
 
 // SU_INTERACT_B: interaction found in the second step of a pair -> the cell's density is in the
@@ -713,7 +715,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
   p.cb = 0; p.k = 0; p.off = 0; p.u1 = p.u2 = p.u3 = 0.f;
   float kx = 0.f;
   int state = SU_FETCH;
-  const int quorum0 = PU.quorum > 0 ? PU.quorum : auto_quorum(P.counters);
+  const int quorum0 = PU.quorum > 0 ? PU.quorum : auto_quorum(P.counters, TL && !MACRO ? 18 : 24);
   int quorum = quorum0;
   bool tail = false;                                         // the work queue is (nearly) empty
 
