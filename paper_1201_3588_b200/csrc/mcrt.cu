@@ -72,6 +72,7 @@ struct mcrt_ctx {
   unsigned long long* d_tally_scratch = nullptr;
   uint32_t* d_perm = nullptr;             // package numbers of a batch grouped by source
   unsigned long long perm_cap = 0;
+  bool group_smem_set = false;            // k_group_by_source may use more than 48 KB of shared memory
   uint16_t* d_keys = nullptr;             // group of every package of the batch (kept between the two grouping passes)
   unsigned long long keys_cap = 0;
   unsigned int* d_srccnt = nullptr;       // [2][nsrc] counts, cursors
@@ -666,7 +667,12 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   int gmode = ctx->order_by_source < 0 ? ((big || n >= (1ull << 21)) ? 2 : 0) : ctx->order_by_source;
   if (gmode == 1 && ctx->nsrc < 2) gmode = 0;
   int sub = 1;                                               // start-direction sub-groups per source
-  if (gmode == 2) sub = ctx->nsrc * 128 <= kMaxOrderedSources ? 128 : (ctx->nsrc * 32 <= kMaxOrderedSources ? 32 : 1);
+  if (gmode == 2) {                                          // the finest direction bins the group table has room for
+    sub = 1;
+    for (int m = 64; m >= 4 && sub == 1; m >>= 1)            // ... and the batch has packages for (256 per group on average)
+      if ((long long)ctx->nsrc * 2 * m * m <= kMaxOrderedSources && ((long long)ctx->nsrc * 2 * m * m * 256 <= (long long)n || m == 4))
+        sub = 2 * m * m;
+  }
   if (gmode && sub * ctx->nsrc <= kMaxOrderedSources && (sub > 1 || ctx->nsrc > 1) && n >= 65536) {
     if (ctx->perm_cap < n) {
       cudaFree(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
@@ -680,10 +686,15 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
     }
     if (!ctx->d_srccnt) CU(cudaMalloc(&ctx->d_srccnt, sizeof(unsigned int) * 2 * kMaxOrderedSources));
     CU(cudaMemsetAsync(ctx->d_srccnt, 0, sizeof(unsigned int) * 2 * kMaxOrderedSources, st));
-    const unsigned gblocks = (unsigned)ctx->sm_count * 8u;
+    // (every block flushes its histogram of all groups: fewer, larger blocks when the groups are many)
+    const unsigned gblocks = (unsigned)ctx->sm_count * (ctx->nsrc * sub > 2048 ? 3u : 8u);
     const size_t gsmem = sizeof(unsigned int) * 2 * (size_t)ctx->nsrc * sub;
+    if (gsmem > (48u << 10) && !ctx->group_smem_set) {
+      CU(cudaFuncSetAttribute(k_group_by_source, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(unsigned int) * 2 * kMaxOrderedSources)));
+      ctx->group_smem_set = true;
+    }
     k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, nullptr, nullptr, ctx->d_keys);
-    k_scan_sources<<<1, 32, 0, st>>>(ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->nsrc * sub);
+    k_scan_sources<<<1, 1024, 0, st>>>(ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->nsrc * sub);
     k_group_by_source<<<gblocks, 256, gsmem, st>>>(P, sub, ctx->d_srccnt, ctx->d_srccnt + kMaxOrderedSources, ctx->d_perm, ctx->d_keys);
     ctx->launches += 3;
     P.perm = ctx->d_perm;
@@ -795,7 +806,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
       CU(cudaMemsetAsync(ctx->d_regcnt, 0, sizeof(unsigned int) * 2 * (size_t)nreg, st));
       const unsigned gblocks = (unsigned)ctx->sm_count * 4u;
       k_region_hist<<<gblocks, 256, sizeof(unsigned int) * nreg, st>>>(list_in, n_in, nreg, ctx->d_regcnt);
-      k_scan_sources<<<1, 32, 0, st>>>(ctx->d_regcnt, ctx->d_regcnt + nreg, nreg);
+      k_scan_sources<<<1, 1024, 0, st>>>(ctx->d_regcnt, ctx->d_regcnt + nreg, nreg);
       k_region_scatter<<<gblocks, 256, sizeof(unsigned int) * 2 * nreg, st>>>(list_in, n_in, nreg, ctx->d_regcnt + nreg, ctx->d_perm);
       PU.base.next = ctx->d_heads + ctx->head; PU.base.next_reset = ctx->d_heads + (ctx->head ^ 1);
       ctx->head ^= 1;
