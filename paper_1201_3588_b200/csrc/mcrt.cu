@@ -339,9 +339,11 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
   ctx->uni = k == 0;
   ctx->lay.N = d->n_root;
   ctx->lay.nbk = (d->n_root + 7) / 8;
-  // automatic: bricks for single-level grids larger than the L2; on two-level grids most crossings are in
-  // subcubes (already blocks of S^3) and the bricked root measured slower (c3 13.3 vs 12.2 ms per batch)
-  ctx->lay.bricked = d->layout == 2 || (d->layout == 0 && k == 0 && n3 * 4 > (48ll << 20));
+  // automatic: bricks for root grids larger than 48 MB -- single-level (c4) and, since the packages of a warp fly
+  // closely together (64 x 128 start-direction bins), two-level ones too: c3 5.89 -> 5.72 ms per launch (it measured
+  // slower before that, 13.3 vs 12.2 ms, when most of its gathers missed the L1 either way); c2 (12.8 MB) keeps
+  // the x-fastest root (2.82 both ways)
+  ctx->lay.bricked = d->layout == 2 || (d->layout == 0 && n3 * 4 > (48ll << 20));
   ctx->store_n3 = slots_of(ctx->lay);
   if (ctx->store_n3 + k * s3 >= (1ll << 31)) {               // padding pushed it over: fall back
     ctx->lay.bricked = 0;
