@@ -789,8 +789,14 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
     PU.upd_lnQ = ctx->d_lnQ; PU.upd_guide = ctx->d_guide; PU.upd_trow = ctx->d_trow; PU.upd_lnrho = ctx->d_lnrho;
     PU.upd_slots = ctx->store_slots; PU.upd_n3 = ctx->uni ? ctx->store_slots : ctx->store_n3;
     void* args[] = {(void*)&PU};
-    CU(cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3((unsigned)threads), args, smem, st));
-    *fused = true;
+    const cudaError_t ce = cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3((unsigned)threads), args, smem, st);
+    if (ce == cudaSuccess) {
+      *fused = true;
+    } else {                                                 // (e.g. the grid cannot be co-resident right now): two launches
+      (void)cudaGetLastError();
+      PU.upd_nT = 0;
+      kern<<<(unsigned)grid, threads, smem, st>>>(PU);
+    }
   } else {
     kern<<<(unsigned)grid, threads, smem, st>>>(PU);
   }
