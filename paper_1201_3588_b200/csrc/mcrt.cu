@@ -22,6 +22,76 @@
 
 using namespace mcrt;
 
+// ---- device memory of the library: a small caching allocator ---------------------------------------------------
+// A job allocates ~25 device arrays in its set-up calls; cudaMalloc / cudaFree cost 40 us apiece on one box and
+// 250 us on another (setup_ms 1.0 ... 6.3 in bench.py's e2e).  Blocks of up to 256 MB that a context gives back are
+// kept (at most 1 GB in all) and handed out again to the next request of exactly the same size -- a second job
+// of the same shape allocates nothing.  mc_free synchronises the device like cudaFree does, so a block is never
+// handed on while a kernel may still use it.
+#include <map>
+#include <mutex>
+namespace {
+std::mutex g_mc_mutex;
+std::multimap<std::pair<int, size_t>, void*> g_mc_cache;      // (device, bytes) -> block
+size_t g_mc_cached = 0;
+std::map<void*, size_t>& g_mc_sizes() { static std::map<void*, size_t> m; return m; }   // live blocks of the library
+constexpr size_t kMcBlockMax = (size_t)256 << 20, kMcTotalMax = (size_t)1 << 30;
+}  // namespace
+template <typename T>
+static cudaError_t mc_malloc(T** p, size_t bytes) {
+  int dev = 0;
+  if (bytes && bytes <= kMcBlockMax && cudaGetDevice(&dev) == cudaSuccess) {
+    std::lock_guard<std::mutex> lock(g_mc_mutex);
+    auto it = g_mc_cache.find({dev, bytes});
+    if (it != g_mc_cache.end()) {
+      *p = static_cast<T*>(it->second);
+      g_mc_cache.erase(it);
+      g_mc_cached -= bytes;
+      return cudaSuccess;
+    }
+  }
+  void* q = nullptr;
+  cudaError_t e = cudaMalloc(&q, bytes);
+  if (e == cudaErrorMemoryAllocation) {                      // give the cache back and try once more
+    (void)cudaGetLastError();
+    std::lock_guard<std::mutex> lock(g_mc_mutex);
+    for (auto& kv : g_mc_cache) { g_mc_sizes().erase(kv.second); cudaFree(kv.second); }
+    g_mc_cache.clear();
+    g_mc_cached = 0;
+    e = cudaMalloc(&q, bytes);
+  }
+  if (e == cudaSuccess) {
+    *p = static_cast<T*>(q);
+    std::lock_guard<std::mutex> lock(g_mc_mutex);
+    g_mc_sizes()[q] = bytes;
+  }
+  return e;
+}
+static cudaError_t mc_free(void* q) {
+  if (!q) return cudaSuccess;
+  size_t bytes = 0;
+  int dev = 0;
+  {
+    std::lock_guard<std::mutex> lock(g_mc_mutex);
+    auto it = g_mc_sizes().find(q);
+    if (it != g_mc_sizes().end()) bytes = it->second;
+  }
+  if (bytes && bytes <= kMcBlockMax && cudaGetDevice(&dev) == cudaSuccess) {
+    cudaDeviceSynchronize();
+    std::lock_guard<std::mutex> lock(g_mc_mutex);
+    if (g_mc_cached + bytes <= kMcTotalMax) {
+      g_mc_cache.insert({{dev, bytes}, q});
+      g_mc_cached += bytes;
+      return cudaSuccess;
+    }
+  }
+  {
+    std::lock_guard<std::mutex> lock(g_mc_mutex);
+    g_mc_sizes().erase(q);
+  }
+  return cudaFree(q);
+}
+
 struct BatchEvents { cudaEvent_t e0, e1, e2; };
 
 struct mcrt_ctx {
@@ -139,27 +209,27 @@ static mcrt_status fail(mcrt_ctx* c, mcrt_status st, const std::string& msg) {
   } while (0)
 
 static void free_opacity(mcrt_ctx* c) {
-  cudaFree(c->d_nu); cudaFree(c->d_dnu); cudaFree(c->d_kabs); cudaFree(c->d_opac);
-  cudaFree(c->d_lnQ); cudaFree(c->d_cdf); cudaFree(c->d_small); cudaFree(c->d_guide);
+  mc_free(c->d_nu); mc_free(c->d_dnu); mc_free(c->d_kabs); mc_free(c->d_opac);
+  mc_free(c->d_lnQ); mc_free(c->d_cdf); mc_free(c->d_small); mc_free(c->d_guide);
   c->d_nu = c->d_dnu = c->d_kabs = nullptr; c->d_opac = nullptr; c->d_lnQ = c->d_cdf = nullptr; c->d_guide = nullptr;
   c->d_small = nullptr;
 }
 static void free_pah(mcrt_ctx* c) {
-  cudaFree(c->d_kabs_eq); cudaFree(c->d_pah_C); cudaFree(c->d_pah_E); cudaFree(c->d_pah_T); cudaFree(c->d_pah_U);
-  cudaFree(c->d_pah_Lam); cudaFree(c->d_pah_W); cudaFree(c->d_pah_P); cudaFree(c->d_pah_J); cudaFree(c->d_pah_next); cudaFree(c->d_pah_q);
-  cudaFree(c->d_pah_cdf); cudaFree(c->d_pah_cold); cudaFree(c->d_pah_cnt); cudaFree(c->d_pah_W32);
+  mc_free(c->d_kabs_eq); mc_free(c->d_pah_C); mc_free(c->d_pah_E); mc_free(c->d_pah_T); mc_free(c->d_pah_U);
+  mc_free(c->d_pah_Lam); mc_free(c->d_pah_W); mc_free(c->d_pah_P); mc_free(c->d_pah_J); mc_free(c->d_pah_next); mc_free(c->d_pah_q);
+  mc_free(c->d_pah_cdf); mc_free(c->d_pah_cold); mc_free(c->d_pah_cnt); mc_free(c->d_pah_W32);
   c->d_pah_W32 = nullptr;
   c->d_kabs_eq = c->d_pah_C = c->d_pah_E = c->d_pah_T = c->d_pah_U = c->d_pah_Lam = c->d_pah_W = c->d_pah_P = nullptr;
   c->d_pah_J = nullptr; c->d_pah_next = nullptr; c->d_pah_q = c->d_pah_cdf = c->d_pah_cold = nullptr; c->d_pah_cnt = nullptr;
   c->pah = false;
 }
 static void free_observer(mcrt_ctx* c) {
-  cudaFree(c->obs.sed_mu); cudaFree(c->obs.image);
+  mc_free(c->obs.sed_mu); mc_free(c->obs.image);
   c->obs.sed_mu = c->obs.image = nullptr;
   c->obs.n_mu = c->obs.n_pix = 0;
 }
 static void free_sources(mcrt_ctx* c) {
-  cudaFree(c->d_src); cudaFree(c->d_csrc); cudaFree(c->d_csrc32);
+  mc_free(c->d_src); mc_free(c->d_csrc); mc_free(c->d_csrc32);
   c->d_src = nullptr; c->d_csrc = nullptr; c->d_csrc32 = nullptr;
 }
 
@@ -175,8 +245,8 @@ static mcrt_status build_region_tables(mcrt_ctx* ctx, const int* lut6N, const in
       const int ir = N - 1 - i;
       if (ir != 0 && ir % shape[a] == 0) marked[(size_t)(2 * a + 1) * N + i] = kLutRegion;              // ir -> ir-1
     }
-  if (!ctx->d_lut_marked) CU(cudaMalloc(&ctx->d_lut_marked, sizeof(int) * marked.size()));
-  if (!ctx->d_lut_plain2) CU(cudaMalloc(&ctx->d_lut_plain2, sizeof(int) * plain2.size()));
+  if (!ctx->d_lut_marked) CU(mc_malloc(&ctx->d_lut_marked, sizeof(int) * marked.size()));
+  if (!ctx->d_lut_plain2) CU(mc_malloc(&ctx->d_lut_plain2, sizeof(int) * plain2.size()));
   CU(cudaMemcpy(ctx->d_lut_marked, marked.data(), sizeof(int) * marked.size(), cudaMemcpyHostToDevice));
   CU(cudaMemcpy(ctx->d_lut_plain2, plain2.data(), sizeof(int) * plain2.size(), cudaMemcpyHostToDevice));
   for (int a = 0; a < 3; ++a) ctx->region_cells[a] = shape[a];
@@ -274,7 +344,7 @@ static mcrt_status prepare_density_bits(mcrt_ctx* ctx) {
   std::vector<uint32_t> bits(words, 0u);
   for (size_t i = 0; i < h.size(); ++i)
     if (have1 && h[i] == v1) bits[i >> 5] |= 1u << (i & 31);
-  CU(cudaMalloc(&ctx->d_bits, 4 * words));
+  CU(mc_malloc(&ctx->d_bits, 4 * words));
   CU(cudaMemcpy(ctx->d_bits, bits.data(), 4 * words, cudaMemcpyHostToDevice));
   ctx->dens_mode = 2;
   ctx->stage_bytes = (unsigned)(4 * words);
@@ -354,13 +424,13 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
   float *st_root = nullptr, *st_sub = nullptr;
   int* d_refidx = nullptr;
   const float *src_root = d->rho_root, *src_sub = d->rho_sub;
-  struct Tmp { float*& a; float*& b; int*& c; ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); } } tmp{st_root, st_sub, d_refidx};
+  struct Tmp { float*& a; float*& b; int*& c; ~Tmp() { mc_free(a); mc_free(b); mc_free(c); } } tmp{st_root, st_sub, d_refidx};
   if (d->mem == MCRT_HOST) {
-    CUG(cudaMalloc(&st_root, sizeof(float) * n3));
+    CUG(mc_malloc(&st_root, sizeof(float) * n3));
     CUG(cudaMemcpy(st_root, d->rho_root, sizeof(float) * n3, cudaMemcpyHostToDevice));
     src_root = st_root;
     if (k > 0) {
-      CUG(cudaMalloc(&st_sub, sizeof(float) * k * s3));
+      CUG(mc_malloc(&st_sub, sizeof(float) * k * s3));
       CUG(cudaMemcpy(st_sub, d->rho_sub, sizeof(float) * k * s3, cudaMemcpyHostToDevice));
       src_sub = st_sub;
     }
@@ -388,13 +458,13 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
       }
     }
   }
-  CUG(cudaMalloc(&ctx->d_rho, sizeof(float) * ctx->store_slots));
-  CUG(cudaMalloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->store_slots));
-  CUG(cudaMalloc(&ctx->d_trow, sizeof(float) * ctx->store_slots));
+  CUG(mc_malloc(&ctx->d_rho, sizeof(float) * ctx->store_slots));
+  CUG(mc_malloc(&ctx->d_tally, sizeof(unsigned long long) * ctx->store_slots));
+  CUG(mc_malloc(&ctx->d_trow, sizeof(float) * ctx->store_slots));
   CUG(cudaMemset(ctx->d_tally, 0, sizeof(unsigned long long) * ctx->store_slots));
   CUG(cudaMemset(ctx->d_trow, 0, sizeof(float) * ctx->store_slots));
   if (k > 0) {
-    CUG(cudaMalloc(&d_refidx, sizeof(int) * n3));
+    CUG(mc_malloc(&d_refidx, sizeof(int) * n3));
     CUG(cudaMemcpy(d_refidx, refidx.data(), sizeof(int) * n3, cudaMemcpyHostToDevice));
   }
   {
@@ -424,7 +494,7 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
         stride *= S;
       }
     }
-    CUG(cudaMalloc(&ctx->d_lut, sizeof(int) * lut.size()));
+    CUG(mc_malloc(&ctx->d_lut, sizeof(int) * lut.size()));
     CUG(cudaMemcpy(ctx->d_lut, lut.data(), sizeof(int) * lut.size(), cudaMemcpyHostToDevice));
     // Region sweeps for single-level bricked grids of at least 256^3 cells (the L2 and more): the root tables once
     // more with a marker on every step that crosses a boundary between regions of 256 x 128 x 128 cells (17 MB of
@@ -451,7 +521,7 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
     k_sanitize<<<(unsigned)((k * s3 + 255) / 256), 256>>>(src_sub, ctx->d_rho + ctx->store_n3, k * s3);
     ctx->launches++;
   }
-  CUG(cudaMalloc(&ctx->d_lnrho, sizeof(float) * ctx->store_slots));
+  CUG(mc_malloc(&ctx->d_lnrho, sizeof(float) * ctx->store_slots));
   k_ln_density<<<(unsigned)((ctx->store_slots + 255) / 256), 256>>>(ctx->d_rho, ctx->d_lnrho, ctx->store_slots);
   ctx->launches++;
   CUG(cudaGetLastError());
@@ -465,10 +535,10 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
       ctx->stage_bytes = (unsigned)(((size_t)ctx->store_slots * 4 + 15) & ~(size_t)15);
       if (ctx->stage_bytes > (size_t)ctx->store_slots * 4) {   // the bulk copy reads whole 16-byte units
         float* padded = nullptr;
-        CUG(cudaMalloc(&padded, ctx->stage_bytes));
+        CUG(mc_malloc(&padded, ctx->stage_bytes));
         CUG(cudaMemset(padded, 0, ctx->stage_bytes));
         CUG(cudaMemcpy(padded, ctx->d_rho, (size_t)ctx->store_slots * 4, cudaMemcpyDeviceToDevice));
-        cudaFree(ctx->d_rho);
+        mc_free(ctx->d_rho);
         ctx->d_rho = padded;
       }
     }
@@ -485,7 +555,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   for (auto& b : ctx->pending) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& b : ctx->spare) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& t : ctx->tickets) {
-    cudaFree(t.snap_abs); cudaFree(t.snap_T); cudaFree(t.snap_small); cudaFreeHost(t.h_small);
+    mc_free(t.snap_abs); mc_free(t.snap_T); mc_free(t.snap_small); cudaFreeHost(t.h_small);
     if (t.ev_snap) cudaEventDestroy(t.ev_snap);
     if (t.ev_done) cudaEventDestroy(t.ev_done);
   }
@@ -494,11 +564,11 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   free_pah(ctx);
   free_sources(ctx);
   free_observer(ctx);
-  cudaFree(ctx->d_rho); cudaFree(ctx->d_lnrho); cudaFree(ctx->d_tally); cudaFree(ctx->d_trow);
-  cudaFree(ctx->d_lut); cudaFree(ctx->d_lut_marked); cudaFree(ctx->d_lut_plain2); cudaFree(ctx->d_rec);
-  cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]); cudaFree(ctx->d_swcnt); cudaFree(ctx->d_regcnt);
-  cudaFree(ctx->d_heads);
-  cudaFree(ctx->d_bits); cudaFree(ctx->d_tally_scratch); cudaFree(ctx->d_perm); cudaFree(ctx->d_keys); cudaFree(ctx->d_srccnt); cudaFree(ctx->d_out_scratch);
+  mc_free(ctx->d_rho); mc_free(ctx->d_lnrho); mc_free(ctx->d_tally); mc_free(ctx->d_trow);
+  mc_free(ctx->d_lut); mc_free(ctx->d_lut_marked); mc_free(ctx->d_lut_plain2); mc_free(ctx->d_rec);
+  mc_free(ctx->d_list[0]); mc_free(ctx->d_list[1]); mc_free(ctx->d_swcnt); mc_free(ctx->d_regcnt);
+  mc_free(ctx->d_heads);
+  mc_free(ctx->d_bits); mc_free(ctx->d_tally_scratch); mc_free(ctx->d_perm); mc_free(ctx->d_keys); mc_free(ctx->d_srccnt); mc_free(ctx->d_out_scratch);
   delete ctx;
   return MCRT_OK;
 }
@@ -537,22 +607,22 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
   double *d_edges = nullptr, *d_w = nullptr;
   float *d_ka = nullptr, *d_ks = nullptr, *d_g = nullptr;
   struct Tmp { double*& a; double*& b; float*& c; float*& d; float*& e;
-               ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); cudaFree(d); cudaFree(e); } } tmp{d_edges, d_w, d_ka, d_ks, d_g};
-  CU(cudaMalloc(&d_edges, 8 * (nb + 1))); CU(cudaMalloc(&d_w, 8 * ns));
-  CU(cudaMalloc(&d_ka, 4 * (size_t)ns * nb)); CU(cudaMalloc(&d_ks, 4 * (size_t)ns * nb));
-  CU(cudaMalloc(&d_g, 4 * (size_t)ns * nb));
+               ~Tmp() { mc_free(a); mc_free(b); mc_free(c); mc_free(d); mc_free(e); } } tmp{d_edges, d_w, d_ka, d_ks, d_g};
+  CU(mc_malloc(&d_edges, 8 * (nb + 1))); CU(mc_malloc(&d_w, 8 * ns));
+  CU(mc_malloc(&d_ka, 4 * (size_t)ns * nb)); CU(mc_malloc(&d_ks, 4 * (size_t)ns * nb));
+  CU(mc_malloc(&d_g, 4 * (size_t)ns * nb));
   CU(cudaMemcpy(d_edges, d->lambda_edges_um, 8 * (nb + 1), cudaMemcpyHostToDevice));
   CU(cudaMemcpy(d_w, d->weight, 8 * ns, cudaMemcpyHostToDevice));
   CU(cudaMemcpy(d_ka, d->kabs, 4 * (size_t)ns * nb, cudaMemcpyHostToDevice));
   CU(cudaMemcpy(d_ks, d->ksca, 4 * (size_t)ns * nb, cudaMemcpyHostToDevice));
   CU(cudaMemcpy(d_g, d->g, 4 * (size_t)ns * nb, cudaMemcpyHostToDevice));
-  CU(cudaMalloc(&ctx->d_nu, 8 * nb)); CU(cudaMalloc(&ctx->d_dnu, 8 * nb)); CU(cudaMalloc(&ctx->d_kabs, 8 * nb));
-  CU(cudaMalloc(&ctx->d_opac, sizeof(float4) * nb));
-  CU(cudaMalloc(&ctx->d_lnQ, 4 * nT));
-  CU(cudaMalloc(&ctx->d_cdf, 4 * (size_t)nT * nb));
-  CU(cudaMalloc(&ctx->d_guide, sizeof(int) * kGuide));
+  CU(mc_malloc(&ctx->d_nu, 8 * nb)); CU(mc_malloc(&ctx->d_dnu, 8 * nb)); CU(mc_malloc(&ctx->d_kabs, 8 * nb));
+  CU(mc_malloc(&ctx->d_opac, sizeof(float4) * nb));
+  CU(mc_malloc(&ctx->d_lnQ, 4 * nT));
+  CU(mc_malloc(&ctx->d_cdf, 4 * (size_t)nT * nb));
+  CU(mc_malloc(&ctx->d_guide, sizeof(int) * kGuide));
   const size_t n_small = 1 + CNT_N + 4 * (size_t)nb;
-  CU(cudaMalloc(&ctx->d_small, 8 * n_small));
+  CU(mc_malloc(&ctx->d_small, 8 * n_small));
   CU(cudaMemset(ctx->d_small, 0, 8 * n_small));
   k_mix_opacity<<<(nb + 127) / 128, 128>>>(nb, ns, d_edges, d_w, d_ka, d_ks, d_g, ctx->root_size,
                                            ctx->d_nu, ctx->d_dnu, ctx->d_kabs, ctx->d_opac);
@@ -605,13 +675,13 @@ mcrt_status mcrt_set_source(mcrt_ctx* ctx, int32_t n_src, const mcrt_source* src
   free_sources(ctx);
   ctx->have_source = false;
   double* d_T = nullptr;
-  struct Tmp { double*& a; ~Tmp() { cudaFree(a); } } tmp{d_T};
-  CU(cudaMalloc(&d_T, 8 * n_src));
+  struct Tmp { double*& a; ~Tmp() { mc_free(a); } } tmp{d_T};
+  CU(mc_malloc(&d_T, 8 * n_src));
   CU(cudaMemcpy(d_T, Tbb.data(), 8 * n_src, cudaMemcpyHostToDevice));
-  CU(cudaMalloc(&ctx->d_src, sizeof(SrcDev) * n_src));
+  CU(mc_malloc(&ctx->d_src, sizeof(SrcDev) * n_src));
   CU(cudaMemcpy(ctx->d_src, h.data(), sizeof(SrcDev) * n_src, cudaMemcpyHostToDevice));
-  CU(cudaMalloc(&ctx->d_csrc, 8 * (size_t)n_src * ctx->nb));
-  CU(cudaMalloc(&ctx->d_csrc32, 4 * (size_t)n_src * ctx->nb));
+  CU(mc_malloc(&ctx->d_csrc, 8 * (size_t)n_src * ctx->nb));
+  CU(mc_malloc(&ctx->d_csrc32, 4 * (size_t)n_src * ctx->nb));
   k_build_source_cdf<<<n_src, 128, 8 * (ctx->nb + 1)>>>(ctx->nb, d_T, ctx->d_nu, ctx->d_dnu, ctx->d_csrc, ctx->d_csrc32);
   ctx->launches++;
   CU(cudaGetLastError());
@@ -648,7 +718,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.tally32 = tally32; P.trow = ctx->d_trow;
   P.opac = ctx->d_opac; P.cdf = ctx->d_cdf; P.csrc = ctx->d_csrc32; P.csrc64 = ctx->d_csrc; P.src = ctx->d_src;
   if (!ctx->d_heads) {
-    CU(cudaMalloc(&ctx->d_heads, 16));
+    CU(mc_malloc(&ctx->d_heads, 16));
     CU(cudaMemset(ctx->d_heads, 0, 16));
   }
   P.next = nullptr; P.next_reset = nullptr;                  // (set at each launch, below)
@@ -677,16 +747,16 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   }
   if (gmode && sub * ctx->nsrc <= kMaxOrderedSources && (sub > 1 || ctx->nsrc > 1) && n >= 65536) {
     if (ctx->perm_cap < n) {
-      cudaFree(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
-      CU(cudaMalloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
+      mc_free(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
+      CU(mc_malloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
       ctx->perm_cap = n;
     }
     if (ctx->keys_cap < n) {
-      cudaFree(ctx->d_keys); ctx->d_keys = nullptr; ctx->keys_cap = 0;
-      CU(cudaMalloc(&ctx->d_keys, sizeof(uint16_t) * (size_t)n));
+      mc_free(ctx->d_keys); ctx->d_keys = nullptr; ctx->keys_cap = 0;
+      CU(mc_malloc(&ctx->d_keys, sizeof(uint16_t) * (size_t)n));
       ctx->keys_cap = n;
     }
-    if (!ctx->d_srccnt) CU(cudaMalloc(&ctx->d_srccnt, sizeof(unsigned int) * 2 * kMaxOrderedSources));
+    if (!ctx->d_srccnt) CU(mc_malloc(&ctx->d_srccnt, sizeof(unsigned int) * 2 * kMaxOrderedSources));
     CU(cudaMemsetAsync(ctx->d_srccnt, 0, sizeof(unsigned int) * 2 * kMaxOrderedSources, st));
     // (every block flushes its histogram of all groups: fewer, larger blocks when the groups are many)
     const unsigned gblocks = (unsigned)ctx->sm_count * (ctx->nsrc * sub > 2048 ? 3u : 8u);
@@ -730,21 +800,21 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   PU.lut2 = 0;
   if (region) {
     if (ctx->rec_cap < n) {
-      cudaFree(ctx->d_rec); cudaFree(ctx->d_list[0]); cudaFree(ctx->d_list[1]);
+      mc_free(ctx->d_rec); mc_free(ctx->d_list[0]); mc_free(ctx->d_list[1]);
       ctx->d_rec = nullptr; ctx->d_list[0] = ctx->d_list[1] = nullptr; ctx->rec_cap = 0;
-      CU(cudaMalloc(&ctx->d_rec, sizeof(float4) * 3 * (size_t)n));
-      CU(cudaMalloc(&ctx->d_list[0], 8 * (size_t)n));
-      CU(cudaMalloc(&ctx->d_list[1], 8 * (size_t)n));
+      CU(mc_malloc(&ctx->d_rec, sizeof(float4) * 3 * (size_t)n));
+      CU(mc_malloc(&ctx->d_list[0], 8 * (size_t)n));
+      CU(mc_malloc(&ctx->d_list[1], 8 * (size_t)n));
       ctx->rec_cap = n;
     }
     if (ctx->perm_cap < n) {
-      cudaFree(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
-      CU(cudaMalloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
+      mc_free(ctx->d_perm); ctx->d_perm = nullptr; ctx->perm_cap = 0;
+      CU(mc_malloc(&ctx->d_perm, sizeof(uint32_t) * (size_t)n));
       ctx->perm_cap = n;
     }
     const int nreg = 4096;                                   // capacity of the histogram (regions <= 4096)
-    if (!ctx->d_swcnt) CU(cudaMalloc(&ctx->d_swcnt, sizeof(unsigned int) * (kMaxSweeps + 2)));
-    if (!ctx->d_regcnt) CU(cudaMalloc(&ctx->d_regcnt, sizeof(unsigned int) * 2 * (size_t)nreg));
+    if (!ctx->d_swcnt) CU(mc_malloc(&ctx->d_swcnt, sizeof(unsigned int) * (kMaxSweeps + 2)));
+    if (!ctx->d_regcnt) CU(mc_malloc(&ctx->d_regcnt, sizeof(unsigned int) * 2 * (size_t)nreg));
     CU(cudaMemsetAsync(ctx->d_swcnt, 0, sizeof(unsigned int) * (kMaxSweeps + 2), st));
     PU.rec = ctx->d_rec; PU.lut = ctx->d_lut_marked;
     PU.list_out = ctx->d_list[0]; PU.list_out_count = ctx->d_swcnt;
@@ -845,7 +915,7 @@ static mcrt_status launch_pah_update(mcrt_ctx* ctx, uint64_t n_cum, cudaStream_t
   long long blocks = only_slot >= 0 ? 1 : (ctx->store_slots + warps - 1) / warps;
   const long long cap = (long long)ctx->sm_count * 16;
   if (blocks > cap) blocks = cap;
-  if (!ctx->d_pah_next) CU(cudaMalloc(&ctx->d_pah_next, 8));
+  if (!ctx->d_pah_next) CU(mc_malloc(&ctx->d_pah_next, 8));
   CU(cudaMemsetAsync(ctx->d_pah_next, 0, 8, st));            // work queue of leaves
   k_pah_update<<<(unsigned)blocks, 32 * (only_slot >= 0 ? 1 : warps), smem, st>>>(
       ctx->pahd, ctx->d_rho, ctx->d_pah_cnt, ctx->d_pah_cdf, ctx->store_slots,
@@ -868,7 +938,7 @@ static mcrt_status launch_update(mcrt_ctx* ctx, const unsigned long long* tally,
   float ln_sub3 = (float)(3.0 * std::log((double)ctx->S));
   if (tally != ctx->d_tally && needs_reorder(ctx)) {               // caller's sum is in slot order (R22)
     if (!ctx->d_tally_scratch) {
-      CU(cudaMalloc(&ctx->d_tally_scratch, 8 * (size_t)ctx->store_slots));
+      CU(mc_malloc(&ctx->d_tally_scratch, 8 * (size_t)ctx->store_slots));
       CU(cudaMemsetAsync(ctx->d_tally_scratch, 0, 8 * (size_t)ctx->store_slots, st));
     }
     mcrt_status rc = api_to_store_u64(ctx, tally, ctx->d_tally_scratch, st);
@@ -1021,7 +1091,7 @@ mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps
     unsigned long long* d_out = (unsigned long long*)n_abs_out;
     unsigned long long* tmp = nullptr;
     if (mem == MCRT_HOST) {
-      if (!ctx->d_out_scratch) CU(cudaMalloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
+      if (!ctx->d_out_scratch) CU(mc_malloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
       tmp = (unsigned long long*)ctx->d_out_scratch; d_out = tmp;
     }
     mcrt_status rc = store_to_api_u64(ctx, ctx->d_tally, d_out, ctx->last_stream);
@@ -1040,7 +1110,7 @@ mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem)
   float* d_T = T_out;
   float* tmp = nullptr;
   if (mem == MCRT_HOST) {
-    if (!ctx->d_out_scratch) CU(cudaMalloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
+    if (!ctx->d_out_scratch) CU(mc_malloc(&ctx->d_out_scratch, 8 * (size_t)ctx->slots));
     tmp = (float*)ctx->d_out_scratch; d_T = tmp;
   }
   {
@@ -1085,18 +1155,18 @@ mcrt_status mcrt_set_pah(mcrt_ctx* ctx, const mcrt_pah_desc* d) {
   free_pah(ctx);
   const int nb = ctx->nb;
   float* d_in = nullptr;
-  struct Tmp { float*& a; ~Tmp() { cudaFree(a); } } tmp{d_in};
-  CU(cudaMalloc(&d_in, 4 * (size_t)nb));
+  struct Tmp { float*& a; ~Tmp() { mc_free(a); } } tmp{d_in};
+  CU(mc_malloc(&d_in, 4 * (size_t)nb));
   CU(cudaMemcpy(d_in, d->kabs_pah, 4 * (size_t)nb, cudaMemcpyHostToDevice));
-  CU(cudaMalloc(&ctx->d_kabs_eq, 8 * (size_t)nb)); CU(cudaMalloc(&ctx->d_pah_q, 4 * (size_t)nb));
-  CU(cudaMalloc(&ctx->d_pah_C, 8 * (size_t)nb)); CU(cudaMalloc(&ctx->d_pah_E, 8 * (size_t)nb));
-  CU(cudaMalloc(&ctx->d_pah_T, 8 * (size_t)K)); CU(cudaMalloc(&ctx->d_pah_U, 8 * (size_t)K));
-  CU(cudaMalloc(&ctx->d_pah_Lam, 8 * (size_t)K)); CU(cudaMalloc(&ctx->d_pah_P, 8 * (size_t)K));
-  CU(cudaMalloc(&ctx->d_pah_W, 8 * (size_t)K * nb)); CU(cudaMalloc(&ctx->d_pah_J, sizeof(int) * (size_t)K * K));
-  CU(cudaMalloc(&ctx->d_pah_W32, 4 * (size_t)K * nb));
-  CU(cudaMalloc(&ctx->d_pah_cold, 4 * (size_t)nb));
-  CU(cudaMalloc(&ctx->d_pah_cnt, sizeof(uint32_t) * (size_t)ctx->store_slots * nb));
-  CU(cudaMalloc(&ctx->d_pah_cdf, sizeof(float) * (size_t)ctx->store_slots * nb));
+  CU(mc_malloc(&ctx->d_kabs_eq, 8 * (size_t)nb)); CU(mc_malloc(&ctx->d_pah_q, 4 * (size_t)nb));
+  CU(mc_malloc(&ctx->d_pah_C, 8 * (size_t)nb)); CU(mc_malloc(&ctx->d_pah_E, 8 * (size_t)nb));
+  CU(mc_malloc(&ctx->d_pah_T, 8 * (size_t)K)); CU(mc_malloc(&ctx->d_pah_U, 8 * (size_t)K));
+  CU(mc_malloc(&ctx->d_pah_Lam, 8 * (size_t)K)); CU(mc_malloc(&ctx->d_pah_P, 8 * (size_t)K));
+  CU(mc_malloc(&ctx->d_pah_W, 8 * (size_t)K * nb)); CU(mc_malloc(&ctx->d_pah_J, sizeof(int) * (size_t)K * K));
+  CU(mc_malloc(&ctx->d_pah_W32, 4 * (size_t)K * nb));
+  CU(mc_malloc(&ctx->d_pah_cold, 4 * (size_t)nb));
+  CU(mc_malloc(&ctx->d_pah_cnt, sizeof(uint32_t) * (size_t)ctx->store_slots * nb));
+  CU(mc_malloc(&ctx->d_pah_cdf, sizeof(float) * (size_t)ctx->store_slots * nb));
   k_pah_split<<<(nb + 127) / 128, 128>>>(nb, ctx->d_kabs, d_in, ctx->d_nu, d->n_C, d->mass_fraction, ctx->d_kabs_eq,
                                          ctx->d_pah_q, ctx->d_pah_C, ctx->d_pah_E);
   // the equilibrium tables from what is left for the grains in equilibrium (R35)
@@ -1143,8 +1213,8 @@ static mcrt_status get_rows(mcrt_ctx* ctx, const T* store, T* out, mcrt_mem mem)
   const size_t bytes = sizeof(T) * (size_t)ctx->slots * ctx->nb;
   T* d_out = out;
   T* tmp = nullptr;
-  struct Tmp { T*& a; ~Tmp() { cudaFree(a); } } guard{tmp};
-  if (mem == MCRT_HOST) { CU(cudaMalloc(&tmp, bytes)); d_out = tmp; }
+  struct Tmp { T*& a; ~Tmp() { mc_free(a); } } guard{tmp};
+  if (mem == MCRT_HOST) { CU(mc_malloc(&tmp, bytes)); d_out = tmp; }
   mcrt_status rc = rows_to_api<T>(ctx, store, d_out, ctx->last_stream);
   if (rc != MCRT_OK) return rc;
   if (mem == MCRT_HOST) return copy_out(ctx, out, tmp, bytes, MCRT_HOST);
@@ -1214,7 +1284,7 @@ mcrt_status mcrt_results_begin(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem 
   unsigned long long* abs_dst = nullptr;
   float* T_dst = nullptr;
   if (out->n_abs) {
-    if (host && !t.snap_abs) CU(cudaMalloc(&t.snap_abs, 8 * (size_t)ctx->slots));
+    if (host && !t.snap_abs) CU(mc_malloc(&t.snap_abs, 8 * (size_t)ctx->slots));
     abs_dst = host ? t.snap_abs : (unsigned long long*)out->n_abs;
     if (needs_reorder(ctx)) {
       mcrt_status rc = store_to_api_u64(ctx, ctx->d_tally, abs_dst, st);
@@ -1224,12 +1294,12 @@ mcrt_status mcrt_results_begin(mcrt_ctx* ctx, const mcrt_results* out, mcrt_mem 
     }
   }
   if (out->T) {
-    if (host && !t.snap_T) CU(cudaMalloc(&t.snap_T, 4 * (size_t)ctx->slots));
+    if (host && !t.snap_T) CU(mc_malloc(&t.snap_T, 4 * (size_t)ctx->slots));
     T_dst = host ? t.snap_T : out->T;
     mcrt_status rc = trow_to_api_T(ctx, T_dst, st);
     if (rc != MCRT_OK) return rc;
   }
-  if (!t.snap_small) { CU(cudaMalloc(&t.snap_small, 8 * n_small)); }
+  if (!t.snap_small) { CU(mc_malloc(&t.snap_small, 8 * n_small)); }
   CU(cudaMemcpyAsync(t.snap_small, ctx->d_small, 8 * n_small, cudaMemcpyDeviceToDevice, st));
   CU(cudaGetLastError());
   CU(cudaEventRecord(t.ev_snap, st));
@@ -1313,11 +1383,11 @@ mcrt_status mcrt_set_observer(mcrt_ctx* ctx, const mcrt_observer_desc* d) {
   CU(cudaDeviceSynchronize());
   free_observer(ctx);
   if (d->n_mu > 0) {
-    CU(cudaMalloc(&ctx->obs.sed_mu, 8 * (size_t)d->n_mu * 3 * ctx->nb));
+    CU(mc_malloc(&ctx->obs.sed_mu, 8 * (size_t)d->n_mu * 3 * ctx->nb));
     CU(cudaMemset(ctx->obs.sed_mu, 0, 8 * (size_t)d->n_mu * 3 * ctx->nb));
   }
   if (d->n_pix > 0) {
-    CU(cudaMalloc(&ctx->obs.image, 8 * (size_t)d->n_pix * d->n_pix));
+    CU(mc_malloc(&ctx->obs.image, 8 * (size_t)d->n_pix * d->n_pix));
     CU(cudaMemset(ctx->obs.image, 0, 8 * (size_t)d->n_pix * d->n_pix));
   }
   ctx->obs.n_mu = d->n_mu; ctx->obs.n_pix = d->n_pix;
@@ -1504,8 +1574,8 @@ mcrt_status mcrt_philox_blocks(const uint32_t* key2, const uint32_t* ctr, uint32
   if (!key2 || !ctr || !out || n < 0) return fail(nullptr, MCRT_EINVAL, "mcrt_philox_blocks: bad arguments");
   if (n == 0) return MCRT_OK;
   uint32_t *d_c = nullptr, *d_o = nullptr;
-  struct Tmp { uint32_t*& a; uint32_t*& b; ~Tmp() { cudaFree(a); cudaFree(b); } } tmp{d_c, d_o};
-  CU(cudaMalloc(&d_c, 16 * (size_t)n)); CU(cudaMalloc(&d_o, 16 * (size_t)n));
+  struct Tmp { uint32_t*& a; uint32_t*& b; ~Tmp() { mc_free(a); mc_free(b); } } tmp{d_c, d_o};
+  CU(mc_malloc(&d_c, 16 * (size_t)n)); CU(mc_malloc(&d_o, 16 * (size_t)n));
   CU(cudaMemcpy(d_c, ctr, 16 * (size_t)n, cudaMemcpyHostToDevice));
   k_philox_blocks<<<(unsigned)((n + 255) / 256), 256>>>(key2[0], key2[1], d_c, d_o, n);
   CU(cudaGetLastError());
@@ -1525,9 +1595,9 @@ mcrt_status mcrt_uniforms(const uint32_t* words, float* u, double* ud, float* ta
   if (!words || !u || !ud || !tau || n < 0) return fail(nullptr, MCRT_EINVAL, "mcrt_uniforms: bad arguments");
   if (n == 0) return MCRT_OK;
   uint32_t* d_w = nullptr; float *d_u = nullptr, *d_t = nullptr; double* d_ud = nullptr;
-  struct Tmp { uint32_t*& a; float*& b; float*& c; double*& d; ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); cudaFree(d); } } tmp{d_w, d_u, d_t, d_ud};
-  CU(cudaMalloc(&d_w, 4 * (size_t)n)); CU(cudaMalloc(&d_u, 4 * (size_t)n)); CU(cudaMalloc(&d_t, 4 * (size_t)n));
-  CU(cudaMalloc(&d_ud, 8 * (size_t)n));
+  struct Tmp { uint32_t*& a; float*& b; float*& c; double*& d; ~Tmp() { mc_free(a); mc_free(b); mc_free(c); mc_free(d); } } tmp{d_w, d_u, d_t, d_ud};
+  CU(mc_malloc(&d_w, 4 * (size_t)n)); CU(mc_malloc(&d_u, 4 * (size_t)n)); CU(mc_malloc(&d_t, 4 * (size_t)n));
+  CU(mc_malloc(&d_ud, 8 * (size_t)n));
   CU(cudaMemcpy(d_w, words, 4 * (size_t)n, cudaMemcpyHostToDevice));
   k_uniforms<<<(unsigned)((n + 255) / 256), 256>>>(d_w, d_u, d_ud, d_t, n);
   CU(cudaGetLastError());
@@ -1550,9 +1620,9 @@ mcrt_status mcrt_gather_calibrate(uint64_t footprint_bytes, uint64_t n_gathers, 
   float *d_a = nullptr, *d_sink = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   struct Tmp { float*& a; float*& b; cudaEvent_t& e0; cudaEvent_t& e1;
-               ~Tmp() { cudaFree(a); cudaFree(b); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); } } tmp{d_a, d_sink, e0, e1};
-  CU(cudaMalloc(&d_a, 4 * (size_t)n_elems));
-  CU(cudaMalloc(&d_sink, 4));
+               ~Tmp() { mc_free(a); mc_free(b); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); } } tmp{d_a, d_sink, e0, e1};
+  CU(mc_malloc(&d_a, 4 * (size_t)n_elems));
+  CU(mc_malloc(&d_sink, 4));
   CU(cudaMemsetAsync(d_a, 0, 4 * (size_t)n_elems, st));
   CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
   const unsigned blocks = (unsigned)sms * 8u, threads = 256u;
