@@ -177,6 +177,35 @@ mcrt_status mcrt_accumulate_update(mcrt_ctx* ctx, const uint32_t* delta_sum_dev,
 mcrt_status mcrt_get_cell_energy(mcrt_ctx* ctx, uint64_t* n_abs_out, double* eps_out, mcrt_mem mem);
 /* T_out[leaf slots] in K; T_min for cells that absorbed nothing or hold no dust. */
 mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem);
+/* The temperatures of mcrt_get_cell_temperature(ctx, T_out, MCRT_HOST), read out WITHOUT allocating
+ * device memory.  Who needs it: the ordinary getter converts the stored temperature rows to kelvin
+ * in slot order (R22) with a kernel, and that kernel needs a device array to write to before the
+ * copy to the host -- the getter cudaMallocs one (4..8 B x leaf slots) the first time it is used
+ * on a context.  Some callers must not, or cannot, do that between batches: a process whose
+ * device memory is already handed out in full to another allocator (a torch caching pool, a fixed
+ * MPS / MIG memory quota) where a late cudaMalloc fails; a host thread that runs while another
+ * thread of the process records a CUDA graph in global capture mode, where any cudaMalloc breaks
+ * the recording; a latency-bound control loop that cannot afford the device-wide synchronisation
+ * a cudaMalloc or cudaFree may imply.  For them the conversion kernel of this call writes into an
+ * array that is part of the library image: MCRT_NOALLOC_MAX_SLOTS floats (4 MiB), which every GPU
+ * that loads libmcrt.so holds from load until the process exits, used or not.
+ *   T_out: HOST pointer, [leaf slots] floats, owned by the caller; K, same values bit for bit as
+ *     the ordinary getter's.  The call returns after the copy to T_out has completed.
+ *   Limit: mcrt_leaf_slots(ctx) <= MCRT_NOALLOC_MAX_SLOTS, else MCRT_EINVAL and a message naming
+ *     both numbers (C0 and C1 fit; the disks and the 512^3 cube do not: use the ordinary getter).
+ *   The context's device must be the current device (MCRT_ESTATE otherwise).
+ *   The first call on a GPU asks the driver once where that GPU's copy of the array lives
+ *     (cudaGetSymbolAddress); later calls reuse the answer.  Make that first call before any
+ *     stream capture starts.
+ *   The call makes no cudaMalloc, cudaFree or other allocating CUDA call, and nothing is freed.
+ *   ONE array per GPU serves every context and every call, and it keeps whatever the previous call
+ *     left in it.  Nothing has to be cleared: each of the [leaf slots] floats copied out is written
+ *     by this call's kernels first, and no float beyond them is read.  Two such calls in flight on
+ *     one GPU at the same time would overwrite each other's temperatures; the library therefore
+ *     takes a process-wide lock for the whole call and does not return before its copy is done.
+ *     Do not work around that (e.g. by copying the array yourself from another stream). */
+#define MCRT_NOALLOC_MAX_SLOTS 1048576
+mcrt_status mcrt_get_cell_temperature_noalloc(mcrt_ctx* ctx, float* T_out_host);
 /* counts_out[3][n_bins]: escaped packages per bin; component 0 = direct (never interacted),
  * 1 = scattered only, 2 = thermal (re-emitted at least once) (R24). */
 mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem);

@@ -92,6 +92,16 @@ static cudaError_t mc_free(void* q) {
   return cudaFree(q);
 }
 
+// ---- device array of mcrt_get_cell_temperature_noalloc (include/mcrt.h) -------------------------------------------
+// Part of the library image: every GPU that loads the library holds these 4 MiB until the process exits.  The
+// name below is only a handle in host code -- it is NOT a device address there; the address of a GPU's copy comes
+// from cudaGetSymbolAddress with that GPU current (noalloc_T_array, once per GPU).
+constexpr long long kNoallocMaxSlots = MCRT_NOALLOC_MAX_SLOTS;
+static __device__ __align__(256) float g_noalloc_T[kNoallocMaxSlots];
+constexpr int kNoallocMaxDevices = 64;
+static float* g_noalloc_T_ptr[kNoallocMaxDevices] = {};      // [device] address of that GPU's copy; nullptr: not asked yet
+static std::mutex g_noalloc_mutex;                           // one call at a time: the array is shared
+
 struct BatchEvents { cudaEvent_t e0, e1, e2; };
 
 struct mcrt_ctx {
@@ -1120,6 +1130,51 @@ mcrt_status mcrt_get_cell_temperature(mcrt_ctx* ctx, float* T_out, mcrt_mem mem)
   CU(cudaGetLastError());
   if (mem == MCRT_HOST) return copy_out(ctx, T_out, tmp, 4 * (size_t)ctx->slots, MCRT_HOST);
   return sync_last(ctx);
+}
+
+// Address of the current GPU's copy of g_noalloc_T (asked once per GPU; the caller holds g_noalloc_mutex).
+static mcrt_status noalloc_T_array(mcrt_ctx* ctx, int dev, float** out) {
+  if (!g_noalloc_T_ptr[dev]) {
+    float* p = nullptr;
+    CU(cudaGetSymbolAddress((void**)&p, g_noalloc_T));
+    if (!p) return fail(ctx, MCRT_ECUDA, "mcrt_get_cell_temperature_noalloc: cudaGetSymbolAddress returned NULL");
+    g_noalloc_T_ptr[dev] = p;
+  }
+  *out = g_noalloc_T_ptr[dev];
+  return MCRT_OK;
+}
+
+// mcrt_get_cell_temperature for callers that cannot allocate device memory (include/mcrt.h says who): the same
+// conversion kernels, writing into the library's own fixed array instead of a cudaMalloc'ed one.  No cudaMalloc /
+// cudaFree / allocating CUDA call on this path; nothing in the array needs clearing (every float copied out is
+// written first).  The lock is held until the copy to the host is complete, so calls never overlap on the GPU.
+mcrt_status mcrt_get_cell_temperature_noalloc(mcrt_ctx* ctx, float* T_out_host) {
+  if (!ctx) return MCRT_EINVAL;
+  if (!T_out_host) return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_temperature_noalloc: NULL output");
+  if (!ctx->have_opacity) return fail(ctx, MCRT_ESTATE, "mcrt_get_cell_temperature_noalloc: opacity not set");
+  if (ctx->slots > kNoallocMaxSlots)
+    return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_temperature_noalloc: the grid has " + std::to_string(ctx->slots) +
+                                      " leaf slots, the library's fixed array holds MCRT_NOALLOC_MAX_SLOTS = " +
+                                      std::to_string(kNoallocMaxSlots) + " (use mcrt_get_cell_temperature, which allocates)");
+  int dev = -1;
+  CU(cudaGetDevice(&dev));
+  if (dev != ctx->device)
+    return fail(ctx, MCRT_ESTATE, "mcrt_get_cell_temperature_noalloc: the context lives on device " +
+                                      std::to_string(ctx->device) + " but device " + std::to_string(dev) + " is current");
+  if (dev < 0 || dev >= kNoallocMaxDevices)
+    return fail(ctx, MCRT_EINVAL, "mcrt_get_cell_temperature_noalloc: device index beyond " + std::to_string(kNoallocMaxDevices - 1));
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  float* d_T = nullptr;
+  {
+    mcrt_status rc = noalloc_T_array(ctx, dev, &d_T);
+    if (rc != MCRT_OK) return rc;
+  }
+  {
+    mcrt_status rc = trow_to_api_T(ctx, d_T, ctx->last_stream);
+    if (rc != MCRT_OK) return rc;
+  }
+  CU(cudaGetLastError());
+  return copy_out(ctx, T_out_host, d_T, 4 * (size_t)ctx->slots, MCRT_HOST);
 }
 
 mcrt_status mcrt_get_sed(mcrt_ctx* ctx, uint64_t* counts_out, mcrt_mem mem) {

@@ -12,6 +12,7 @@ import numpy as np
 from . import build as _build
 
 MCRT_HOST, MCRT_DEVICE = 0, 1
+NOALLOC_MAX_SLOTS = 1 << 20          # MCRT_NOALLOC_MAX_SLOTS of include/mcrt.h
 _lib = None
 
 
@@ -65,7 +66,7 @@ SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opac
            "mcrt_update_temperature", "mcrt_store_slots", "mcrt_delta_words", "mcrt_transport_batch_delta",
            "mcrt_accumulate_update", "mcrt_get_results", "mcrt_results_begin", "mcrt_results_wait",
            "mcrt_get_cell_energy",
-           "mcrt_get_cell_temperature", "mcrt_get_sed", "mcrt_set_pah", "mcrt_get_pah_absorbed",
+           "mcrt_get_cell_temperature", "mcrt_get_cell_temperature_noalloc", "mcrt_get_sed", "mcrt_set_pah", "mcrt_get_pah_absorbed",
            "mcrt_get_pah_emission_cdf", "mcrt_get_pah_temperature_distribution", "mcrt_set_observer",
            "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
            "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_tail_mode", "mcrt_set_source_order",
@@ -104,6 +105,8 @@ def lib():
         L.mcrt_results_wait.argtypes = [vp, i32]
         L.mcrt_get_cell_energy.argtypes = [vp, vp, C.POINTER(C.c_double), C.c_int]
         L.mcrt_get_cell_temperature.argtypes = [vp, vp, C.c_int]
+        L.mcrt_get_cell_temperature_noalloc.argtypes = [vp, vp]
+        L.mcrt_get_cell_temperature_noalloc.restype = C.c_int
         L.mcrt_get_sed.argtypes = [vp, vp, C.c_int]
         L.mcrt_set_pah.argtypes = [vp, C.POINTER(_PahDesc)]
         L.mcrt_get_pah_absorbed.argtypes = [vp, vp, C.c_int]
@@ -379,6 +382,19 @@ class Context:
         out, p, mem = self._out((self.slots,), np.float32, device, out)
         self._check(lib().mcrt_get_cell_temperature(self.h, p, mem),
                     "mcrt_get_cell_temperature")
+        return out
+
+    def get_cell_temperature_noalloc(self, out=None):
+        """Temperatures [leaf slots] in K as a numpy array, read out without any device allocation
+        by the library (mcrt_get_cell_temperature_noalloc): for callers that cannot cudaMalloc
+        between batches -- all device memory already owned by another pool or a fixed quota,
+        another thread recording a CUDA graph, a loop that cannot take an allocation's stall.
+        Grids of up to NOALLOC_MAX_SLOTS leaf slots; larger ones raise McrtError.  Same values
+        bit for bit as get_cell_temperature().  One library-owned array per GPU serves all
+        calls, so the library runs them one at a time."""
+        out, p, _ = self._out((self.slots,), np.float32, False, out)
+        self._check(lib().mcrt_get_cell_temperature_noalloc(self.h, p),
+                    "mcrt_get_cell_temperature_noalloc")
         return out
 
     def get_sed(self, device=False, out=None):
