@@ -36,7 +36,9 @@
 // R35..R40; tests/test_oracle_pah.py): the temperature distribution P(T) is pinned by its two
 // physical limits (strong heating -> a narrow peak at the equilibrium temperature; rare hard
 // photons -> the cooling-curve distribution C(T)/Lambda(T)), by the balance of mean heating and
-// mean cooling, and by the exact split of absorptions between PAH and equilibrium grains.
+// mean cooling, and by the exact split of absorptions between PAH and equilibrium grains; the photon rates per
+// molecule that feed it (pah_rates, R40) by the energy identity with a molecule count formed in the test from
+// the inputs (root leaves and sub-cells), joined to the solver through heating = cooling.
 // The WHOLE interaction loop (flights, scattering, absorption + re-emission, cubes and subcubes) at any optical
 // depth is pinned by two situations in which the mathematics fixes its answer (tests/test_oracle_invariants.py):
 // mean-chord invariance (a body in a uniform isotropic field: the expected absorbed count of every leaf, the

@@ -210,3 +210,58 @@ def test_pah_run_heats_up_and_emits_in_the_bands(oracle_mod):
     # deterministic function of the tallies: recomputing from the counts reproduces the rows
     o.pah_update(cumP, 30000)
     assert np.array_equal(o.pah_cdf(), cdf)
+
+
+def test_photon_rates_per_molecule_from_the_leaf_tallies(oracle_mod):
+    """R40 (`pah_rates`, the input of O12): the absorption rate of ONE molecule in bin j is the leaf's
+    absorbed PAH power in that bin, counts_j L_tot / N_cum, divided by the photon energy h nu_j and by
+    the number of molecules in the leaf.  The molecule count is formed HERE from the inputs --
+    mass fraction x rho x V / (N_C x 12 u), V = root_size^3 for a cube and (root_size / S)^3 for a
+    subcube -- so a missing N_C, a missing mass fraction or a wrong sub-cell volume fails:
+      sum_j R_j h nu_j n_mol = sum_j counts_j L_tot / N_cum            (energy, to 1e-12)
+      sum_k P_k Lambda(T_k) n_mol = the same power                     (joins R to the pinned solver)
+    on root leaves and sub-cells of a two-level grid after a real PAH run (the PAH sits
+    in a heating bath fixed by the radiation field; the bath here is the leaf's own tally)."""
+    O = oracle_mod
+    wl = W.c2(n_root=8, n_packets=120_000, batch=40_000)
+    assert wl.sub == 4 and wl.refine is not None and wl.refine.sum() > 0
+    pah = W.pah_share(wl, n_C=60, mass_fraction=0.05, uv_share=0.5, band_share=0.3)
+    o = O.Oracle(wl)
+    o.set_pah(pah.n_C, pah.mass_fraction, pah.kabs, n_Tp=96, T_hi=2.0e4)
+    o.run()
+    counts, total = o.pah_absorbed()
+    assert total > 500                                                  # (a 4000 K star: few hard photons)
+    n3, S = wl.n_root ** 3, wl.sub
+    edges_cm = np.asarray(wl.lambda_edges_um, np.float64) * 1e-4
+    E = H * CL / np.sqrt(edges_cm[:-1] * edges_cm[1:])                  # h nu_j at the bin centres (R4)
+    L_tot = sum(s.L for s in wl.sources)
+    n_cum = wl.n_packets
+    g = o.pah_grid()
+    per_leaf = counts.sum(axis=1)
+    hot = np.flatnonzero(per_leaf > 0)
+    roots, subs = hot[hot < n3], hot[hot >= n3]
+    assert len(roots) > 3 and len(subs) > 3                             # both kinds of leaf
+    picked = list(roots[np.argsort(per_leaf[roots])[-4:]]) + list(subs[np.argsort(per_leaf[subs])[-6:]]) + [int(subs[0])]
+    for slot in picked:
+        if slot < n3:
+            rho, V = float(wl.rho_root[slot]), wl.root_size ** 3
+        else:
+            rho, V = float(wl.rho_sub[slot - n3]), (wl.root_size / S) ** 3
+        assert rho > 0
+        n_mol = pah.mass_fraction * rho * V / (pah.n_C * M_C)
+        R = o.pah_rates(slot, counts[slot], n_cum)
+        power = float(counts[slot].astype(np.float64).sum()) * L_tot / n_cum
+        assert float((R * E).sum()) * n_mol == pytest.approx(power, rel=1e-12)
+        assert np.allclose(R * E * n_mol, counts[slot].astype(np.float64) * L_tot / n_cum, rtol=1e-12, atol=0.0)
+        P, _ = o.pah_solve(R)
+        assert P[-1] < 1e-12
+        assert float((P[1:] * g["Lam"][1:]).sum()) * n_mol == pytest.approx(power, rel=1e-8)
+    # twice the packages behind the same counts: every package carries half the energy
+    R1, R2 = o.pah_rates(picked[0], counts[picked[0]], n_cum), o.pah_rates(picked[0], counts[picked[0]], 2 * n_cum)
+    assert np.allclose(R2, 0.5 * R1, rtol=1e-15)
+    # a leaf without dust, or without absorptions, has no rates
+    empty = np.flatnonzero(np.concatenate([wl.rho_root, wl.rho_sub]) == 0)
+    empty = [e for e in empty if e >= n3 or not wl.refine[e]]
+    if empty:
+        assert o.pah_rates(int(empty[0]), np.ones(o.nb, np.uint64), n_cum) is None
+    assert o.pah_rates(int(picked[0]), np.zeros(o.nb, np.uint64), n_cum) is None
