@@ -284,59 +284,97 @@ def time_steps(torch, ctx, wl, runner, stream, world, steps, warmup, flush, barr
                 launches=ctx.kernel_launches() - launches_before, one_step=one_step)
 
 
+# Minimum lane-instructions the method needs per unit of work (DESIGN.md section 7 derives each figure): the walk
+# step is the SASS instruction count of the committed loop (29 per step + 4.5 of loop overhead per step of the PTX
+# step pair, profiles/r02_summary.md; a two-level grid needs at least that much per crossing); the event figures are
+# hand counts of the arithmetic each event cannot do without (Philox block, -ln, DDA set-up; HG draw + rotation;
+# tally + temperature gather + 7 CDF probes + isotropic draw; emission: source CDF search + direction + start cell,
+# escape tally, lane refill).  Constants of the code, not of a capture: the fraction is reproducible from the
+# line's own counters.
+MIN_LANE_INSTR = {"crossing": 33.5, "flight": 95.0, "scattering": 50.0, "absorption": 57.0, "packet": 70.0}
+
+
+def lane_issue_peak():
+    """Lane-instructions per second the GPU can issue: SMs x 4 schedulers x 32 lanes x max SM clock."""
+    return issue_peak() * 32.0
+
+
 def rooflines(wl, name, d, tr_s, steps, gather_peak):
-    """The bound that holds for this workload and the secondary figures (DESIGN.md sections 7, 8).
-    L2-resident density array: the walk is bound by the rate at which the SMs' L1TEX units serve
-    scattered 4-byte gathers (calibrated live, mcrt_gather_calibrate, at this footprint); density
-    array at or above the L2 size: HBM, algorithmic bytes against the measured copy bandwidth."""
+    """roofline of the transport kernel, every figure from THIS run's counters and kernel times (DESIGN.md
+    sections 7, 8).  `frac` is algorithmic work / live kernel time / peak:
+      density array L2-resident (all but C4): bound "alu" -- the minimum lane-instructions of the method
+        (MIN_LANE_INSTR x this run's crossings, flights, scatterings, absorptions, packages) against
+        148 SMs x 4 schedulers x 32 lanes x sm_max_mhz;
+      density array beyond the L2 (C4): bound "hbm" -- SURVEY.md 8(d)(iii) algorithmic bytes against the
+        measured copy bandwidth (MEASURED_PEAKS.json).
+    Inside it, always: "gather" = BASELINE.json's own metric, crossings/s against the independent-gather rate
+    calibrated live at this footprint (mcrt_gather_calibrate); "hbm" and "alu" = the two algorithmic figures;
+    "issue_active" = executed-instruction UTILISATION from the committed ncu capture (not a roofline fraction,
+    never enters frac; stale if the kernel changed after the capture named beside it)."""
     peak, peak_src = measured_peaks()
     bytes_alg, per_cross, per_abs = algorithmic_bytes(wl, d["crossings"], d["absorptions"])
     hbm_achieved = bytes_alg / tr_s / 1e9 if tr_s > 0 else 0.0
     foot = int(wl.leaf_slots) * 4
-    hbm = {"bound": "hbm", "kernel": "k_transport_u", "achieved": hbm_achieved, "peak": peak, "unit": "GB/s",
-           "frac": hbm_achieved / peak, "traffic": ncu_traffic(name), "peak_source": peak_src,
+    cap = ncu_capture(name)
+    hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": peak, "unit": "GB/s",
+           "frac": hbm_achieved / peak, "peak_source": peak_src,
            "algorithmic_bytes": {"per_crossing": per_cross, "per_absorption": per_abs,
-                                 "per_launch": bytes_alg / steps},
-           "kernel_ms": 1e3 * tr_s / steps}
-    if hbm["traffic"]:
-        hbm["traffic_over_algorithmic"] = hbm["traffic"] / (bytes_alg / steps)
-        hbm["dram_rate_gbs_from_capture"] = hbm["traffic"] / (tr_s / steps) / 1e9
+                                 "per_launch": bytes_alg / steps}}
+    traffic = ncu_traffic(name)
+    if traffic:
+        hbm["traffic_over_algorithmic"] = traffic / (bytes_alg / steps)
+    work = (MIN_LANE_INSTR["crossing"] * d["crossings"] + MIN_LANE_INSTR["flight"] * d["flights"]
+            + MIN_LANE_INSTR["scattering"] * d["scatterings"] + MIN_LANE_INSTR["absorption"] * d["absorptions"]
+            + MIN_LANE_INSTR["packet"] * d["emitted"])
+    alu_ach = work / tr_s / 1e9 if tr_s > 0 else 0.0
+    alu_pk = lane_issue_peak() / 1e9
+    alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_pk, "unit": "G lane-instructions/s", "frac": alu_ach / alu_pk,
+           "peak_source": "148 SMs x 4 warp schedulers x 32 lanes x sm_max_mhz (MEASURED_PEAKS.json, else 1965 MHz)",
+           "algorithmic_work": {"min_lane_instructions_per": MIN_LANE_INSTR, "per_launch": work / steps,
+                                "counters_per_launch": {k: d[k] / steps for k in ("crossings", "flights", "scatterings",
+                                                                                  "absorptions", "emitted")}}}
     gather = None
     if gather_peak:
         g_ach = d["crossings"] / tr_s if tr_s > 0 else 0.0
         gather = {"footprint_bytes": foot, "peak_gathers_per_s": gather_peak, "achieved_gathers_per_s": g_ach,
                   "frac": g_ach / gather_peak,
-                  "what": "peak = independent hash-indexed 4-byte gathers/s over an array of the density "
-                          "footprint at full occupancy (mcrt_gather_calibrate); achieved = cell crossings/s "
-                          "of k_transport_u.  A fraction above 1 means the walk's locality (bricks, grouped "
-                          "hand-out) lets one sector serve several crossings: then it is no ceiling and the "
-                          "hbm figures are the ones that bound"}
-    cap = ncu_capture(name)
+                  "what": "BASELINE.json metric '% of gather-BW roofline': peak = independent hash-indexed 4-byte "
+                          "gathers/s over an array of the density footprint at full occupancy (mcrt_gather_calibrate, "
+                          "measured in this run); achieved = cell crossings/s of k_transport_u.  Above 1 the walk's "
+                          "locality (bricks, grouped hand-out) lets one sector serve several crossings: no ceiling then"}
     resident = foot <= 0.75 * L2_BYTES
+    head = alu if resident else hbm
+    roof = {"bound": head["bound"], "kernel": "k_transport_u", "achieved": head["achieved"], "peak": head["peak"],
+            "unit": head["unit"], "frac": head["frac"], "peak_source": head["peak_source"],
+            "traffic": traffic, "traffic_source": cap.get("capture") if traffic else None,
+            "kernel_ms": 1e3 * tr_s / steps,
+            "why_this_bound": ("density array L2-resident: DRAM moves a few per cent of the algorithmic bytes, the "
+                               "kernel is limited by instruction issue at 18-22 of 32 lanes (profiles/)" if resident else
+                               "density array beyond the L2: the gathers' sectors come from HBM (region sweeps keep "
+                               "the traffic near the algorithmic bytes)"),
+            "alu": alu, "hbm": hbm, "gather": gather}
     if cap.get("warp_instructions_per_launch"):
-        # The committed capture of this workload shows what binds it: the issue slots (65-85 % busy, DRAM at
-        # a few per cent of its peak -- C4 too since it is swept region by region --, L1TEX wavefronts well
-        # below their peak).  achieved = the capture's warp instructions per step (all launches of the
-        # transport kernel in a batch) / the kernel time measured HERE; peak = SMs x 4 schedulers x max clock.
         ipl = float(cap["warp_instructions_per_launch"])
-        ach = ipl / (tr_s / steps) / 1e9 if tr_s > 0 else 0.0
-        pk = issue_peak() / 1e9
-        roof = {"bound": "alu", "kernel": "k_transport_u", "achieved": ach, "peak": pk, "unit": "G warp instructions/s",
-                "frac": ach / pk, "traffic": hbm["traffic"],
-                "peak_source": "148 SMs x 4 warp schedulers x 1 instruction/clock x sm_max_mhz (MEASURED_PEAKS.json)",
-                "instructions_per_launch_from_capture": ipl, "lanes_per_instruction": cap.get("lanes_per_instruction"),
-                "useful_lane_frac": (ach / pk) * float(cap.get("lanes_per_instruction", 32.0)) / 32.0,
-                "kernel_ms": 1e3 * tr_s / steps, "hbm": hbm}
-    elif resident and gather:
-        roof = {"bound": "l1tex-gather", "kernel": "k_transport_u", "achieved": 4e-9 * gather["achieved_gathers_per_s"],
-                "peak": 4e-9 * gather_peak, "unit": "GB/s", "frac": gather["frac"], "traffic": hbm["traffic"],
-                "peak_source": "calibrated live: scattered 4-byte gathers over the density footprint x 4 B "
-                               "(density array is L2-resident: DRAM moves ~1 % of the algorithmic bytes)",
-                "algorithmic_bytes": {"per_crossing": 4, "per_launch": 4.0 * d["crossings"] / steps},
-                "kernel_ms": 1e3 * tr_s / steps, "hbm": hbm}
-    else:
-        roof = hbm
+        roof["issue_active"] = {
+            "frac_of_issue_slots": (ipl / (tr_s / steps)) / issue_peak() if tr_s > 0 else 0.0,
+            "warp_instructions_per_launch_from_capture": ipl,
+            "lanes_per_instruction_from_capture": cap.get("lanes_per_instruction"),
+            "capture": cap.get("capture"),
+            "what": "utilisation (executed instructions of a committed ncu capture / this run's kernel time), "
+                    "not an algorithmic fraction; never enters roofline.frac"}
     return roof, gather
+
+
+def update_roofline(wl, store_slots, up_s, steps):
+    """k_update_temperature: a stream over the storage slots -- reads the cumulative tally (u64) and ln rho
+    (fp32), writes the temperature row (fp32): 16 B per slot against the measured copy bandwidth."""
+    if not up_s or up_s <= 0:
+        return None
+    peak, peak_src = measured_peaks()
+    ach = 16.0 * store_slots * steps / up_s / 1e9
+    return {"bound": "hbm", "kernel": "k_update_temperature", "achieved": ach, "peak": peak, "unit": "GB/s",
+            "frac": ach / peak, "peak_source": peak_src, "algorithmic_bytes": {"per_slot": 16, "per_launch": 16.0 * store_slots},
+            "kernel_ms": 1e3 * up_s / steps}
 
 
 def measure_workload(torch, mcrt, wl, name, steps, warmup, stream, flush, args, calibrate=True):
@@ -353,15 +391,21 @@ def measure_workload(torch, mcrt, wl, name, steps, warmup, stream, flush, args, 
     gpeak = mcrt.gather_calibrate(int(wl.leaf_slots) * 4, 1 << 30, stream)[0] if calibrate else None
     roof, gather = rooflines(wl, name, r["d"], tr_s, steps, gpeak)
     d = r["d"]
+    up_s = float(r["t_up"].sum()) * 1e-3
     out = {"config": describe(wl, name), "steps": steps, "warmup": warmup,
            "packets_per_s": d["emitted"] / secs, "crossings_per_s": d["crossings"] / secs,
            "ms_per_step": 1e3 * secs / steps, "kernel_ms": 1e3 * tr_s / steps,
-           "update_ms": float(r["t_up"].sum()) / steps, "lost": d["lost"],
+           "update_ms": 1e3 * up_s / steps, "lost": d["lost"],
            "crossings_per_packet": d["crossings"] / max(d["emitted"], 1),
            "bound": roof["bound"], "roofline_frac": roof["frac"],
-           "hbm_algorithmic_frac": (roof.get("hbm") or roof)["frac"],
+           "alu_algorithmic_frac": roof["alu"]["frac"],
+           "hbm_algorithmic_frac": roof["hbm"]["frac"],
            "gather_frac": gather["frac"] if gather else None,
-           "traffic_over_algorithmic": (roof.get("hbm") or roof).get("traffic_over_algorithmic")}
+           "traffic_over_algorithmic": roof["hbm"].get("traffic_over_algorithmic"),
+           "update_roofline": update_roofline(wl, ctx.store_slots(), up_s, steps)}
+    if name.endswith("_pah"):       # the batch-end time of a PAH run is k_pah_update (P(T) of every leaf) + k_update_temperature
+        out["pah_update_ms"] = out["update_ms"]
+        out["update_roofline"] = None
     ctx.destroy()
     return out
 
@@ -460,6 +504,8 @@ def run_gpu(args, wl, name):
             dist.destroy_process_group()
         return
     secs = total_ms * 1e-3
+    store_slots = ctx.store_slots()
+    ctx.destroy()
     tr_s = float(t_tr.sum()) * 1e-3                          # dominant kernel: this rank's launches
     roof, gather = rooflines(wl, name, d, tr_s, args.steps, gpeak)
     roof["kernel_share_of_step"] = tr_s / (float(sum(step_ms)) * 1e-3)
@@ -477,18 +523,17 @@ def run_gpu(args, wl, name):
            "kernel_ms_per_step": {"transport": tr_ms / args.steps, "temperature_update": up_ms / args.steps},
            "wall_ms_per_step_incl_flush": 1e3 * r["t_wall"] / args.steps,
            "roofline": roof, "gpu_launches": launches, "clocks": clocks}
-    if gather is not None:
-        out["gather_roofline"] = gather
+    out["update_roofline"] = update_roofline(wl, store_slots, up_ms * 1e-3, args.steps)
     if e2e is not None:
         out["e2e"] = e2e
-    ctx.destroy()
     # ---- every other config of BASELINE.json, at reduced step counts, in the same invocation ----
     if world == 1 and not args.no_per_config:
         per = {name: {k: v for k, v in (("packets_per_s", out["value"]), ("crossings_per_s", out["crossings_per_s"]),
                                          ("ms_per_step", out["ms_per_step"]),
                                          ("kernel_ms", roof["kernel_ms"]), ("bound", roof["bound"]),
                                          ("roofline_frac", roof["frac"]),
-                                         ("hbm_algorithmic_frac", (roof.get("hbm") or roof)["frac"]),
+                                         ("alu_algorithmic_frac", roof["alu"]["frac"]),
+                                         ("hbm_algorithmic_frac", roof["hbm"]["frac"]),
                                          ("gather_frac", gather["frac"] if gather else None), ("lost", n_lost))}}
         for wname, wsteps in PER_CONFIG:
             if wname == name:
@@ -577,7 +622,12 @@ def run_e2e(args, wl, mcrt, torch, dist, rank, world, stream, repeats=3):
     order = sorted(range(repeats), key=lambda i: jobs[i]["job_ms"])
     out = dict(jobs[order[repeats // 2]])
     out["job_ms_all"] = [j["job_ms"] for j in jobs]
-    out["what"] += f"; the job is run {repeats} times from scratch, the median job is reported"
+    out["cold_first_job"] = {"value": jobs[0]["value"], "job_ms": jobs[0]["job_ms"], "setup_ms": jobs[0]["setup_ms"],
+                             "what": "the first of the jobs: its device blocks are not all in the library's cache yet "
+                                     "(only those the benchmark's own context of the same shape gave back)"}
+    out["what"] += (f"; the job is run {repeats} times, each with a new context from host arrays; the MEDIAN job is "
+                    "reported: a WARM-POOL job -- the library caches the device blocks a destroyed context gives back "
+                    "(mcrt_release_cached_memory frees them), so jobs 2 and 3 allocate nothing; cold_first_job is the first")
     return out
 
 

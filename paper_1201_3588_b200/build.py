@@ -26,7 +26,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 
 def _sources():
     return sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC)
-                  if f.endswith((".cu", ".cuh", ".h"))) + [os.path.join(INCLUDE, "mcrt.h")]
+                  if f.endswith((".cu", ".cuh", ".h"))) + [os.path.join(INCLUDE, "mcrt.h"), os.path.join(INCLUDE, "mcrt_dev.h")]
 
 
 def needs_build(path: str = LIB_PATH) -> bool:

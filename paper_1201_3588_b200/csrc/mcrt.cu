@@ -3,6 +3,7 @@
 // of the method (table build, emission, walk, interactions, tallies, temperature update) runs in
 // the kernels of transport.cuh / tables.cuh.  There is no CPU fallback.
 #include "mcrt.h"
+#include "mcrt_dev.h"
 
 #include <cmath>
 #include <cstdio>
@@ -31,22 +32,52 @@ using namespace mcrt;
 #include <map>
 #include <mutex>
 namespace {
-std::mutex g_mc_mutex;
-std::multimap<std::pair<int, size_t>, void*> g_mc_cache;      // (device, bytes) -> block
-size_t g_mc_cached = 0;
-std::map<void*, size_t>& g_mc_sizes() { static std::map<void*, size_t> m; return m; }   // live blocks of the library
+// Process-lifetime singletons, never destroyed: a context may be destroyed (Python's Context.__del__) after the
+// static destructors of this library have run.
+struct McBlock { int device; size_t bytes; };
+struct McState {
+  std::mutex mutex;
+  std::multimap<std::pair<int, size_t>, void*> cache;         // (owning device, bytes) -> block
+  size_t cached = 0;
+  std::map<void*, McBlock> live;                              // every block of the library: the device it was allocated on
+};
+McState& mc_state() { static McState* s = new McState; return *s; }
 constexpr size_t kMcBlockMax = (size_t)256 << 20, kMcTotalMax = (size_t)1 << 30;
+
+// Makes `dev` the current device for its lifetime (blocks are synchronised and freed on the device that owns them).
+struct DeviceScope {
+  int prev = -1; bool switched = false;
+  explicit DeviceScope(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev && dev >= 0) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceScope() { if (switched) cudaSetDevice(prev); }
+};
+
+// Frees every cached block (the caller holds the lock).
+size_t mc_release_cache_locked(McState& S) {
+  const size_t bytes = S.cached;
+  for (auto& kv : S.cache) {
+    DeviceScope scope(kv.first.first);
+    S.live.erase(kv.second);
+    cudaFree(kv.second);
+  }
+  S.cache.clear();
+  S.cached = 0;
+  return bytes;
+}
 }  // namespace
 template <typename T>
 static cudaError_t mc_malloc(T** p, size_t bytes) {
+  McState& S = mc_state();
   int dev = 0;
-  if (bytes && bytes <= kMcBlockMax && cudaGetDevice(&dev) == cudaSuccess) {
-    std::lock_guard<std::mutex> lock(g_mc_mutex);
-    auto it = g_mc_cache.find({dev, bytes});
-    if (it != g_mc_cache.end()) {
+  const bool have_dev = cudaGetDevice(&dev) == cudaSuccess;
+  if (bytes && bytes <= kMcBlockMax && have_dev) {
+    std::lock_guard<std::mutex> lock(S.mutex);
+    auto it = S.cache.find({dev, bytes});
+    if (it != S.cache.end()) {
       *p = static_cast<T*>(it->second);
-      g_mc_cache.erase(it);
-      g_mc_cached -= bytes;
+      S.cache.erase(it);
+      S.cached -= bytes;
       return cudaSuccess;
     }
   }
@@ -54,40 +85,41 @@ static cudaError_t mc_malloc(T** p, size_t bytes) {
   cudaError_t e = cudaMalloc(&q, bytes);
   if (e == cudaErrorMemoryAllocation) {                      // give the cache back and try once more
     (void)cudaGetLastError();
-    std::lock_guard<std::mutex> lock(g_mc_mutex);
-    for (auto& kv : g_mc_cache) { g_mc_sizes().erase(kv.second); cudaFree(kv.second); }
-    g_mc_cache.clear();
-    g_mc_cached = 0;
+    {
+      std::lock_guard<std::mutex> lock(S.mutex);
+      mc_release_cache_locked(S);
+    }
     e = cudaMalloc(&q, bytes);
   }
   if (e == cudaSuccess) {
     *p = static_cast<T*>(q);
-    std::lock_guard<std::mutex> lock(g_mc_mutex);
-    g_mc_sizes()[q] = bytes;
+    std::lock_guard<std::mutex> lock(S.mutex);
+    S.live[q] = McBlock{have_dev ? dev : -1, bytes};
   }
   return e;
 }
 static cudaError_t mc_free(void* q) {
   if (!q) return cudaSuccess;
-  size_t bytes = 0;
-  int dev = 0;
+  McState& S = mc_state();
+  McBlock blk{-1, 0};
   {
-    std::lock_guard<std::mutex> lock(g_mc_mutex);
-    auto it = g_mc_sizes().find(q);
-    if (it != g_mc_sizes().end()) bytes = it->second;
+    std::lock_guard<std::mutex> lock(S.mutex);
+    auto it = S.live.find(q);
+    if (it != S.live.end()) blk = it->second;
   }
-  if (bytes && bytes <= kMcBlockMax && cudaGetDevice(&dev) == cudaSuccess) {
+  DeviceScope scope(blk.device);                             // the device the block lives on, whichever is current
+  if (blk.bytes && blk.bytes <= kMcBlockMax && blk.device >= 0) {
     cudaDeviceSynchronize();
-    std::lock_guard<std::mutex> lock(g_mc_mutex);
-    if (g_mc_cached + bytes <= kMcTotalMax) {
-      g_mc_cache.insert({{dev, bytes}, q});
-      g_mc_cached += bytes;
+    std::lock_guard<std::mutex> lock(S.mutex);
+    if (S.cached + blk.bytes <= kMcTotalMax) {
+      S.cache.insert({{blk.device, blk.bytes}, q});
+      S.cached += blk.bytes;
       return cudaSuccess;
     }
   }
   {
-    std::lock_guard<std::mutex> lock(g_mc_mutex);
-    g_mc_sizes().erase(q);
+    std::lock_guard<std::mutex> lock(S.mutex);
+    S.live.erase(q);
   }
   return cudaFree(q);
 }
@@ -204,7 +236,7 @@ struct mcrt_ctx {
   std::string err;
 };
 
-static std::string g_err;   // errors raised without a context
+static thread_local std::string g_err;   // errors raised without a context (per calling thread)
 
 static mcrt_status fail(mcrt_ctx* c, mcrt_status st, const std::string& msg) {
   if (c) c->err = msg; else g_err = msg;
@@ -561,6 +593,7 @@ mcrt_status mcrt_grid_create(const mcrt_grid_desc* d, mcrt_ctx** out) {
 
 mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   if (!ctx) return MCRT_EINVAL;
+  DeviceScope scope(ctx->device);                            // the context's GPU, whichever is current in the caller
   cudaDeviceSynchronize();                                   // nothing of this context may still be running
   for (auto& b : ctx->pending) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& b : ctx->spare) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
@@ -605,7 +638,10 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
   if (nT == 0) { nT = 801; Tmin = 1.0; Tmax = 1.0e4; }
   if (nT < 2 || nT > 8192 || !(Tmin > 0) || !(Tmax > Tmin))
     return fail(ctx, MCRT_EINVAL, "mcrt_set_opacity: bad temperature table");
+  for (auto& t : ctx->tickets)
+    if (t.busy) return fail(ctx, MCRT_ESTATE, "mcrt_set_opacity: a read-out ticket is in flight (call mcrt_results_wait first)");
   CU(cudaDeviceSynchronize());
+  for (auto& t : ctx->tickets) { mc_free(t.snap_small); t.snap_small = nullptr; }   // sized by n_bins
   free_opacity(ctx);
   free_pah(ctx);                                            // a PAH is declared against an opacity set
   free_sources(ctx);
@@ -1696,6 +1732,12 @@ mcrt_status mcrt_gather_calibrate(uint64_t footprint_bytes, uint64_t n_gathers, 
   *gathers_per_s = sec > 0 ? (double)turns * (double)per_turn / sec : 0.0;
   if (seconds) *seconds = sec;
   return MCRT_OK;
+}
+
+int64_t mcrt_release_cached_memory(void) {
+  McState& S = mc_state();
+  std::lock_guard<std::mutex> lock(S.mutex);
+  return (int64_t)mc_release_cache_locked(S);
 }
 
 const char* mcrt_last_error(const mcrt_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }

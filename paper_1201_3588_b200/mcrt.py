@@ -60,19 +60,23 @@ class _Results(C.Structure):
                 ("eps", C.POINTER(C.c_double))]
 
 
-# every symbol include/mcrt.h declares
-SYMBOLS = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opacity",
-           "mcrt_set_source", "mcrt_run_batch", "mcrt_transport_batch",
-           "mcrt_update_temperature", "mcrt_store_slots", "mcrt_delta_words", "mcrt_transport_batch_delta",
-           "mcrt_accumulate_update", "mcrt_get_results", "mcrt_results_begin", "mcrt_results_wait",
-           "mcrt_get_cell_energy",
-           "mcrt_get_cell_temperature", "mcrt_get_cell_temperature_noalloc", "mcrt_get_sed", "mcrt_set_pah", "mcrt_get_pah_absorbed",
-           "mcrt_get_pah_emission_cdf", "mcrt_get_pah_temperature_distribution", "mcrt_set_observer",
-           "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters",
-           "mcrt_reset_tallies", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_tail_mode", "mcrt_set_source_order",
-           "mcrt_set_density_staging", "mcrt_density_staging", "mcrt_set_region_sweeps", "mcrt_get_region_sweep_counts",
-           "mcrt_get_batch_times", "mcrt_get_tables",
-           "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks", "mcrt_uniforms", "mcrt_gather_calibrate", "mcrt_last_error")
+# every symbol include/mcrt.h declares (the stable boundary) ...
+SYMBOLS_STABLE = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_set_opacity",
+                  "mcrt_set_source", "mcrt_run_batch", "mcrt_transport_batch",
+                  "mcrt_update_temperature", "mcrt_store_slots", "mcrt_delta_words", "mcrt_transport_batch_delta",
+                  "mcrt_accumulate_update", "mcrt_get_results", "mcrt_results_begin", "mcrt_results_wait",
+                  "mcrt_get_cell_energy", "mcrt_get_cell_temperature", "mcrt_get_cell_temperature_noalloc",
+                  "mcrt_get_sed", "mcrt_set_pah", "mcrt_get_pah_absorbed",
+                  "mcrt_get_pah_emission_cdf", "mcrt_get_pah_temperature_distribution", "mcrt_set_observer",
+                  "mcrt_get_sed_mu", "mcrt_get_image", "mcrt_get_counters", "mcrt_reset_tallies",
+                  "mcrt_release_cached_memory", "mcrt_last_error")
+# ... and include/mcrt_dev.h (tuning knobs, measurement tools, test hooks)
+SYMBOLS_DEV = ("mcrt_gather_calibrate", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_tail_mode",
+               "mcrt_set_source_order", "mcrt_set_density_staging", "mcrt_density_staging",
+               "mcrt_set_region_sweeps", "mcrt_get_region_sweep_counts", "mcrt_get_batch_times",
+               "mcrt_get_tables", "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks",
+               "mcrt_uniforms")
+SYMBOLS = SYMBOLS_STABLE + SYMBOLS_DEV
 
 
 def lib():
@@ -139,6 +143,8 @@ def lib():
         L.mcrt_uniforms.argtypes = [vp, vp, vp, vp, i64]
         L.mcrt_gather_calibrate.argtypes = [u64, u64, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
         L.mcrt_gather_calibrate.restype = C.c_int
+        L.mcrt_release_cached_memory.restype = i64
+        L.mcrt_release_cached_memory.argtypes = []
         L.mcrt_last_error.restype = C.c_char_p
         L.mcrt_last_error.argtypes = [vp]
         for name in ("mcrt_grid_create", "mcrt_destroy", "mcrt_set_opacity", "mcrt_set_source",
@@ -481,6 +487,10 @@ class Context:
                     "mcrt_get_tables")
         return opac, lnQ, cdf
 
+    def store_slots(self):
+        """Length of the library's internal storage of the leaf arrays (>= slots: bricks are padded)."""
+        return int(lib().mcrt_store_slots(self.h))
+
     def kernel_launches(self):
         return int(lib().mcrt_kernel_launches(self.h))
 
@@ -552,6 +562,12 @@ def gather_calibrate(footprint_bytes, n_gathers=1 << 30, stream=None):
     if rc != 0:
         raise McrtError(f"mcrt_gather_calibrate: status {rc}: {lib().mcrt_last_error(None).decode()}")
     return g.value, sec.value
+
+
+def release_cached_memory():
+    """Give the device blocks the library caches after contexts were destroyed back to the driver;
+    returns the bytes released."""
+    return int(lib().mcrt_release_cached_memory())
 
 
 def debug_violations():

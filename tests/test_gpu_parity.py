@@ -636,6 +636,42 @@ def test_combined_and_overlapped_read_out(M, maker):
     ctx.results_wait(h1), ctx.results_wait(h2)
 
 
+def test_set_opacity_with_more_bins_after_a_read_out(M):
+    """a read-out ticket's device snapshot of the small tallies is sized by n_bins.
+    Re-setting the opacity with MORE bins after mcrt_get_results must not let the next read-out copy
+    past the old block (which the caching allocator places beside the library's own tables): the
+    context re-used with 4096 bins gives exactly what a fresh context gives, its tables included,
+    and mcrt_set_opacity is refused while a ticket is still in flight."""
+    small = W.sphere(n_root=16, n_bins=16, n_packets=20_000, batch=20_000)
+    big = W.sphere(n_root=16, n_bins=4096, n_packets=20_000, batch=20_000)
+    mk = lambda wl, c: dict(sed=np.zeros((3, wl.n_bins), np.uint64), emitted_per_bin=np.zeros(wl.n_bins, np.uint64),
+                            n_abs=np.zeros(c.slots, np.uint64), T=np.zeros(c.slots, np.float32))
+    ctx = M.run_workload(small)
+    ctx.get_results(mk(small, ctx))                            # both tickets now own snapshots sized for 16 bins
+    ctx.get_results(mk(small, ctx))
+    h = ctx.results_begin(mk(small, ctx))
+    with pytest.raises(M.McrtError, match="ticket is in flight"):
+        ctx.set_opacity(big.lambda_edges_um, big.weight, big.kabs, big.ksca, big.g)
+    ctx.results_wait(h)
+    ctx.set_opacity(big.lambda_edges_um, big.weight, big.kabs, big.ksca, big.g)
+    ctx.set_source(big.sources)
+    ctx.reset_tallies(3)
+    fresh = M.from_workload(big)
+    tables = [t.copy() for t in ctx.get_tables()]
+    for first, cnt in big.batches():
+        ctx.run_batch(big.seed, first, cnt)
+        fresh.run_batch(big.seed, first, cnt)
+    for _ in range(3):                                         # both tickets, and the first one again
+        a, b = ctx.get_results(mk(big, ctx)), fresh.get_results(mk(big, fresh))
+        for k in ("sed", "emitted_per_bin", "n_abs", "T"):
+            assert np.array_equal(a[k], b[k]), k
+        assert a["counters"] == b["counters"] and a["counters"]["emitted"] == big.n_packets
+        assert a["sed"].sum() == big.n_packets
+    for t0, t1, t2 in zip(tables, ctx.get_tables(), fresh.get_tables()):
+        assert np.array_equal(t0, t1) and np.array_equal(t1, t2)   # no table was written over
+    assert M.release_cached_memory() >= 0
+
+
 def test_automatic_walk_quorum_does_not_change_results(M):
     """quorum 0 = chosen by the kernel from the job's crossings per flight."""
     wl = W.c2(n_root=32, n_packets=3 << 17, batch=1 << 17)
