@@ -33,8 +33,8 @@ UNIT = "packets/s"
 def make_workload(name: str):
     """Bench workloads.  c1_tau1 = BASELINE.json configs[1] at tau_V = 1 (the configuration the
     10^8 packets/s target is quoted on)."""
-    if name == "c1_tau1_pah":                                # row f2: the tau_V = 1 sphere with a transiently heated PAH
-        return W.c1(tau_v=1.0)
+    if name.endswith("_pah"):                                # row f2: the same workload with a transiently heated PAH
+        return make_workload(name[:-4])
     if name.startswith("c1_tau"):
         return W.c1(tau_v=float(name[6:]))
     if name == "c0":
@@ -455,7 +455,7 @@ def measure_tau_sweep(torch, mcrt, repeats=3):
 
 
 PER_CONFIG = (("c0", 6), ("c1_tau0.1", 4), ("c1_tau10", 4), ("c1_tau100", 4), ("c2", 3), ("c3", 3), ("c4", 3),
-              ("c1_tau1_pah", 4))
+              ("c1_tau1_pah", 4), ("c2_pah", 3))
 
 
 def run_gpu(args, wl, name):
