@@ -74,6 +74,12 @@ int32_t mcrt_density_staging(const mcrt_ctx* ctx);
  * 2^21 packages).  Batches below 65536 packages are never reordered; more than 64 sources fall
  * back to mode 1, more than 2048 to 0.  Integer tallies: results do not depend on it. */
 mcrt_status mcrt_set_source_order(mcrt_ctx* ctx, int32_t mode);
+/* The re-emission bin of an absorbed package is the first bin whose cumulative emission reaches the
+ * package's uniform (Eqn 11.67; R11), found by bisection of a table row.  on != 0
+ * (the default): a guide table built with the rows (32 slices of the uniform per row) hands the
+ * bisection the few bins of the uniform's slice -- one load instead of its first four or five
+ * probes; on = 0: plain bisection of the whole row.  The bin found is the same, bit for bit. */
+mcrt_status mcrt_set_cdf_guide(mcrt_ctx* ctx, int32_t on);
 /* Device times in ms of the mcrt_run_batch calls made since the previous call of this function
  * (oldest first, at most `cap`), split into the two kernels of a batch (transport, temperature
  * update), from CUDA events recorded on each batch's stream.  Synchronises with those streams.

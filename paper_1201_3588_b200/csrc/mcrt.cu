@@ -153,6 +153,8 @@ struct mcrt_ctx {
   float4* d_opac = nullptr;
   float *d_lnQ = nullptr, *d_cdf = nullptr;
   int* d_guide = nullptr;                 // [kGuide] bracket guide of the ln Q table (tables.cuh)
+  uint32_t* d_cdf_guide = nullptr;        // [nT][kCdfGuide] bracket guide of the emission rows (tables.cuh)
+  int cdf_guide_off = 0;                  // mcrt_set_cdf_guide(0): plain bisection (for the bit-identity test)
   // sources
   int nsrc = 0;
   SrcDev* d_src = nullptr;
@@ -252,7 +254,8 @@ static mcrt_status fail(mcrt_ctx* c, mcrt_status st, const std::string& msg) {
 
 static void free_opacity(mcrt_ctx* c) {
   mc_free(c->d_nu); mc_free(c->d_dnu); mc_free(c->d_kabs); mc_free(c->d_opac);
-  mc_free(c->d_lnQ); mc_free(c->d_cdf); mc_free(c->d_small); mc_free(c->d_guide);
+  mc_free(c->d_lnQ); mc_free(c->d_cdf); mc_free(c->d_small); mc_free(c->d_guide); mc_free(c->d_cdf_guide);
+  c->d_cdf_guide = nullptr;
   c->d_nu = c->d_dnu = c->d_kabs = nullptr; c->d_opac = nullptr; c->d_lnQ = c->d_cdf = nullptr; c->d_guide = nullptr;
   c->d_small = nullptr;
 }
@@ -667,6 +670,7 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
   CU(mc_malloc(&ctx->d_lnQ, 4 * nT));
   CU(mc_malloc(&ctx->d_cdf, 4 * (size_t)nT * nb));
   CU(mc_malloc(&ctx->d_guide, sizeof(int) * kGuide));
+  CU(mc_malloc(&ctx->d_cdf_guide, sizeof(uint32_t) * (size_t)nT * kCdfGuide));
   const size_t n_small = 1 + CNT_N + 4 * (size_t)nb;
   CU(mc_malloc(&ctx->d_small, 8 * n_small));
   CU(cudaMemset(ctx->d_small, 0, 8 * n_small));
@@ -675,7 +679,8 @@ mcrt_status mcrt_set_opacity(mcrt_ctx* ctx, const mcrt_opacity_desc* d) {
   k_build_emission_rows<<<nT, 128, 8 * (nb + 1)>>>(nb, nT, Tmin, Tmax, ctx->d_nu, ctx->d_dnu,
                                                    ctx->d_kabs, ctx->d_lnQ, ctx->d_cdf);
   k_build_guide<<<kGuide / 256, 256>>>(ctx->d_lnQ, nT, ctx->d_guide);
-  ctx->launches += 3;
+  k_build_cdf_guide<<<nT, kCdfGuide>>>(ctx->d_cdf, nb, nT, ctx->d_cdf_guide);
+  ctx->launches += 4;
   CU(cudaGetLastError());
   CU(cudaDeviceSynchronize());
   ctx->have_opacity = true;
@@ -762,6 +767,7 @@ static mcrt_status launch_transport(mcrt_ctx* ctx, uint64_t seed, uint64_t first
   const int nb = ctx->nb;
   TransportParams P;
   P.rho = ctx->d_rho; P.tally = ctx->d_tally; P.tally32 = tally32; P.trow = ctx->d_trow;
+  P.cdf_guide = ctx->cdf_guide_off ? nullptr : ctx->d_cdf_guide;
   P.opac = ctx->d_opac; P.cdf = ctx->d_cdf; P.csrc = ctx->d_csrc32; P.csrc64 = ctx->d_csrc; P.src = ctx->d_src;
   if (!ctx->d_heads) {
     CU(mc_malloc(&ctx->d_heads, 16));
@@ -1264,11 +1270,12 @@ mcrt_status mcrt_set_pah(mcrt_ctx* ctx, const mcrt_pah_desc* d) {
   k_build_emission_rows<<<ctx->nT, 128, 8 * (nb + 1)>>>(nb, ctx->nT, ctx->Tmin, ctx->Tmax, ctx->d_nu, ctx->d_dnu,
                                                         ctx->d_kabs_eq, ctx->d_lnQ, ctx->d_cdf);
   k_build_guide<<<kGuide / 256, 256>>>(ctx->d_lnQ, ctx->nT, ctx->d_guide);
+  k_build_cdf_guide<<<ctx->nT, kCdfGuide>>>(ctx->d_cdf, nb, ctx->nT, ctx->d_cdf_guide);
   k_pah_states<<<K, 128>>>(nb, K, T_lo, T_hi, d->n_C, theta, ctx->d_nu, ctx->d_dnu, ctx->d_pah_C, ctx->d_pah_T,
                            ctx->d_pah_U, ctx->d_pah_Lam, ctx->d_pah_W, ctx->d_pah_W32);
   k_pah_thresholds<<<(K * K + 255) / 256, 256>>>(nb, K, ctx->d_pah_E, ctx->d_pah_U, ctx->d_pah_J);
   k_pah_cold_row<<<1, 32>>>(nb, ctx->d_pah_W, ctx->d_pah_cold);
-  ctx->launches += 6;
+  ctx->launches += 7;
   CU(cudaGetLastError());
   ctx->pahd.nC = d->n_C; ctx->pahd.K = K; ctx->pahd.nb = nb; ctx->pahd.fP = d->mass_fraction; ctx->pahd.theta = theta;
   ctx->pahd.E = ctx->d_pah_E; ctx->pahd.U = ctx->d_pah_U; ctx->pahd.Lam = ctx->d_pah_Lam; ctx->pahd.W = ctx->d_pah_W;
@@ -1600,6 +1607,12 @@ mcrt_status mcrt_set_density_staging(mcrt_ctx* ctx, int32_t mode) {
 }
 
 int32_t mcrt_density_staging(const mcrt_ctx* ctx) { return ctx ? staging_mode(ctx) : -1; }
+
+mcrt_status mcrt_set_cdf_guide(mcrt_ctx* ctx, int32_t on) {
+  if (!ctx) return MCRT_EINVAL;
+  ctx->cdf_guide_off = on ? 0 : 1;
+  return MCRT_OK;
+}
 
 mcrt_status mcrt_set_source_order(mcrt_ctx* ctx, int32_t mode) {
   if (!ctx) return MCRT_EINVAL;

@@ -70,6 +70,29 @@ __global__ void k_build_emission_rows(int nb, int nT, double Tmin, double Tmax,
     cdf[(size_t)k * nb + j] = (j == nb - 1 || !(Q > 0)) ? 1.f : (float)(s_term[j] / Q);
 }
 
+// Bracket guide of the emission rows: the re-emission bin is "the first j with C[j] >= u" (R11), found by bisection
+// of a 128...200-entry row -- 7-8 dependent loads from the L2 per absorption.  For u in [k/G, (k+1)/G) that bin lies
+// in [g_k, g_{k+1}], g_k = first j with C[j] >= k/G (C is non-decreasing and ends in 1): the pair is stored as one
+// word, lo | hi << 16, so ONE load narrows the search to the few bins of that slice.  Built from the fp32 rows with
+// the search's own comparison; k/G is exact in fp32, so the bin found is the bisection's, bit for bit.
+constexpr int kCdfGuide = 32;
+__global__ void k_build_cdf_guide(const float* __restrict__ cdf, int nb, int nT, uint32_t* __restrict__ guide) {
+  const int row = blockIdx.x, k = threadIdx.x;
+  if (row >= nT || k >= kCdfGuide) return;
+  const float* c = cdf + (size_t)row * nb;
+  uint32_t g[2];
+  for (int e = 0; e < 2; ++e) {
+    const float u = (float)(k + e) * (1.f / (float)kCdfGuide);
+    int lo = 0, hi = nb - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (c[mid] >= u) hi = mid; else lo = mid + 1;
+    }
+    g[e] = (uint32_t)lo;
+  }
+  guide[(size_t)row * kCdfGuide + k] = g[0] | (g[1] << 16);
+}
+
 // Source spectra: blackbody truncated to the band, same midpoint rule (R5, R6).  Kept in fp64: the
 // emission bin is settled once per package with the fp64 uniform, so emitted-per-bin is exact; the
 // fp32 copy serves the search loop that emission shares with re-emission.

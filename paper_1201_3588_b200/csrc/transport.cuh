@@ -55,6 +55,7 @@ struct TransportParams {
   const float* __restrict__ trow;              // [slots] temperature as table row coordinate
   const float4* __restrict__ opac;             // [nb] (kappa_ext*root_size, albedo, g, kappa_abs)
   const float* __restrict__ cdf;               // [nT][nb] emission inverse-CDF rows
+  const uint32_t* __restrict__ cdf_guide;      // [nT][kCdfGuide] bracket of the search in a row (tables.cuh), or NULL
   const float* __restrict__ csrc;              // [nsrc][nb] source spectrum CDFs, fp32 copy: searched in the same
                                                // instruction stream as the re-emission rows ...
   const double* __restrict__ csrc64;           // ... and the fp64 table that settles the bin exactly
@@ -139,6 +140,16 @@ __device__ __forceinline__ void draw4(unsigned long long seed, unsigned long lon
   uint32_t x[4];
   draw4w(seed, pid, k, tag, x);
   u[0] = u01(x[0]); u[1] = u01(x[1]); u[2] = u01(x[2]); u[3] = u01(x[3]);
+}
+
+// first j with cdf[j] >= u, known to lie in [lo, hi] (the whole row, or the bracket a guide table gives)
+template <typename T>
+__device__ __forceinline__ int search_cdf_range(const T* __restrict__ cdf, int lo, int hi, T u) {
+  while (lo < hi) {
+    int mid = (lo + hi) >> 1;
+    if (__ldg(cdf + mid) >= u) hi = mid; else lo = mid + 1;
+  }
+  return lo;
 }
 
 // first j with cdf[j] >= u

@@ -855,6 +855,7 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
         const float* row;
         float us;
         int s = 0;
+        int lo = 0, hi = P.nb - 1;                           // where the bin search starts (narrowed by the rows' guide)
         if (is_new) {                                        // O4: source by luminosity (fp64, exact)
           const double u0 = u01d(xw[0]);
           while (s < P.nsrc - 1 && P.src[s].lcdf < u0) ++s;
@@ -889,9 +890,13 @@ __global__ void __launch_bounds__(256, MINBLOCKS) k_transport_u(const TransportP
             int rw = (u01(xw[1]) < w && k0 + 1 < P.nT) ? k0 + 1 : k0; // R11 stochastic row choice
             row = P.cdf + (size_t)rw * P.nb;
             us = u01(xw[0]);
+            if (P.cdf_guide) {                               // one load instead of the first four or five probes
+              const uint32_t g = __ldg(P.cdf_guide + rw * kCdfGuide + (int)(us * (float)kCdfGuide));
+              lo = (int)(g & 0xffffu); hi = (int)(g >> 16);
+            }
           }
         }
-        bin = search_cdf<float>(row, P.nb, us);              // one search loop for emission and re-emission
+        bin = search_cdf_range<float>(row, lo, hi, us);      // one search loop for emission and re-emission
         if (is_new) {
           // the emission bin is settled in fp64 against the fp64 table with the oracle's uniform: the fp32
           // search lands within a bin or two of "first j with C[j] >= u", a short walk ends exactly on it

@@ -72,7 +72,7 @@ SYMBOLS_STABLE = ("mcrt_grid_create", "mcrt_destroy", "mcrt_leaf_slots", "mcrt_s
                   "mcrt_release_cached_memory", "mcrt_last_error")
 # ... and include/mcrt_dev.h (tuning knobs, measurement tools, test hooks)
 SYMBOLS_DEV = ("mcrt_gather_calibrate", "mcrt_set_launch", "mcrt_set_walk_quorum", "mcrt_set_tail_mode",
-               "mcrt_set_source_order", "mcrt_set_density_staging", "mcrt_density_staging",
+               "mcrt_set_source_order", "mcrt_set_cdf_guide", "mcrt_set_density_staging", "mcrt_density_staging",
                "mcrt_set_region_sweeps", "mcrt_get_region_sweep_counts", "mcrt_get_batch_times",
                "mcrt_get_tables", "mcrt_kernel_launches", "mcrt_debug_violations", "mcrt_philox_blocks",
                "mcrt_uniforms")
@@ -125,6 +125,8 @@ def lib():
         L.mcrt_set_walk_quorum.argtypes = [vp, i32]
         L.mcrt_set_tail_mode.argtypes = [vp, i32]
         L.mcrt_set_source_order.argtypes = [vp, i32]
+        L.mcrt_set_cdf_guide.argtypes = [vp, i32]
+        L.mcrt_set_cdf_guide.restype = C.c_int
         L.mcrt_set_region_sweeps.argtypes = [vp, i32, i32, i32, i32]
         L.mcrt_set_region_sweeps.restype = C.c_int
         L.mcrt_get_region_sweep_counts.argtypes = [vp, vp, i32, C.POINTER(i32)]
@@ -467,6 +469,9 @@ class Context:
 
     def density_staging(self):
         return int(lib().mcrt_density_staging(self.h))
+
+    def set_cdf_guide(self, on=True):
+        self._check(lib().mcrt_set_cdf_guide(self.h, 1 if on else 0), "mcrt_set_cdf_guide")
 
     def set_source_order(self, mode):
         self._check(lib().mcrt_set_source_order(self.h, int(mode)), "mcrt_set_source_order")

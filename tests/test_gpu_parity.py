@@ -672,6 +672,26 @@ def test_set_opacity_with_more_bins_after_a_read_out(M):
     assert M.release_cached_memory() >= 0
 
 
+@pytest.mark.parametrize("maker", [lambda: W.c1(tau_v=10.0, n_packets=3 << 17, batch=1 << 17),
+                                   lambda: W.c2(n_root=32, n_packets=3 << 17, batch=1 << 17),
+                                   lambda: W.sphere(n_root=16, n_bins=4096, tau_v=5.0, n_packets=60_000, batch=20_000),
+                                   lambda: W.sphere(n_root=16, n_bins=3, tau_v=5.0, n_packets=60_000, batch=20_000)])
+def test_cdf_guide_does_not_change_results(M, maker):
+    """The bracket guide of the emission rows (mcrt_set_cdf_guide, tables.cuh k_build_cdf_guide) only shortens
+    the bisection that finds the re-emission bin: with and without it every tally is identical, over
+    several batches (the temperatures, hence the rows searched, move), with 3, 128, 200 and 4096 bins."""
+    wl = maker()
+    a = M.from_workload(wl)
+    a.set_cdf_guide(False)
+    b = M.from_workload(wl)                                     # the default: guide on
+    for first, cnt in wl.batches():
+        a.run_batch(wl.seed, first, cnt)
+        b.run_batch(wl.seed, first, cnt)
+    _assert_identical(a, b)
+    c = b.get_counters()
+    assert c["emitted"] == wl.n_packets and c["absorptions"] > 10_000
+
+
 def test_automatic_walk_quorum_does_not_change_results(M):
     """quorum 0 = chosen by the kernel from the job's crossings per flight."""
     wl = W.c2(n_root=32, n_packets=3 << 17, batch=1 << 17)
