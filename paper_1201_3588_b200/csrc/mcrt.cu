@@ -53,6 +53,14 @@ struct DeviceScope {
   ~DeviceScope() { if (switched) cudaSetDevice(prev); }
 };
 
+// While one of these is alive on a thread, mc_free on that thread skips its device synchronisation: the caller has
+// synchronised the device itself and launches nothing until the scope ends (mcrt_destroy: one wait, not one per block).
+thread_local int tl_mc_device_idle = 0;
+struct DeviceIdleScope {
+  DeviceIdleScope() { ++tl_mc_device_idle; }
+  ~DeviceIdleScope() { --tl_mc_device_idle; }
+};
+
 // Frees every cached block (the caller holds the lock).
 size_t mc_release_cache_locked(McState& S) {
   const size_t bytes = S.cached;
@@ -109,7 +117,7 @@ static cudaError_t mc_free(void* q) {
   }
   DeviceScope scope(blk.device);                             // the device the block lives on, whichever is current
   if (blk.bytes && blk.bytes <= kMcBlockMax && blk.device >= 0) {
-    cudaDeviceSynchronize();
+    if (!tl_mc_device_idle) cudaDeviceSynchronize();
     std::lock_guard<std::mutex> lock(S.mutex);
     if (S.cached + blk.bytes <= kMcTotalMax) {
       S.cache.insert({{blk.device, blk.bytes}, q});
@@ -598,6 +606,7 @@ mcrt_status mcrt_destroy(mcrt_ctx* ctx) {
   if (!ctx) return MCRT_EINVAL;
   DeviceScope scope(ctx->device);                            // the context's GPU, whichever is current in the caller
   cudaDeviceSynchronize();                                   // nothing of this context may still be running
+  DeviceIdleScope idle;                                      // ... and nothing is launched below: the frees need not wait again
   for (auto& b : ctx->pending) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& b : ctx->spare) { cudaEventDestroy(b.e0); cudaEventDestroy(b.e1); cudaEventDestroy(b.e2); }
   for (auto& t : ctx->tickets) {

@@ -672,6 +672,31 @@ def test_set_opacity_with_more_bins_after_a_read_out(M):
     assert M.release_cached_memory() >= 0
 
 
+def test_cached_device_memory_is_reused_and_can_be_released(M):
+    """the library keeps the device blocks of a destroyed context (up to 1 GB) for the next
+    context of the same shape; mcrt_release_cached_memory hands them back to the driver (so that torch,
+    NCCL or the caller's own cudaMalloc can have them) and reports the bytes; a context created
+    afterwards allocates afresh and gives the same results."""
+    import torch
+    wl = W.sphere(n_root=128, n_packets=50_000, batch=25_000)     # 2 M cells: blocks of 8-16 MB, well above the driver's 2 MB slabs
+    M.release_cached_memory()
+    ctx = M.run_workload(wl)
+    sed = ctx.get_sed().copy()
+    torch.cuda.synchronize()
+    free_live = torch.cuda.mem_get_info()[0]
+    ctx.destroy()
+    assert torch.cuda.mem_get_info()[0] <= free_live + (1 << 20)   # destroyed, but the blocks stay with the library
+    again = M.run_workload(wl)                                      # ... and serve the next context of this shape
+    assert np.array_equal(again.get_sed(), sed)
+    again.destroy()
+    released = M.release_cached_memory()
+    assert released >= 128 ** 3 * (4 + 4 + 8 + 4)                   # at least density, ln density, tally, temperature rows
+    assert torch.cuda.mem_get_info()[0] >= free_live + released // 2
+    assert M.release_cached_memory() == 0
+    fresh = M.run_workload(wl)
+    assert np.array_equal(fresh.get_sed(), sed)
+
+
 @pytest.mark.parametrize("maker", [lambda: W.c1(tau_v=10.0, n_packets=3 << 17, batch=1 << 17),
                                    lambda: W.c2(n_root=32, n_packets=3 << 17, batch=1 << 17),
                                    lambda: W.sphere(n_root=16, n_bins=4096, tau_v=5.0, n_packets=60_000, batch=20_000),
