@@ -300,6 +300,10 @@ def lognormal_field(n: int, corr_cells: float, sigma_ln: float, seed: int) -> np
 
 def c4(n_root=512, n_packets=1_000_000_000, batch=1 << 24, seed=1, tau_v=10.0,
        corr_cells=8.0) -> Workload:
+    """BASELINE.json configs[4]: clumpy cube, ten interior stars + an external field.  Deviation from
+    SURVEY.md 8(d), which proposed drawing the field and the star positions from Philox SETUP blocks:
+    they come from numpy's default_rng(seed) / default_rng(seed + 1000) -- an input generator shared by
+    both sides needs no tie to the method's own generator, and neither side redraws them."""
     h = 1.0 * AU
     edges = lambda_edges(128, 0.05, 1000.0)
     w, kabs, ksca, g = _grey_single_species(edges, 0.6, 0.5)
